@@ -1,0 +1,161 @@
+"""CPU oracle of the KineticXGPU collision operator -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` / `--impl reference`
+legs may import this package.  It shares no code with `paper_2607_00755_b200/` and never
+imports it.  The arithmetic lives in `kx_oracle.c` (plain C, literal loops in the paper's
+notation); this file only compiles it with gcc and marshals numpy arrays through ctypes.
+
+Steps and citations: see the header of `kx_oracle.c` (eq. 4.4,
+4.6, 4.7, B.15-B.20, C.1-C.9).  Pins: tests/test_oracle_pins.py.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "kx_oracle.c")
+_LIB = os.path.join(_HERE, "libokx.so")
+_lib = None
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+
+
+def build(force: bool = False) -> str:
+    """Compile kx_oracle.c -> libokx.so (gcc -O2 -ffp-contract=off -fopenmp)."""
+    if force or (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.check_call(cmd)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_LIB)
+        _lib.okx_kinematics.argtypes = [C.c_int, _dp, _dp, C.c_double, _dp, _dp, _dp]
+        _lib.okx_kinematics.restype = None
+        _lib.okx_build.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double, C.c_double,
+                                   _dp, _ip, _dp]
+        _lib.okx_build.restype = C.c_long
+        _lib.okx_collide.argtypes = [C.c_int, C.c_int, _dp, _dp, _ip, _dp, C.c_int, C.c_double,
+                                     _dp, _dp, _dp]
+        _lib.okx_collide.restype = None
+        _lib.okx_project.argtypes = [C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp]
+        _lib.okx_project.restype = None
+        _lib.okx_moments.argtypes = [C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp]
+        _lib.okx_moments.restype = None
+        _lib.okx_evolve.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double,
+                                    C.c_double, C.c_int, C.c_double, C.c_double, _dp, C.c_int, C.c_int,
+                                    _dp, _dp, _dp, _dp, C.c_int, C.c_int, _dp, _dp, _dp]
+        _lib.okx_evolve.restype = C.c_int
+        _lib.okx_F_quadrature.argtypes = [C.c_double] * 6 + [C.c_int, _dp, _dp]
+        _lib.okx_F_quadrature.restype = C.c_double
+        _lib.okx_F_closed.argtypes = [C.c_double] * 6
+        _lib.okx_F_closed.restype = C.c_double
+    return _lib
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _c(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+LOG, LINEAR = 0, 1
+EULER, HEUN, RK4 = 0, 1, 2
+
+
+def kinematics(p, dp, m):
+    """O1: returns E, K, h."""
+    p, dp = _c(p), _c(dp)
+    n = p.size
+    E, K, h = np.empty(n), np.empty(n), np.empty(n)
+    _load().okx_kinematics(n, _d(p), _d(dp), float(m), _d(E), _d(K), _d(h))
+    return E, K, h
+
+
+class Tables:
+    """Dense W[i,n,m], jL[i,n,m] (-1 = dropped), wR[i,n,m] from the quadruple loop (O2-O7)."""
+
+    def __init__(self, p, dp, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0):
+        self.p, self.dp = _c(p), _c(dp)
+        self.m, self.g_chi, self.M2_0, self.m_med = float(m), float(g_chi), float(M2_0), float(m_med)
+        n = self.N = self.p.size
+        self.W = np.empty((n, n, n))
+        self.jL = np.empty((n, n, n), dtype=np.int32)
+        self.wR = np.empty((n, n, n))
+        self.kept = _load().okx_build(n, _d(self.p), _d(self.dp), self.m, self.g_chi, self.M2_0,
+                                      self.m_med, _d(self.W), self.jL.ctypes.data_as(_ip), _d(self.wR))
+        self.E, self.K, self.h = kinematics(self.p, self.dp, self.m)
+
+
+def collide(T: Tables, f, interp=LOG, f_floor=1e-300):
+    """O8-O9: returns gain, loss, C_raw, each [B,N]."""
+    f = _c(np.atleast_2d(f))
+    B, n = f.shape
+    assert n == T.N
+    g, l, c = np.empty((B, n)), np.empty((B, n)), np.empty((B, n))
+    _load().okx_collide(n, B, _d(f), _d(T.W), T.jL.ctypes.data_as(_ip), _d(T.wR), int(interp),
+                        float(f_floor), _d(g), _d(l), _d(c))
+    return g, l, c
+
+
+def project(T: Tables, f, Craw, eps_supp=1e-12):
+    """O10: returns C_proj [B,N] and diag [B,4] = eps_N, eps_E, R_N, R_E."""
+    f, Craw = _c(np.atleast_2d(f)), _c(np.atleast_2d(Craw))
+    B, n = f.shape
+    out, diag = np.empty((B, n)), np.empty((B, 4))
+    for b in range(B):
+        fb, cb, ob, db = f[b], Craw[b], out[b], diag[b]
+        _load().okx_project(n, _d(fb), _d(cb), _d(T.h), _d(T.E), float(eps_supp), _d(ob), _d(db))
+    return out, diag
+
+
+def moments(T: Tables, f):
+    """O11: returns [B,4] = n, rho, <p>, <p^2>."""
+    f = _c(np.atleast_2d(f))
+    out = np.empty((f.shape[0], 4))
+    for b in range(f.shape[0]):
+        _load().okx_moments(T.N, _d(f[b]), _d(T.p), _d(T.h), _d(T.E), T.g_chi, _d(out[b]))
+    return out
+
+
+def evolve(p, dp, f, *, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, interp=LOG, f_floor=1e-300,
+           eps_supp=1e-12, method=RK4, tau=None, rate=None, mass=None, kappa=None, project=True,
+           G=None, amp=None, want_diag=False):
+    """O12: fixed-step integration; returns f_final [B,N] (and diag [S,B,6] if want_diag)."""
+    p, dp = _c(p), _c(dp)
+    f = _c(np.atleast_2d(f)).copy()
+    B, n = f.shape
+    tau = _c(tau)
+    S = tau.size - 1
+    rate = None if rate is None else _c(rate)
+    mass = None if mass is None else _c(mass)
+    kappa = None if kappa is None else _c(kappa)
+    nsrc = 0 if G is None else int(np.atleast_2d(G).shape[0])
+    G = None if G is None else _c(np.atleast_2d(G))
+    amp = None if amp is None else _c(np.atleast_2d(amp))
+    diag = np.zeros((S, B, 6)) if want_diag else None
+    rc = _load().okx_evolve(n, B, _d(p), _d(dp), float(m), float(g_chi), float(M2_0), float(m_med),
+                            int(interp), float(f_floor), float(eps_supp), _d(f), int(method), S,
+                            _d(tau), _d(rate), _d(mass), _d(kappa), int(bool(project)), nsrc,
+                            _d(G), _d(amp), _d(diag))
+    assert rc == 0
+    return (f, diag) if want_diag else f
+
+
+def F_quadrature(pi, pn, pm, m, M2_0, m_med, mu, wmu):
+    mu, wmu = _c(mu), _c(wmu)
+    return _load().okx_F_quadrature(pi, pn, pm, m, M2_0, m_med, mu.size, _d(mu), _d(wmu))
+
+
+def F_closed(pi, pn, pm, m, M2_0, m_med):
+    return _load().okx_F_closed(pi, pn, pm, m, M2_0, m_med)

@@ -1,0 +1,392 @@
+/*
+ * kx_oracle.c -- plain, slow, obviously-correct CPU oracle for the discretized 2->2 elastic
+ * self-collision operator of KineticXGPU (arxiv/paper_2607_00755).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may call it.  It shares no code, header,
+ * table or constant with paper_2607_00755_b200/csrc (the CUDA path) and neither includes the other.
+ *
+ * The method is a discretization, so the oracle follows the paper's algorithm step by step in the
+ * paper's notation; citations are PAPER.md line numbers.
+ *   build   : literal quadruple loop (i, n, m, j)          -- eq. 4.4, 4.7, B.15-B.19
+ *   evaluate: literal triple loop over dense W[i][n][m]     -- eq. 4.6 with 2.6, B.18, B.20
+ *   project : App. C, eq. C.2-C.8 ; diagnostics C.1, C.9
+ *   moments : eq. B.1-B.2
+ *   evolve  : fixed-step Euler / Heun / RK4 on eq. 4.9
+ * No symmetry reduction, no sparsity tricks, no blocking, no fusion.  Sums use long double
+ * accumulators (x87 80-bit on x86-64).  Compile with -O2 -ffp-contract=off.
+ *
+ * Readings of the paper (D1-D13) are listed in DESIGN.md.  Pins: tests/test_oracle_pins.py
+ * (P1-P10).  Functions with no pin outside themselves: none on the hot path; the paper's
+ * Fig. 2 / Table 1 / Figs. 4-8, 12-13 comparisons are "parity unpinned" (need BEST and SM tables).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define OKX_PI 3.14159265358979323846264338327950288L
+
+/* ---- O1: kinematics.  E_i = sqrt(p_i^2+m^2); K_i = E_i - m written as
+ * p_i^2/(E_i+m) (reading D3: same number, no cancellation); h_i = p_i^2 dp_i (eq. B.1). */
+void okx_kinematics(int N, const double *p, const double *dp, double m,
+                    double *E, double *K, double *h)
+{
+    for (int i = 0; i < N; ++i) {
+        E[i] = sqrt(p[i] * p[i] + m * m);
+        K[i] = (p[i] * p[i]) / (E[i] + m);
+        h[i] = (p[i] * p[i]) * dp[i];
+    }
+}
+
+/* Antiderivative of 1/(Q^2+c2)^2 (reading D5), long double.  c2 may have either sign; Q^2+c2>0. */
+static long double okx_anti(long double Q, long double c2)
+{
+    if (c2 > 0.0L) {
+        long double c = sqrtl(c2);
+        return Q / (2.0L * c2 * (Q * Q + c2)) + atanl(Q / c) / (2.0L * c2 * c);
+    } else {
+        long double k2 = -c2, k = sqrtl(k2);
+        return -Q / (2.0L * k2 * (Q * Q - k2)) + logl((Q + k) / (Q - k)) / (4.0L * k2 * k);
+    }
+}
+
+/* J = int_{Q-}^{Q+} |M|^2(Q) dQ.  Contact: |M|^2 = M2_0 (eq. B.17).
+ * Mediator (reading D5): |M|^2 = M2_0/(1+(-t)/m_med^2)^2 with -t = Q^2-(E_i-E_n)^2, so
+ * J = M2_0 m_med^4 int dQ/(Q^2+c2)^2, c2 = m_med^2-(E_i-E_n)^2 = m_med^2-(K_i-K_n)^2. */
+static double okx_J(double Qm, double Qp, double M2_0, double m_med, double Ki, double Kn)
+{
+    if (!(Qp > Qm)) return 0.0;
+    if (m_med <= 0.0) return M2_0 * (Qp - Qm);
+    long double dK = (long double)Ki - (long double)Kn;
+    long double mm = (long double)m_med * (long double)m_med;
+    long double c2 = mm - dK * dK;
+    long double a = Qm, b = Qp, val;
+    if (fabsl(c2) < 1e-6L * a * b) {
+        /* series in c2: 1/(Q^2+c2)^2 = sum_k (k+1)(-c2)^k Q^(-2k-4) */
+        val = 0.0L;
+        long double pw = 1.0L;
+        for (int k = 0; k < 8; ++k) {
+            long double e = (long double)(2 * k + 3);
+            val += pw * (long double)(k + 1) * (powl(a, -e) - powl(b, -e)) / e;
+            pw *= -c2;
+        }
+    } else {
+        val = okx_anti(b, c2) - okx_anti(a, c2);
+    }
+    return (double)((long double)M2_0 * mm * mm * val);
+}
+
+/* ---- O2-O7: build W_inm, jL(i,n,m), omega_R(i,n,m) for every ORDERED triple; the fourth loop is the
+ * bracket scan over j.  jL = -1 marks a dropped triple (W = 0).  Returns the number of kept triples. */
+long okx_build(int N, const double *p, const double *dp, double m, double g_chi,
+               double M2_0, double m_med, double *W, int32_t *jL, double *wR)
+{
+    double *E = malloc(sizeof(double) * N), *K = malloc(sizeof(double) * N), *h = malloc(sizeof(double) * N);
+    okx_kinematics(N, p, dp, m, E, K, h);
+    const double pi3 = (double)(OKX_PI * OKX_PI * OKX_PI);
+    long kept = 0;
+#pragma omp parallel for schedule(dynamic) reduction(+ : kept)
+    for (int i = 0; i < N; ++i)
+        for (int n = 0; n < N; ++n)
+            for (int mm = 0; mm < N; ++mm) {
+                size_t idx = ((size_t)i * N + n) * N + mm;
+                W[idx] = 0.0; jL[idx] = -1; wR[idx] = 0.0;
+                /* O2: energy conservation, eq. 4.4: E_j = E_n+E_m-E_i  <=>  K~ = K_n+K_m-K_i */
+                double Kt = (K[n] + K[mm]) - K[i];
+                /* D4: snap ties at the domain edge */
+                double tau = 32.0 * 2.220446049250313e-16 * (K[n] + K[mm] + K[i]);
+                if (Kt < K[0] && Kt >= K[0] - tau) Kt = K[0];
+                if (Kt > K[N - 1] && Kt <= K[N - 1] + tau) Kt = K[N - 1];
+                /* O3: keep iff E_j >= m and q_min <= q_j <= q_max <=> K_0 <= K~ <= K_{N-1} */
+                if (!(Kt >= K[0] && Kt <= K[N - 1])) continue;
+                /* O4 */
+                double pj = sqrt(Kt * (Kt + 2.0 * m));
+                /* O5: eq. B.15-B.16 */
+                double Qm = fmax(fabs(p[i] - p[n]), fabs(p[mm] - pj));
+                double Qp = fmin(p[i] + p[n], p[mm] + pj);
+                double J = okx_J(Qm, Qp, M2_0, m_med, K[i], K[n]);
+                /* O6: eq. 4.7 with F of eq. B.17 */
+                double w = dp[n] * dp[mm] / (2.0 * E[i] * g_chi);
+                w = w * (1.0 / (64.0 * pi3 * p[i]));
+                w = w * (p[n] * p[mm] / (E[n] * E[mm]));
+                w = w * J;
+                /* O7: bracket scan, largest j with K_j <= K~ <= K_{j+1}; eq. B.19 */
+                int jb = -1;
+                for (int j = 0; j <= N - 2; ++j)
+                    if (K[j] <= Kt && Kt <= K[j + 1]) jb = j;
+                if (jb < 0) continue; /* cannot happen after O3 */
+                W[idx] = w;
+                jL[idx] = jb;
+                wR[idx] = (Kt - K[jb]) / (K[jb + 1] - K[jb]);
+                kept += 1;
+            }
+    free(E); free(K); free(h);
+    return kept;
+}
+
+/* ---- O8-O9: evaluate.  interp 0 = LOG (eq. B.20 at eta=0; reading D7),
+ * 1 = LINEAR.  gain_i = sum_nm W f_n f_m ; loss_i = f_i sum_nm W f_j~ ; C_raw = gain - loss
+ * (eq. 4.6 with the dilute factor of eq. 2.6). f is [B,N] row-major. */
+void okx_collide(int N, int B, const double *f, const double *W, const int32_t *jL, const double *wR,
+                 int interp, double f_floor, double *gain, double *loss, double *C)
+{
+#pragma omp parallel for collapse(2) schedule(dynamic)
+    for (int b = 0; b < B; ++b)
+        for (int i = 0; i < N; ++i) {
+            const double *fb = f + (size_t)b * N;
+            long double g = 0.0L, l = 0.0L;
+            for (int n = 0; n < N; ++n)
+                for (int mm = 0; mm < N; ++mm) {
+                    size_t idx = ((size_t)i * N + n) * N + mm;
+                    int j = jL[idx];
+                    if (j < 0) continue;
+                    double w = W[idx];
+                    double oR = wR[idx], oL = 1.0 - oR;
+                    double fj;
+                    if (interp == 0) {
+                        /* D8: y = ln(max(f, f_floor)) */
+                        double yL = log(fmax(fb[j], f_floor)), yR = log(fmax(fb[j + 1], f_floor));
+                        fj = exp(oL * yL + oR * yR);
+                    } else {
+                        fj = oL * fb[j] + oR * fb[j + 1];
+                    }
+                    g += (long double)w * (long double)fb[n] * (long double)fb[mm];
+                    l += (long double)w * (long double)fj;
+                }
+            double gi = (double)g, li = (double)((long double)fb[i] * l);
+            if (gain) gain[(size_t)b * N + i] = gi;
+            if (loss) loss[(size_t)b * N + i] = li;
+            if (C) C[(size_t)b * N + i] = (double)(g - (long double)fb[i] * l);
+        }
+}
+
+/* ---- O10: two-moment projection, App. C eq. C.2-C.8, support mask C.4 with
+ * f_max = max_i |f_i|; degenerate cases per reading D9.  diag (may be NULL) receives
+ * eps_N, eps_E (C.1, raw), R_N, R_E (C.9).  One distribution. */
+void okx_project(int N, const double *f, const double *Craw, const double *h, const double *E,
+                 double eps_supp, double *Cproj, double *diag)
+{
+    long double R0 = 0, R1 = 0, S0 = 0, S1 = 0;
+    double fmax = 0.0;
+    for (int i = 0; i < N; ++i) {
+        R0 += (long double)h[i] * Craw[i];
+        R1 += (long double)h[i] * E[i] * Craw[i];
+        S0 += (long double)h[i] * fabs(Craw[i]);
+        S1 += (long double)h[i] * E[i] * fabs(Craw[i]);
+        if (fabs(f[i]) > fmax) fmax = fabs(f[i]);
+    }
+    long double A00 = 0, A01 = 0, A11 = 0;
+    double *xi = malloc(sizeof(double) * N);
+    for (int i = 0; i < N; ++i) {
+        double r = (fmax > 0.0) ? fabs(f[i]) / fmax : 0.0;
+        xi[i] = (r > eps_supp) ? r : 0.0;
+        A00 += (long double)h[i] * xi[i];
+        A01 += (long double)h[i] * E[i] * xi[i];
+        A11 += (long double)h[i] * E[i] * E[i] * xi[i];
+    }
+    long double alpha = 0, beta = 0;
+    if (fmax > 0.0 && A00 > 0.0L) {
+        long double det = A00 * A11 - A01 * A01;
+        if (det <= 1e-14L * A00 * A11) { alpha = R0 / A00; beta = 0; }
+        else { alpha = (R0 * A11 - R1 * A01) / det; beta = (R1 * A00 - R0 * A01) / det; }
+    }
+    long double D0 = 0, D1 = 0;
+    for (int i = 0; i < N; ++i) {
+        double corr = (double)((long double)xi[i] * (alpha + beta * (long double)E[i]));
+        Cproj[i] = Craw[i] - corr;
+        D0 += (long double)h[i] * fabs(corr);
+        D1 += (long double)h[i] * E[i] * fabs(corr);
+    }
+    if (diag) {
+        diag[0] = (S0 > 0) ? (double)(R0 / S0) : 0.0;
+        diag[1] = (S1 > 0) ? (double)(R1 / S1) : 0.0;
+        diag[2] = (S0 > 0) ? (double)(D0 / S0) : 0.0;
+        diag[3] = (S1 > 0) ? (double)(D1 / S1) : 0.0;
+    }
+    free(xi);
+}
+
+/* ---- O11: moments, eq. B.2 with the factor g_chi/(2 pi^2);
+ * <p^k> = sum h p^k f / sum h f.  out = n, rho, <p>, <p^2>. */
+void okx_moments(int N, const double *f, const double *p, const double *h, const double *E,
+                 double g_chi, double *out)
+{
+    long double s0 = 0, s1 = 0, sp = 0, sp2 = 0;
+    for (int i = 0; i < N; ++i) {
+        s0 += (long double)h[i] * f[i];
+        s1 += (long double)h[i] * E[i] * f[i];
+        sp += (long double)h[i] * p[i] * f[i];
+        sp2 += (long double)h[i] * p[i] * p[i] * f[i];
+    }
+    long double fac = (long double)g_chi / (2.0L * OKX_PI * OKX_PI);
+    out[0] = (double)(fac * s0);
+    out[1] = (double)(fac * s1);
+    out[2] = (s0 != 0) ? (double)(sp / s0) : 0.0;
+    out[3] = (s0 != 0) ? (double)(sp2 / s0) : 0.0;
+}
+
+/* ---- O12: fixed-step integrators on  df/dtau = kappa_b R(tau) C[f; m(tau)] + sum_s amp_s(step) G_s
+ * (eq. 4.9; regime description PAPER.md:225-227; reading D11/D12: source amplitude is
+ * constant over a step, expansion enters through rate[] and mass[]).
+ * method 0 Euler, 1 Heun, 2 RK4.  rate/mass are [2S+1] (nodes and midpoints) or NULL.  When mass is
+ * given the tables are rebuilt (O1-O7) at every stage.  project != 0 applies O10.
+ * diag: NULL or [S,B,6] = eps_N, eps_E, R_N, R_E (of the step's first stage), n, rho (after the step). */
+typedef struct {
+    int N; const double *p, *dp; double m, g_chi, M2_0, m_med; int interp; double f_floor, eps_supp;
+    double *W; int32_t *jL; double *wR; double *E, *K, *h; double cur_m;
+} okx_ctx;
+
+static void okx_rhs(okx_ctx *c, const double *f, double mass, int use_mass, double kR, int project,
+                    int nsrc, const double *G, const double *ampk, double *k, double *diag4)
+{
+    int N = c->N;
+    if (use_mass && mass != c->cur_m) {
+        okx_build(N, c->p, c->dp, mass, c->g_chi, c->M2_0, c->m_med, c->W, c->jL, c->wR);
+        okx_kinematics(N, c->p, c->dp, mass, c->E, c->K, c->h);
+        c->cur_m = mass;
+    }
+    double *Craw = malloc(sizeof(double) * N), *Cp = malloc(sizeof(double) * N);
+    okx_collide(N, 1, f, c->W, c->jL, c->wR, c->interp, c->f_floor, NULL, NULL, Craw);
+    if (project) okx_project(N, f, Craw, c->h, c->E, c->eps_supp, Cp, diag4);
+    else { memcpy(Cp, Craw, sizeof(double) * N); if (diag4) okx_project(N, f, Craw, c->h, c->E, c->eps_supp, Craw, diag4); }
+    for (int i = 0; i < N; ++i) {
+        double s = 0.0;
+        for (int q = 0; q < nsrc; ++q) s += ampk[q] * G[(size_t)q * N + i];
+        k[i] = kR * Cp[i] + s;
+    }
+    free(Craw); free(Cp);
+}
+
+int okx_evolve(int N, int B, const double *p, const double *dp, double m, double g_chi,
+               double M2_0, double m_med, int interp, double f_floor, double eps_supp,
+               double *f, int method, int S, const double *tau, const double *rate,
+               const double *mass, const double *kappa, int project,
+               int nsrc, const double *G, const double *amp, double *diag)
+{
+    size_t N3 = (size_t)N * N * N;
+    okx_ctx c = { N, p, dp, m, g_chi, M2_0, m_med, interp, f_floor, eps_supp,
+                  malloc(sizeof(double) * N3), malloc(sizeof(int32_t) * N3), malloc(sizeof(double) * N3),
+                  malloc(sizeof(double) * N), malloc(sizeof(double) * N), malloc(sizeof(double) * N), m };
+    okx_build(N, p, dp, m, g_chi, M2_0, m_med, c.W, c.jL, c.wR);
+    okx_kinematics(N, p, dp, m, c.E, c.K, c.h);
+    double *k1 = malloc(sizeof(double) * N), *k2 = malloc(sizeof(double) * N), *k3 = malloc(sizeof(double) * N),
+           *k4 = malloc(sizeof(double) * N), *ft = malloc(sizeof(double) * N), *ampk = malloc(sizeof(double) * (nsrc > 0 ? nsrc : 1));
+    int use_mass = mass != NULL;
+    /* the step loop is outermost so that a time-dependent mass needs one rebuild per stage, shared by all b */
+    for (int s = 0; s < S; ++s) {
+        double dt = tau[s + 1] - tau[s];
+        double R0 = rate ? rate[2 * s] : 1.0, Rh = rate ? rate[2 * s + 1] : 1.0, R1 = rate ? rate[2 * s + 2] : 1.0;
+        double m0 = use_mass ? mass[2 * s] : m, mh = use_mass ? mass[2 * s + 1] : m, m1 = use_mass ? mass[2 * s + 2] : m;
+        for (int q = 0; q < nsrc; ++q) ampk[q] = amp[(size_t)q * S + s];
+        /* stage-major over b so each rebuild is reused by every member */
+        if (method == 0) {
+            for (int b = 0; b < B; ++b) {
+                double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+                okx_rhs(&c, fb, m0, use_mass, kb * R0, project, nsrc, G, ampk, k1, diag ? diag + ((size_t)s * B + b) * 6 : NULL);
+                for (int i = 0; i < N; ++i) fb[i] = fb[i] + dt * k1[i];
+            }
+        } else if (method == 1) {
+            double *K1 = malloc(sizeof(double) * N * B);
+            for (int b = 0; b < B; ++b) {
+                double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+                okx_rhs(&c, fb, m0, use_mass, kb * R0, project, nsrc, G, ampk, K1 + (size_t)b * N, diag ? diag + ((size_t)s * B + b) * 6 : NULL);
+            }
+            for (int b = 0; b < B; ++b) {
+                double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N, *kk = K1 + (size_t)b * N;
+                for (int i = 0; i < N; ++i) ft[i] = fb[i] + dt * kk[i];
+                okx_rhs(&c, ft, m1, use_mass, kb * R1, project, nsrc, G, ampk, k2, NULL);
+                for (int i = 0; i < N; ++i) fb[i] = fb[i] + 0.5 * dt * (kk[i] + k2[i]);
+            }
+            free(K1);
+        } else {
+            double *K1 = malloc(sizeof(double) * N * B), *K2 = malloc(sizeof(double) * N * B), *K3 = malloc(sizeof(double) * N * B);
+            for (int b = 0; b < B; ++b) {
+                double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+                okx_rhs(&c, fb, m0, use_mass, kb * R0, project, nsrc, G, ampk, K1 + (size_t)b * N, diag ? diag + ((size_t)s * B + b) * 6 : NULL);
+            }
+            for (int b = 0; b < B; ++b) {
+                double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+                for (int i = 0; i < N; ++i) ft[i] = fb[i] + 0.5 * dt * K1[(size_t)b * N + i];
+                okx_rhs(&c, ft, mh, use_mass, kb * Rh, project, nsrc, G, ampk, K2 + (size_t)b * N, NULL);
+            }
+            for (int b = 0; b < B; ++b) {
+                double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+                for (int i = 0; i < N; ++i) ft[i] = fb[i] + 0.5 * dt * K2[(size_t)b * N + i];
+                okx_rhs(&c, ft, mh, use_mass, kb * Rh, project, nsrc, G, ampk, K3 + (size_t)b * N, NULL);
+            }
+            for (int b = 0; b < B; ++b) {
+                double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+                for (int i = 0; i < N; ++i) ft[i] = fb[i] + dt * K3[(size_t)b * N + i];
+                okx_rhs(&c, ft, m1, use_mass, kb * R1, project, nsrc, G, ampk, k4, NULL);
+                for (int i = 0; i < N; ++i)
+                    fb[i] = fb[i] + (dt / 6.0) * (K1[(size_t)b * N + i] + 2.0 * K2[(size_t)b * N + i] + 2.0 * K3[(size_t)b * N + i] + k4[i]);
+            }
+            free(K1); free(K2); free(K3);
+        }
+        if (diag) {
+            double mend = use_mass ? m1 : m;
+            if (use_mass && mend != c.cur_m) { okx_kinematics(N, p, dp, mend, c.E, c.K, c.h); }
+            for (int b = 0; b < B; ++b) {
+                double mo[4];
+                okx_moments(N, f + (size_t)b * N, p, c.h, c.E, g_chi, mo);
+                diag[((size_t)s * B + b) * 6 + 4] = mo[0];
+                diag[((size_t)s * B + b) * 6 + 5] = mo[1];
+            }
+            if (use_mass && mend != c.cur_m) { okx_kinematics(N, p, dp, c.cur_m, c.E, c.K, c.h); }
+        }
+    }
+    free(k1); free(k2); free(k3); free(k4); free(ft); free(ampk);
+    free(c.W); free(c.jL); free(c.wR); free(c.E); free(c.K); free(c.h);
+    return 0;
+}
+
+/* ---- Pin helper (P9), NOT on the evaluate path: the reduced kernel F(p_i,p_n,p_m) by the
+ * mu-quadrature of eq. B.5-B.12, nodes/weights supplied by the caller.
+ * If m_med > 0 the integrand carries |M|^2(t(mu)), t = 2m^2-2E_iE_n+2p_ip_n mu (reading D5). */
+double okx_F_quadrature(double pi_, double pn, double pm, double m, double M2_0, double m_med,
+                        int nmu, const double *mu, const double *wmu)
+{
+    double Ei = sqrt(pi_ * pi_ + m * m), En = sqrt(pn * pn + m * m), Em = sqrt(pm * pm + m * m);
+    long double acc = 0.0L;
+    for (int q = 0; q < nmu; ++q) {
+        double u = mu[q];
+        double A0 = m * m + En * Em - En * Ei - Em * Ei + pi_ * pn * u;   /* B.5 */
+        double A1 = pi_ * pm - pn * pm * u;                                 /* B.6 */
+        double K2 = pn * pn * pm * pm * (1.0 - u * u);                      /* B.7 */
+        double a = -(K2 + A1 * A1), b = -2.0 * A0 * A1, c = K2 - A0 * A0;   /* B.8 */
+        double disc = b * b - 4.0 * a * c;
+        if (!(disc > 0.0) || !(a < 0.0)) continue;
+        double sq = sqrt(disc);
+        double r1 = (-b + sq) / (2.0 * a), r2 = (-b - sq) / (2.0 * a);      /* B.10 */
+        double lo = fmin(r1, r2), hi = fmax(r1, r2);
+        if (hi <= -1.0 || lo >= 1.0) continue;
+        double vm = fmax(lo, -1.0), vp = fmin(hi, 1.0);
+        double am = fmax(-1.0, fmin(1.0, (2.0 * a * vm + b) / sq));
+        double ap = fmax(-1.0, fmin(1.0, (2.0 * a * vp + b) / sq));
+        double I = (asin(am) - asin(ap)) / sqrt(-a);                        /* B.11 */
+        double M2 = M2_0;
+        if (m_med > 0.0) {
+            double t = 2.0 * m * m - 2.0 * Ei * En + 2.0 * pi_ * pn * u;
+            double d = 1.0 + (-t) / (m_med * m_med);
+            M2 = M2_0 / (d * d);
+        }
+        acc += (long double)wmu[q] * I * M2;
+    }
+    double pref = 1.0 / (4.0 * pow(2.0 * (double)OKX_PI, 4)) * (pn * pm) * (pn * pm) / (En * Em); /* B.12 */
+    return pref * (double)acc;
+}
+
+/* The closed-form F used inside okx_build for one triple (exposed for the P9 pin): eq. B.17 / D5. */
+double okx_F_closed(double pi_, double pn, double pm, double m, double M2_0, double m_med)
+{
+    double Ei = sqrt(pi_ * pi_ + m * m), En = sqrt(pn * pn + m * m), Em = sqrt(pm * pm + m * m);
+    double Ki = pi_ * pi_ / (Ei + m), Kn = pn * pn / (En + m), Km = pm * pm / (Em + m);
+    double Kt = (Kn + Km) - Ki;
+    if (Kt < 0.0) return 0.0;
+    double pj = sqrt(Kt * (Kt + 2.0 * m));
+    double Qm = fmax(fabs(pi_ - pn), fabs(pm - pj)), Qp = fmin(pi_ + pn, pm + pj);
+    double J = okx_J(Qm, Qp, M2_0, m_med, Ki, Kn);
+    const double pi3 = (double)(OKX_PI * OKX_PI * OKX_PI);
+    return (1.0 / (64.0 * pi3 * pi_)) * (pn * pm / (En * Em)) * J;
+}

@@ -1,0 +1,324 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these retype the oracle's formulas: they are closed forms, invariants, special cases and a
+brute-force angular quadrature chosen so that a dropped term, wrong sign/index or transposed operand
+in `oracle/kx_oracle.c` fails at least one of them.  CPU only.
+"""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.integrate import quad
+
+import kx_inputs as kin
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+# ------------------------------------------------------------------ P1: W_inm = W_imn (B.17 symmetric)
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_P1_W_symmetric(oracle, cfg):
+    c = kin.config(cfg, N=48 if cfg == 3 else None)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    if c["m_med"] <= 0:     # contact: B.17 is symmetric in n<->m.  A t-channel |M|^2(t), t=(p_i-p_n)^2, is not (D5)
+        assert np.abs(T.W - T.W.transpose(0, 2, 1)).max() <= 1e-11 * np.abs(T.W).max()
+    assert (T.jL == T.jL.transpose(0, 2, 1)).all()          # the index map always is
+    assert (T.W >= 0).all() and T.kept == int((T.jL >= 0).sum())
+
+
+# ------------------------------------------------------------------ P2: overlap invariance, massless = 2 min(p)
+def test_P2_massless_overlap_is_twice_min(oracle):
+    rng = np.random.default_rng(7)
+    for _ in range(200):
+        pi, pn, pm = rng.uniform(0.05, 5.0, size=3)
+        pj = pn + pm - pi
+        F = oracle.F_closed(pi, pn, pm, 0.0, 1.0, 0.0)
+        if pj <= 0:
+            assert F == 0.0
+            continue
+        expect = 2.0 * min(pi, pn, pm, pj) / (64.0 * math.pi ** 3 * pi)       # p/E = 1 at m = 0
+        assert F == pytest.approx(expect, rel=1e-12, abs=1e-18)
+
+
+def test_P2_permutation_invariance_massive(oracle):
+    """[min(a+b,c+d)-max(|a-b|,|c-d|)]_+ is invariant under all 24 permutations of (p_i,p_n,p_m,p_j):
+    exchanging the roles (i<->n) and (i,n)<->(m,j) must leave p_i*E_n*E_m*F/(p_n p_m) unchanged."""
+    rng = np.random.default_rng(8)
+    m = 1.0
+    E = lambda p: math.sqrt(p * p + m * m)
+    for _ in range(100):
+        pi, pn, pm = rng.uniform(0.05, 4.0, size=3)
+        Ej = E(pn) + E(pm) - E(pi)
+        if Ej <= m * (1 + 1e-9):
+            continue
+        pj = math.sqrt(Ej * Ej - m * m)
+        ov = lambda a, b, c: oracle.F_closed(a, b, c, m, 1.0, 0.0) * a * E(b) * E(c) / (b * c)
+        base = ov(pi, pn, pm)
+        # (i,n,m,j) -> (n,i,j,m): chi_n chi_i <- chi_j chi_m has the same overlap
+        assert ov(pn, pi, pj) == pytest.approx(base, rel=1e-9, abs=1e-15)
+        assert ov(pi, pm, pn) == pytest.approx(base, rel=1e-9, abs=1e-15)
+        assert ov(pj, pm, pn) == pytest.approx(base, rel=1e-9, abs=1e-15)
+
+
+# ------------------------------------------------------------------ P3: zeros of W only from the validity test
+def test_P3_zeros_only_from_validity(oracle):
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    kept = T.jL >= 0
+    # interior kept triples (strictly inside the K range) have a strictly positive overlap
+    Kt = T.K[None, :, None] + T.K[None, None, :] - T.K[:, None, None]
+    interior = kept & (Kt > T.K[0] * (1 + 1e-9)) & (Kt < T.K[-1] * (1 - 1e-9))
+    assert (T.W[interior] > 0).all()
+    assert (T.W[~kept] == 0).all()
+    # validity is exactly E_j >= m, q_min <= q_j <= q_max away from ties
+    far = np.abs(Kt - T.K[0]) > 1e-9
+    far &= np.abs(Kt - T.K[-1]) > 1e-9
+    assert (kept[far] == ((Kt >= T.K[0]) & (Kt <= T.K[-1]))[far]).all()
+
+
+# ------------------------------------------------------------------ P4: exact conservation special case
+@pytest.mark.parametrize("interp", [0, 1])
+def test_P4_exact_conservation_massless_uniform(oracle, interp):
+    N, D = 40, 0.25
+    p = D * np.arange(1, N + 1)
+    dp = np.full(N, D)
+    T = oracle.Tables(p, dp, 0.0)
+    assert np.all((T.wR[T.jL >= 0] < 1e-12) | (T.wR[T.jL >= 0] > 1 - 1e-12))   # every j~ on-grid
+    f = kin.bimodal(p, (2.0, 6.0), (0.5, 1.0))[None, :]
+    g, l, C = oracle.collide(T, f, interp)
+    h, E = T.h, T.E
+    epsN = (h * C[0]).sum() / (h * np.abs(C[0])).sum()
+    epsE = (h * E * C[0]).sum() / (h * E * np.abs(C[0])).sum()
+    assert abs(epsN) <= 1e-14 and abs(epsE) <= 1e-14
+    # total gain = total loss, and energy-weighted too (number / energy conservation, eq. 2.7 / 4.8)
+    assert (h * g[0]).sum() == pytest.approx((h * l[0]).sum(), rel=1e-13)
+
+
+def test_P4_exchange_symmetry_of_W(oracle):
+    """Detailed-balance structure: h_i W_inm = h_n W_{n,i,j} on the exact grid (exchange (i,j)<->(n,m))."""
+    N, D = 24, 0.5
+    p = D * np.arange(1, N + 1)
+    T = oracle.Tables(p, np.full(N, D), 0.0)
+    checked = 0
+    for i, n, m in itertools.product(range(N), repeat=3):
+        j = n + m - i                                    # p_j = p_n + p_m - p_i  ->  index n+m-i+... (p_k=(k+1)D)
+        jj = (n + 1) + (m + 1) - (i + 1) - 1
+        if 0 <= jj < N and T.jL[i, n, m] >= 0:
+            lhs = T.h[i] * T.W[i, n, m]
+            rhs = T.h[n] * T.W[n, i, jj]
+            assert lhs == pytest.approx(rhs, rel=1e-12, abs=1e-300)
+            checked += 1
+    assert checked > 1000
+
+
+# ------------------------------------------------------------------ P5: thermal fixed point under LOG
+@pytest.mark.parametrize("cfg,Tchi", [(1, 1.3), (3, 0.7)])
+def test_P5_thermal_fixed_point(oracle, cfg, Tchi):
+    c = kin.config(cfg, N=64 if cfg == 3 else None)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    f = (0.37 * np.exp(-T.E / Tchi))[None, :]
+    g, l, C = oracle.collide(T, f, 0)
+    assert np.abs(C).max() <= 1e-13 * np.abs(g).max()
+    # LINEAR does not have this property: O(Delta^2) residual (P8)
+    g1, l1, C1 = oracle.collide(T, f, 1)
+    assert np.abs(C1).max() > 1e-8 * np.abs(g1).max()
+
+
+# ------------------------------------------------------------------ P6: projection conserves both moments
+def test_P6_projection_and_steps_conserve(oracle):
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    g, l, C = oracle.collide(T, c["f"], 0)
+    Cp, diag = oracle.project(T, c["f"], C)
+    sc = (T.h * np.abs(C[0])).sum()
+    assert abs((T.h * Cp[0]).sum()) <= 1e-14 * sc
+    assert abs((T.h * T.E * Cp[0]).sum()) <= 1e-14 * (T.h * T.E * np.abs(C[0])).sum()
+    # diag = eps_N, eps_E (C.1) and R_N, R_E (C.9), recomputed here from their definitions
+    assert diag[0, 0] == pytest.approx((T.h * C[0]).sum() / sc, rel=1e-10)
+    assert diag[0, 2] == pytest.approx((T.h * np.abs(Cp[0] - C[0])).sum() / sc, rel=1e-10)
+    # 50 RK4 steps: number and energy drift <= 1e-12 relative per step
+    nu_max = (l[0] / c["f"][0]).max()
+    S = 50
+    tau = np.arange(S + 1) * (0.2 / nu_max)
+    f1 = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.RK4, tau=tau)
+    n0, n1 = oracle.moments(T, c["f"])[0], oracle.moments(T, f1)[0]
+    assert abs(n1[0] / n0[0] - 1) <= 1e-12 * S and abs(n1[1] / n0[1] - 1) <= 1e-12 * S
+    assert np.abs(f1 - c["f"]).max() > 1e-3 * c["f"].max()          # it did move
+
+
+def test_P6_relaxes_towards_maxwell_boltzmann(oracle):
+    """Config 1 run: Euler steps with the projected LOG operator approach z*exp(-E/T) (H-theorem)."""
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    g, l, C = oracle.collide(T, c["f"], 0)
+    nu_max = (l[0] / c["f"][0]).max()
+
+    def dist_to_mb(f):
+        # least-squares fit of ln f = ln z - E/T on the populated bins
+        msk = f > 1e-8 * f.max()
+        A = np.stack([np.ones(msk.sum()), -T.E[msk]], axis=1)
+        coef, res, *_ = np.linalg.lstsq(A, np.log(f[msk]), rcond=None)
+        return float(np.sqrt(((A @ coef - np.log(f[msk])) ** 2).mean()))
+
+    d0 = dist_to_mb(c["f"][0])
+    f = c["f"]
+    for S in (200, 2000):
+        tau = np.arange(S + 1) * (0.2 / nu_max)
+        f = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.EULER, tau=tau)
+        d = dist_to_mb(f[0])
+        assert d < d0
+        d0 = d
+    assert (f > 0).all()
+
+
+# ------------------------------------------------------------------ P7: normalisation against eq. 2.4 (closed form)
+def test_P7_loss_frequency_closed_form(oracle):
+    """m=0, contact, f = z exp(-p/T): eq. 2.4 with the massless two-body phase space 1/(8 pi) gives
+    nu(p) = loss/f = |M|^2 z T^2 / (64 pi^3 p), and gain = nu f.  The discrete operator converges to it."""
+    z, Tt, M2 = 0.8, 1.0, 2.5
+    errs = []
+    for N in (100, 200):
+        D = 30.0 / N
+        p = D * np.arange(1, N + 1)
+        T = oracle.Tables(p, np.full(N, D), 0.0, 1.0, M2, 0.0)
+        f = (z * np.exp(-p / Tt))[None, :]
+        g, l, C = oracle.collide(T, f, 0)
+        nu = l[0] / f[0]
+        exact = M2 * z * Tt ** 2 / (64 * math.pi ** 3 * p)
+        win = (p > 0.5) & (p < 8.0)
+        errs.append(np.abs(nu[win] / exact[win] - 1).max())
+        assert np.abs(g[0][win] / (exact * f[0])[win] - 1).max() < 0.09
+    assert errs[0] < 0.08 and errs[1] < 0.025 and errs[1] < 0.4 * errs[0]
+
+
+# ------------------------------------------------------------------ P8: residuals shrink with N
+def test_P8_raw_residuals_decrease_with_N(oracle):
+    res = []
+    for N in (32, 64, 128):
+        p = kin.log_grid(N, 1e-3, 1e2)
+        dp = kin.trapezoid_widths(p)
+        T = oracle.Tables(p, dp, 1.0)
+        f = kin.two_bump_eq51(p)[None, :]
+        g, l, C = oracle.collide(T, f, 0)
+        Cp, diag = oracle.project(T, f, C)
+        res.append(np.abs(diag[0]))
+    assert res[2][0] < res[0][0] and res[2][1] < res[0][1]        # eps_N, eps_E
+    assert res[2][2] < res[0][2] and res[2][3] < res[0][3]        # R_N, R_E (Fig. 9)
+
+
+# ------------------------------------------------------------------ P9: brute-force angular quadrature (B.5-B.12) = B.17
+@pytest.mark.parametrize("m_med", [0.0, 0.5])
+def test_P9_closed_form_equals_mu_quadrature(oracle, m_med):
+    mu, w = np.polynomial.legendre.leggauss(6000)
+    rng = np.random.default_rng(11)
+    done = 0
+    while done < 12:
+        pi, pn, pm = rng.uniform(0.1, 3.0, size=3)
+        Fc = oracle.F_closed(pi, pn, pm, 1.0, 1.7, m_med)
+        if Fc <= 0:
+            continue
+        Fq = oracle.F_quadrature(pi, pn, pm, 1.0, 1.7, m_med, mu, w)
+        assert Fq == pytest.approx(Fc, rel=2e-3)
+        done += 1
+
+
+def test_P9_mediator_J_against_numerical_integration(oracle):
+    """D5: F_closed(m_med)/F_closed(contact) = m_med^4 * int dQ/(Q^2+c^2)^2 / (Q+ - Q-), checked by adaptive quadrature (scipy QUADPACK)."""
+    rng = np.random.default_rng(12)
+    m = 1.0
+    done = 0
+    while done < 20:
+        pi, pn, pm = rng.uniform(0.05, 6.0, size=3)
+        m_med = float(rng.choice([0.05, 0.5, 3.0]))
+        Fc0 = oracle.F_closed(pi, pn, pm, m, 1.0, 0.0)
+        if Fc0 <= 0:
+            continue
+        Ei, En, Em = (math.sqrt(x * x + m * m) for x in (pi, pn, pm))
+        pj = math.sqrt((En + Em - Ei) ** 2 - m * m)
+        Qm, Qp = max(abs(pi - pn), abs(pm - pj)), min(pi + pn, pm + pj)
+        dE2 = (Ei - En) ** 2
+        integrand = lambda Q: 1.0 / (1.0 + (Q * Q - dE2) / m_med ** 2) ** 2
+        simpson, _ = quad(integrand, Qm, Qp, epsabs=0, epsrel=1e-13, limit=400)
+        ratio = oracle.F_closed(pi, pn, pm, m, 1.0, m_med) / Fc0
+        assert ratio == pytest.approx(simpson / (Qp - Qm), rel=1e-8)
+        done += 1
+
+
+# ------------------------------------------------------------------ P10: the paper's printed projection sizes (soft)
+def test_P10_paper_projection_correction_trend(oracle):
+    rows = [ln.split() for ln in open(os.path.join(HERE, "golden", "paper_projection_correction.txt"))
+            if ln.strip() and not ln.startswith("#")]
+    paper = {int(r[0]): float(r[1]) for r in rows}
+    got = {}
+    for N in paper:
+        p = kin.log_grid(N, 1e-3, 1e2)
+        T = oracle.Tables(p, kin.trapezoid_widths(p), 1.0)
+        f = kin.two_bump_eq51(p)[None, :]
+        g, l, C = oracle.collide(T, f, 0)
+        Cp, _ = oracle.project(T, f, C)
+        got[N] = 100 * np.abs(Cp - C).max() / np.abs(C).max()
+    # soft: same order of magnitude as PAPER.md:468 (Bose factors and eps_supp differ) and ~N^-2 trend
+    for N, v in paper.items():
+        assert v / 10 < got[N] < v * 10, (N, got[N], v)
+    assert got[256] < got[96] / 3
+
+
+# ------------------------------------------------------------------ moments: closed form (B.2)
+def test_moments_closed_form(oracle):
+    """n = g/(2 pi^2) sum h f: for f=exp(-p) on a fine uniform grid -> g/(2 pi^2) * 2 (int p^2 e^-p = 2);
+    <p> = 3, <p^2> = 12 ; rho(m=0) = g/(2 pi^2) * 6."""
+    N = 4000
+    p = np.linspace(0.005, 40.0, N)
+    dp = kin.trapezoid_widths(p)
+    T = oracle.Tables.__new__(oracle.Tables)
+    T.N, T.p, T.g_chi = N, p, 2.0
+    T.E, T.K, T.h = oracle.kinematics(p, dp, 0.0)
+    mo = oracle.moments(T, np.exp(-p)[None, :])[0]
+    fac = 2.0 / (2 * math.pi ** 2)
+    assert mo[0] == pytest.approx(fac * 2.0, rel=1e-4)
+    assert mo[1] == pytest.approx(fac * 6.0, rel=1e-4)
+    assert mo[2] == pytest.approx(3.0, rel=1e-4)
+    assert mo[3] == pytest.approx(12.0, rel=1e-4)
+
+
+# ------------------------------------------------------------------ integrator (O12): closed forms and convergence order
+def test_evolve_sources_only_closed_form(oracle):
+    """kappa = 0 switches the collision term off: f(S) = f(0) + sum_k amp[:,k] dtau_k G exactly, any method."""
+    c = kin.config(5, N=24, B=3)
+    sch = kin.config5_schedule(c["p"], c["dp"], B=3, S=40)
+    expect = (sch["amp"] * np.diff(sch["tau"])[None, :]).sum(axis=1) @ sch["G"]
+    for method in (oracle.EULER, oracle.HEUN, oracle.RK4):
+        f = oracle.evolve(c["p"], c["dp"], c["f"], method=method, tau=sch["tau"], rate=sch["rate"],
+                          mass=None, kappa=np.zeros(3), G=sch["G"], amp=sch["amp"])
+        assert np.allclose(f, expect[None, :], rtol=1e-13, atol=0)
+
+
+def test_evolve_convergence_order_and_rate_scaling(oracle):
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    g, l, C = oracle.collide(T, c["f"], 0)
+    t_end = 8.0 / (l[0] / c["f"][0]).max()
+
+    def run(method, S, **kw):
+        return oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=method, tau=np.linspace(0, t_end, S + 1), **kw)
+
+    ref = run(oracle.RK4, 256)
+    errs = {}
+    for method, order in ((oracle.EULER, 1), (oracle.HEUN, 2), (oracle.RK4, 4)):
+        e1 = np.abs(run(method, 8) - ref).max()
+        e2 = np.abs(run(method, 16) - ref).max()
+        errs[method] = (e1, e2)
+        assert e1 / e2 > 0.6 * 2 ** order, (method, e1, e2)
+    # a constant rate R and coupling kappa multiply the operator: (R=2, kappa=3, t) == (R=1, kappa=1, 6t)
+    S = 16
+    a = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.RK4, tau=np.linspace(0, t_end / 6, S + 1),
+                      rate=np.full(2 * S + 1, 2.0), kappa=np.array([3.0]))
+    b = run(oracle.RK4, S)
+    assert np.allclose(a, b, rtol=1e-12, atol=1e-300)
+    # a mass schedule that is constant equals the static run (per-stage rebuild path)
+    d = oracle.evolve(c["p"], c["dp"], c["f"], m=0.3, method=oracle.HEUN, tau=np.linspace(0, t_end, 5),
+                      mass=np.full(9, c["m"]))
+    e = run(oracle.HEUN, 4)
+    assert np.array_equal(d, e)
