@@ -46,7 +46,7 @@ def _load():
         _lib.okx_collide.argtypes = [C.c_int, C.c_int, _dp, _dp, _ip, _dp, C.c_int, C.c_double,
                                      _dp, _dp, _dp]
         _lib.okx_collide.restype = None
-        _lib.okx_project.argtypes = [C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp]
+        _lib.okx_project.argtypes = [C.c_int, _dp, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp]
         _lib.okx_project.restype = None
         _lib.okx_moments.argtypes = [C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp]
         _lib.okx_moments.restype = None
@@ -115,7 +115,7 @@ def project(T: Tables, f, Craw, eps_supp=1e-12):
     out, diag = np.empty((B, n)), np.empty((B, 4))
     for b in range(B):
         fb, cb, ob, db = f[b], Craw[b], out[b], diag[b]
-        _load().okx_project(n, _d(fb), _d(cb), _d(T.h), _d(T.E), float(eps_supp), _d(ob), _d(db))
+        _load().okx_project(n, _d(fb), _d(cb), _d(T.h), _d(T.E), _d(T.K), float(eps_supp), _d(ob), _d(db))
     return out, diag
 
 

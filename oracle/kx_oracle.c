@@ -163,45 +163,54 @@ void okx_collide(int N, int B, const double *f, const double *W, const int32_t *
 
 /* ---- O10: two-moment projection, App. C eq. C.2-C.8, support mask C.4 with
  * f_max = max_i |f_i|; degenerate cases per reading D9.  diag (may be NULL) receives
- * eps_N, eps_E (C.1, raw), R_N, R_E (C.9).  One distribution. */
+ * eps_N, eps_E (C.1, raw), R_N, R_E (C.9).  One distribution.
+ *
+ * Reading D3 applied to App. C: the correction xi_i (alpha + beta E_i) lives in span{1, E_i} =
+ * span{1, K_i} (E_i = m + K_i), and the two conditions (C.5) "sum h C = 0, sum h E C = 0" are
+ * equivalent to "sum h C = 0, sum h K C = 0".  The 2x2 system (C.7) is therefore solved in the
+ * basis {1, K_i}: alpha' + beta K_i with alpha' = alpha + beta m.  Same projection, but the
+ * determinant A00*A11 - A01^2 no longer cancels catastrophically when K << m (with the literal
+ * E-basis even long double loses the result at m/T = 1e3: 1e-10 of max gain, measured against
+ * exact rational arithmetic; pin tests/test_oracle_pins.py::test_P6_projection_exact_rational). */
 void okx_project(int N, const double *f, const double *Craw, const double *h, const double *E,
-                 double eps_supp, double *Cproj, double *diag)
+                 const double *K, double eps_supp, double *Cproj, double *diag)
 {
-    long double R0 = 0, R1 = 0, S0 = 0, S1 = 0;
+    long double R0 = 0, R1 = 0, RK = 0, S0 = 0, S1 = 0;
     double fmax = 0.0;
     for (int i = 0; i < N; ++i) {
-        R0 += (long double)h[i] * Craw[i];
+        R0 += (long double)h[i] * Craw[i];                    /* C.2 */
         R1 += (long double)h[i] * E[i] * Craw[i];
+        RK += (long double)h[i] * K[i] * Craw[i];             /* = R1 - m R0 */
         S0 += (long double)h[i] * fabs(Craw[i]);
         S1 += (long double)h[i] * E[i] * fabs(Craw[i]);
         if (fabs(f[i]) > fmax) fmax = fabs(f[i]);
     }
-    long double A00 = 0, A01 = 0, A11 = 0;
+    long double A00 = 0, A0K = 0, AKK = 0;
     double *xi = malloc(sizeof(double) * N);
     for (int i = 0; i < N; ++i) {
-        double r = (fmax > 0.0) ? fabs(f[i]) / fmax : 0.0;
+        double r = (fmax > 0.0) ? fabs(f[i]) / fmax : 0.0;    /* C.4 */
         xi[i] = (r > eps_supp) ? r : 0.0;
-        A00 += (long double)h[i] * xi[i];
-        A01 += (long double)h[i] * E[i] * xi[i];
-        A11 += (long double)h[i] * E[i] * E[i] * xi[i];
+        A00 += (long double)h[i] * xi[i];                     /* C.6 in the {1,K} basis */
+        A0K += (long double)h[i] * K[i] * xi[i];
+        AKK += (long double)h[i] * K[i] * K[i] * xi[i];
     }
-    long double alpha = 0, beta = 0;
+    long double alpha = 0, beta = 0;                          /* correction = xi (alpha + beta K) */
     if (fmax > 0.0 && A00 > 0.0L) {
-        long double det = A00 * A11 - A01 * A01;
-        if (det <= 1e-14L * A00 * A11) { alpha = R0 / A00; beta = 0; }
-        else { alpha = (R0 * A11 - R1 * A01) / det; beta = (R1 * A00 - R0 * A01) / det; }
+        long double det = A00 * AKK - A0K * A0K;              /* C.8 */
+        if (det <= 1e-14L * A00 * AKK) { alpha = R0 / A00; beta = 0; }   /* D9: number only */
+        else { alpha = (R0 * AKK - RK * A0K) / det; beta = (RK * A00 - R0 * A0K) / det; }
     }
     long double D0 = 0, D1 = 0;
     for (int i = 0; i < N; ++i) {
-        double corr = (double)((long double)xi[i] * (alpha + beta * (long double)E[i]));
-        Cproj[i] = Craw[i] - corr;
+        double corr = (double)((long double)xi[i] * (alpha + beta * (long double)K[i]));
+        Cproj[i] = Craw[i] - corr;                            /* C.3 */
         D0 += (long double)h[i] * fabs(corr);
         D1 += (long double)h[i] * E[i] * fabs(corr);
     }
     if (diag) {
-        diag[0] = (S0 > 0) ? (double)(R0 / S0) : 0.0;
+        diag[0] = (S0 > 0) ? (double)(R0 / S0) : 0.0;         /* C.1 */
         diag[1] = (S1 > 0) ? (double)(R1 / S1) : 0.0;
-        diag[2] = (S0 > 0) ? (double)(D0 / S0) : 0.0;
+        diag[2] = (S0 > 0) ? (double)(D0 / S0) : 0.0;         /* C.9 */
         diag[3] = (S1 > 0) ? (double)(D1 / S1) : 0.0;
     }
     free(xi);
@@ -248,8 +257,8 @@ static void okx_rhs(okx_ctx *c, const double *f, double mass, int use_mass, doub
     }
     double *Craw = malloc(sizeof(double) * N), *Cp = malloc(sizeof(double) * N);
     okx_collide(N, 1, f, c->W, c->jL, c->wR, c->interp, c->f_floor, NULL, NULL, Craw);
-    if (project) okx_project(N, f, Craw, c->h, c->E, c->eps_supp, Cp, diag4);
-    else { memcpy(Cp, Craw, sizeof(double) * N); if (diag4) okx_project(N, f, Craw, c->h, c->E, c->eps_supp, Craw, diag4); }
+    if (project) okx_project(N, f, Craw, c->h, c->E, c->K, c->eps_supp, Cp, diag4);
+    else { memcpy(Cp, Craw, sizeof(double) * N); if (diag4) okx_project(N, f, Craw, c->h, c->E, c->K, c->eps_supp, Craw, diag4); }
     for (int i = 0; i < N; ++i) {
         double s = 0.0;
         for (int q = 0; q < nsrc; ++q) s += ampk[q] * G[(size_t)q * N + i];

@@ -148,6 +148,35 @@ def test_P6_projection_and_steps_conserve(oracle):
     assert np.abs(f1 - c["f"]).max() > 1e-3 * c["f"].max()          # it did move
 
 
+@pytest.mark.parametrize("m", [1.0, 30.0, 1000.0])
+def test_P6_projection_exact_rational(oracle, m):
+    """App. C solved LITERALLY (eq. C.2-C.8, basis {1, E_i}) in exact rational arithmetic on the same doubles.
+    The oracle solves the same system in the basis {1, K_i} (reading D3); the projections must coincide, also at
+    m/T = 1e3 where the E-basis determinant cancels to 4e-10 of its terms.  The energies of the exact solve are
+    E_i = m + K_i taken exactly (the stable kinetic energies of O1 define the grid; the rounded double
+    sqrt(p^2+m^2) differs from m + K_i by up to 1e-10 K_i at this mass, which alone moves the result by 3e-13)."""
+    from fractions import Fraction as Fr
+    N = 48
+    p = kin.log_grid(N, 1e-3, 100.0)
+    T = oracle.Tables(p, kin.trapezoid_widths(p), m)
+    f = kin.bimodal(p, (3.0, 8.0), (1.0, 2.0))[None, :]
+    g, l, C = oracle.collide(T, f, 0)
+    Cp, _ = oracle.project(T, f, C, eps_supp=1e-12)
+    h, E, c = [Fr(x) for x in T.h], [Fr(m) + Fr(x) for x in T.K], [Fr(x) for x in C[0]]
+    fmax = float(np.abs(f[0]).max())
+    xi = [Fr(abs(float(x)) / fmax) if abs(float(x)) / fmax > 1e-12 else Fr(0) for x in f[0]]     # C.4
+    R0 = sum(a * b for a, b in zip(h, c))                                                           # C.2
+    R1 = sum(a * e * b for a, e, b in zip(h, E, c))
+    A00 = sum(a * x for a, x in zip(h, xi))                                                         # C.6
+    A01 = sum(a * e * x for a, e, x in zip(h, E, xi))
+    A11 = sum(a * e * e * x for a, e, x in zip(h, E, xi))
+    det = A00 * A11 - A01 * A01                                                                     # C.8
+    al, be = (R0 * A11 - R1 * A01) / det, (R1 * A00 - R0 * A01) / det
+    exact = np.array([float(ci - x * (al + be * e)) for ci, x, e in zip(c, xi, E)])                 # C.3
+    assert np.abs(Cp[0] - exact).max() <= 1e-15 * np.abs(g).max()
+    assert np.abs(exact - C[0]).max() > 1e-4 * np.abs(g).max()          # the correction is not trivially zero
+
+
 def test_P6_relaxes_towards_maxwell_boltzmann(oracle):
     """Config 1 run: Euler steps with the projected LOG operator approach z*exp(-E/T) (H-theorem)."""
     c = kin.config(1)
