@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py -- C[f] evaluations per second on BASELINE config 3 (N=256 log grid, B=64 members, mediator |M|^2, fp64).
+
+A step is one pass of the whole hot path over one batch: kx_collide on f[B,N] (prep -> gain/loss contraction ->
+reduction + raw operator).  `value` = all ranks' B*K evaluations / max-over-ranks device time, inputs resident in
+HBM; `e2e` = the same through kx_collide_host (pinned host f in, C out, copies inside the timed region).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--mode log|linear] [--project]
+    torchrun --nproc-per-node N ... bench.py --gpus N ...
+
+N > 1: the path partitions over independent distributions, so every rank evaluates its own batch of B members
+(weak scaling, no data-path collective).  --impl reference times the CPU oracle as it stands (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import kx_inputs as kin  # noqa: E402
+
+METRIC = "C[f] evals/s (fp64, N=256, B=64)"
+UNIT = "C[f]/s"
+WORKLOAD = "cfg3: N=256 log p/T in [1e-3,50], B=64 seeded bimodal f, |M|^2 ~ 1/(1+q^2/m_med^2)^2, m_med=0.5"
+# FP64-pipe instructions per (entry, member) of the LOG/table kernel, counted from the source and checked in SASS
+# (DESIGN.md "Kernels"): gain DMUL+DFMA, argument DFMA, exp2 3 DADD + 3 DFMA + DMUL + DFMA, loss DFMA.
+FP64_INST = {"log": 12, "linear": 4}
+FP64_FLOP = {"log": 19, "linear": 7}      # DFMA = 2 flop, DADD/DMUL = 1
+SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM (37 TFLOP/s nominal at 1.965 GHz)
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        return json.load(open(path)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 2 + k and r[2 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _inputs(rank: int, B: int):
+    c = kin.config(3, B=B)
+    if rank:   # every rank its own members: seeds 3000 + rank*B + b
+        c["f"] = np.stack([kin._random_bimodal(c["p"], 3000 + rank * B + b) for b in range(B)])
+    return c
+
+
+def cpu_oracle(c, members: int, steps: int = 1, warmup: int = 0):
+    """The oracle as it stands, timed on the host cores on a bounded sample: dense tables built once (timed
+    separately), then `members` members of the batch evaluated per step (evaluate phase O8-O9)."""
+    import oracle
+    t0 = time.perf_counter()
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    t_build = time.perf_counter() - t0
+    fs = np.ascontiguousarray(c["f"][:members])
+    for _ in range(warmup):
+        oracle.collide(T, fs, oracle.LOG)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.collide(T, fs, oracle.LOG)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    return dict(value=members / dt, unit=UNIT, cores=os.cpu_count(), kind="oracle",
+                sample=f"{members} of {len(c['f'])} members of cfg3 per step, evaluate phase (O8-O9) over the dense N^3 tables, "
+                       f"{steps} step(s); table build (O1-O7) {t_build:.1f} s not included",
+                ms_per_step=dt * 1e3, build_s=t_build)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    c = _inputs(0, 64)
+    members = 16
+    cb = cpu_oracle(c, members, steps=args.steps, warmup=min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": cb["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": cb["sample"]},
+            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="kx", choices=["kx", "reference"])
+    ap.add_argument("--mode", default="log", choices=["log", "linear"])
+    ap.add_argument("--project", action="store_true", help="time the projected operator (App. C) instead of the raw one")
+    ap.add_argument("--batch", type=int, default=64)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2607_00755_b200 as kx
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libkx has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    B, K, Wm = args.batch, args.steps, max(args.warmup, 3)
+    c = _inputs(rank, B)
+    h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], device=local,
+                  interp=kx.INTERP_LOG if args.mode == "log" else kx.INTERP_LINEAR)
+    info = h.info()
+    dev = torch.device("cuda", local)
+    f = torch.tensor(c["f"], dtype=torch.float64, device=dev)
+    C = torch.empty_like(f)
+    flags = kx.PROJECT if args.project else 0
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)    # 256 MiB > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        h.collide(f, flags=flags, out=C)
+
+    for _ in range(Wm):
+        flush.zero_()
+        step()
+    barrier()
+
+    # ---- timed region: K steps, L2 flushed before each, device time from CUDA events on the launching stream
+    sampler = ClockSampler(local)
+    sampler.start()
+    h.profile(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    barrier()
+    for k in range(K):
+        flush.zero_()
+        ev[k][0].record(stream)
+        step()
+        ev[k][1].record(stream)
+    barrier()
+    t_cold = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    kern_ms, kern_n = h.profile_read()
+    h.profile(False)
+
+    # ---- same K steps back to back (tensor L2-resident, as inside an integrator)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    a.record(stream)
+    for k in range(K):
+        step()
+    b.record(stream)
+    barrier()
+    t_warm = a.elapsed_time(b) * 1e-3
+
+    # ---- end to end through host buffers
+    fh = torch.tensor(c["f"], dtype=torch.float64).pin_memory()
+    Ch = torch.empty_like(fh).pin_memory()
+    for _ in range(3):
+        h.collide_host(fh, Ch, flags=flags)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(K):
+        h.collide_host(fh, Ch, flags=flags)
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    clocks = sampler.stop()
+
+    times = torch.tensor([t_cold, t_warm, t_e2e, kern_ms * 1e-3], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    t_cold, t_warm, t_e2e, t_kern = [float(x) for x in times.cpu()]
+    same = bool(torch.isfinite(C).all())
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks, peak_src = _peaks()
+    sm_max_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    nnz = info["nnz"]
+    kern_s = t_kern / max(kern_n, 1)
+    if args.mode == "log":
+        # plain FP64 ALU bound: one exp per (entry, member); peak = SMs x 64 FMA lanes x 2 flop x max SM clock
+        peak = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_hz / 1e12
+        ach = nnz * B * FP64_FLOP["log"] / kern_s / 1e12
+        roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": None, "kernel": "k_contract<8,LOG_TAB>", "kernel_ms": kern_s * 1e3,
+                "peak_source": f"148 SMs x 64 FP64 FMA lanes x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src})",
+                "fp64_inst_per_entry_member": FP64_INST["log"], "flop_per_entry_member": FP64_FLOP["log"],
+                "pipe_frac": nnz * B * FP64_INST["log"] / kern_s / (SM_COUNT * FP64_LANES_PER_SM * sm_max_hz)}
+    else:
+        peak = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_hz / 1e12
+        ach = nnz * B * FP64_FLOP["linear"] / kern_s / 1e12
+        roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": None, "kernel": "k_contract<8,LINEAR>", "kernel_ms": kern_s * 1e3,
+                "peak_source": f"148 SMs x 64 FP64 FMA lanes x 2 x {sm_max_hz / 1e6:.0f} MHz ({peak_src})"}
+    line = {
+        "metric": METRIC, "value": world * B * K / t_cold, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": t_cold / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "N": 256, "B_per_gpu": B, "mode": args.mode, "projected": bool(args.project),
+                   "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "l2": "flushed before every timed step (256 MiB write)",
+                   "parallelism": f"independent batches x{world}" if world > 1 else "single GPU"},
+        "value_l2_warm": world * B * K / t_warm, "ms_per_step_l2_warm": t_warm / K * 1e3,
+        "calls_per_s": world * K / t_cold,
+        "e2e": {"value": world * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": B * 256 * 8,
+                "d2h_bytes_per_step": B * 256 * 8, "ms_per_step": t_e2e / K * 1e3},
+        "gpu_launches": 3 * K, "clocks": clocks, "roofline": roof, "finite": same,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        cb = cpu_oracle(c, members=B, steps=3, warmup=1)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line), flush=True)
+    h.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,168 @@
+/*
+ * kx.h -- C ABI of libkx: the discretized 2->2 elastic self-collision operator C[f] of KineticXGPU
+ * (arxiv/paper_2607_00755) as hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * What the library computes (citations are PAPER.md line numbers; readings D1-D13 are in DESIGN.md):
+ *   kinematics        E_i = sqrt(p_i^2+m^2), K_i = E_i-m, h_i = p_i^2 dp_i          eq. B.1
+ *   index map         E_j~ = E_n+E_m-E_i, bracket j_L and weight omega_R            eq. 4.4, B.19
+ *   kernel tensor     W_inm = dp_n dp_m F_inm / (2 E_i g_chi)                        eq. 4.7, B.15-B.17
+ *   operator          C_i = sum_{n,m} W_inm (f_n f_m - f_i f_j~)                     eq. 4.6 with eq. 2.6
+ *   interpolation     f_j~ = exp(w_L ln f_L + w_R ln f_R)  (LOG)  or  w_L f_L + w_R f_R (LINEAR)   eq. B.20
+ *   projection        C^proj = C^raw - xi_i (alpha + beta E_i)                       App. C, eq. C.2-C.8
+ *   moments           n = g/(2 pi^2) sum h f, rho = g/(2 pi^2) sum h E f             eq. B.2
+ *   time stepping     df/dtau = kappa_b R(tau) C^proj[f; m(tau)] + sum_s amp_s G_s   eq. 4.9
+ *
+ * Conventions
+ *   - Every function returns kx_status_t (KX_OK = 0).  No exceptions, no abort(), no global state.
+ *     kx_last_error(h) returns a handle-owned, NUL-terminated description of the last failure.
+ *   - Pointers are marked HOST or DEVICE.  DEVICE pointers are caller-owned allocations on the
+ *     handle's device (e.g. torch.Tensor.data_ptr()), 16-byte aligned, row-major [B,N] fp64.
+ *     HOST arrays are read during the call and may be freed afterwards.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  kx_collide*,
+ *     kx_moments and kx_set_mass only enqueue work on it and return without synchronising, except
+ *     that the first call with a larger batch B than seen before grows the handle's workspace
+ *     (cudaMalloc, implicit sync).  kx_build, kx_evolve, kx_collide_host and kx_tensor_export
+ *     synchronise the stream before returning.
+ *   - The handle owns the kernel tensor and all workspaces.  One host thread at a time per handle.
+ *   - There is no CPU fallback: every entry point fails with KX_ERR_CUDA when no sm_100 device
+ *     is usable.
+ */
+#ifndef KX_H_
+#define KX_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct kx_handle_s* kx_handle_t;
+
+typedef enum {
+    KX_OK = 0,
+    KX_ERR_INVALID_ARG = 1,   /* null pointer, N<4 or N>1024, non-monotone grid, dp<=0, B<1, misaligned pointer */
+    KX_ERR_ALLOC = 2,         /* host or device allocation failed */
+    KX_ERR_CUDA = 3,          /* CUDA runtime error (message in kx_last_error) */
+    KX_ERR_UNSUPPORTED = 4,   /* option not implemented (fp32 mode) */
+    KX_ERR_NONFINITE = 5      /* kx_evolve produced a NaN/Inf in f */
+} kx_status_t;
+
+/* interpolation of f at the off-grid fourth momentum (reading D7) */
+#define KX_INTERP_LOG     0   /* eq. B.20 at eta=0: f_j~ = exp(w_L y_L + w_R y_R), y = ln max(f, f_floor) (default) */
+#define KX_INTERP_LINEAR  1   /* f_j~ = w_L f_L + w_R f_R (operator exactly bilinear) */
+/* storage of the kernel tensor */
+#define KX_STORE_SYM_ROWS 0   /* symmetry-reduced (n<=m, W_inm+W_imn), structural zeros dropped, row-compressed */
+/* precision */
+#define KX_FP64 0
+#define KX_FP32 1             /* not implemented: KX_ERR_UNSUPPORTED */
+/* exp used by the LOG loss term */
+#define KX_EXP_TABLE 0        /* 128-entry table + degree-4 polynomial, <= 1 ulp-level error (default) */
+#define KX_EXP_LIBM  1        /* CUDA math library exp2() */
+/* flags of kx_collide / kx_evolve */
+#define KX_PROJECT 1u         /* apply the two-moment projection of App. C */
+#define KX_DIAG    2u         /* kx_evolve: fill ctl->diag */
+/* integrators of kx_evolve (fixed step) */
+#define KX_EULER 0
+#define KX_HEUN  1
+#define KX_RK4   2
+
+/* Momentum grid (HOST): p ascending and > 0, dp > 0 (bin widths / quadrature weights, reading D1). eq. 4.5 */
+typedef struct { int32_t n; const double* p; const double* dp; } kx_grid_t;
+/* Species: mass m >= 0 and internal degrees of freedom g_chi > 0 (eq. 4.2) */
+typedef struct { double m; double g_chi; } kx_species_t;
+/* |M|^2 = M2_0 (m_med <= 0: contact, eq. B.17) or M2_0 / (1 + (-t)/m_med^2)^2, t = (p_i-p_n)^2 (reading D5) */
+typedef struct { double M2_0; double m_med; } kx_msq_t;
+/* Options; pass NULL for the defaults {LOG, SYM_ROWS, FP64, EXP_TABLE, 1e-300, 1e-12} */
+typedef struct {
+    int32_t interp;      /* KX_INTERP_*  */
+    int32_t storage;     /* KX_STORE_*   */
+    int32_t precision;   /* KX_FP64      */
+    int32_t exp_impl;    /* KX_EXP_*     */
+    double  f_floor;     /* y = ln max(f, f_floor), reading D8; must be >= 1e-300 and > 0 */
+    double  eps_supp;    /* support threshold of eq. C.4, reading D9 */
+} kx_opts_t;
+
+/* a1-a3: build kinematics, the energy-conserving index map and the kernel tensor ON THE DEVICE.
+ * `device` is the CUDA ordinal.  Synchronises `stream`.  *out is NULL on failure. */
+kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq_t* msq,
+                     const kx_opts_t* opts, int device, void* stream, kx_handle_t* out);
+
+/* Re-run a1-a3 for a new kinematic mass (p_i = q_i/a changes with time; reading D12).
+ * Asynchronous: the new number of non-zeros stays on the device (kx_info synchronises to read it). */
+kx_status_t kx_set_mass(kx_handle_t h, double m, void* stream);
+
+/* a4-a7: C[b,i] = sum_{n,m} W_inm (f_n f_m - f_i f_j~) for B distributions (eq. 4.6).
+ * f, C: DEVICE [B,N].  flags: 0 = raw operator, KX_PROJECT = App. C projection applied.
+ * In place (C == f) is not allowed. */
+kx_status_t kx_collide(kx_handle_t h, const double* f, double* C, int32_t B, uint32_t flags, void* stream);
+
+/* a4, a5 separately: gain[b,i] = sum W f_n f_m, loss[b,i] = f_i sum W f_j~ (DEVICE [B,N]; either may be NULL). */
+kx_status_t kx_collide_parts(kx_handle_t h, const double* f, double* gain, double* loss, int32_t B, void* stream);
+
+/* General form: any of C, gain, loss, diag may be NULL.  diag: DEVICE [B,4] = eps_N, eps_E (eq. C.1,
+ * PAPER.md:415, of the raw operator) and R_N, R_E (eq. C.9; zero unless KX_PROJECT). */
+kx_status_t kx_collide_ex(kx_handle_t h, const double* f, double* C, double* gain, double* loss,
+                          double* diag, int32_t B, uint32_t flags, void* stream);
+
+/* Same operator with HOST buffers f[B,N] -> C[B,N]: host->device copy, kx_collide, device->host copy
+ * on `stream`, then synchronises.  Pinned host memory makes the copies asynchronous. */
+kx_status_t kx_collide_host(kx_handle_t h, const double* f_host, double* C_host, int32_t B,
+                            uint32_t flags, void* stream);
+
+/* a9: moments of eq. B.2.  f: DEVICE [B,N]; n, rho, p1 = <p>, p2 = <p^2>: DEVICE [B], any may be NULL. */
+kx_status_t kx_moments(kx_handle_t h, const double* f, int32_t B,
+                       double* n, double* rho, double* p1, double* p2, void* stream);
+
+/* Source terms of eq. 4.1/4.9: sum_s amp[s,k] G[s,i] during step k (constant over the step's stages, D11). */
+typedef struct {
+    int32_t nsrc;          /* 0..8 */
+    const double* G;       /* DEVICE [nsrc,N] source shapes */
+    const double* amp;     /* HOST [nsrc,S] rate of source s during step k, per unit tau */
+} kx_source_t;
+
+typedef struct {
+    int32_t method;        /* KX_EULER | KX_HEUN | KX_RK4 */
+    int32_t S;             /* number of steps */
+    const double* tau;     /* HOST [S+1] nodes of the integration variable (t, or u = ln a, eq. 4.9) */
+    const double* rate;    /* HOST [2S+1] multiplier R at nodes and midpoints (1/H, eq. 4.9); NULL => 1 */
+    const double* mass;    /* HOST [2S+1] kinematic mass at nodes and midpoints; NULL => static tensor.
+                              When given, a1-a3 are re-evaluated at every stage (reading D12). */
+    const double* kappa;   /* HOST [B] per-member coupling multiplier; NULL => 1 */
+    uint32_t flags;        /* KX_PROJECT | KX_DIAG */
+    double* diag;          /* DEVICE [S,B,6]: eps_N, eps_E, R_N, R_E of each step's first stage, then
+                              n, rho after the step (with the end-of-step mass); or NULL */
+} kx_evolve_t;
+
+/* a8: S fixed steps of df/dtau = kappa_b R C[f; m] + sources, every stage = contraction + projection +
+ * fused Runge-Kutta update on the device.  f: DEVICE [B,N], in/out.  src may be NULL.
+ * Synchronises; returns KX_ERR_NONFINITE if f left the finite range.  On return with a mass
+ * schedule, the handle's tensor is the one of the last stage evaluated. */
+kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
+                      const kx_evolve_t* ctl, void* stream);
+
+/* Number of stored (i, n<=m) entries, bytes of tensor data one kx_collide streams, grid size.
+ * Synchronises the device.  Any output pointer may be NULL. */
+kx_status_t kx_info(kx_handle_t h, int64_t* nnz, int64_t* tensor_bytes, int32_t* n);
+
+/* Copy the stored tensor to HOST arrays (testing the builder entry by entry): rowptr[N+1]; for entry e of
+ * row i: W[e] = W_inm + W_imn (n<m) or W_inn; omega[e] = omega_R; nmj[e] = n | m<<10 | j_L<<20.
+ * cap = capacity of W/omega/nmj in entries; fails with KX_ERR_INVALID_ARG if cap < nnz. */
+kx_status_t kx_tensor_export(kx_handle_t h, int64_t cap, int64_t* rowptr, double* W, double* omega, uint32_t* nmj);
+
+/* Copy the device kinematics to HOST arrays of length N (any may be NULL): E_i, K_i, h_i. */
+kx_status_t kx_kinematics_export(kx_handle_t h, double* E, double* K, double* hw);
+
+/* Measurement aid (bench.py): while enabled, every launch of the contraction kernel (a4/a5, the dominant kernel)
+ * is bracketed by two CUDA events recorded on the caller's stream.  kx_profile_read synchronises the device,
+ * returns the summed kernel time in milliseconds and the number of launches since the last read, and resets. */
+kx_status_t kx_profile(kx_handle_t h, int32_t enable);
+kx_status_t kx_profile_read(kx_handle_t h, double* contract_ms, int64_t* launches);
+
+const char* kx_last_error(kx_handle_t h);   /* h may be NULL: returns the last build failure */
+void        kx_destroy(kx_handle_t h);
+int32_t     kx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KX_H_ */

@@ -46,6 +46,9 @@ def _load():
         _lib.okx_collide.argtypes = [C.c_int, C.c_int, _dp, _dp, _ip, _dp, C.c_int, C.c_double,
                                      _dp, _dp, _dp]
         _lib.okx_collide.restype = None
+        _lib.okx_collide_rows.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double,
+                                          C.c_double, _dp, C.c_int, _ip, C.c_int, C.c_double, _dp, _dp, _dp]
+        _lib.okx_collide_rows.restype = None
         _lib.okx_project.argtypes = [C.c_int, _dp, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp]
         _lib.okx_project.restype = None
         _lib.okx_moments.argtypes = [C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp]
@@ -105,6 +108,18 @@ def collide(T: Tables, f, interp=LOG, f_floor=1e-300):
     g, l, c = np.empty((B, n)), np.empty((B, n)), np.empty((B, n))
     _load().okx_collide(n, B, _d(f), _d(T.W), T.jL.ctypes.data_as(_ip), _d(T.wR), int(interp),
                         float(f_floor), _d(g), _d(l), _d(c))
+    return g, l, c
+
+
+def collide_rows(p, dp, f, rows, *, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, interp=LOG, f_floor=1e-300):
+    """O2-O9 for the selected rows i only (no stored tables): returns gain, loss, C_raw, each [B, len(rows)]."""
+    p, dp = _c(p), _c(dp)
+    f = _c(np.atleast_2d(f))
+    B, n = f.shape
+    rows = np.ascontiguousarray(rows, dtype=np.int32)
+    g, l, c = np.empty((B, rows.size)), np.empty((B, rows.size)), np.empty((B, rows.size))
+    _load().okx_collide_rows(n, B, _d(p), _d(dp), float(m), float(g_chi), float(M2_0), float(m_med), _d(f),
+                             rows.size, rows.ctypes.data_as(_ip), int(interp), float(f_floor), _d(g), _d(l), _d(c))
     return g, l, c
 
 

@@ -77,49 +77,58 @@ static double okx_J(double Qm, double Qp, double M2_0, double m_med, double Ki, 
     return (double)((long double)M2_0 * mm * mm * val);
 }
 
-/* ---- O2-O7: build W_inm, jL(i,n,m), omega_R(i,n,m) for every ORDERED triple; the fourth loop is the
- * bracket scan over j.  jL = -1 marks a dropped triple (W = 0).  Returns the number of kept triples. */
+/* ---- O2-O7 for ONE ordered triple (i,n,m): W_inm, bracket jL (-1 = dropped) and omega_R; the fourth loop is
+ * the bracket scan over j.  Returns 1 if the triple is kept. */
+static int okx_triple(int N, const double *p, const double *dp, const double *E, const double *K,
+                      double m, double g_chi, double M2_0, double m_med, int i, int n, int mm,
+                      double *W, int32_t *jL, double *wR)
+{
+    const double pi3 = (double)(OKX_PI * OKX_PI * OKX_PI);
+    *W = 0.0; *jL = -1; *wR = 0.0;
+    /* O2: energy conservation, eq. 4.4: E_j = E_n+E_m-E_i  <=>  K~ = K_n+K_m-K_i */
+    double Kt = (K[n] + K[mm]) - K[i];
+    /* D4: snap ties at the domain edge */
+    double tau = 32.0 * 2.220446049250313e-16 * (K[n] + K[mm] + K[i]);
+    if (Kt < K[0] && Kt >= K[0] - tau) Kt = K[0];
+    if (Kt > K[N - 1] && Kt <= K[N - 1] + tau) Kt = K[N - 1];
+    /* O3: keep iff E_j >= m and q_min <= q_j <= q_max <=> K_0 <= K~ <= K_{N-1} */
+    if (!(Kt >= K[0] && Kt <= K[N - 1])) return 0;
+    /* O4 */
+    double pj = sqrt(Kt * (Kt + 2.0 * m));
+    /* O5: eq. B.15-B.16 */
+    double Qm = fmax(fabs(p[i] - p[n]), fabs(p[mm] - pj));
+    double Qp = fmin(p[i] + p[n], p[mm] + pj);
+    double J = okx_J(Qm, Qp, M2_0, m_med, K[i], K[n]);
+    /* O6: eq. 4.7 with F of eq. B.17 */
+    double w = dp[n] * dp[mm] / (2.0 * E[i] * g_chi);
+    w = w * (1.0 / (64.0 * pi3 * p[i]));
+    w = w * (p[n] * p[mm] / (E[n] * E[mm]));
+    w = w * J;
+    /* O7: bracket scan, largest j with K_j <= K~ <= K_{j+1}; eq. B.19 */
+    int jb = -1;
+    for (int j = 0; j <= N - 2; ++j)
+        if (K[j] <= Kt && Kt <= K[j + 1]) jb = j;
+    if (jb < 0) return 0; /* cannot happen after O3 */
+    *W = w;
+    *jL = jb;
+    *wR = (Kt - K[jb]) / (K[jb + 1] - K[jb]);
+    return 1;
+}
+
+/* ---- O2-O7: build W_inm, jL(i,n,m), omega_R(i,n,m) for every ORDERED triple (literal quadruple loop).
+ * jL = -1 marks a dropped triple (W = 0).  Returns the number of kept triples. */
 long okx_build(int N, const double *p, const double *dp, double m, double g_chi,
                double M2_0, double m_med, double *W, int32_t *jL, double *wR)
 {
     double *E = malloc(sizeof(double) * N), *K = malloc(sizeof(double) * N), *h = malloc(sizeof(double) * N);
     okx_kinematics(N, p, dp, m, E, K, h);
-    const double pi3 = (double)(OKX_PI * OKX_PI * OKX_PI);
     long kept = 0;
 #pragma omp parallel for schedule(dynamic) reduction(+ : kept)
     for (int i = 0; i < N; ++i)
         for (int n = 0; n < N; ++n)
             for (int mm = 0; mm < N; ++mm) {
                 size_t idx = ((size_t)i * N + n) * N + mm;
-                W[idx] = 0.0; jL[idx] = -1; wR[idx] = 0.0;
-                /* O2: energy conservation, eq. 4.4: E_j = E_n+E_m-E_i  <=>  K~ = K_n+K_m-K_i */
-                double Kt = (K[n] + K[mm]) - K[i];
-                /* D4: snap ties at the domain edge */
-                double tau = 32.0 * 2.220446049250313e-16 * (K[n] + K[mm] + K[i]);
-                if (Kt < K[0] && Kt >= K[0] - tau) Kt = K[0];
-                if (Kt > K[N - 1] && Kt <= K[N - 1] + tau) Kt = K[N - 1];
-                /* O3: keep iff E_j >= m and q_min <= q_j <= q_max <=> K_0 <= K~ <= K_{N-1} */
-                if (!(Kt >= K[0] && Kt <= K[N - 1])) continue;
-                /* O4 */
-                double pj = sqrt(Kt * (Kt + 2.0 * m));
-                /* O5: eq. B.15-B.16 */
-                double Qm = fmax(fabs(p[i] - p[n]), fabs(p[mm] - pj));
-                double Qp = fmin(p[i] + p[n], p[mm] + pj);
-                double J = okx_J(Qm, Qp, M2_0, m_med, K[i], K[n]);
-                /* O6: eq. 4.7 with F of eq. B.17 */
-                double w = dp[n] * dp[mm] / (2.0 * E[i] * g_chi);
-                w = w * (1.0 / (64.0 * pi3 * p[i]));
-                w = w * (p[n] * p[mm] / (E[n] * E[mm]));
-                w = w * J;
-                /* O7: bracket scan, largest j with K_j <= K~ <= K_{j+1}; eq. B.19 */
-                int jb = -1;
-                for (int j = 0; j <= N - 2; ++j)
-                    if (K[j] <= Kt && Kt <= K[j + 1]) jb = j;
-                if (jb < 0) continue; /* cannot happen after O3 */
-                W[idx] = w;
-                jL[idx] = jb;
-                wR[idx] = (Kt - K[jb]) / (K[jb + 1] - K[jb]);
-                kept += 1;
+                kept += okx_triple(N, p, dp, E, K, m, g_chi, M2_0, m_med, i, n, mm, &W[idx], &jL[idx], &wR[idx]);
             }
     free(E); free(K); free(h);
     return kept;
@@ -159,6 +168,48 @@ void okx_collide(int N, int B, const double *f, const double *W, const int32_t *
             if (loss) loss[(size_t)b * N + i] = li;
             if (C) C[(size_t)b * N + i] = (double)(g - (long double)fb[i] * l);
         }
+}
+
+/* ---- O2-O9 for SELECTED rows i only, without storing the tables: the same per-triple code (okx_triple) and the
+ * same accumulation as okx_collide, used to sample the operator at sizes where the dense N^3 tables are too
+ * slow to build (N = 512).  rows[nrows]; outputs are [B, nrows]. */
+void okx_collide_rows(int N, int B, const double *p, const double *dp, double m, double g_chi,
+                      double M2_0, double m_med, const double *f, int nrows, const int32_t *rows,
+                      int interp, double f_floor, double *gain, double *loss, double *C)
+{
+    double *E = malloc(sizeof(double) * N), *K = malloc(sizeof(double) * N), *h = malloc(sizeof(double) * N);
+    okx_kinematics(N, p, dp, m, E, K, h);
+#pragma omp parallel for schedule(dynamic)
+    for (int r = 0; r < nrows; ++r) {
+        int i = rows[r];
+        long double *g = calloc(B, sizeof(long double)), *l = calloc(B, sizeof(long double));
+        for (int n = 0; n < N; ++n)
+            for (int mm = 0; mm < N; ++mm) {
+                double w, oR; int32_t j;
+                if (!okx_triple(N, p, dp, E, K, m, g_chi, M2_0, m_med, i, n, mm, &w, &j, &oR)) continue;
+                double oL = 1.0 - oR;
+                for (int b = 0; b < B; ++b) {
+                    const double *fb = f + (size_t)b * N;
+                    double fj;
+                    if (interp == 0) {
+                        double yL = log(fmax(fb[j], f_floor)), yR = log(fmax(fb[j + 1], f_floor));
+                        fj = exp(oL * yL + oR * yR);
+                    } else {
+                        fj = oL * fb[j] + oR * fb[j + 1];
+                    }
+                    g[b] += (long double)w * (long double)fb[n] * (long double)fb[mm];
+                    l[b] += (long double)w * (long double)fj;
+                }
+            }
+        for (int b = 0; b < B; ++b) {
+            long double fi = f[(size_t)b * N + i];
+            if (gain) gain[(size_t)b * nrows + r] = (double)g[b];
+            if (loss) loss[(size_t)b * nrows + r] = (double)(fi * l[b]);
+            if (C) C[(size_t)b * nrows + r] = (double)(g[b] - fi * l[b]);
+        }
+        free(g); free(l);
+    }
+    free(E); free(K); free(h);
 }
 
 /* ---- O10: two-moment projection, App. C eq. C.2-C.8, support mask C.4 with

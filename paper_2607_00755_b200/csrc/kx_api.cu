@@ -1,0 +1,487 @@
+// kx_api.cu -- the C ABI of include/kx.h: argument checks, memory ownership and launch sequencing.
+// All arithmetic of the path runs in the kernels of kx_build.cu / kx_contract.cu; nothing here computes
+// a physical quantity on the host except the 256-entry exp2 table (a constant, not data dependent).
+#include "kx_internal.cuh"
+
+#include <math.h>
+#include <new>
+#include <vector>
+
+namespace {
+
+std::string g_build_err;
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+inline long long tri_entries(int N) { return (long long)N * ((long long)N * (N + 1) / 2); }
+
+template <typename T>
+cudaError_t dalloc(T** p, size_t count) { return cudaMalloc((void**)p, count * sizeof(T)); }
+
+void free_tensor(kx_handle_s* h)
+{
+    cudaFree(h->d.W); cudaFree(h->d.omega); cudaFree(h->d.nmj);
+    h->d.W = nullptr; h->d.omega = nullptr; h->d.nmj = nullptr;
+    h->cap = 0;
+}
+
+kx_status_t alloc_tensor(kx_handle_s* h, long long cap)
+{
+    free_tensor(h);
+    if (cap < 1) cap = 1;
+    KX_CUDA(dalloc(&h->d.W, (size_t)cap));
+    KX_CUDA(dalloc(&h->d.omega, (size_t)cap));
+    KX_CUDA(dalloc(&h->d.nmj, (size_t)cap));
+    h->cap = cap;
+    return KX_OK;
+}
+
+void free_ws(kx_handle_s* h)
+{
+    cudaFree(h->yd); cudaFree(h->part); cudaFree(h->fstage); cudaFree(h->k1); cudaFree(h->k2);
+    cudaFree(h->k3); cudaFree(h->Cbuf); cudaFree(h->hostio);
+    h->yd = h->part = h->fstage = h->k1 = h->k2 = h->k3 = h->Cbuf = h->hostio = nullptr;
+    h->wsB = 0; h->ws_tasks = 0;
+}
+
+// the smallest chunk is 1024 entries, so a row of len entries has at most len/1024+1 tasks
+inline long long max_tasks(const kx_handle_s* h) { return h->cap / 1024 + h->d.N + 1; }
+
+kx_status_t ensure_ws(kx_handle_s* h, int B)
+{
+    const long long need_tasks = max_tasks(h);
+    if (B <= h->wsB && need_tasks <= h->ws_tasks) return KX_OK;
+    const int nB = B > h->wsB ? B : h->wsB;
+    free_ws(h);
+    const size_t bn = (size_t)nB * h->d.N;
+    KX_CUDA(dalloc(&h->yd, bn * 2));
+    KX_CUDA(dalloc(&h->part, (size_t)need_tasks * nB * 2));
+    KX_CUDA(dalloc(&h->fstage, bn));
+    KX_CUDA(dalloc(&h->k1, bn));
+    KX_CUDA(dalloc(&h->k2, bn));
+    KX_CUDA(dalloc(&h->k3, bn));
+    KX_CUDA(dalloc(&h->Cbuf, bn + (size_t)nB));   // + kappa[B]
+    KX_CUDA(dalloc(&h->hostio, bn * 2));
+    h->wsB = nB; h->ws_tasks = need_tasks;
+    return KX_OK;
+}
+
+long long nnz_estimate(const kx_handle_s* h)
+{
+    if (!h->nnz_stale) return h->nnz;
+    return (long long)(0.66 * (double)tri_entries(h->d.N));
+}
+
+// (re)build the task table when the chunk size changes or the tensor was rebuilt
+kx_status_t ensure_tasks(kx_handle_s* h, int B, cudaStream_t s)
+{
+    const int chunk = kx_pick_chunk(nnz_estimate(h), h->d.N, B, h->sm_count);
+    if (chunk != h->d.chunk || h->chunk_for_B == 0) {
+        h->d.chunk = chunk;
+        KX_CUDA(kx_launch_tasks(h->d, chunk, s));
+        h->chunk_for_B = B;
+    }
+    return KX_OK;
+}
+
+// a1-a3 for mass m; the capacity must already cover the result
+kx_status_t rebuild(kx_handle_s* h, double m, cudaStream_t s)
+{
+    h->d.m = m;
+    KX_CUDA(kx_launch_kinematics(h->d, m, s));
+    KX_CUDA(kx_launch_runs(h->d, s));
+    KX_CUDA(kx_launch_fill(h->d, s));
+    h->nnz_stale = true;
+    h->chunk_for_B = 0;
+    return KX_OK;
+}
+
+kx_status_t check_batch(kx_handle_s* h, const void* f, int B)
+{
+    if (!f || B < 1) { h->err = "f is NULL or B < 1"; return KX_ERR_INVALID_ARG; }
+    if (((uintptr_t)f & 15u) != 0) { h->err = "device pointer not 16-byte aligned"; return KX_ERR_INVALID_ARG; }
+    return KX_OK;
+}
+
+kx_status_t collide_impl(kx_handle_s* h, const double* f, double* C, double* gain, double* loss, double* diag,
+                         int B, unsigned flags, cudaStream_t s)
+{
+    kx_status_t rc = check_batch(h, f, B);
+    if (rc != KX_OK) return rc;
+    if (C == f) { h->err = "in-place kx_collide (C == f) is not allowed"; return KX_ERR_INVALID_ARG; }
+    if ((rc = ensure_ws(h, B)) != KX_OK) return rc;
+    if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
+    KX_CUDA(kx_launch_prep(h->d, f, h->yd, B, s));
+    if (h->profiling) {
+        if (h->prof_used == h->prof_events.size()) {
+            cudaEvent_t a, b;
+            KX_CUDA(cudaEventCreate(&a));
+            KX_CUDA(cudaEventCreate(&b));
+            h->prof_events.emplace_back(a, b);
+        }
+        KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].first, s));
+    }
+    KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, s));
+    if (h->profiling) {
+        KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].second, s));
+        h->prof_used++;
+    }
+    KxStage st = {};
+    st.flags = flags & KX_PROJECT;
+    st.C = C; st.gain = gain; st.loss = loss; st.diag = diag; st.diag_stride = 4;
+    st.evolve = 0;
+    KX_CUDA(kx_launch_finish(h->d, f, h->part, B, st, s));
+    return KX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t kx_version(void) { return 100; }
+
+const char* kx_last_error(kx_handle_t h) { return h ? h->err.c_str() : g_build_err.c_str(); }
+
+void kx_destroy(kx_handle_t h)
+{
+    if (!h) return;
+    {
+        DeviceGuard g(h->device);
+        free_tensor(h);
+        free_ws(h);
+        cudaFree(h->dev_blob);
+        for (auto& ev : h->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+    }
+    delete h;
+}
+
+kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq_t* msq,
+                     const kx_opts_t* opts, int device, void* stream, kx_handle_t* out)
+{
+    if (out) *out = nullptr;
+    if (!grid || !sp || !msq || !out || !grid->p || !grid->dp) { g_build_err = "null argument"; return KX_ERR_INVALID_ARG; }
+    const int N = grid->n;
+    if (N < 4 || N > KX_MAX_N) { g_build_err = "N must be in [4, 1024]"; return KX_ERR_INVALID_ARG; }
+    for (int i = 0; i < N; ++i) {
+        if (!(grid->p[i] > 0.0) || !(grid->dp[i] > 0.0) || !isfinite(grid->p[i]) || !isfinite(grid->dp[i]) ||
+            (i > 0 && !(grid->p[i] > grid->p[i - 1]))) {
+            g_build_err = "grid must have p ascending and > 0, dp > 0";
+            return KX_ERR_INVALID_ARG;
+        }
+    }
+    if (!(sp->m >= 0.0) || !(sp->g_chi > 0.0) || !isfinite(sp->m)) { g_build_err = "need m >= 0 and g_chi > 0"; return KX_ERR_INVALID_ARG; }
+    if (!isfinite(msq->M2_0) || !isfinite(msq->m_med)) { g_build_err = "non-finite |M|^2 parameters"; return KX_ERR_INVALID_ARG; }
+    kx_opts_t o = {KX_INTERP_LOG, KX_STORE_SYM_ROWS, KX_FP64, KX_EXP_TABLE, 1e-300, 1e-12};
+    if (opts) o = *opts;
+    if (o.precision != KX_FP64) { g_build_err = "fp32 mode is not implemented"; return KX_ERR_UNSUPPORTED; }
+    if (o.storage != KX_STORE_SYM_ROWS) { g_build_err = "unknown storage mode"; return KX_ERR_UNSUPPORTED; }
+    if (o.interp != KX_INTERP_LOG && o.interp != KX_INTERP_LINEAR) { g_build_err = "unknown interpolation"; return KX_ERR_INVALID_ARG; }
+    if (o.exp_impl != KX_EXP_TABLE && o.exp_impl != KX_EXP_LIBM) { g_build_err = "unknown exp_impl"; return KX_ERR_INVALID_ARG; }
+    if (!(o.f_floor >= 1e-300) || !(o.eps_supp >= 0.0)) { g_build_err = "need f_floor >= 1e-300 and eps_supp >= 0"; return KX_ERR_INVALID_ARG; }
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        g_build_err = "no usable CUDA device (libkx has no CPU fallback)";
+        return KX_ERR_CUDA;
+    }
+    DeviceGuard guard(device);
+    if (!guard.ok) { g_build_err = "cudaSetDevice failed"; return KX_ERR_CUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || prop.major != 10) {
+        g_build_err = "libkx is built for sm_100a (B200) only";
+        return KX_ERR_CUDA;
+    }
+
+    kx_handle_s* h = new (std::nothrow) kx_handle_s();
+    if (!h) { g_build_err = "out of host memory"; return KX_ERR_ALLOC; }
+    h->device = device;
+    h->sm_count = prop.multiProcessorCount;
+    h->nnz_stale = true;
+    KxDev& d = h->d;
+    d = KxDev{};
+    d.N = N; d.interp = o.interp; d.exp_impl = o.exp_impl; d.chunk = 0;
+    d.m = sp->m; d.g_chi = sp->g_chi; d.M2_0 = msq->M2_0; d.m_med = msq->m_med;
+    d.f_floor = o.f_floor; d.eps_supp = o.eps_supp;
+    cudaStream_t s = (cudaStream_t)stream;
+
+    auto fail = [&](kx_status_t rc) { g_build_err = h->err; kx_destroy(h); return rc; };
+    auto body = [&]() -> kx_status_t {
+        // one blob: 8 double arrays [N], exp table, int tables
+        const size_t nd = (size_t)8 * N + (1u << KX_EXP_BITS);
+        const size_t n2 = (size_t)N * N;
+        const size_t bytes = nd * 8 + (n2 * 2 + (n2 + 1) + 2 * (size_t)(N + 1) + 4) * 4;
+        KX_CUDA(cudaMalloc(&h->dev_blob, bytes));
+        double* dp_ = (double*)h->dev_blob;
+        double* P = dp_;            dp_ += N;
+        double* DP = dp_;           dp_ += N;
+        d.E = dp_;                  dp_ += N;
+        d.K = dp_;                  dp_ += N;
+        d.h = dp_;                  dp_ += N;
+        d.invdK = dp_;              dp_ += N;
+        d.arow = dp_;               dp_ += N;
+        d.ccol = dp_;               dp_ += N;
+        double* tab = dp_;          dp_ += (1u << KX_EXP_BITS);
+        int* ip = (int*)dp_;
+        d.run_mlo = ip;             ip += n2;
+        d.run_len = ip;             ip += n2;
+        d.run_off = (unsigned*)ip;  ip += n2 + 1;
+        d.rowptr = (unsigned*)ip;   ip += N + 1;
+        d.taskptr = (unsigned*)ip;  ip += N + 1;
+        h->flag = ip;
+        d.p = P; d.dp = DP; d.exptab = tab;
+        std::vector<double> t(1u << KX_EXP_BITS);
+        for (unsigned k = 0; k < (1u << KX_EXP_BITS); ++k)
+            t[k] = (double)exp2l((long double)k / (long double)(1u << KX_EXP_BITS));
+        KX_CUDA(cudaMemcpyAsync(P, grid->p, (size_t)N * 8, cudaMemcpyHostToDevice, s));
+        KX_CUDA(cudaMemcpyAsync(DP, grid->dp, (size_t)N * 8, cudaMemcpyHostToDevice, s));
+        KX_CUDA(cudaMemcpyAsync(tab, t.data(), t.size() * 8, cudaMemcpyHostToDevice, s));
+        KX_CUDA(cudaMemsetAsync(h->flag, 0, 4, s));
+        KX_CUDA(kx_launch_kinematics(d, d.m, s));
+        KX_CUDA(kx_launch_runs(d, s));
+        unsigned nnz = 0;
+        KX_CUDA(cudaMemcpyAsync(&nnz, d.run_off + n2, 4, cudaMemcpyDeviceToHost, s));
+        KX_CUDA(cudaStreamSynchronize(s));
+        kx_status_t rc = alloc_tensor(h, (long long)nnz);
+        if (rc != KX_OK) return rc;
+        KX_CUDA(kx_launch_fill(d, s));
+        KX_CUDA(cudaStreamSynchronize(s));
+        h->nnz = nnz; h->nnz_stale = false; h->chunk_for_B = 0;
+        return KX_OK;
+    };
+    kx_status_t rc = body();
+    if (rc != KX_OK) return fail(rc);
+    *out = h;
+    return KX_OK;
+}
+
+kx_status_t kx_set_mass(kx_handle_t h, double m, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    if (!(m >= 0.0) || !isfinite(m)) { h->err = "need finite m >= 0"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const long long ub = tri_entries(h->d.N);
+    if (h->cap < ub) {   // the new mass may keep more triples: size for every (i, n<=m)
+        KX_CUDA(cudaStreamSynchronize(s));
+        kx_status_t rc = alloc_tensor(h, ub);
+        if (rc != KX_OK) return rc;
+    }
+    return rebuild(h, m, s);
+}
+
+kx_status_t kx_collide_ex(kx_handle_t h, const double* f, double* C, double* gain, double* loss,
+                          double* diag, int32_t B, uint32_t flags, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    return collide_impl(h, f, C, gain, loss, diag, B, flags, (cudaStream_t)stream);
+}
+
+kx_status_t kx_collide(kx_handle_t h, const double* f, double* C, int32_t B, uint32_t flags, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    if (!C) { h->err = "C is NULL"; return KX_ERR_INVALID_ARG; }
+    return kx_collide_ex(h, f, C, nullptr, nullptr, nullptr, B, flags, stream);
+}
+
+kx_status_t kx_collide_parts(kx_handle_t h, const double* f, double* gain, double* loss, int32_t B, void* stream)
+{
+    return kx_collide_ex(h, f, nullptr, gain, loss, nullptr, B, 0u, stream);
+}
+
+kx_status_t kx_collide_host(kx_handle_t h, const double* f_host, double* C_host, int32_t B,
+                            uint32_t flags, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    if (!f_host || !C_host || B < 1) { h->err = "null host buffer or B < 1"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    kx_status_t rc = ensure_ws(h, B);
+    if (rc != KX_OK) return rc;
+    const size_t bn = (size_t)B * h->d.N;
+    double* fd = h->hostio;
+    double* Cd = h->hostio + (size_t)h->wsB * h->d.N;
+    KX_CUDA(cudaMemcpyAsync(fd, f_host, bn * 8, cudaMemcpyHostToDevice, s));
+    rc = collide_impl(h, fd, Cd, nullptr, nullptr, nullptr, B, flags, s);
+    if (rc != KX_OK) return rc;
+    KX_CUDA(cudaMemcpyAsync(C_host, Cd, bn * 8, cudaMemcpyDeviceToHost, s));
+    KX_CUDA(cudaStreamSynchronize(s));
+    return KX_OK;
+}
+
+kx_status_t kx_moments(kx_handle_t h, const double* f, int32_t B,
+                       double* n, double* rho, double* p1, double* p2, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    kx_status_t rc = check_batch(h, f, B);
+    if (rc != KX_OK) return rc;
+    DeviceGuard guard(h->device);
+    KX_CUDA(kx_launch_moments(h->d, f, B, n, rho, p1, p2, 1, (cudaStream_t)stream));
+    return KX_OK;
+}
+
+kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
+                      const kx_evolve_t* ctl, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    kx_status_t rc = check_batch(h, f, B);
+    if (rc != KX_OK) return rc;
+    if (!ctl || !ctl->tau || ctl->S < 0) { h->err = "ctl, ctl->tau must be set and S >= 0"; return KX_ERR_INVALID_ARG; }
+    if (ctl->method != KX_EULER && ctl->method != KX_HEUN && ctl->method != KX_RK4) { h->err = "unknown method"; return KX_ERR_INVALID_ARG; }
+    const int nsrc = src ? src->nsrc : 0;
+    if (nsrc < 0 || nsrc > KX_MAX_SRC || (nsrc > 0 && (!src->G || !src->amp))) { h->err = "bad source description"; return KX_ERR_INVALID_ARG; }
+    if ((ctl->flags & KX_DIAG) && !ctl->diag) { h->err = "KX_DIAG needs ctl->diag"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const int N = h->d.N, S = ctl->S;
+    if (ctl->mass && h->cap < tri_entries(N)) {
+        KX_CUDA(cudaStreamSynchronize(s));
+        if ((rc = alloc_tensor(h, tri_entries(N))) != KX_OK) return rc;
+        if ((rc = rebuild(h, h->d.m, s)) != KX_OK) return rc;
+    }
+    if ((rc = ensure_ws(h, B)) != KX_OK) return rc;
+    double* kappa_d = nullptr;
+    if (ctl->kappa) {
+        kappa_d = h->Cbuf + (size_t)h->wsB * N;
+        KX_CUDA(cudaMemcpyAsync(kappa_d, ctl->kappa, (size_t)B * 8, cudaMemcpyHostToDevice, s));
+    }
+    KX_CUDA(cudaMemsetAsync(h->flag, 0, 4, s));
+    const bool diag = (ctl->flags & KX_DIAG) != 0;
+    const int nstage = ctl->method == KX_EULER ? 1 : (ctl->method == KX_HEUN ? 2 : 4);
+    double kin_mass = h->d.m;        // mass of the kinematics arrays on the device
+    double ten_mass = h->d.m;        // mass the tensor was built for
+    bool have_yd = false;            // yd already holds the current stage input (written by the last finish)
+
+    for (int k = 0; k < S; ++k) {
+        const double dt = ctl->tau[k + 1] - ctl->tau[k];
+        for (int stg = 0; stg < nstage; ++stg) {
+            // node (0), midpoint (1) or end (2) of the step for this stage
+            int pos;
+            if (ctl->method == KX_EULER) pos = 0;
+            else if (ctl->method == KX_HEUN) pos = stg == 0 ? 0 : 2;
+            else pos = stg == 0 ? 0 : (stg == 3 ? 2 : 1);
+            const double R = ctl->rate ? ctl->rate[2 * k + pos] : 1.0;
+            if (ctl->mass) {
+                const double m = ctl->mass[2 * k + pos];
+                if (m != ten_mass || m != kin_mass) {
+                    if ((rc = rebuild(h, m, s)) != KX_OK) return rc;
+                    ten_mass = kin_mass = m;
+                }
+            }
+            if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
+            const double* fin = stg == 0 ? f : h->fstage;
+            if (!have_yd) KX_CUDA(kx_launch_prep(h->d, fin, h->yd, B, s));
+            KX_CUDA(kx_launch_contract(h->d, h->sm_count, fin, h->yd, h->part, B, s));
+            KxStage st = {};
+            st.flags = ctl->flags & KX_PROJECT;
+            st.diag = (diag && stg == 0) ? ctl->diag + (size_t)k * B * 6 : nullptr;
+            st.diag_stride = 6;
+            st.evolve = 1; st.rk_method = ctl->method; st.rk_stage = stg;
+            st.dt = dt; st.rate = R; st.kappa = kappa_d;
+            st.nsrc = nsrc; st.G = nsrc ? src->G : nullptr;
+            for (int q = 0; q < nsrc; ++q) st.amp[q] = src->amp[(size_t)q * S + k];
+            st.f = f; st.fstage = h->fstage; st.k1 = h->k1; st.k2 = h->k2; st.k3 = h->k3;
+            st.ydnext = h->yd; st.flag = h->flag;
+            KX_CUDA(kx_launch_finish(h->d, fin, h->part, B, st, s));
+            have_yd = true;
+        }
+        if (diag) {
+            if (ctl->mass) {
+                const double mend = ctl->mass[2 * k + 2];
+                if (mend != kin_mass) { KX_CUDA(kx_launch_kinematics(h->d, mend, s)); kin_mass = mend; }
+            }
+            double* dg = ctl->diag + (size_t)k * B * 6;
+            KX_CUDA(kx_launch_moments(h->d, f, B, dg + 4, dg + 5, nullptr, nullptr, 6, s));
+        }
+    }
+    if (ctl->mass && kin_mass != ten_mass) {   // leave the handle consistent
+        if ((rc = rebuild(h, kin_mass, s)) != KX_OK) return rc;
+    }
+    int flag = 0;
+    KX_CUDA(cudaMemcpyAsync(&flag, h->flag, 4, cudaMemcpyDeviceToHost, s));
+    KX_CUDA(cudaStreamSynchronize(s));
+    if (flag) { h->err = "kx_evolve: f became non-finite"; return KX_ERR_NONFINITE; }
+    return KX_OK;
+}
+
+kx_status_t kx_profile(kx_handle_t h, int32_t enable)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    h->profiling = enable != 0;
+    return KX_OK;
+}
+
+kx_status_t kx_profile_read(kx_handle_t h, double* contract_ms, int64_t* launches)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    KX_CUDA(cudaDeviceSynchronize());
+    double sum = 0.0;
+    for (size_t k = 0; k < h->prof_used; ++k) {
+        float ms = 0.f;
+        KX_CUDA(cudaEventElapsedTime(&ms, h->prof_events[k].first, h->prof_events[k].second));
+        sum += ms;
+    }
+    if (contract_ms) *contract_ms = sum;
+    if (launches) *launches = (int64_t)h->prof_used;
+    h->prof_used = 0;
+    return KX_OK;
+}
+
+kx_status_t kx_info(kx_handle_t h, int64_t* nnz, int64_t* tensor_bytes, int32_t* n)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    KX_CUDA(cudaDeviceSynchronize());
+    if (h->nnz_stale) {
+        unsigned v = 0;
+        KX_CUDA(cudaMemcpy(&v, h->d.run_off + (size_t)h->d.N * h->d.N, 4, cudaMemcpyDeviceToHost));
+        h->nnz = v; h->nnz_stale = false;
+    }
+    if (nnz) *nnz = h->nnz;
+    if (tensor_bytes) *tensor_bytes = h->nnz * 20;   // W 8 + omega 8 + n|m|j 4
+    if (n) *n = h->d.N;
+    return KX_OK;
+}
+
+kx_status_t kx_tensor_export(kx_handle_t h, int64_t cap, int64_t* rowptr, double* W, double* omega, uint32_t* nmj)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    int64_t nnz = 0;
+    kx_status_t rc = kx_info(h, &nnz, nullptr, nullptr);
+    if (rc != KX_OK) return rc;
+    if (cap < nnz) { h->err = "kx_tensor_export: capacity below nnz"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    const int N = h->d.N;
+    if (rowptr) {
+        std::vector<unsigned> rp(N + 1);
+        KX_CUDA(cudaMemcpy(rp.data(), h->d.rowptr, (size_t)(N + 1) * 4, cudaMemcpyDeviceToHost));
+        for (int i = 0; i <= N; ++i) rowptr[i] = rp[i];
+    }
+    if (W) KX_CUDA(cudaMemcpy(W, h->d.W, (size_t)nnz * 8, cudaMemcpyDeviceToHost));
+    if (omega) KX_CUDA(cudaMemcpy(omega, h->d.omega, (size_t)nnz * 8, cudaMemcpyDeviceToHost));
+    if (nmj) KX_CUDA(cudaMemcpy(nmj, h->d.nmj, (size_t)nnz * 4, cudaMemcpyDeviceToHost));
+    return KX_OK;
+}
+
+kx_status_t kx_kinematics_export(kx_handle_t h, double* E, double* K, double* hw)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    KX_CUDA(cudaDeviceSynchronize());
+    const size_t b = (size_t)h->d.N * 8;
+    if (E) KX_CUDA(cudaMemcpy(E, h->d.E, b, cudaMemcpyDeviceToHost));
+    if (K) KX_CUDA(cudaMemcpy(K, h->d.K, b, cudaMemcpyDeviceToHost));
+    if (hw) KX_CUDA(cudaMemcpy(hw, h->d.h, b, cudaMemcpyDeviceToHost));
+    return KX_OK;
+}
+
+}  // extern "C"

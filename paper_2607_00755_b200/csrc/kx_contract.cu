@@ -1,0 +1,449 @@
+// kx_contract.cu -- steps a4-a9: gain/loss contraction, raw operator, projection, fused RK stage, moments.
+//
+//   a4  gain_i = sum_{n<=m} Wsym[i,nm] f_n f_m                              eq. 4.6 with 2.6
+//   a5  nu_i   = sum_{n<=m} Wsym[i,nm] f_j~,  loss_i = f_i nu_i
+//       LOG:    f_j~ = 2^(y_L + omega_R (y_R - y_L)),  y = log2 max(f, f_floor)   eq. B.20 at eta=0, D7/D8
+//       LINEAR: f_j~ = f_L + omega_R (f_R - f_L)                                  eq. B.19
+//   a6  C_raw = gain - f_i nu_i
+//   a7  projection C.2-C.8 in the basis {1, K_i} (same span as {1, E_i}, well conditioned), diag C.1, C.9
+//   a8  Runge-Kutta stage update fused into the finishing kernel                   eq. 4.9
+//   a9  moments                                                                    eq. B.2
+//
+// Work decomposition of the contraction: row i of the row-compressed tensor is cut into tasks of `chunk`
+// entries; a persistent CTA loops over tasks, each thread owns entries e0+tid, e0+tid+256, ... and keeps
+// BT gain and BT loss accumulators (one per batch member of its group) in registers; a fixed-order
+// shuffle/shared-memory reduction writes one partial per (task, b); the finishing kernel adds the
+// partials of a row in task order.  No atomics: results are bit-reproducible.
+//
+// Compiled with --fmad=false; every fused multiply-add below is an explicit fma().
+#include "kx_internal.cuh"
+
+namespace {
+
+// ---------------------------------------------------------------- exp2 for the LOG loss term
+// 2^t = 2^k * T[idx] * 2^r,  t = k + idx/256 + r, |r| <= 2^-9.  Adding 1.5*2^44 leaves round(256 t) in the
+// low mantissa bits (one DADD), T is a 256-entry table replicated 16x in shared memory so that the
+// 64-bit gather is bank-conflict free, 2^r = 1 + r q(r) with q the degree-3 Chebyshev interpolant of
+// (2^r-1)/r on |r| <= 1.01*2^-9 (polynomial error 5e-18), and 2^k is added to the exponent field by the
+// integer pipe.  FP64-pipe cost: 2 DADD + 1 DADD + 3 DFMA + 1 DMUL + 1 DFMA = 8.  Valid for
+// -1021 < t < 1023 (f_floor >= 1e-300 keeps t >= -997).
+__device__ __forceinline__ double kx_exp2_tab(double t, const double* __restrict__ tab_lane)
+{
+    const double MAG = 26388279066624.0;                 // 1.5 * 2^44
+    const double C1 = 0.6931471805599427, C2 = 0.24022650695910042,
+                 C3 = 0.05550411385340617, C4 = 0.009618129707037269;
+    double tm = t + MAG;
+    int nlo = __double2loint(tm);
+    double r = t - (tm - MAG);
+    double T = tab_lane[(nlo & ((1 << KX_EXP_BITS) - 1)) * KX_EXP_REP];
+    double q = fma(fma(fma(C4, r, C3), r, C2), r, C1);
+    double s = r * q;
+    double res = fma(T, s, T);
+    int hi = __double2hiint(res) + ((nlo >> KX_EXP_BITS) << 20);
+    return __hiloint2double(hi, __double2loint(res));
+}
+
+// ---------------------------------------------------------------- prep: (y_j, y_{j+1}-y_j) per (b, j)
+__device__ __forceinline__ double kx_yval(double f, int interp, double f_floor)
+{
+    return interp == KX_INTERP_LOG ? log2(fmax(f, f_floor)) : f;
+}
+
+__global__ void k_prep(KxDev d, const double* __restrict__ f, double2* __restrict__ yd, int B)
+{
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    int b = blockIdx.y;
+    if (j >= d.N) return;
+    const double* fb = f + (size_t)b * d.N;
+    double y0 = kx_yval(fb[j], d.interp, d.f_floor);
+    double y1 = (j + 1 < d.N) ? kx_yval(fb[j + 1], d.interp, d.f_floor) : y0;
+    yd[(size_t)b * d.N + j] = make_double2(y0, y1 - y0);
+}
+
+// ---------------------------------------------------------------- contraction
+enum { MODE_LOG_TAB = 0, MODE_LOG_LIBM = 1, MODE_LINEAR = 2 };
+
+template <int BT, int MODE>
+__global__ void __launch_bounds__(KX_CTA, 2)
+k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd,
+           double* __restrict__ part, int B)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = d.N;
+    double2* s_yd = reinterpret_cast<double2*>(smem_raw);                 // [BT][N]
+    double* s_f = reinterpret_cast<double*>(s_yd + (size_t)BT * N);       // [BT][N]
+    double* s_red = s_f + (size_t)BT * N;                                 // [8][2*BT]
+    double* s_tab = s_red + (KX_CTA / 32) * 2 * BT;                       // [256][16] (MODE_LOG_TAB)
+    unsigned* s_tp = reinterpret_cast<unsigned*>(s_tab + (MODE == MODE_LOG_TAB ? (KX_EXP_REP << KX_EXP_BITS) : 0)); // [N+1]
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b0 = blockIdx.y * BT;
+    const int nb = min(BT, B - b0);
+
+    for (int k = tid; k < BT * N; k += KX_CTA) {
+        int b = k / N, j = k - b * N;
+        if (b < nb) {
+            s_yd[k] = yd[(size_t)(b0 + b) * N + j];
+            s_f[k] = f[(size_t)(b0 + b) * N + j];
+        } else {                                  // ragged last group: harmless values, results discarded
+            s_yd[k] = make_double2(0.0, 0.0);
+            s_f[k] = 0.0;
+        }
+    }
+    if (MODE == MODE_LOG_TAB)
+        for (int k = tid; k < (KX_EXP_REP << KX_EXP_BITS); k += KX_CTA) s_tab[k] = d.exptab[k / KX_EXP_REP];
+    for (int k = tid; k <= N; k += KX_CTA) s_tp[k] = d.taskptr[k];
+    __syncthreads();
+
+    const unsigned ntasks = s_tp[N];
+    const double* tab_lane = s_tab + (lane & (KX_EXP_REP - 1));
+    const unsigned chunk = (unsigned)d.chunk;
+
+    for (unsigned task = blockIdx.x; task < ntasks; task += gridDim.x) {
+        // row of this task: largest i with taskptr[i] <= task
+        int lo = 0, hi = N - 1;
+        while (lo < hi) {
+            int mid = (lo + hi + 1) >> 1;
+            if (s_tp[mid] <= task) lo = mid; else hi = mid - 1;
+        }
+        const int i = lo;
+        const unsigned r0 = d.rowptr[i], r1 = d.rowptr[i + 1];
+        const unsigned e0 = r0 + (task - s_tp[i]) * chunk;
+        const unsigned e1 = min(e0 + chunk, r1);
+
+        double g[BT], l[BT];
+#pragma unroll
+        for (int b = 0; b < BT; ++b) { g[b] = 0.0; l[b] = 0.0; }
+
+        unsigned e = e0 + tid;
+        double W = 0.0, om = 0.0;
+        unsigned pk = 0;
+        if (e < e1) { W = d.W[e]; om = d.omega[e]; pk = d.nmj[e]; }
+        while (e < e1) {
+            const double Wc = W, omc = om;
+            const unsigned pkc = pk;
+            e += KX_CTA;
+            if (e < e1) { W = d.W[e]; om = d.omega[e]; pk = d.nmj[e]; }   // prefetch the next entry
+            const int n = pkc & 1023, m = (pkc >> 10) & 1023, j = pkc >> 20;
+#pragma unroll
+            for (int b = 0; b < BT; ++b) {
+                const double pn = s_f[b * N + n] * s_f[b * N + m];
+                g[b] = fma(Wc, pn, g[b]);
+                const double2 y = s_yd[b * N + j];
+                const double t = fma(omc, y.y, y.x);
+                double x;
+                if (MODE == MODE_LOG_TAB) x = kx_exp2_tab(t, tab_lane);
+                else if (MODE == MODE_LOG_LIBM) x = exp2(t);
+                else x = t;
+                l[b] = fma(Wc, x, l[b]);
+            }
+        }
+        // fixed-order reduction: xor butterfly inside the warp, then warps 0..7 in order
+#pragma unroll
+        for (int b = 0; b < BT; ++b) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                g[b] += __shfl_xor_sync(0xffffffffu, g[b], o);
+                l[b] += __shfl_xor_sync(0xffffffffu, l[b], o);
+            }
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int b = 0; b < BT; ++b) {
+                s_red[warp * 2 * BT + 2 * b] = g[b];
+                s_red[warp * 2 * BT + 2 * b + 1] = l[b];
+            }
+        }
+        __syncthreads();
+        if (tid < 2 * BT) {
+            double acc = 0.0;
+#pragma unroll
+            for (int w = 0; w < KX_CTA / 32; ++w) acc += s_red[w * 2 * BT + tid];
+            const int b = tid >> 1;
+            if (b < nb) part[((size_t)task * B + (b0 + b)) * 2 + (tid & 1)] = acc;
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------- block reductions (256 threads, fixed order)
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* s_red /* [NV*8] */)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+    __syncthreads();
+    if (lane == 0)
+#pragma unroll
+        for (int k = 0; k < NV; ++k) s_red[k * 8 + warp] = v[k];
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        double a = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) a += s_red[k * 8 + w];
+        v[k] = a;
+    }
+}
+
+__device__ __forceinline__ double block_max(double v, double* s_red)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    __syncthreads();
+    if (lane == 0) s_red[warp] = v;
+    __syncthreads();
+    double a = s_red[0];
+#pragma unroll
+    for (int w = 1; w < 8; ++w) a = fmax(a, s_red[w]);
+    return a;
+}
+
+// ---------------------------------------------------------------- finishing kernel: one CTA per member b
+constexpr int kMaxPerThread = KX_MAX_N / KX_CTA;   // 4
+
+__global__ void __launch_bounds__(KX_CTA)
+k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ part, int B, KxStage st)
+{
+    __shared__ double s_red[8 * 8];
+    __shared__ double s_y[KX_MAX_N];
+    const int N = d.N, tid = threadIdx.x, b = blockIdx.x;
+    const double* fb = fin + (size_t)b * N;
+
+    double C[kMaxPerThread], fi[kMaxPerThread], hi_[kMaxPerThread], Ei[kMaxPerThread], Ki[kMaxPerThread];
+#pragma unroll
+    for (int q = 0; q < kMaxPerThread; ++q) {
+        const int i = tid + q * KX_CTA;
+        C[q] = 0.0; fi[q] = 0.0; hi_[q] = 0.0; Ei[q] = 0.0; Ki[q] = 0.0;
+        if (i < N) {
+            const unsigned t0 = d.taskptr[i], t1 = d.taskptr[i + 1];
+            double g = 0.0, nu = 0.0;
+            for (unsigned t = t0; t < t1; ++t) {
+                g += part[((size_t)t * B + b) * 2];
+                nu += part[((size_t)t * B + b) * 2 + 1];
+            }
+            fi[q] = fb[i];
+            C[q] = fma(-fi[q], nu, g);                            // a6
+            hi_[q] = d.h[i]; Ei[q] = d.E[i]; Ki[q] = d.K[i];
+            if (st.gain) st.gain[(size_t)b * N + i] = g;
+            if (st.loss) st.loss[(size_t)b * N + i] = fi[q] * nu;
+        }
+    }
+
+    const bool project = (st.flags & KX_PROJECT) != 0;
+    if (project || st.diag) {
+        // C.2 and the denominators of C.1 / C.9
+        double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        double fm = 0.0;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) {
+            const double hc = hi_[q] * C[q];
+            v[0] += hc;                       // R0 = sum h C
+            v[1] += hc * Ki[q];               // RK = sum h K C
+            v[2] += hc * Ei[q];               // R1 = sum h E C
+            v[3] += fabs(hc);                 // S0
+            v[4] += fabs(hc) * Ei[q];         // S1
+            fm = fmax(fm, fabs(fi[q]));
+        }
+        block_sum<5>(v, s_red);
+        const double fmax_ = block_max(fm, s_red);
+        const double R0 = v[0], RK = v[1], R1 = v[2], S0 = v[3], S1 = v[4];
+        double alpha = 0.0, beta = 0.0, D0 = 0.0, D1 = 0.0;
+        if (project) {
+            double xi[kMaxPerThread];
+            double a[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+            for (int q = 0; q < kMaxPerThread; ++q) {
+                const double r = fmax_ > 0.0 ? fabs(fi[q]) / fmax_ : 0.0;     // C.4
+                xi[q] = r > d.eps_supp ? r : 0.0;
+                const double hx = hi_[q] * xi[q];
+                a[0] += hx;                   // A00
+                a[1] += hx * Ki[q];           // A0K
+                a[2] += hx * Ki[q] * Ki[q];   // AKK
+            }
+            block_sum<3>(a, s_red);
+            const double A00 = a[0], A0K = a[1], AKK = a[2];
+            if (fmax_ > 0.0 && A00 > 0.0) {
+                const double det = A00 * AKK - A0K * A0K;                    // C.8
+                if (det <= 1e-14 * A00 * AKK) { alpha = R0 / A00; beta = 0.0; }   // D9
+                else { alpha = (R0 * AKK - RK * A0K) / det; beta = (RK * A00 - R0 * A0K) / det; }
+            }
+            double dsum[2] = {0.0, 0.0};
+#pragma unroll
+            for (int q = 0; q < kMaxPerThread; ++q) {
+                const double corr = xi[q] * (alpha + beta * Ki[q]);
+                C[q] = C[q] - corr;                                          // C.3
+                dsum[0] += hi_[q] * fabs(corr);
+                dsum[1] += hi_[q] * Ei[q] * fabs(corr);
+            }
+            if (st.diag) { block_sum<2>(dsum, s_red); D0 = dsum[0]; D1 = dsum[1]; }
+        }
+        if (st.diag && tid == 0) {
+            double* dg = st.diag + (size_t)b * st.diag_stride;
+            dg[0] = S0 > 0.0 ? R0 / S0 : 0.0;       // eps_N, C.1
+            dg[1] = S1 > 0.0 ? R1 / S1 : 0.0;       // eps_E
+            dg[2] = S0 > 0.0 ? D0 / S0 : 0.0;       // R_N, C.9
+            dg[3] = S1 > 0.0 ? D1 / S1 : 0.0;       // R_E
+        }
+    }
+
+    if (st.C) {
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) {
+            const int i = tid + q * KX_CTA;
+            if (i < N) st.C[(size_t)b * N + i] = C[q];
+        }
+    }
+    if (!st.evolve) return;
+
+    // ---- a8: k = kappa_b R C + sum_s amp_s G_s, then the Runge-Kutta bookkeeping of this stage
+    const double kR = (st.kappa ? st.kappa[b] : 1.0) * st.rate;
+    const double dt = st.dt;
+    bool bad = false;
+#pragma unroll
+    for (int q = 0; q < kMaxPerThread; ++q) {
+        const int i = tid + q * KX_CTA;
+        if (i >= N) continue;
+        const size_t o = (size_t)b * N + i;
+        double s = 0.0;
+        for (int r = 0; r < st.nsrc; ++r) s += st.amp[r] * st.G[(size_t)r * N + i];
+        const double k = kR * C[q] + s;
+        const double f0 = st.f[o];
+        double next;      // input of the next operator evaluation
+        if (st.rk_method == KX_EULER) {
+            next = f0 + dt * k;
+            st.f[o] = next;
+        } else if (st.rk_method == KX_HEUN) {
+            if (st.rk_stage == 0) { st.k1[o] = k; next = f0 + dt * k; st.fstage[o] = next; }
+            else { next = f0 + 0.5 * dt * (st.k1[o] + k); st.f[o] = next; }
+        } else {
+            if (st.rk_stage == 0) { st.k1[o] = k; next = f0 + 0.5 * dt * k; st.fstage[o] = next; }
+            else if (st.rk_stage == 1) { st.k2[o] = k; next = f0 + 0.5 * dt * k; st.fstage[o] = next; }
+            else if (st.rk_stage == 2) { st.k3[o] = k; next = f0 + dt * k; st.fstage[o] = next; }
+            else { next = f0 + (dt / 6.0) * (st.k1[o] + 2.0 * st.k2[o] + 2.0 * st.k3[o] + k); st.f[o] = next; }
+        }
+        if (!isfinite(next)) bad = true;
+        s_y[i] = kx_yval(next, d.interp, d.f_floor);
+    }
+    if (bad) atomicOr(st.flag, 1);
+    __syncthreads();
+    if (st.ydnext) {
+        double2* ydn = reinterpret_cast<double2*>(st.ydnext) + (size_t)b * N;
+        for (int i = tid; i < N; i += KX_CTA) {
+            const double y0 = s_y[i], y1 = (i + 1 < N) ? s_y[i + 1] : y0;
+            ydn[i] = make_double2(y0, y1 - y0);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- a9: moments, eq. B.2
+__global__ void __launch_bounds__(KX_CTA)
+k_moments(KxDev d, const double* __restrict__ f, double* n, double* rho, double* p1, double* p2, int stride)
+{
+    __shared__ double s_red[8 * 8];
+    const int N = d.N, b = blockIdx.x;
+    double v[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int i = threadIdx.x; i < N; i += KX_CTA) {
+        const double hf = d.h[i] * f[(size_t)b * N + i];
+        const double p = d.p[i];
+        v[0] += hf;
+        v[1] += hf * d.E[i];
+        v[2] += hf * p;
+        v[3] += hf * p * p;
+    }
+    block_sum<4>(v, s_red);
+    if (threadIdx.x == 0) {
+        const double fac = d.g_chi / (2.0 * 3.14159265358979323846 * 3.14159265358979323846);
+        if (n) n[(size_t)b * stride] = fac * v[0];
+        if (rho) rho[(size_t)b * stride] = fac * v[1];
+        if (p1) p1[(size_t)b * stride] = v[0] != 0.0 ? v[2] / v[0] : 0.0;
+        if (p2) p2[(size_t)b * stride] = v[0] != 0.0 ? v[3] / v[0] : 0.0;
+    }
+}
+
+template <int BT, int MODE>
+cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, const double* yd,
+                              double* part, int B, cudaStream_t s)
+{
+    const int N = d.N;
+    size_t smem = (size_t)BT * N * 24 + (size_t)(KX_CTA / 32) * 2 * BT * 8
+                + (MODE == MODE_LOG_TAB ? (size_t)(KX_EXP_REP << KX_EXP_BITS) * 8 : 0) + (size_t)(N + 1) * 4;
+    cudaError_t e = cudaFuncSetAttribute(k_contract<BT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_contract<BT, MODE>, KX_CTA, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    const int groups = (B + BT - 1) / BT;
+    int gx = (sm_count * occ + groups - 1) / groups;
+    if (gx < 1) gx = 1;
+    dim3 grid(gx, groups);
+    k_contract<BT, MODE><<<grid, KX_CTA, smem, s>>>(d, f, reinterpret_cast<const double2*>(yd), part, B);
+    return cudaGetLastError();
+}
+
+template <int BT>
+cudaError_t launch_contract_m(const KxDev& d, int sm_count, const double* f, const double* yd,
+                              double* part, int B, cudaStream_t s)
+{
+    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, s);
+    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, s);
+    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, s);
+}
+
+}  // namespace
+
+int kx_pick_bt(int N, int B)
+{
+    int cap = N > 512 ? 4 : 8;
+    int bt = 1;
+    while (bt < B && bt < cap) bt <<= 1;
+    return bt;
+}
+
+int kx_pick_chunk(long long nnz_est, int N, int B, int sm_count)
+{
+    const int bt = kx_pick_bt(N, B);
+    const long long groups = (B + bt - 1) / bt;
+    long long c = nnz_est * groups / ((long long)sm_count * 12);
+    c = (c / KX_CTA) * KX_CTA;
+    if (c < 1024) c = 1024;
+    if (c > 8192) c = 8192;
+    return (int)c;
+}
+
+cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, cudaStream_t s)
+{
+    dim3 grid((d.N + 255) / 256, B);
+    k_prep<<<grid, 256, 0, s>>>(d, f, reinterpret_cast<double2*>(yd), B);
+    return cudaGetLastError();
+}
+
+cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
+                               double* part, int B, cudaStream_t s)
+{
+    switch (kx_pick_bt(d.N, B)) {
+        case 1: return launch_contract_m<1>(d, sm_count, f, yd, part, B, s);
+        case 2: return launch_contract_m<2>(d, sm_count, f, yd, part, B, s);
+        case 4: return launch_contract_m<4>(d, sm_count, f, yd, part, B, s);
+        default: return launch_contract_m<8>(d, sm_count, f, yd, part, B, s);
+    }
+}
+
+cudaError_t kx_launch_finish(const KxDev& d, const double* fin, const double* part, int B,
+                             const KxStage& st, cudaStream_t s)
+{
+    k_finish<<<B, KX_CTA, 0, s>>>(d, fin, part, B, st);
+    return cudaGetLastError();
+}
+
+cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
+                              double* p1, double* p2, int stride, cudaStream_t s)
+{
+    k_moments<<<B, KX_CTA, 0, s>>>(d, f, n, rho, p1, p2, stride);
+    return cudaGetLastError();
+}

@@ -1,0 +1,114 @@
+// kx_internal.cuh -- shared declarations of libkx's translation units (NOT part of the ABI).
+// The CUDA path shares nothing with oracle/: no header, table, constant generator or helper.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "../../include/kx.h"
+
+#define KX_MAX_N      1024     // n, m, j_L are packed 10 bits each
+#define KX_MAX_SRC    8
+#define KX_CTA        256      // threads per CTA of the contraction kernels
+#define KX_EXP_BITS   8        // 2^8-entry exp2 table
+#define KX_EXP_REP    16       // table replicated once per bank pair: conflict-free 64-bit gathers
+
+// Device-side view of a handle: plain pointers, passed by value to every kernel.
+struct KxDev {
+    int N;
+    int interp;          // KX_INTERP_*
+    int exp_impl;        // KX_EXP_*
+    int chunk;           // entries per contraction task
+    double m, g_chi, M2_0, m_med, f_floor, eps_supp;
+    // grid and kinematics [N]
+    const double *p, *dp;
+    double *E, *K, *h;        // eq. B.1; K_i = E_i - m evaluated as p^2/(E+m)
+    double *invdK;            // 1/(K_{j+1}-K_j), j < N-1
+    double *arow;             // 1/(2 E_i g_chi) * 1/(64 pi^3 p_i)
+    double *ccol;             // dp_n p_n / E_n
+    // run table of the builder [N*N]: for (i,n) the valid m form one interval [mlo, mlo+len)
+    int *run_mlo, *run_len;
+    unsigned *run_off;        // [N*N+1] exclusive scan of run_len; run_off[N*N] = nnz
+    // row-compressed symmetric tensor
+    unsigned *rowptr;         // [N+1]
+    double *W;                // [cap] W_inm + W_imn (n<m) or W_inn
+    double *omega;            // [cap] omega_R of eq. B.19
+    unsigned *nmj;            // [cap] n | m<<10 | jL<<20
+    // contraction tasks: row i is cut into ceil(len_i/chunk) tasks
+    unsigned *taskptr;        // [N+1] exclusive scan; taskptr[N] = ntasks
+    const double *exptab;     // [2^KX_EXP_BITS] 2^(k/2^KX_EXP_BITS)
+};
+
+struct kx_handle_s {
+    KxDev d;
+    int device;
+    int sm_count;
+    long long cap;            // capacity of W/omega/nmj in entries
+    long long nnz;            // host copy, valid when !nnz_stale
+    bool nnz_stale;
+    int chunk_for_B;          // the batch size taskptr was last built for (0 = none)
+    // workspaces, grown on demand
+    int wsB;                  // batch capacity of the buffers below
+    long long ws_tasks;       // task capacity of `part`
+    double *yd;               // [wsB, N, 2]  LOG: (log2 f_j, log2 f_{j+1} - log2 f_j); LINEAR: (f_j, f_{j+1}-f_j)
+    double *part;             // [ws_tasks, wsB, 2] per-task partial (gain, loss frequency)
+    double *fstage, *k1, *k2, *k3, *Cbuf;   // [wsB, N] evolve buffers
+    double *hostio;           // [wsB, N] x2 staging for kx_collide_host
+    int *flag;                // device non-finite flag
+    void *dev_blob;           // one allocation holding the [N]-sized arrays
+    bool profiling;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;
+    size_t prof_used;
+    std::string err;
+};
+
+#define KX_CUDA(call)                                                                          \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            char buf_[512];                                                                    \
+            snprintf(buf_, sizeof buf_, "%s:%d: %s -> %s", __FILE__, __LINE__, #call,           \
+                     cudaGetErrorString(e_));                                                  \
+            h->err = buf_;                                                                     \
+            return KX_ERR_CUDA;                                                                \
+        }                                                                                      \
+    } while (0)
+
+// ---- launchers implemented in kx_build.cu
+cudaError_t kx_launch_kinematics(const KxDev& d, double m, cudaStream_t s);
+cudaError_t kx_launch_runs(const KxDev& d, cudaStream_t s);      // run table + scan + rowptr
+cudaError_t kx_launch_fill(const KxDev& d, cudaStream_t s);      // W, omega, nmj
+cudaError_t kx_launch_tasks(const KxDev& d, int chunk, cudaStream_t s);
+
+// ---- launchers implemented in kx_contract.cu
+struct KxStage {             // what the finishing kernel does after the reduction
+    unsigned flags;          // KX_PROJECT
+    double *C, *gain, *loss, *diag;       // outputs of kx_collide_ex (any may be null); diag stride 4
+    int diag_stride;
+    // evolve: mode 0 = none; otherwise the Runge-Kutta update below
+    int rk_method, rk_stage;
+    double dt, rate;
+    const double *kappa;     // device [B] or null
+    int nsrc;
+    const double *G;         // device [nsrc,N]
+    double amp[KX_MAX_SRC];
+    double *f;               // state [B,N]
+    double *fstage;          // stage input written by this stage for the next one
+    double *k1, *k2, *k3;
+    double *ydnext;          // where to write yd of the next stage input (fused prep) or null
+    int *flag;
+    int evolve;
+};
+cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, cudaStream_t s);
+cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
+                               double* part, int B, cudaStream_t s);
+cudaError_t kx_launch_finish(const KxDev& d, const double* f, const double* part, int B,
+                             const KxStage& st, cudaStream_t s);
+cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
+                              double* p1, double* p2, int stride, cudaStream_t s);
+int kx_pick_bt(int N, int B);
+int kx_pick_chunk(long long nnz_est, int N, int B, int sm_count);

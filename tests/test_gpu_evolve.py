@@ -1,0 +1,171 @@
+"""kx_evolve (a8) against the oracle's fixed-step integrators (O12) on the BASELINE configs 1, 2 and 5."""
+import numpy as np
+import pytest
+
+import kx_inputs as kin
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    return torch
+
+
+def _dev(torch, a):
+    return torch.tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda")
+
+
+def _nu_max(oracle, c):
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g, l, C = oracle.collide(T, c["f"], 0)
+    return T, float((l[0] / c["f"][0]).max())
+
+
+def test_cfg1_euler_200_steps(torch_cuda, oracle):
+    """Config 1: one C[f] plus 200 explicit-Euler steps toward Maxwell-Boltzmann, number/energy conserved."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(1)
+    T, nu = _nu_max(oracle, c)
+    S = 200
+    tau = np.arange(S + 1) * (0.2 / nu)                      # reading D13
+    f_ref, d_ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.EULER, tau=tau, want_diag=True)
+    h = kx.Handle(c["p"], c["dp"], c["m"])
+    f = _dev(torch, c["f"])
+    diag = h.evolve(f, tau, method=kx.EULER, want_diag=True).cpu().numpy()
+    got = f.cpu().numpy()
+    assert np.abs(got - f_ref).max() <= 1e-10 * np.abs(f_ref).max()
+    assert np.allclose(diag[:, :, 4:], d_ref[:, :, 4:], rtol=1e-12, atol=0)          # n, rho after each step
+    assert np.allclose(diag[:, :, :4], d_ref[:, :, :4], rtol=1e-6, atol=1e-12)        # eps_N, eps_E, R_N, R_E
+    # conserved moments drift <= 1e-12 relative per step
+    n0 = oracle.moments(T, c["f"])[0]
+    assert np.abs(diag[:, 0, 4] / n0[0] - 1).max() <= 1e-12 * S
+    assert np.abs(diag[:, 0, 5] / n0[1] - 1).max() <= 1e-12 * S
+    assert np.abs(np.diff(diag[:, 0, 4])).max() <= 1e-12 * n0[0]
+    h.close()
+
+
+@pytest.mark.parametrize("method", ["HEUN", "RK4"])
+def test_cfg2_relaxation_chunks(torch_cuda, oracle, method):
+    """Config 2: fixed-dt relaxation in chunks of 10 steps; f compared at the chunk boundaries."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(2)
+    T, nu = _nu_max(oracle, c)
+    dt = 0.5 / nu
+    h = kx.Handle(c["p"], c["dp"], c["m"])
+    f = _dev(torch, c["f"])
+    f_ref = c["f"].copy()
+    for chunk in range(3):
+        tau = (chunk * 10 + np.arange(11)) * dt
+        f_ref = oracle.evolve(c["p"], c["dp"], f_ref, m=c["m"], method=getattr(oracle, method), tau=tau)
+        h.evolve(f, tau, method=getattr(kx, method))
+        assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-10 * np.abs(f_ref).max()
+    mo = h.moments(f).cpu().numpy()[:, 0]
+    m0 = oracle.moments(T, c["f"])[0]
+    assert abs(mo[0] / m0[0] - 1) <= 3e-11 and abs(mo[1] / m0[1] - 1) <= 3e-11
+    h.close()
+
+
+def test_cfg2_reaches_maxwell_boltzmann(torch_cuda):
+    """Config 2 run to its stopping rule ||f - f_MB|| / ||f_MB|| < 1e-6 with f_MB = z exp(-E/T) fitted to the
+    conserved number and energy (device run only; the oracle comparison is in the chunk test above)."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    from scipy.optimize import brentq
+    c = kin.config(2)
+    h = kx.Handle(c["p"], c["dp"], c["m"])
+    E, K, hw = h.kinematics_export()
+    f = _dev(torch, c["f"])
+    loss = h.collide_parts(f)[1].cpu().numpy()[0]
+    dt = 0.5 / float((loss / c["f"][0]).max())
+    n0, rho0 = (hw * c["f"][0]).sum(), (hw * E * c["f"][0]).sum()
+
+    def mean_E(Tt):
+        w = hw * np.exp(-(E - E[0]) / Tt)
+        return (w * E).sum() / w.sum() - rho0 / n0
+    Tt = brentq(mean_E, 0.05, 50.0, xtol=1e-14)
+    fmb = np.exp(-E / Tt)
+    fmb *= n0 / (hw * fmb).sum()
+    dist = None
+    for chunk in range(400):
+        h.evolve(f, (chunk * 10 + np.arange(11)) * dt, method=kx.RK4)
+        g = f.cpu().numpy()[0]
+        dist = np.linalg.norm(g - fmb) / np.linalg.norm(fmb)
+        if dist < 1e-6:
+            break
+    assert dist < 1e-6, dist
+    assert (g > 0).all()
+    h.close()
+
+
+def test_cfg5_reduced_freeze_in(torch_cuda, oracle):
+    """Config 5 on a reduced copy (N=64, S=300, B=4): two sources, time-dependent mass (tensor rebuilt at every
+    stage), per-member coupling, rate schedule, projection and diagnostics."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    B, S = 4, 300
+    c = kin.config(5, N=64, B=B)
+    sch = kin.config5_schedule(c["p"], c["dp"], B=B, S=S)
+    f_ref, d_ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.RK4, tau=sch["tau"],
+                                 rate=sch["rate"], mass=sch["mass"], kappa=sch["kappa"], G=sch["G"],
+                                 amp=sch["amp"], want_diag=True)
+    h = kx.Handle(c["p"], c["dp"], c["m"])
+    f = _dev(torch, c["f"])
+    diag = h.evolve(f, sch["tau"], method=kx.RK4, rate=sch["rate"], mass=sch["mass"], kappa=sch["kappa"],
+                    G=_dev(torch, sch["G"]), amp=sch["amp"], want_diag=True).cpu().numpy()
+    got = f.cpu().numpy()
+    assert np.abs(got - f_ref).max() <= 1e-9 * np.abs(f_ref).max()
+    assert np.allclose(diag[:, :, 4:], d_ref[:, :, 4:], rtol=1e-10, atol=0)
+    # exact invariant: every member holds the injected number sum_k amp dtau = (#active steps) * 1e-3
+    hsum = (c["p"] ** 2 * c["dp"] * got).sum(axis=1)
+    injected = (sch["amp"] * np.diff(sch["tau"])[None, :]).sum()
+    assert np.abs(hsum / injected - 1).max() <= 1e-11
+    # warmness <p^2>/<p>^2 per member matches the oracle's moments
+    T = oracle.Tables(c["p"], c["dp"], float(sch["mass"][-1]))
+    mo = h.moments(f).cpu().numpy().T
+    assert np.allclose(mo, oracle.moments(T, f_ref), rtol=1e-9, atol=0)
+    h.close()
+
+
+def test_cfg5_sources_only_and_heun_euler_mass(torch_cuda, oracle):
+    """kappa = 0 switches collisions off: f = sum_k amp dtau G exactly (any method); Euler/Heun with a mass
+    schedule and diagnostics exercise the end-of-step kinematics path."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    B, S = 2, 40
+    c = kin.config(5, N=32, B=B)
+    sch = kin.config5_schedule(c["p"], c["dp"], B=B, S=S)
+    expect = (sch["amp"] * np.diff(sch["tau"])[None, :]).sum(axis=1) @ sch["G"]
+    h = kx.Handle(c["p"], c["dp"], c["m"])
+    G = _dev(torch, sch["G"])
+    for method in ("EULER", "HEUN", "RK4"):
+        f = _dev(torch, c["f"])
+        h.evolve(f, sch["tau"], method=getattr(kx, method), rate=sch["rate"], kappa=np.zeros(B), G=G, amp=sch["amp"])
+        assert np.allclose(f.cpu().numpy(), expect[None, :], rtol=1e-13, atol=0)
+    for method in ("EULER", "HEUN"):
+        f_ref, d_ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=getattr(oracle, method), tau=sch["tau"],
+                                     rate=sch["rate"], mass=sch["mass"], kappa=sch["kappa"], G=sch["G"],
+                                     amp=sch["amp"], want_diag=True)
+        f = _dev(torch, c["f"])
+        diag = h.evolve(f, sch["tau"], method=getattr(kx, method), rate=sch["rate"], mass=sch["mass"],
+                        kappa=sch["kappa"], G=G, amp=sch["amp"], want_diag=True).cpu().numpy()
+        assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-9 * np.abs(f_ref).max()
+        assert np.allclose(diag[:, :, 4:], d_ref[:, :, 4:], rtol=1e-10, atol=0)
+    h.close()
+
+
+def test_nonfinite_is_reported(torch_cuda):
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(1)
+    h = kx.Handle(c["p"], c["dp"], c["m"])
+    f = _dev(torch, c["f"] * 1e200)
+    with pytest.raises(kx.KxError) as ei:
+        h.evolve(f, np.arange(6) * 1e200, method=kx.EULER)
+    assert ei.value.status == 5
+    h.close()

@@ -1,0 +1,247 @@
+"""GPU-vs-oracle parity through the C ABI (libkx) on the seeded inputs of kx_inputs.
+
+Bar (BASELINE.json north_star): max-abs error <= 1e-11 relative to max_i |gain_i| per distribution in fp64;
+integer work (which triples are kept, the bracket index j_L) bit-exact.  The oracle (oracle/) is the CPU
+reference; nothing here feeds a GPU value back into it.
+"""
+import numpy as np
+import pytest
+
+import kx_inputs as kin
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    return torch
+
+
+def _handle(c, **kw):
+    import paper_2607_00755_b200 as kx
+    return kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], **kw)
+
+
+def _dev(torch, a):
+    return torch.tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda")
+
+
+def _relerr(got, ref, gain):
+    """max_i |got-ref| / max_i |gain_i|, per member, worst member."""
+    scale = np.abs(gain).max(axis=1, keepdims=True)
+    return float((np.abs(got - ref) / scale).max())
+
+
+# --------------------------------------------------------------------------------------- a1-a3: builder
+@pytest.mark.parametrize("cfg,N", [(1, None), (2, 96), (3, 72), (4, 80), (5, 64)])
+def test_builder_entry_by_entry(torch_cuda, oracle, cfg, N):
+    c = kin.config(cfg, N=N)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    h = _handle(c)
+    t = h.tensor_export()
+    n_, m_, j_, rp = t["n"], t["m"], t["jL"], t["rowptr"]
+    nn = T.N
+    i_ = np.repeat(np.arange(nn), np.diff(rp))
+    # kinematics
+    E, K, hw = h.kinematics_export()
+    assert np.array_equal(K, T.K) and np.array_equal(E, T.E) and np.array_equal(hw, T.h)
+    # which (i, n<=m) triples are kept: exact
+    kept = T.jL >= 0
+    iu, nu, mu = np.nonzero(kept & (np.arange(nn)[None, :, None] <= np.arange(nn)[None, None, :]))
+    assert len(iu) == len(i_) == h.info()["nnz"]
+    assert np.array_equal(i_, iu) and np.array_equal(n_, nu) and np.array_equal(m_, mu)   # same deterministic order
+    assert (n_ <= m_).all()
+    # bracket index: exact; omega_R and W: rounding level
+    assert np.array_equal(j_, T.jL[i_, n_, m_])
+    assert np.abs(t["omega"] - T.wR[i_, n_, m_]).max() <= 4e-16
+    Wsym = np.where(n_ == m_, T.W[i_, n_, m_], T.W[i_, n_, m_] + T.W[i_, m_, n_])
+    rowmax = np.array([Wsym[rp[i]:rp[i + 1]].max() if rp[i + 1] > rp[i] else 1.0 for i in range(nn)])[i_]
+    tol = 1e-13 if c["m_med"] <= 0 else 2e-12        # mediator: closed form in double vs long double
+    assert (np.abs(t["W"] - Wsym) <= tol * rowmax + 1e-14 * np.abs(Wsym)).all()
+    assert np.median(np.abs(t["W"] - Wsym)[Wsym > 0] / Wsym[Wsym > 0]) < 1e-15
+    h.close()
+
+
+# --------------------------------------------------------------------------------------- a4-a6: operator
+@pytest.mark.parametrize("cfg,N,B,interp", [
+    (1, None, None, 0), (1, None, None, 1),
+    (2, None, None, 0), (2, None, None, 1),
+    (3, 96, 5, 0), (3, 96, 9, 1), (3, 33, 3, 0),
+    (4, 100, 8, 0), (4, 100, 2, 0),
+])
+def test_collide_parity(torch_cuda, oracle, cfg, N, B, interp):
+    torch = torch_cuda
+    c = kin.config(cfg, N=N, B=B)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, c["f"], interp)
+    h = _handle(c, interp=interp)
+    f = _dev(torch, c["f"])
+    g, l = h.collide_parts(f)
+    C = h.collide(f)
+    assert _relerr(g.cpu().numpy(), g0, g0) <= TOL
+    assert _relerr(l.cpu().numpy(), l0, g0) <= TOL
+    assert _relerr(C.cpu().numpy(), C0, g0) <= TOL
+    # typical error is far below the bar
+    assert _relerr(C.cpu().numpy(), C0, g0) <= 2e-13
+    h.close()
+
+
+def test_collide_full_cfg3_all_members(torch_cuda, oracle):
+    """BASELINE config 3 at full size (N=256, B=64, mediator |M|^2), every member, in the bench's launch configuration."""
+    torch = torch_cuda
+    c = kin.config(3)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, c["f"], 0)
+    h = _handle(c)
+    f = _dev(torch, c["f"])
+    o = h.collide_ex(f, flags=0, want=("C", "gain", "loss"))
+    assert _relerr(o["gain"].cpu().numpy(), g0, g0) <= TOL
+    assert _relerr(o["loss"].cpu().numpy(), l0, g0) <= TOL
+    assert _relerr(o["C"].cpu().numpy(), C0, g0) <= TOL
+    # projected
+    Cp0, d0 = oracle.project(T, c["f"], C0)
+    o = h.collide_ex(f, flags=1, want=("C", "diag"))
+    assert _relerr(o["C"].cpu().numpy(), Cp0, g0) <= TOL
+    assert np.allclose(o["diag"].cpu().numpy(), d0, rtol=1e-9, atol=1e-13)
+    # library exp2 gives the same operator
+    h2 = _handle(c, exp_impl=1)
+    assert _relerr(h2.collide(f).cpu().numpy(), C0, g0) <= TOL
+    h.close(); h2.close()
+
+
+@pytest.mark.parametrize("B", [1, 8])
+def test_collide_cfg4_full_size_sampled_rows(torch_cuda, oracle, B):
+    """BASELINE config 4 (N=512): the dense oracle tables are too slow to build, so rows are sampled one by one."""
+    torch = torch_cuda
+    c = kin.config(4, B=B)
+    rows = np.array([0, 1, 2, 31, 32, 100, 255, 256, 300, 400, 480, 509, 510, 511])
+    g0, l0, C0 = oracle.collide_rows(c["p"], c["dp"], c["f"], rows, m=c["m"], M2_0=c["M2_0"], m_med=c["m_med"])
+    h = _handle(c)
+    f = _dev(torch, c["f"])
+    o = h.collide_ex(f, flags=0, want=("C", "gain", "loss"))
+    gmax = np.abs(o["gain"].cpu().numpy()).max(axis=1, keepdims=True)
+    for key, ref in (("gain", g0), ("loss", l0), ("C", C0)):
+        got = o[key].cpu().numpy()[:, rows]
+        assert (np.abs(got - ref) / gmax).max() <= TOL, key
+    # properties that hold at any size: projected operator has vanishing number and energy moments
+    E, K, hw = h.kinematics_export()
+    Cp = h.collide(f, flags=1).cpu().numpy()
+    Craw = o["C"].cpu().numpy()
+    assert (np.abs((hw * Cp).sum(axis=1)) <= 1e-13 * (hw * np.abs(Craw)).sum(axis=1)).all()
+    assert (np.abs((hw * E * Cp).sum(axis=1)) <= 1e-13 * (hw * E * np.abs(Craw)).sum(axis=1)).all()
+    info = h.info()
+    assert 0.6 < info["nnz"] / (512 * 512 * 513 / 2) < 0.7
+    h.close()
+
+
+def test_thermal_fixed_point_on_gpu(torch_cuda):
+    """P5 on the device: C_raw[z exp(-E/T)] vanishes term by term under LOG interpolation."""
+    torch = torch_cuda
+    c = kin.config(3)
+    h = _handle(c)
+    E, K, hw = h.kinematics_export()
+    f = _dev(torch, np.stack([0.37 * np.exp(-E / 0.7), 2.0 * np.exp(-E / 3.0)]))
+    o = h.collide_ex(f, want=("C", "gain"))
+    assert (o["C"].abs().amax(dim=1) <= 3e-13 * o["gain"].abs().amax(dim=1)).all()
+    h.close()
+
+
+# --------------------------------------------------------------------------------------- edge cases
+def test_edge_cases(torch_cuda, oracle):
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    # smallest grid, zeros / floor in f, negative values, ragged batch
+    p = kin.uniform_grid(4, 0.5, 2.0)
+    dp = kin.trapezoid_widths(p)
+    f = np.array([[1.0, 0.5, 0.0, 1e-310], [0.0, 0.0, 0.0, 0.0], [1.0, -0.5, 0.3, 0.2]])
+    T = oracle.Tables(p, dp, 0.3)
+    h = kx.Handle(p, dp, 0.3)
+    for interp in (0, 1):
+        hh = kx.Handle(p, dp, 0.3, interp=interp)
+        g0, l0, C0 = oracle.collide(T, f, interp)
+        C = hh.collide(_dev(torch, f)).cpu().numpy()
+        scale = max(np.abs(g0).max(), 1e-300)
+        assert np.abs(C - C0).max() <= TOL * scale
+        Cp0, d0 = oracle.project(T, f, C0)
+        o = hh.collide_ex(_dev(torch, f), flags=1, want=("C", "diag"))
+        assert np.abs(o["C"].cpu().numpy() - Cp0).max() <= TOL * scale       # includes the f == 0 member (D9)
+        hh.close()
+    # error behaviour
+    fz = _dev(torch, f)
+    with pytest.raises(kx.KxError):
+        h.collide(fz, out=fz)                                 # in place
+    with pytest.raises(ValueError):
+        h.collide(_dev(torch, np.zeros((2, 5))))              # wrong N
+    big = torch.zeros(3 * 4 + 1, dtype=torch.float64, device="cuda")
+    mis = big[1:].view(3, 4)
+    with pytest.raises(kx.KxError):
+        h.collide(mis)                                        # misaligned pointer
+    for bad in (dict(p=p[::-1].copy(), dp=dp), dict(p=p, dp=-dp), dict(p=p[:3], dp=dp[:3])):
+        with pytest.raises(kx.KxError):
+            kx.Handle(bad["p"], bad["dp"], 0.3)
+    with pytest.raises(kx.KxError):
+        kx.Handle(p, dp, 0.3, f_floor=0.0)
+    h.close()
+
+
+def test_host_buffer_call(torch_cuda, oracle):
+    torch = torch_cuda
+    c = kin.config(3, N=64, B=4)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, c["f"], 0)
+    h = _handle(c)
+    fh = torch.tensor(c["f"]).pin_memory()
+    Ch = torch.empty_like(fh).pin_memory()
+    h.collide_host(fh, Ch)
+    assert _relerr(Ch.numpy(), C0, g0) <= TOL
+    Cn = np.empty_like(c["f"])
+    h.collide_host(c["f"], Cn)                                # pageable numpy buffers work too
+    assert np.array_equal(Cn, Ch.numpy())
+    h.close()
+
+
+def test_bitwise_reproducible(torch_cuda):
+    torch = torch_cuda
+    c = kin.config(3, N=128, B=16)
+    h = _handle(c)
+    f = _dev(torch, c["f"])
+    a = h.collide(f, flags=1).clone()
+    for _ in range(3):
+        assert torch.equal(h.collide(f, flags=1), a)
+    h2 = _handle(c)
+    assert torch.equal(h2.collide(f, flags=1), a)
+    # a member's result does not depend on its batch neighbours
+    assert torch.equal(h.collide(f[3:4].contiguous(), flags=1)[0], a[3])
+    h.close(); h2.close()
+
+
+# --------------------------------------------------------------------------------------- a7, a9
+@pytest.mark.parametrize("m", [1.0, 1000.0])
+def test_projection_and_moments_parity(torch_cuda, oracle, m):
+    torch = torch_cuda
+    c = kin.config(5, N=96, B=3)
+    p, dp = c["p"], c["dp"]
+    f = np.stack([kin.bimodal(p, (3.0, 30.0), (1.0, 3.0)), kin.bimodal(p, (1.0, 8.0), (0.5, 2.0)),
+                  kin.two_bump_eq51(p)])
+    T = oracle.Tables(p, dp, m)
+    g0, l0, C0 = oracle.collide(T, f, 0)
+    Cp0, d0 = oracle.project(T, f, C0)
+    import paper_2607_00755_b200 as kx
+    h = kx.Handle(p, dp, m)
+    o = h.collide_ex(_dev(torch, f), flags=1)
+    assert _relerr(o["C"].cpu().numpy(), Cp0, g0) <= TOL
+    assert np.allclose(o["diag"].cpu().numpy(), d0, rtol=1e-8, atol=1e-13)
+    mo = h.moments(_dev(torch, f)).cpu().numpy().T
+    assert np.allclose(mo, oracle.moments(T, f), rtol=1e-13, atol=0)
+    # kx_set_mass: rebuilding for another mass equals a fresh build
+    h.set_mass(2.5)
+    T2 = oracle.Tables(p, dp, 2.5)
+    g2, l2, C2 = oracle.collide(T2, f, 0)
+    assert _relerr(h.collide(_dev(torch, f)).cpu().numpy(), C2, g2) <= TOL
+    assert h.info()["nnz"] == int(((T2.jL >= 0) & (np.arange(96)[None, :, None] <= np.arange(96)[None, None, :])).sum())
+    h.close()

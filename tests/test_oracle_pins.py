@@ -351,3 +351,16 @@ def test_evolve_convergence_order_and_rate_scaling(oracle):
                       mass=np.full(9, c["m"]))
     e = run(oracle.HEUN, 4)
     assert np.array_equal(d, e)
+
+
+# ------------------------------------------------------------------ row-sampled evaluator = full evaluator
+@pytest.mark.parametrize("cfg,interp", [(1, 0), (3, 0), (3, 1)])
+def test_collide_rows_equals_full_tables(oracle, cfg, interp):
+    """okx_collide_rows (used to sample N=512) walks the same triples as the dense-table path: identical results."""
+    c = kin.config(cfg, N=40 if cfg == 3 else None, B=3 if cfg == 3 else None)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g, l, C = oracle.collide(T, c["f"], interp)
+    rows = np.array([0, 1, 7, T.N // 2, T.N - 2, T.N - 1])
+    gr, lr, Cr = oracle.collide_rows(c["p"], c["dp"], c["f"], rows, m=c["m"], g_chi=c["g_chi"], M2_0=c["M2_0"],
+                                     m_med=c["m_med"], interp=interp)
+    assert np.array_equal(gr, g[:, rows]) and np.array_equal(lr, l[:, rows]) and np.array_equal(Cr, C[:, rows])
