@@ -51,7 +51,12 @@ typedef enum {
 #define KX_INTERP_LOG     0   /* eq. B.20 at eta=0: f_j~ = exp(w_L y_L + w_R y_R), y = ln max(f, f_floor) (default) */
 #define KX_INTERP_LINEAR  1   /* f_j~ = w_L f_L + w_R f_R (operator exactly bilinear) */
 /* storage of the kernel tensor */
-#define KX_STORE_SYM_ROWS 0   /* symmetry-reduced (n<=m, W_inm+W_imn), structural zeros dropped, row-compressed */
+#define KX_STORE_SYM_ROWS 0   /* symmetry-reduced (n<=m, W_inm+W_imn), structural zeros dropped, row-compressed;
+                                 evaluated by the streaming kernel, one exp per (entry, member) in LOG mode */
+#define KX_STORE_TILED    1   /* default: SYM_ROWS plus the 16-row tiled operand of the FP64 tensor-core (DMMA)
+                                 contraction: gain as (n<=m) x members GEMM, LOG loss through the Chebyshev moments
+                                 of each (i, bracket) bucket; members with a bracket whose
+                                 interpolation error bound exceeds 1e-15 max f fall back to the streaming kernel */
 /* precision */
 #define KX_FP64 0
 #define KX_FP32 1             /* not implemented: KX_ERR_UNSUPPORTED */
@@ -72,12 +77,14 @@ typedef struct { int32_t n; const double* p; const double* dp; } kx_grid_t;
 typedef struct { double m; double g_chi; } kx_species_t;
 /* |M|^2 = M2_0 (m_med <= 0: contact, eq. B.17) or M2_0 / (1 + (-t)/m_med^2)^2, t = (p_i-p_n)^2 (reading D5) */
 typedef struct { double M2_0; double m_med; } kx_msq_t;
-/* Options; pass NULL for the defaults {LOG, SYM_ROWS, FP64, EXP_TABLE, 1e-300, 1e-12} */
+/* Options; pass NULL for the defaults {LOG, TILED, FP64, EXP_TABLE, 0, 0, 1e-300, 1e-12} */
 typedef struct {
     int32_t interp;      /* KX_INTERP_*  */
     int32_t storage;     /* KX_STORE_*   */
     int32_t precision;   /* KX_FP64      */
     int32_t exp_impl;    /* KX_EXP_*     */
+    int32_t loss_nodes;  /* KX_STORE_TILED + LOG: Chebyshev nodes per bracket, 8|16|24|32; 0 = default (24) */
+    int32_t reserved;    /* must be 0 */
     double  f_floor;     /* y = ln max(f, f_floor), reading D8; must be >= 1e-300 and > 0 */
     double  eps_supp;    /* support threshold of eq. C.4, reading D9 */
 } kx_opts_t;
@@ -140,7 +147,8 @@ typedef struct {
 kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
                       const kx_evolve_t* ctl, void* stream);
 
-/* Number of stored (i, n<=m) entries, bytes of tensor data one kx_collide streams, grid size.
+/* Number of stored (i, n<=m) entries, bytes of tensor data one kx_collide streams (the tiled operand when
+ * it is in use, else 20 bytes per entry), grid size.
  * Synchronises the device.  Any output pointer may be NULL. */
 kx_status_t kx_info(kx_handle_t h, int64_t* nnz, int64_t* tensor_bytes, int32_t* n);
 

@@ -44,12 +44,63 @@ kx_status_t alloc_tensor(kx_handle_s* h, long long cap)
     return KX_OK;
 }
 
+void free_tiled(kx_handle_s* h)
+{
+    cudaFree(h->t.A); cudaFree(h->t.desc);
+    h->t.A = nullptr; h->t.desc = nullptr;
+    h->cap_groups = 0; h->tiled_ok = false;
+}
+
+kx_status_t alloc_tiled(kx_handle_s* h, long long groups)
+{
+    free_tiled(h);
+    if (groups < 1) groups = 1;
+    KX_CUDA(dalloc(&h->t.A, (size_t)groups * KX_GROUP_DBL));
+    KX_CUDA(dalloc(&h->t.desc, (size_t)groups * 4));
+    h->cap_groups = groups;
+    return KX_OK;
+}
+
+// upper bound of the groups of the tiled storage for ANY mass: every (n <= m) pair in every tile
+inline long long tiled_groups_bound(const kx_handle_s* h)
+{
+    const long long N = h->d.N, NT = h->t.NT;
+    const long long quads_per_tile = (N * (N + 1) / 2 + 3) / 4 + N;     // each run rounds up by < 1 quad
+    return NT * ((quads_per_tile + 3) / 4 + h->t.LG);
+}
+
+// a2-a3 in the tiled layout for the current kinematics (the run table of kx_launch_runs must be current)
+kx_status_t build_tiled(kx_handle_s* h, cudaStream_t s, bool may_sync)
+{
+    KX_CUDA(kx_launch_tile_runs(h->d, h->t, s));
+    if (may_sync) {
+        unsigned g = 0;
+        KX_CUDA(cudaMemcpyAsync(&g, h->t.vtptr + 2 * h->t.NT, 4, cudaMemcpyDeviceToHost, s));
+        KX_CUDA(cudaStreamSynchronize(s));
+        h->groups = g;
+        if (h->cap_groups < (long long)g) {
+            kx_status_t rc = alloc_tiled(h, g);
+            if (rc != KX_OK) return rc;
+        }
+    } else if (h->cap_groups < tiled_groups_bound(h)) {
+        h->err = "internal: tiled capacity too small for an asynchronous rebuild";
+        return KX_ERR_ALLOC;
+    }
+    const long long used = may_sync ? h->groups : h->cap_groups;
+    KX_CUDA(cudaMemsetAsync(h->t.A, 0, (size_t)used * KX_GROUP_DBL * 8, s));
+    KX_CUDA(kx_launch_tile_fill(h->d, h->t, s));
+    h->tiled_ok = true;
+    return KX_OK;
+}
+
 void free_ws(kx_handle_s* h)
 {
     cudaFree(h->yd); cudaFree(h->part); cudaFree(h->fstage); cudaFree(h->k1); cudaFree(h->k2);
     cudaFree(h->k3); cudaFree(h->Cbuf); cudaFree(h->hostio);
+    cudaFree(h->XT); cudaFree(h->fmax); cudaFree(h->mflag); cudaFree(h->tpart);
     h->yd = h->part = h->fstage = h->k1 = h->k2 = h->k3 = h->Cbuf = h->hostio = nullptr;
-    h->wsB = 0; h->ws_tasks = 0;
+    h->XT = h->fmax = h->tpart = nullptr; h->mflag = nullptr;
+    h->wsB = 0; h->ws_tasks = 0; h->ws_xstride = 0; h->tslots = 0;
 }
 
 // the smallest chunk is 1024 entries, so a row of len entries has at most len/1024+1 tasks
@@ -70,6 +121,16 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
     KX_CUDA(dalloc(&h->k3, bn));
     KX_CUDA(dalloc(&h->Cbuf, bn + (size_t)nB));   // + kappa[B]
     KX_CUDA(dalloc(&h->hostio, bn * 2));
+    if (h->storage == KX_STORE_TILED) {
+        const int xs = kx_xstride(nB);
+        const long long slots = (long long)h->sm_count + 2 * h->t.NT + 1;
+        KX_CUDA(dalloc(&h->XT, (size_t)h->t.xrows * xs));
+        KX_CUDA(cudaMemset(h->XT, 0, (size_t)h->t.xrows * xs * 8));      // padding rows stay zero for good
+        KX_CUDA(dalloc(&h->fmax, (size_t)nB));
+        KX_CUDA(dalloc(&h->mflag, (size_t)nB));
+        KX_CUDA(dalloc(&h->tpart, (size_t)slots * xs * 16));
+        h->ws_xstride = xs; h->tslots = slots;
+    }
     h->wsB = nB; h->ws_tasks = need_tasks;
     return KX_OK;
 }
@@ -101,6 +162,57 @@ kx_status_t rebuild(kx_handle_s* h, double m, cudaStream_t s)
     KX_CUDA(kx_launch_fill(h->d, s));
     h->nnz_stale = true;
     h->chunk_for_B = 0;
+    h->tiled_ok = false;
+    return KX_OK;
+}
+
+// the tiled operand is rebuilt lazily: kx_set_mass and mass schedules only refresh the streaming storage
+kx_status_t ensure_tiled(kx_handle_s* h, cudaStream_t s)
+{
+    if (h->storage != KX_STORE_TILED || h->tiled_ok) return KX_OK;
+    return build_tiled(h, s, true);
+}
+
+// one evaluation of a4-a5 into the partial buffers; returns through *st the fields the finishing kernel needs
+kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bool use_tiled, KxStage* st,
+                        cudaStream_t s)
+{
+    auto prof_begin = [&]() -> kx_status_t {
+        if (!h->profiling) return KX_OK;
+        if (h->prof_used == h->prof_events.size()) {
+            cudaEvent_t a, b;
+            KX_CUDA(cudaEventCreate(&a));
+            KX_CUDA(cudaEventCreate(&b));
+            h->prof_events.emplace_back(a, b);
+        }
+        KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].first, s));
+        return KX_OK;
+    };
+    auto prof_end = [&]() -> kx_status_t {
+        if (!h->profiling) return KX_OK;
+        KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].second, s));
+        h->prof_used++;
+        return KX_OK;
+    };
+    kx_status_t rc;
+    if (use_tiled) {
+        const int xs = h->ws_xstride;
+        const int G = kx_dmma_ctas(h->sm_count, h->groups);
+        KX_CUDA(kx_launch_xt(h->d, h->t, f, h->yd, h->XT, xs, h->fmax, h->mflag, B, s));
+        if ((rc = prof_begin()) != KX_OK) return rc;
+        KX_CUDA(kx_launch_dmma(h->d, h->t, G, h->XT, xs, h->tpart, B, s));
+        if ((rc = prof_end()) != KX_OK) return rc;
+        if (h->d.interp == KX_INTERP_LOG)      // exact streaming path for flagged members only (LINEAR is exact)
+            KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, h->mflag, s));
+        st->tpart = h->tpart; st->vtptr = h->t.vtptr; st->mflag = h->d.interp == KX_INTERP_LOG ? h->mflag : nullptr;
+        st->NT = h->t.NT; st->nctas = G; st->xstride = xs;
+    } else {
+        if (!have_yd) KX_CUDA(kx_launch_prep(h->d, f, h->yd, B, s));
+        if ((rc = prof_begin()) != KX_OK) return rc;
+        KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, nullptr, s));
+        if ((rc = prof_end()) != KX_OK) return rc;
+        st->tpart = nullptr; st->vtptr = nullptr; st->mflag = nullptr;
+    }
     return KX_OK;
 }
 
@@ -119,22 +231,9 @@ kx_status_t collide_impl(kx_handle_s* h, const double* f, double* C, double* gai
     if (C == f) { h->err = "in-place kx_collide (C == f) is not allowed"; return KX_ERR_INVALID_ARG; }
     if ((rc = ensure_ws(h, B)) != KX_OK) return rc;
     if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
-    KX_CUDA(kx_launch_prep(h->d, f, h->yd, B, s));
-    if (h->profiling) {
-        if (h->prof_used == h->prof_events.size()) {
-            cudaEvent_t a, b;
-            KX_CUDA(cudaEventCreate(&a));
-            KX_CUDA(cudaEventCreate(&b));
-            h->prof_events.emplace_back(a, b);
-        }
-        KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].first, s));
-    }
-    KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, s));
-    if (h->profiling) {
-        KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].second, s));
-        h->prof_used++;
-    }
+    if ((rc = ensure_tiled(h, s)) != KX_OK) return rc;
     KxStage st = {};
+    if ((rc = launch_eval(h, f, B, false, h->storage == KX_STORE_TILED, &st, s)) != KX_OK) return rc;
     st.flags = flags & KX_PROJECT;
     st.C = C; st.gain = gain; st.loss = loss; st.diag = diag; st.diag_stride = 4;
     st.evolve = 0;
@@ -156,8 +255,10 @@ void kx_destroy(kx_handle_t h)
     {
         DeviceGuard g(h->device);
         free_tensor(h);
+        free_tiled(h);
         free_ws(h);
         cudaFree(h->dev_blob);
+        cudaFree(h->tiled_blob);
         for (auto& ev : h->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     }
     delete h;
@@ -179,10 +280,15 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     }
     if (!(sp->m >= 0.0) || !(sp->g_chi > 0.0) || !isfinite(sp->m)) { g_build_err = "need m >= 0 and g_chi > 0"; return KX_ERR_INVALID_ARG; }
     if (!isfinite(msq->M2_0) || !isfinite(msq->m_med)) { g_build_err = "non-finite |M|^2 parameters"; return KX_ERR_INVALID_ARG; }
-    kx_opts_t o = {KX_INTERP_LOG, KX_STORE_SYM_ROWS, KX_FP64, KX_EXP_TABLE, 1e-300, 1e-12};
+    kx_opts_t o = {KX_INTERP_LOG, KX_STORE_TILED, KX_FP64, KX_EXP_TABLE, 0, 0, 1e-300, 1e-12};
     if (opts) o = *opts;
+    if (o.loss_nodes == 0) o.loss_nodes = 24;
     if (o.precision != KX_FP64) { g_build_err = "fp32 mode is not implemented"; return KX_ERR_UNSUPPORTED; }
-    if (o.storage != KX_STORE_SYM_ROWS) { g_build_err = "unknown storage mode"; return KX_ERR_UNSUPPORTED; }
+    if (o.storage != KX_STORE_SYM_ROWS && o.storage != KX_STORE_TILED) { g_build_err = "unknown storage mode"; return KX_ERR_UNSUPPORTED; }
+    if (o.loss_nodes != 8 && o.loss_nodes != 16 && o.loss_nodes != 24 && o.loss_nodes != 32) {
+        g_build_err = "loss_nodes must be 0 (default 24), 8, 16, 24 or 32";
+        return KX_ERR_INVALID_ARG;
+    }
     if (o.interp != KX_INTERP_LOG && o.interp != KX_INTERP_LINEAR) { g_build_err = "unknown interpolation"; return KX_ERR_INVALID_ARG; }
     if (o.exp_impl != KX_EXP_TABLE && o.exp_impl != KX_EXP_LIBM) { g_build_err = "unknown exp_impl"; return KX_ERR_INVALID_ARG; }
     if (!(o.f_floor >= 1e-300) || !(o.eps_supp >= 0.0)) { g_build_err = "need f_floor >= 1e-300 and eps_supp >= 0"; return KX_ERR_INVALID_ARG; }
@@ -205,8 +311,10 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     h->device = device;
     h->sm_count = prop.multiProcessorCount;
     h->nnz_stale = true;
+    h->storage = o.storage;
     KxDev& d = h->d;
     d = KxDev{};
+    h->t = KxTiled{};
     d.N = N; d.interp = o.interp; d.exp_impl = o.exp_impl; d.chunk = 0;
     d.m = sp->m; d.g_chi = sp->g_chi; d.M2_0 = msq->M2_0; d.m_med = msq->m_med;
     d.f_floor = o.f_floor; d.eps_supp = o.eps_supp;
@@ -254,6 +362,44 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         KX_CUDA(kx_launch_fill(d, s));
         KX_CUDA(cudaStreamSynchronize(s));
         h->nnz = nnz; h->nnz_stale = false; h->chunk_for_B = 0;
+        if (h->storage == KX_STORE_TILED) {
+            KxTiled& t = h->t;
+            t.NT = (N + KX_TI - 1) / KX_TI;
+            t.Q = d.interp == KX_INTERP_LOG ? o.loss_nodes : 2;
+            t.LQ = ((N - 1) * t.Q + 3) / 4;
+            t.LG = (t.LQ + 3) / 4;
+            t.ones_row = N;
+            t.loss_row0 = N + 1;
+            t.xrows = t.loss_row0 + 16 * t.LG;
+            // small tables: trun_mlo, trun_q [NT*N], trun_off [NT*(N+1)], vtptr [2NT+1], dct [Q*Q], nodes [Q]
+            const size_t tn = (size_t)t.NT * N;
+            const size_t ints = tn * 2 + (size_t)t.NT * (N + 1) + (size_t)(2 * t.NT + 1);
+            const size_t ints_pad = (ints + 1) & ~(size_t)1;
+            KX_CUDA(cudaMalloc(&h->tiled_blob, ints_pad * 4 + ((size_t)t.Q * t.Q + t.Q) * 8));
+            int* tp = (int*)h->tiled_blob;
+            t.trun_mlo = tp;                 tp += tn;
+            t.trun_q = (unsigned*)tp;        tp += tn;
+            t.trun_off = (unsigned*)tp;      tp += (size_t)t.NT * (N + 1);
+            t.vtptr = (unsigned*)tp;
+            double* dd = (double*)((int*)h->tiled_blob + ints_pad);
+            t.dct = dd; t.nodes = dd + (size_t)t.Q * t.Q;
+            // constants of the discrete Chebyshev transform (not data dependent), in long double
+            const int Q = t.Q;
+            std::vector<double> tab((size_t)Q * Q + Q);
+            const long double pi = 3.14159265358979323846264338327950288L;
+            for (int c = 0; c < Q; ++c)
+                for (int q = 0; q < Q; ++q)
+                    tab[(size_t)c * Q + q] = (double)((c == 0 ? 1.0L : 2.0L) / Q * cosl(c * (2 * q + 1) * pi / (2 * Q)));
+            for (int q = 0; q < Q; ++q) tab[(size_t)Q * Q + q] = (double)(0.5L * (1.0L + cosl((2 * q + 1) * pi / (2 * Q))));
+            long double lf = 1.0L;           // log2(2 / Q!)
+            for (int k = 2; k <= Q; ++k) lf -= log2l((long double)k);
+            t.flag_log2 = (double)lf;
+            KX_CUDA(cudaMemcpyAsync(dd, tab.data(), tab.size() * 8, cudaMemcpyHostToDevice, s));
+            KX_CUDA(cudaStreamSynchronize(s));
+            kx_status_t rc2 = build_tiled(h, s, true);
+            if (rc2 != KX_OK) return rc2;
+            KX_CUDA(cudaStreamSynchronize(s));
+        }
         return KX_OK;
     };
     kx_status_t rc = body();
@@ -359,6 +505,10 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
     double kin_mass = h->d.m;        // mass of the kinematics arrays on the device
     double ten_mass = h->d.m;        // mass the tensor was built for
     bool have_yd = false;            // yd already holds the current stage input (written by the last finish)
+    // a static tensor is evaluated through the tiled (DMMA) operand; with a mass schedule every stage has new
+    // kinematics, and re-deriving the Chebyshev moments per stage costs more than the exact streaming path
+    const bool use_tiled = h->storage == KX_STORE_TILED && !ctl->mass;
+    if (use_tiled && (rc = ensure_tiled(h, s)) != KX_OK) return rc;
 
     for (int k = 0; k < S; ++k) {
         const double dt = ctl->tau[k + 1] - ctl->tau[k];
@@ -378,9 +528,8 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
             }
             if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
             const double* fin = stg == 0 ? f : h->fstage;
-            if (!have_yd) KX_CUDA(kx_launch_prep(h->d, fin, h->yd, B, s));
-            KX_CUDA(kx_launch_contract(h->d, h->sm_count, fin, h->yd, h->part, B, s));
             KxStage st = {};
+            if ((rc = launch_eval(h, fin, B, have_yd, use_tiled, &st, s)) != KX_OK) return rc;
             st.flags = ctl->flags & KX_PROJECT;
             st.diag = (diag && stg == 0) ? ctl->diag + (size_t)k * B * 6 : nullptr;
             st.diag_stride = 6;
@@ -389,9 +538,9 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
             st.nsrc = nsrc; st.G = nsrc ? src->G : nullptr;
             for (int q = 0; q < nsrc; ++q) st.amp[q] = src->amp[(size_t)q * S + k];
             st.f = f; st.fstage = h->fstage; st.k1 = h->k1; st.k2 = h->k2; st.k3 = h->k3;
-            st.ydnext = h->yd; st.flag = h->flag;
+            st.ydnext = use_tiled ? nullptr : h->yd; st.flag = h->flag;
             KX_CUDA(kx_launch_finish(h->d, fin, h->part, B, st, s));
-            have_yd = true;
+            have_yd = !use_tiled;
         }
         if (diag) {
             if (ctl->mass) {
@@ -447,7 +596,10 @@ kx_status_t kx_info(kx_handle_t h, int64_t* nnz, int64_t* tensor_bytes, int32_t*
         h->nnz = v; h->nnz_stale = false;
     }
     if (nnz) *nnz = h->nnz;
-    if (tensor_bytes) *tensor_bytes = h->nnz * 20;   // W 8 + omega 8 + n|m|j 4
+    if (tensor_bytes) {
+        if (h->storage == KX_STORE_TILED && h->tiled_ok) *tensor_bytes = h->groups * (KX_GROUP_DBL * 8 + 16);
+        else *tensor_bytes = h->nnz * 20;            // W 8 + omega 8 + n|m|j 4
+    }
     if (n) *n = h->d.N;
     return KX_OK;
 }

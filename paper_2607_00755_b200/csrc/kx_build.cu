@@ -15,18 +15,11 @@
 //
 // Compiled with --fmad=false: validity decisions and omega must not depend on FMA contraction.
 #include "kx_internal.cuh"
-#include <float.h>
+#include "kx_entry.cuh"
 
 namespace {
 
-constexpr double kPi = 3.14159265358979323846;
-
-// ---------------------------------------------------------------- a1
-__device__ __forceinline__ void kin_point(double p, double m, double& E, double& K)
-{
-    E = sqrt(p * p + m * m);
-    K = (p * p) / (E + m);
-}
+using namespace kxe;
 
 __global__ void k_kinematics(KxDev d, double m)
 {
@@ -46,20 +39,6 @@ __global__ void k_kinematics(KxDev d, double m)
     } else {
         d.invdK[i] = 0.0;
     }
-}
-
-// ---------------------------------------------------------------- a2: validity (reading D4)
-// tau = 32 eps (K_n+K_m+K_i); a triple is kept iff K_0 - tau <= K~ <= K_{N-1} + tau, and K~ is then
-// clamped into [K_0, K_{N-1}].
-__device__ __forceinline__ bool keep_lo(double Kn, double Km, double Ki, double K0)
-{
-    double S = Kn + Km, Kt = S - Ki, tau = (32.0 * DBL_EPSILON) * (S + Ki);
-    return Kt >= K0 - tau;
-}
-__device__ __forceinline__ bool keep_hi(double Kn, double Km, double Ki, double KN1)
-{
-    double S = Kn + Km, Kt = S - Ki, tau = (32.0 * DBL_EPSILON) * (S + Ki);
-    return Kt <= KN1 + tau;
 }
 
 // one thread per (i,n): the interval of kept m in [n, N)
@@ -128,42 +107,6 @@ __global__ void __launch_bounds__(1024) k_scan_runs(KxDev d)
     for (int i = t; i <= d.N; i += 1024) d.rowptr[i] = d.run_off[i * d.N];
 }
 
-// ---------------------------------------------------------------- a3: J = int_{Q-}^{Q+} |M|^2 dQ
-// contact: M2_0 (Q+ - Q-)                                                eq. B.17
-// mediator (reading D5): M2_0 m_med^4 int dQ/(Q^2+c2)^2, c2 = m_med^2 - (K_i-K_n)^2.  The difference of
-// the antiderivative Q/(2c2(Q^2+c2)) + atan(Q/c)/(2c^3) between a=Q- and b=Q+ is combined analytically
-// (no subtraction of two large terms); a series in c2 covers |c2| << a^2.
-__device__ double kx_J(double a, double b, double dK, double M2_0, double m_med)
-{
-    if (!(b > a)) return 0.0;
-    double d = b - a;
-    if (m_med <= 0.0) return M2_0 * d;
-    double mm = m_med * m_med;
-    double c2 = mm - dK * dK;
-    double ab = a * b;
-    double val;
-    if (fabs(c2) <= 0.05 * (a * a)) {
-        // 1/(Q^2+c2)^2 = sum_k (k+1) (-c2)^k Q^(-2k-4);  |c2|/a^2 <= 0.05: 14 terms reach 1e-17
-        double u = 1.0 / (a * a), v = 1.0 / (b * b);
-        double ta = u / a, tb = v / b, pw = 1.0;
-        val = 0.0;
-#pragma unroll 1
-        for (int k = 0; k < 14; ++k) {
-            val += pw * (double)(k + 1) * (ta - tb) / (double)(2 * k + 3);
-            pw *= -c2; ta *= u; tb *= v;
-        }
-    } else if (c2 > 0.0) {
-        double c = sqrt(c2);
-        val = d * (c2 - ab) / (2.0 * c2 * (a * a + c2) * (b * b + c2))
-            + atan2(c * d, c2 + ab) / (2.0 * c2 * c);
-    } else {
-        double k2 = -c2, k = sqrt(k2);
-        val = d * (ab + k2) / (2.0 * k2 * ((a - k) * (a + k)) * ((b - k) * (b + k)))
-            + log1p(-2.0 * k * d / ((b - k) * (a + k))) / (4.0 * k2 * k);
-    }
-    return M2_0 * (mm * mm) * val;
-}
-
 // one warp per run (i,n); lanes over m.  Writes W (symmetrised), omega_R and n|m<<10|jL<<20.
 __global__ void __launch_bounds__(256) k_fill(KxDev d)
 {
@@ -184,21 +127,10 @@ __global__ void __launch_bounds__(256) k_fill(KxDev d)
         const double pref_in = d.arow[i] * d.ccol[n];
         for (int k = lane; k < len; k += 32) {
             const int m = mlo + k;
-            const double Km = K[m], pm = P[m];
-            double Kt = (Kn + Km) - Ki;
-            Kt = fmin(fmax(Kt, K0), KN1);                 // D4: the kept triple's K~ snapped into the domain
-            const double pj = sqrt(Kt * (Kt + 2.0 * d.m)); // eq. 4.4
-            // eq. B.15-B.16
-            double J = kx_J(fmax(fabs(pi_ - pn), fabs(pm - pj)), fmin(pi_ + pn, pm + pj), Ki - Kn, d.M2_0, d.m_med);
-            if (m != n)   // the (i,m,n) ordering: second half of the symmetrised entry
-                J += kx_J(fmax(fabs(pi_ - pm), fabs(pn - pj)), fmin(pi_ + pm, pn + pj), Ki - Km, d.M2_0, d.m_med);
-            const double W = pref_in * d.ccol[m] * J;
-            // bracket: largest j in [0, N-2] with K_j <= K~
-            int lo = 0, hi = N - 2;
-            while (lo < hi) {
-                int mid = (lo + hi + 1) >> 1;
-                if (K[mid] <= Kt) lo = mid; else hi = mid - 1;
-            }
+            const double Km = K[m];
+            const double Kt = kx_Kt(Kn, Km, Ki, K0, KN1);       // D4: the kept triple's K~ snapped into the domain
+            const double W = kx_Wsym(d, P, n, m, pi_, pn, Ki, Kn, Km, Kt, pref_in);
+            const int lo = kx_bracket(K, N, Kt);
             const double om = (Kt - K[lo]) / (K[lo + 1] - K[lo]);   // eq. B.19
             const size_t e = (size_t)off + k;
             d.W[e] = W;

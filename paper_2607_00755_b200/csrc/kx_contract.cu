@@ -66,7 +66,7 @@ enum { MODE_LOG_TAB = 0, MODE_LOG_LIBM = 1, MODE_LINEAR = 2 };
 template <int BT, int MODE>
 __global__ void __launch_bounds__(KX_CTA, 2)
 k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd,
-           double* __restrict__ part, int B)
+           double* __restrict__ part, int B, const int* __restrict__ mflag)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = d.N;
@@ -79,6 +79,11 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int b0 = blockIdx.y * BT;
     const int nb = min(BT, B - b0);
+    if (mflag) {          // tiled path: only member groups holding a flagged member take the exact streaming path
+        int any = 0;
+        for (int b = 0; b < nb; ++b) any |= mflag[b0 + b];
+        if (!any) return;
+    }
 
     for (int k = tid; k < BT * N; k += KX_CTA) {
         int b = k / N, j = k - b * N;
@@ -213,6 +218,7 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
     __shared__ double s_y[KX_MAX_N];
     const int N = d.N, tid = threadIdx.x, b = blockIdx.x;
     const double* fb = fin + (size_t)b * N;
+    const bool tiled = st.tpart != nullptr && !(st.mflag && st.mflag[b]);
 
     double C[kMaxPerThread], fi[kMaxPerThread], hi_[kMaxPerThread], Ei[kMaxPerThread], Ki[kMaxPerThread];
 #pragma unroll
@@ -220,11 +226,31 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
         const int i = tid + q * KX_CTA;
         C[q] = 0.0; fi[q] = 0.0; hi_[q] = 0.0; Ei[q] = 0.0; Ki[q] = 0.0;
         if (i < N) {
-            const unsigned t0 = d.taskptr[i], t1 = d.taskptr[i + 1];
             double g = 0.0, nu = 0.0;
-            for (unsigned t = t0; t < t1; ++t) {
-                g += part[((size_t)t * B + b) * 2];
-                nu += part[((size_t)t * B + b) * 2 + 1];
+            if (tiled) {
+                // partials of the DMMA kernel: virtual tiles 2t (gain) and 2t+1 (nu); the CTAs whose group range
+                // meets a virtual tile are c(first group)..c(last group), slot = c + vt, added in slot order
+                const unsigned Gtot = st.vtptr[2 * st.NT];
+                const int tile = i >> 4, il = i & 15;
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+                    const int vt = 2 * tile + half;
+                    const unsigned a0 = st.vtptr[vt], a1 = st.vtptr[vt + 1];
+                    double acc = 0.0;
+                    if (a1 > a0) {
+                        const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.nctas - 1ull) / Gtot);
+                        const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.nctas - 1ull) / Gtot);
+                        for (unsigned c = c0; c <= c1; ++c)
+                            acc += st.tpart[((size_t)(c + vt) * st.xstride + b) * 16 + il];
+                    }
+                    if (half == 0) g = acc; else nu = acc;
+                }
+            } else {
+                const unsigned t0 = d.taskptr[i], t1 = d.taskptr[i + 1];
+                for (unsigned t = t0; t < t1; ++t) {
+                    g += part[((size_t)t * B + b) * 2];
+                    nu += part[((size_t)t * B + b) * 2 + 1];
+                }
             }
             fi[q] = fb[i];
             C[q] = fma(-fi[q], nu, g);                            // a6
@@ -367,7 +393,7 @@ k_moments(KxDev d, const double* __restrict__ f, double* n, double* rho, double*
 
 template <int BT, int MODE>
 cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, const double* yd,
-                              double* part, int B, cudaStream_t s)
+                              double* part, int B, const int* mflag, cudaStream_t s)
 {
     const int N = d.N;
     size_t smem = (size_t)BT * N * 24 + (size_t)(KX_CTA / 32) * 2 * BT * 8
@@ -382,17 +408,17 @@ cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, con
     int gx = (sm_count * occ + groups - 1) / groups;
     if (gx < 1) gx = 1;
     dim3 grid(gx, groups);
-    k_contract<BT, MODE><<<grid, KX_CTA, smem, s>>>(d, f, reinterpret_cast<const double2*>(yd), part, B);
+    k_contract<BT, MODE><<<grid, KX_CTA, smem, s>>>(d, f, reinterpret_cast<const double2*>(yd), part, B, mflag);
     return cudaGetLastError();
 }
 
 template <int BT>
 cudaError_t launch_contract_m(const KxDev& d, int sm_count, const double* f, const double* yd,
-                              double* part, int B, cudaStream_t s)
+                              double* part, int B, const int* mflag, cudaStream_t s)
 {
-    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, s);
-    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, s);
-    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, s);
+    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, mflag, s);
+    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, mflag, s);
+    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, mflag, s);
 }
 
 }  // namespace
@@ -424,13 +450,13 @@ cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, c
 }
 
 cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
-                               double* part, int B, cudaStream_t s)
+                               double* part, int B, const int* mflag, cudaStream_t s)
 {
     switch (kx_pick_bt(d.N, B)) {
-        case 1: return launch_contract_m<1>(d, sm_count, f, yd, part, B, s);
-        case 2: return launch_contract_m<2>(d, sm_count, f, yd, part, B, s);
-        case 4: return launch_contract_m<4>(d, sm_count, f, yd, part, B, s);
-        default: return launch_contract_m<8>(d, sm_count, f, yd, part, B, s);
+        case 1: return launch_contract_m<1>(d, sm_count, f, yd, part, B, mflag, s);
+        case 2: return launch_contract_m<2>(d, sm_count, f, yd, part, B, mflag, s);
+        case 4: return launch_contract_m<4>(d, sm_count, f, yd, part, B, mflag, s);
+        default: return launch_contract_m<8>(d, sm_count, f, yd, part, B, mflag, s);
     }
 }
 

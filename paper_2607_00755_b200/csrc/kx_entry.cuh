@@ -1,0 +1,102 @@
+// kx_entry.cuh -- device functions that evaluate ONE entry of the kernel tensor (steps a2-a3), shared by
+// every builder kernel of libkx so that all storage layouts take bit-identical decisions and values.
+// NOT shared with oracle/.  Compiled with --fmad=false.
+#pragma once
+#include "kx_internal.cuh"
+#include <float.h>
+
+namespace kxe {
+
+constexpr double kPi = 3.14159265358979323846;
+
+// ---------------------------------------------------------------- a1
+__device__ __forceinline__ void kin_point(double p, double m, double& E, double& K)
+{
+    E = sqrt(p * p + m * m);
+    K = (p * p) / (E + m);
+}
+
+// ---------------------------------------------------------------- a2: validity (reading D4)
+// tau = 32 eps (K_n+K_m+K_i); a triple is kept iff K_0 - tau <= K~ <= K_{N-1} + tau, and K~ is then
+// clamped into [K_0, K_{N-1}].
+__device__ __forceinline__ bool keep_lo(double Kn, double Km, double Ki, double K0)
+{
+    double S = Kn + Km, Kt = S - Ki, tau = (32.0 * DBL_EPSILON) * (S + Ki);
+    return Kt >= K0 - tau;
+}
+__device__ __forceinline__ bool keep_hi(double Kn, double Km, double Ki, double KN1)
+{
+    double S = Kn + Km, Kt = S - Ki, tau = (32.0 * DBL_EPSILON) * (S + Ki);
+    return Kt <= KN1 + tau;
+}
+
+// ---------------------------------------------------------------- a3: J = int_{Q-}^{Q+} |M|^2 dQ
+// contact: M2_0 (Q+ - Q-)                                                eq. B.17
+// mediator (reading D5): M2_0 m_med^4 int dQ/(Q^2+c2)^2, c2 = m_med^2 - (K_i-K_n)^2.  The difference of
+// the antiderivative Q/(2c2(Q^2+c2)) + atan(Q/c)/(2c^3) between a=Q- and b=Q+ is combined analytically
+// (no subtraction of two large terms); a series in c2 covers |c2| << a^2.
+static __device__ double kx_J(double a, double b, double dK, double M2_0, double m_med)
+{
+    if (!(b > a)) return 0.0;
+    double d = b - a;
+    if (m_med <= 0.0) return M2_0 * d;
+    double mm = m_med * m_med;
+    double c2 = mm - dK * dK;
+    double ab = a * b;
+    double val;
+    if (fabs(c2) <= 0.05 * (a * a)) {
+        // 1/(Q^2+c2)^2 = sum_k (k+1) (-c2)^k Q^(-2k-4);  |c2|/a^2 <= 0.05: 14 terms reach 1e-17
+        double u = 1.0 / (a * a), v = 1.0 / (b * b);
+        double ta = u / a, tb = v / b, pw = 1.0;
+        val = 0.0;
+#pragma unroll 1
+        for (int k = 0; k < 14; ++k) {
+            val += pw * (double)(k + 1) * (ta - tb) / (double)(2 * k + 3);
+            pw *= -c2; ta *= u; tb *= v;
+        }
+    } else if (c2 > 0.0) {
+        double c = sqrt(c2);
+        val = d * (c2 - ab) / (2.0 * c2 * (a * a + c2) * (b * b + c2))
+            + atan2(c * d, c2 + ab) / (2.0 * c2 * c);
+    } else {
+        double k2 = -c2, k = sqrt(k2);
+        val = d * (ab + k2) / (2.0 * k2 * ((a - k) * (a + k)) * ((b - k) * (b + k)))
+            + log1p(-2.0 * k * d / ((b - k) * (a + k))) / (4.0 * k2 * k);
+    }
+    return M2_0 * (mm * mm) * val;
+}
+
+
+// K~ of a KEPT triple, snapped into the domain (reading D4)                       eq. 4.4
+__device__ __forceinline__ double kx_Kt(double Kn, double Km, double Ki, double K0, double KN1)
+{
+    double Kt = (Kn + Km) - Ki;
+    return fmin(fmax(Kt, K0), KN1);
+}
+
+// symmetrised kernel-tensor entry W_inm + W_imn (n < m) or W_inn for a kept triple     eq. 4.7 + B.15-B.17
+__device__ __forceinline__ double kx_Wsym(const KxDev& d, const double* __restrict__ P, int n, int m,
+                                          double pi_, double pn, double Ki, double Kn, double Km, double Kt,
+                                          double pref_in)
+{
+    const double pm = P[m];
+    const double pj = sqrt(Kt * (Kt + 2.0 * d.m));   // eq. 4.4
+    // eq. B.15-B.16
+    double J = kx_J(fmax(fabs(pi_ - pn), fabs(pm - pj)), fmin(pi_ + pn, pm + pj), Ki - Kn, d.M2_0, d.m_med);
+    if (m != n)   // the (i,m,n) ordering: second half of the symmetrised entry
+        J += kx_J(fmax(fabs(pi_ - pm), fabs(pn - pj)), fmin(pi_ + pm, pn + pj), Ki - Km, d.M2_0, d.m_med);
+    return pref_in * d.ccol[m] * J;
+}
+
+// bracket: largest j in [0, N-2] with K_j <= K~                                   eq. B.19
+__device__ __forceinline__ int kx_bracket(const double* __restrict__ K, int N, double Kt)
+{
+    int lo = 0, hi = N - 2;
+    while (lo < hi) {
+        int mid = (lo + hi + 1) >> 1;
+        if (K[mid] <= Kt) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+}  // namespace kxe

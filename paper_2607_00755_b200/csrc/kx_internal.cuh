@@ -16,6 +16,9 @@
 #define KX_CTA        256      // threads per CTA of the contraction kernels
 #define KX_EXP_BITS   8        // 2^8-entry exp2 table
 #define KX_EXP_REP    16       // table replicated once per bank pair: conflict-free 64-bit gathers
+#define KX_TI         16       // rows i per tile of the tiled (DMMA) storage: two 8-row MMA blocks
+#define KX_QMAX       32       // largest number of Chebyshev nodes of the compressed LOG loss term
+#define KX_GROUP_DBL  256      // doubles of tensor data per group: 4 quads x 2 row blocks x 32 lanes
 
 // Device-side view of a handle: plain pointers, passed by value to every kernel.
 struct KxDev {
@@ -43,12 +46,58 @@ struct KxDev {
     const double *exptab;     // [2^KX_EXP_BITS] 2^(k/2^KX_EXP_BITS)
 };
 
+// Tiled storage (KX_STORE_TILED), the operand of the DMMA contraction kernel (kx_tiled.cu).
+//
+// Rows i are cut into tiles of KX_TI = 16.  Each tile has two "virtual tiles" of work, both of the form
+//     out[b, i] += sum_k X[b, k] * A[k, i]                      (k in quads of 4, quads in groups of 4)
+//   gain (vt = 2t):   k = (n, m) with n <= m;  A = W_inm + W_imn (0 where the triple is dropped for row i),
+//                     X = f_n f_m.  For fixed (tile, n) the m with any kept row form one interval: a "run",
+//                     padded to a multiple of 4.
+//   loss (vt = 2t+1): k = (j, c), c < Q;  A = M_c(i,j) = sum_{(n<=m) in bracket j of row i} Wsym T_c(2 omega_R - 1)
+//                     (Chebyshev moments of the bucket), X = a_c(b,j) = Chebyshev coefficients of the
+//                     degree-(Q-1) interpolant of omega -> f_j^(1-omega) f_(j+1)^omega (LOG) or the exact
+//                     two coefficients (LINEAR, Q = 2).
+// A group (4 quads) stores its 256 doubles in MMA-fragment order: [quad][row block rb][lane], the lane's
+// element being A[k = 4 quad + lane%4][i = 16 t + 8 rb + lane/4].  desc[quad] = xrow | srow << 20: the
+// row of XT holding X for k = 4 quad (rows xrow..xrow+3) and the row whose values scale it (f_n; the
+// ones row for loss quads).
+struct KxTiled {
+    int NT;                   // number of tiles = ceil(N / 16)
+    int Q;                    // Chebyshev coefficients per bracket (LINEAR: 2)
+    int LQ;                   // loss quads per tile = ceil((N-1) Q / 4)
+    int LG;                   // loss groups per tile = ceil(LQ / 4)
+    int ones_row;             // = N: row of XT filled with 1
+    int loss_row0;            // = N + 1: first Chebyshev-coefficient row of XT
+    int xrows;                // rows of XT = loss_row0 + 16 LG
+    int *trun_mlo;            // [NT*N] first m of the run (tile, n)
+    unsigned *trun_q;         // [NT*N] quads of the run
+    unsigned *trun_off;       // [NT*(N+1)] exclusive scan of trun_q inside the tile; [t*(N+1)+N] = quads of tile t
+    unsigned *vtptr;          // [2 NT + 1] exclusive scan of groups per virtual tile
+    double *A;                // [groups][256]
+    unsigned *desc;           // [groups][4]
+    const double *dct;        // [Q*Q] (2 - delta_c0)/Q cos(c theta_q), theta_q = (2q+1) pi / (2Q)
+    const double *nodes;      // [Q] omega_q = (1 + cos theta_q)/2
+    double flag_log2;         // log2(2 / Q!) - log2(eps_flag) ... see kx_tiled.cu k_xt
+};
+
 struct kx_handle_s {
     KxDev d;
     int device;
     int sm_count;
     long long cap;            // capacity of W/omega/nmj in entries
     long long nnz;            // host copy, valid when !nnz_stale
+    KxTiled t;                // tiled storage (valid when tiled_ok)
+    int storage;              // KX_STORE_*
+    bool tiled_ok;            // t.A / t.desc describe the current kinematics
+    long long cap_groups;     // capacity of t.A / t.desc in groups
+    long long groups;         // host copy of vtptr[2 NT]
+    int ws_xstride;           // columns of XT (batch capacity padded)
+    double *XT;               // [t.xrows, ws_xstride] operand rows: f^T, ones, Chebyshev coefficients
+    double *fmax;             // [wsB] max_i f[b,i]
+    int *mflag;               // [wsB] member needs the exact streaming path (a bracket failed the error bound)
+    double *tpart;            // [tslots, ws_xstride, 16] partials of the DMMA kernel
+    long long tslots;
+    void *tiled_blob;         // one allocation holding the small tables of KxTiled
     bool nnz_stale;
     int chunk_for_B;          // the batch size taskptr was last built for (0 = none)
     // workspaces, grown on demand
@@ -100,15 +149,29 @@ struct KxStage {             // what the finishing kernel does after the reducti
     double *fstage;          // stage input written by this stage for the next one
     double *k1, *k2, *k3;
     double *ydnext;          // where to write yd of the next stage input (fused prep) or null
+    // tiled path: partials of the DMMA kernel; members with mflag != 0 take the streaming partials instead
+    const double *tpart;     // [slots, xstride, 16] or null (streaming path only)
+    const unsigned *vtptr;
+    const int *mflag;
+    int NT, nctas, xstride;
     int *flag;
     int evolve;
 };
 cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, cudaStream_t s);
 cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
-                               double* part, int B, cudaStream_t s);
+                               double* part, int B, const int* mflag, cudaStream_t s);
 cudaError_t kx_launch_finish(const KxDev& d, const double* f, const double* part, int B,
                              const KxStage& st, cudaStream_t s);
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
                               double* p1, double* p2, int stride, cudaStream_t s);
+// ---- tiled path (kx_tiled_build.cu, kx_tiled.cu)
+cudaError_t kx_launch_tile_runs(const KxDev& d, const KxTiled& t, cudaStream_t s);     // runs, scans, vtptr
+cudaError_t kx_launch_tile_fill(const KxDev& d, const KxTiled& t, cudaStream_t s);     // A, desc (gain + loss)
+cudaError_t kx_launch_xt(const KxDev& d, const KxTiled& t, const double* f, double* yd, double* XT, int xstride,
+                         double* fmax, int* mflag, int B, cudaStream_t s);
+cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, int G, const double* XT, int xstride,
+                           double* tpart, int B, cudaStream_t s);
+int kx_xstride(int B);
+int kx_dmma_ctas(int sm_count, long long groups);
 int kx_pick_bt(int N, int B);
 int kx_pick_chunk(long long nnz_est, int N, int B, int sm_count);
