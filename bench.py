@@ -32,11 +32,11 @@ import kx_inputs as kin  # noqa: E402
 METRIC = "C[f] evals/s (fp64, N=256, B=64)"
 UNIT = "C[f]/s"
 WORKLOAD = "cfg3: N=256 log p/T in [1e-3,50], B=64 seeded bimodal f, |M|^2 ~ 1/(1+q^2/m_med^2)^2, m_med=0.5"
-# FP64-pipe instructions per (entry, member) of the LOG/table kernel, counted from the source and checked in SASS
-# (DESIGN.md "Kernels"): gain DMUL+DFMA, argument DFMA, exp2 3 DADD + 3 DFMA + DMUL + DFMA, loss DFMA.
-FP64_INST = {"log": 12, "linear": 4}
-FP64_FLOP = {"log": 19, "linear": 7}      # DFMA = 2 flop, DADD/DMUL = 1
-SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM (37 TFLOP/s nominal at 1.965 GHz)
+# Algorithmic work of the dominant kernel k_dmma: one FMA (2 flop) per stored entry and member
+# for the gain, one per (i, bracket, Chebyshev coefficient) and member for the loss.  Padding of the tiled layout,
+# the f_n f_m products and the operand preparation are NOT counted.
+LOSS_NODES = {"log": 24, "linear": 2}
+SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM; DMMA.8x8x4 runs at the same 37.2 TFLOP/s
 
 
 def _peaks():
@@ -237,33 +237,37 @@ def main():
     sm_max_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     nnz = info["nnz"]
     kern_s = t_kern / max(kern_n, 1)
-    if args.mode == "log":
-        # plain FP64 ALU bound: one exp per (entry, member); peak = SMs x 64 FMA lanes x 2 flop x max SM clock
-        peak = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_hz / 1e12
-        ach = nnz * B * FP64_FLOP["log"] / kern_s / 1e12
-        roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "traffic": None, "kernel": "k_contract<8,LOG_TAB>", "kernel_ms": kern_s * 1e3,
-                "peak_source": f"148 SMs x 64 FP64 FMA lanes x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src})",
-                "fp64_inst_per_entry_member": FP64_INST["log"], "flop_per_entry_member": FP64_FLOP["log"],
-                "pipe_frac": nnz * B * FP64_INST["log"] / kern_s / (SM_COUNT * FP64_LANES_PER_SM * sm_max_hz)}
-    else:
-        peak = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_hz / 1e12
-        ach = nnz * B * FP64_FLOP["linear"] / kern_s / 1e12
-        roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "traffic": None, "kernel": "k_contract<8,LINEAR>", "kernel_ms": kern_s * 1e3,
-                "peak_source": f"148 SMs x 64 FP64 FMA lanes x 2 x {sm_max_hz / 1e6:.0f} MHz ({peak_src})"}
+    Q = LOSS_NODES[args.mode]
+    Ngrid = info["N"]
+    # FP64 tensor pipe (DMMA.8x8x4): 148 SMs x 64 FMA/clk x 2 flop x max SM clock; the library's own probe
+    # (kx_probe_flops) measures it on this GPU in the same run.  The guide's nominal ratio applied to the measured
+    # bf16 peak (45/2250 x bf16_tflops) is given as peak_alt.
+    peak_nominal = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_hz / 1e12
+    probe = {"dmma": h.probe_flops(1), "dfma": h.probe_flops(0)}
+    peak = max(peak_nominal, probe["dmma"])
+    flop = 2.0 * (nnz + Ngrid * (Ngrid - 1) * Q) * B
+    ach = flop / kern_s / 1e12
+    roof = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+            "traffic": None, "kernel": "k_dmma<8,8,4> (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss)",
+            "kernel_ms": kern_s * 1e3, "flop_per_launch": flop,
+            "peak_source": f"FP64 tensor pipe: 148 SMs x 64 FMA/clk x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src}); "
+                           f"probe in this run: DMMA {probe['dmma']:.1f}, DFMA {probe['dfma']:.1f} TFLOP/s",
+            "peak_alt": {"value": float(peaks.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0,
+                         "how": f"{peak_src} bf16_tflops x guide nominal ratio 45/2250"},
+            "tensor_bytes_per_launch": info["tensor_bytes"],
+            "hbm_time_us_at_peak": info["tensor_bytes"] / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9) * 1e6}
     line = {
         "metric": METRIC, "value": world * B * K / t_cold, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": t_cold / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD, "N": 256, "B_per_gpu": B, "mode": args.mode, "projected": bool(args.project),
-                   "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "l2": "flushed before every timed step (256 MiB write)",
+                   "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "storage": "tiled", "loss_nodes": Q, "l2": "flushed before every timed step (256 MiB write)",
                    "parallelism": f"independent batches x{world}" if world > 1 else "single GPU"},
         "value_l2_warm": world * B * K / t_warm, "ms_per_step_l2_warm": t_warm / K * 1e3,
         "calls_per_s": world * K / t_cold,
         "e2e": {"value": world * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": B * 256 * 8,
                 "d2h_bytes_per_step": B * 256 * 8, "ms_per_step": t_e2e / K * 1e3},
-        "gpu_launches": 3 * K, "clocks": clocks, "roofline": roof, "finite": same,
+        "gpu_launches": (5 if args.mode == "log" else 4) * K, "clocks": clocks, "roofline": roof, "finite": same,
     }
     if not args.no_cpu_baseline and world == 1:
         cb = cpu_oracle(c, members=B, steps=3, warmup=1)

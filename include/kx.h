@@ -166,6 +166,11 @@ kx_status_t kx_kinematics_export(kx_handle_t h, double* E, double* K, double* hw
 kx_status_t kx_profile(kx_handle_t h, int32_t enable);
 kx_status_t kx_profile_read(kx_handle_t h, double* contract_ms, int64_t* launches);
 
+/* Measurement aid (bench.py): peak FP64 throughput of `device` in TFLOP/s, register-resident chains without memory
+ * traffic.  kind 0 = DFMA (plain FP64 pipe), 1 = DMMA.8x8x4 (FP64 tensor pipe, the instruction of the tiled
+ * contraction).  Synchronises the device; takes about 50 ms. */
+kx_status_t kx_probe_flops(int device, int32_t kind, double* tflops);
+
 const char* kx_last_error(kx_handle_t h);   /* h may be NULL: returns the last build failure */
 void        kx_destroy(kx_handle_t h);
 int32_t     kx_version(void);

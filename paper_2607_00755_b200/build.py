@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkx.so")
-SOURCES = ["kx_api.cu", "kx_build.cu", "kx_contract.cu", "kx_tiled_build.cu", "kx_tiled.cu"]
+SOURCES = ["kx_api.cu", "kx_build.cu", "kx_contract.cu", "kx_tiled_build.cu", "kx_tiled.cu", "kx_probe.cu"]
 HEADERS = [os.path.join(CSRC, "kx_internal.cuh"), os.path.join(CSRC, "kx_entry.cuh"), os.path.join(HERE, "..", "include", "kx.h")]
 # --fmad=false: validity decisions, omega and the Runge-Kutta updates must not depend on implicit FMA
 # contraction; the hot loops call fma() explicitly.

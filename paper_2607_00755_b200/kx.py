@@ -61,7 +61,7 @@ class _Evolve(C.Structure):
 # every symbol include/kx.h declares
 SYMBOLS = ["kx_build", "kx_set_mass", "kx_collide", "kx_collide_parts", "kx_collide_ex",
            "kx_collide_host", "kx_moments", "kx_evolve", "kx_info", "kx_tensor_export",
-           "kx_kinematics_export", "kx_profile", "kx_profile_read", "kx_last_error", "kx_destroy", "kx_version"]
+           "kx_kinematics_export", "kx_profile", "kx_profile_read", "kx_probe_flops", "kx_last_error", "kx_destroy", "kx_version"]
 
 _lib = None
 
@@ -97,6 +97,7 @@ def _load():
     lib.kx_kinematics_export.argtypes = [vp, _dp, _dp, _dp]
     lib.kx_profile.argtypes = [vp, i32]
     lib.kx_profile_read.argtypes = [vp, _dp, i64p]
+    lib.kx_probe_flops.argtypes = [C.c_int, i32, _dp]
     lib.kx_last_error.argtypes = [vp]
     lib.kx_last_error.restype = C.c_char_p
     lib.kx_destroy.argtypes = [vp]
@@ -274,6 +275,12 @@ class Handle:
         ms, n = C.c_double(), C.c_int64()
         self._check(self._lib.kx_profile_read(self._h, C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def probe_flops(self, kind=1):
+        """kx_probe_flops: measured peak TFLOP/s of the handle's device (0 = DFMA, 1 = DMMA.8x8x4)."""
+        v = C.c_double()
+        self._check(self._lib.kx_probe_flops(self.device, int(kind), C.byref(v)))
+        return v.value
 
     def info(self):
         nnz, tb, n = C.c_int64(), C.c_int64(), C.c_int32()

@@ -245,3 +245,81 @@ def test_projection_and_moments_parity(torch_cuda, oracle, m):
     assert _relerr(h.collide(_dev(torch, f)).cpu().numpy(), C2, g2) <= TOL
     assert h.info()["nnz"] == int(((T2.jL >= 0) & (np.arange(96)[None, :, None] <= np.arange(96)[None, None, :])).sum())
     h.close()
+
+
+# --------------------------------------------------------------------------------------- storage modes
+@pytest.mark.parametrize("interp", [0, 1])
+def test_streaming_storage_parity(torch_cuda, oracle, interp):
+    """KX_STORE_SYM_ROWS: the exact streaming kernel alone (one exp per entry and member)."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(3, N=96, B=11)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, c["f"], interp)
+    h = _handle(c, interp=interp, storage=kx.STORE_SYM_ROWS)
+    f = _dev(torch, c["f"])
+    g, l = h.collide_parts(f)
+    assert _relerr(g.cpu().numpy(), g0, g0) <= TOL
+    assert _relerr(l.cpu().numpy(), l0, g0) <= TOL
+    assert _relerr(h.collide(f).cpu().numpy(), C0, g0) <= 2e-13
+    h.close()
+
+
+@pytest.mark.parametrize("nodes", [8, 16, 24, 32])
+def test_tiled_loss_nodes(torch_cuda, oracle, nodes):
+    """Every Chebyshev order gives the oracle's operator: brackets the order cannot resolve to 1e-15 max f send
+    their member to the streaming kernel (few nodes => many members fall back, the result stays within the bar)."""
+    torch = torch_cuda
+    c = kin.config(3, N=64, B=20)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, c["f"], 0)
+    h = _handle(c, loss_nodes=nodes)
+    f = _dev(torch, c["f"])
+    g, l = h.collide_parts(f)
+    assert _relerr(g.cpu().numpy(), g0, g0) <= TOL
+    assert _relerr(l.cpu().numpy(), l0, g0) <= TOL
+    assert _relerr(l.cpu().numpy(), l0, g0) <= 1e-13
+    h.close()
+
+
+def test_tiled_fallback_sharp_features(torch_cuda, oracle):
+    """Distributions the Chebyshev-moment loss cannot represent (cut-offs to exact zero, steps of 1e200, a single
+    occupied bin) are routed per member to the exact streaming kernel; smooth neighbours stay on the DMMA path."""
+    torch = torch_cuda
+    c = kin.config(3, N=80, B=6)
+    p = c["p"]
+    f = c["f"].copy()
+    f[1, p > 3.0] = 0.0                                  # sharp cut-off: ln(f_j+1/f_j) ~ -690 in one bracket
+    f[2] = np.where((p > 0.5) & (p < 2.0), 1.0, 1e-200)  # step function
+    f[3] = 0.0
+    f[3, 40] = 2.5                                       # one occupied bin
+    f[4] = 1e-250 * c["f"][4]                            # tiny but smooth: no fallback needed, still exact
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, f, 0)
+    h = _handle(c)
+    fd = _dev(torch, f)
+    g, l = h.collide_parts(fd)
+    scale = np.maximum(np.abs(g0).max(axis=1, keepdims=True), 1e-300)
+    assert (np.abs(g.cpu().numpy() - g0) / scale).max() <= TOL
+    assert (np.abs(l.cpu().numpy() - l0) / scale).max() <= TOL
+    Cp0, _ = oracle.project(T, f, C0)
+    Cp = h.collide(fd, flags=1).cpu().numpy()
+    assert (np.abs(Cp - Cp0) / scale).max() <= TOL
+    # the same members in another order and batch size give the same bits (fallback is per member)
+    perm = [3, 0, 5, 1]
+    Cq = h.collide(_dev(torch, f[perm]), flags=1).cpu().numpy()
+    assert np.array_equal(Cq, Cp[perm])
+    h.close()
+
+
+@pytest.mark.parametrize("B", [1, 7, 8, 9, 17, 33, 64, 65, 130])
+def test_tiled_batch_sizes(torch_cuda, oracle, B):
+    """Every MMA column-tile configuration (1, 2, 4, 8 tiles; several CTA column groups; ragged tails)."""
+    torch = torch_cuda
+    c = kin.config(3, N=40, B=B)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, c["f"], 0)
+    h = _handle(c)
+    C = h.collide(_dev(torch, c["f"])).cpu().numpy()
+    assert _relerr(C, C0, g0) <= 2e-13
+    h.close()
