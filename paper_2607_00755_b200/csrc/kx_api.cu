@@ -47,7 +47,7 @@ kx_status_t alloc_tensor(kx_handle_s* h, long long cap)
 void free_tiled(kx_handle_s* h)
 {
     cudaFree(h->t.A); cudaFree(h->t.desc);
-    h->t.A = nullptr; h->t.desc = nullptr;
+    h->t.A = nullptr; h->t.desc = nullptr;     // t.AL has a fixed size: freed in kx_destroy
     h->cap_groups = 0; h->tiled_ok = false;
 }
 
@@ -66,7 +66,7 @@ inline long long tiled_groups_bound(const kx_handle_s* h)
 {
     const long long N = h->d.N, NT = h->t.NT;
     const long long quads_per_tile = (N * (N + 1) / 2 + 3) / 4 + N;     // each run rounds up by < 1 quad
-    return NT * ((quads_per_tile + 3) / 4 + h->t.LG);
+    return NT * ((quads_per_tile + 3) / 4);
 }
 
 // a2-a3 in the tiled layout for the current kinematics (the run table of kx_launch_runs must be current)
@@ -75,7 +75,7 @@ kx_status_t build_tiled(kx_handle_s* h, cudaStream_t s, bool may_sync)
     KX_CUDA(kx_launch_tile_runs(h->d, h->t, s));
     if (may_sync) {
         unsigned g = 0;
-        KX_CUDA(cudaMemcpyAsync(&g, h->t.vtptr + 2 * h->t.NT, 4, cudaMemcpyDeviceToHost, s));
+        KX_CUDA(cudaMemcpyAsync(&g, h->t.vtptr + h->t.NT, 4, cudaMemcpyDeviceToHost, s));
         KX_CUDA(cudaStreamSynchronize(s));
         h->groups = g;
         if (h->cap_groups < (long long)g) {
@@ -97,10 +97,10 @@ void free_ws(kx_handle_s* h)
 {
     cudaFree(h->yd); cudaFree(h->part); cudaFree(h->fstage); cudaFree(h->k1); cudaFree(h->k2);
     cudaFree(h->k3); cudaFree(h->Cbuf); cudaFree(h->hostio);
-    cudaFree(h->XT); cudaFree(h->fmax); cudaFree(h->mflag); cudaFree(h->tpart);
+    cudaFree(h->XT); cudaFree(h->fmax); cudaFree(h->mflag); cudaFree(h->gpart); cudaFree(h->lpart);
     h->yd = h->part = h->fstage = h->k1 = h->k2 = h->k3 = h->Cbuf = h->hostio = nullptr;
-    h->XT = h->fmax = h->tpart = nullptr; h->mflag = nullptr;
-    h->wsB = 0; h->ws_tasks = 0; h->ws_xstride = 0; h->tslots = 0;
+    h->XT = h->fmax = h->gpart = h->lpart = nullptr; h->mflag = nullptr;
+    h->wsB = 0; h->ws_tasks = 0; h->ws_xstride = 0;
 }
 
 // the smallest chunk is 1024 entries, so a row of len entries has at most len/1024+1 tasks
@@ -123,13 +123,13 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
     KX_CUDA(dalloc(&h->hostio, bn * 2));
     if (h->storage == KX_STORE_TILED) {
         const int xs = kx_xstride(nB);
-        const long long slots = (long long)h->sm_count + 2 * h->t.NT + 1;
         KX_CUDA(dalloc(&h->XT, (size_t)h->t.xrows * xs));
         KX_CUDA(cudaMemset(h->XT, 0, (size_t)h->t.xrows * xs * 8));      // padding rows stay zero for good
         KX_CUDA(dalloc(&h->fmax, (size_t)nB));
         KX_CUDA(dalloc(&h->mflag, (size_t)nB));
-        KX_CUDA(dalloc(&h->tpart, (size_t)slots * xs * 16));
-        h->ws_xstride = xs; h->tslots = slots;
+        KX_CUDA(dalloc(&h->gpart, (size_t)(8 * h->sm_count + h->t.NT + 1) * xs * 16));
+        KX_CUDA(dalloc(&h->lpart, (size_t)(h->sm_count + h->t.RS + 1) * xs * 256));
+        h->ws_xstride = xs;
     }
     h->wsB = nB; h->ws_tasks = need_tasks;
     return KX_OK;
@@ -197,21 +197,22 @@ kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bo
     kx_status_t rc;
     if (use_tiled) {
         const int xs = h->ws_xstride;
-        const int G = kx_dmma_ctas(h->sm_count, h->groups);
+        kx_dmma_split(h->d, h->t, h->sm_count, h->groups, B, &h->GG, &h->GL);
         KX_CUDA(kx_launch_xt(h->d, h->t, f, h->yd, h->XT, xs, h->fmax, h->mflag, B, s));
         if ((rc = prof_begin()) != KX_OK) return rc;
-        KX_CUDA(kx_launch_dmma(h->d, h->t, G, h->XT, xs, h->tpart, B, s));
+        KX_CUDA(kx_launch_dmma(h->d, h->t, h->groups, h->GG, h->GL, f, h->XT, xs, h->gpart, h->lpart, B, s));
         if ((rc = prof_end()) != KX_OK) return rc;
         if (h->d.interp == KX_INTERP_LOG)      // exact streaming path for flagged members only (LINEAR is exact)
-            KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, h->mflag, s));
-        st->tpart = h->tpart; st->vtptr = h->t.vtptr; st->mflag = h->d.interp == KX_INTERP_LOG ? h->mflag : nullptr;
-        st->NT = h->t.NT; st->nctas = G; st->xstride = xs;
+            KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, h->mflag, true, s));
+        st->gpart = h->gpart; st->lpart = h->lpart; st->vtptr = h->t.vtptr;
+        st->mflag = h->d.interp == KX_INTERP_LOG ? h->mflag : nullptr;
+        st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS; st->GW = 8 * h->GG; st->GL = h->GL; st->xstride = xs;
     } else {
         if (!have_yd) KX_CUDA(kx_launch_prep(h->d, f, h->yd, B, s));
         if ((rc = prof_begin()) != KX_OK) return rc;
-        KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, nullptr, s));
+        KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, nullptr, !have_yd, s));
         if ((rc = prof_end()) != KX_OK) return rc;
-        st->tpart = nullptr; st->vtptr = nullptr; st->mflag = nullptr;
+        st->gpart = nullptr; st->lpart = nullptr; st->vtptr = nullptr; st->mflag = nullptr;
     }
     return KX_OK;
 }
@@ -259,6 +260,7 @@ void kx_destroy(kx_handle_t h)
         free_ws(h);
         cudaFree(h->dev_blob);
         cudaFree(h->tiled_blob);
+        cudaFree(h->t.AL);
         for (auto& ev : h->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     }
     delete h;
@@ -366,14 +368,18 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
             KxTiled& t = h->t;
             t.NT = (N + KX_TI - 1) / KX_TI;
             t.Q = d.interp == KX_INTERP_LOG ? o.loss_nodes : 2;
-            t.LQ = ((N - 1) * t.Q + 3) / 4;
-            t.LG = (t.LQ + 3) / 4;
+            t.LC = ((N - 1) * t.Q + 15) / 16;
+            t.NR8 = (N + 7) / 8;
+            t.RS = (N + 255) / 256;
             t.ones_row = N;
-            t.loss_row0 = N + 1;
-            t.xrows = t.loss_row0 + 16 * t.LG;
-            // small tables: trun_mlo, trun_q [NT*N], trun_off [NT*(N+1)], vtptr [2NT+1], dct [Q*Q], nodes [Q]
+            t.loss_row0 = N + 4;
+            t.xrows = t.loss_row0 + 16 * t.LC;
+            // loss operand: fixed size; the padding (k >= (N-1) Q, rows >= N) stays zero for good
+            KX_CUDA(dalloc(&t.AL, (size_t)t.LC * t.NR8 * 128));
+            KX_CUDA(cudaMemsetAsync(t.AL, 0, (size_t)t.LC * t.NR8 * 128 * 8, s));
+            // small tables: trun_mlo, trun_q [NT*N], trun_off [NT*(N+1)], vtptr [NT+1], dct [Q*Q], nodes [Q]
             const size_t tn = (size_t)t.NT * N;
-            const size_t ints = tn * 2 + (size_t)t.NT * (N + 1) + (size_t)(2 * t.NT + 1);
+            const size_t ints = tn * 2 + (size_t)t.NT * (N + 1) + (size_t)(t.NT + 1);
             const size_t ints_pad = (ints + 1) & ~(size_t)1;
             KX_CUDA(cudaMalloc(&h->tiled_blob, ints_pad * 4 + ((size_t)t.Q * t.Q + t.Q) * 8));
             int* tp = (int*)h->tiled_blob;
@@ -597,7 +603,8 @@ kx_status_t kx_info(kx_handle_t h, int64_t* nnz, int64_t* tensor_bytes, int32_t*
     }
     if (nnz) *nnz = h->nnz;
     if (tensor_bytes) {
-        if (h->storage == KX_STORE_TILED && h->tiled_ok) *tensor_bytes = h->groups * (KX_GROUP_DBL * 8 + 16);
+        if (h->storage == KX_STORE_TILED && h->tiled_ok)
+            *tensor_bytes = h->groups * (KX_GROUP_DBL * 8 + 16) + (long long)h->t.LC * h->t.NR8 * 1024;
         else *tensor_bytes = h->nnz * 20;            // W 8 + omega 8 + n|m|j 4
     }
     if (n) *n = h->d.N;

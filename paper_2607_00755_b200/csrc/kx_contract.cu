@@ -79,6 +79,8 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int b0 = blockIdx.y * BT;
     const int nb = min(BT, B - b0);
+    kx_pdl_trigger();
+    kx_pdl_wait();
     if (mflag) {          // tiled path: only member groups holding a flagged member take the exact streaming path
         int any = 0;
         for (int b = 0; b < nb; ++b) any |= mflag[b0 + b];
@@ -218,7 +220,8 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
     __shared__ double s_y[KX_MAX_N];
     const int N = d.N, tid = threadIdx.x, b = blockIdx.x;
     const double* fb = fin + (size_t)b * N;
-    const bool tiled = st.tpart != nullptr && !(st.mflag && st.mflag[b]);
+    kx_pdl_wait();
+    const bool tiled = st.gpart != nullptr && !(st.mflag && st.mflag[b]);
 
     double C[kMaxPerThread], fi[kMaxPerThread], hi_[kMaxPerThread], Ei[kMaxPerThread], Ki[kMaxPerThread];
 #pragma unroll
@@ -228,22 +231,29 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
         if (i < N) {
             double g = 0.0, nu = 0.0;
             if (tiled) {
-                // partials of the DMMA kernel: virtual tiles 2t (gain) and 2t+1 (nu); the CTAs whose group range
-                // meets a virtual tile are c(first group)..c(last group), slot = c + vt, added in slot order
-                const unsigned Gtot = st.vtptr[2 * st.NT];
-                const int tile = i >> 4, il = i & 15;
-#pragma unroll
-                for (int half = 0; half < 2; ++half) {
-                    const int vt = 2 * tile + half;
-                    const unsigned a0 = st.vtptr[vt], a1 = st.vtptr[vt + 1];
-                    double acc = 0.0;
+                // partials of the DMMA kernel.  gain: tile = i/16, groups [a0,a1) of the tile were taken by the gain
+                // workers c0..c1 (equal ranges of the Gtot groups), slot = c + tile.  loss: supertile = i/256, chunk units
+                // [sp LC, (sp+1) LC) of the RS LC units were taken by the loss CTAs c0..c1, slot = c + sp.  Both are
+                // added in slot order.
+                {
+                    const unsigned Gtot = st.vtptr[st.NT];
+                    const int tile = i >> 4, il = i & 15;
+                    const unsigned a0 = st.vtptr[tile], a1 = st.vtptr[tile + 1];
                     if (a1 > a0) {
-                        const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.nctas - 1ull) / Gtot);
-                        const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.nctas - 1ull) / Gtot);
+                        const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.GW - 1ull) / Gtot);
+                        const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.GW - 1ull) / Gtot);
                         for (unsigned c = c0; c <= c1; ++c)
-                            acc += st.tpart[((size_t)(c + vt) * st.xstride + b) * 16 + il];
+                            g += st.gpart[((size_t)(c + tile) * st.xstride + b) * 16 + il];
                     }
-                    if (half == 0) g = acc; else nu = acc;
+                }
+                {
+                    const unsigned U = (unsigned)st.RS * (unsigned)st.LC;
+                    const unsigned sp = (unsigned)i >> 8, il = (unsigned)i & 255u;
+                    const unsigned a0 = sp * (unsigned)st.LC, a1 = a0 + (unsigned)st.LC;
+                    const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.GL - 1ull) / U);
+                    const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.GL - 1ull) / U);
+                    for (unsigned c = c0; c <= c1; ++c)
+                        nu += st.lpart[((size_t)(c + sp) * st.xstride + b) * 256 + il];
                 }
             } else {
                 const unsigned t0 = d.taskptr[i], t1 = d.taskptr[i + 1];
@@ -393,7 +403,7 @@ k_moments(KxDev d, const double* __restrict__ f, double* n, double* rho, double*
 
 template <int BT, int MODE>
 cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, const double* yd,
-                              double* part, int B, const int* mflag, cudaStream_t s)
+                              double* part, int B, const int* mflag, bool pdl, cudaStream_t s)
 {
     const int N = d.N;
     size_t smem = (size_t)BT * N * 24 + (size_t)(KX_CTA / 32) * 2 * BT * 8
@@ -408,17 +418,16 @@ cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, con
     int gx = (sm_count * occ + groups - 1) / groups;
     if (gx < 1) gx = 1;
     dim3 grid(gx, groups);
-    k_contract<BT, MODE><<<grid, KX_CTA, smem, s>>>(d, f, reinterpret_cast<const double2*>(yd), part, B, mflag);
-    return cudaGetLastError();
+    return kx_launch(k_contract<BT, MODE>, grid, dim3(KX_CTA), smem, s, pdl, d, f, reinterpret_cast<const double2*>(yd), part, B, mflag);
 }
 
 template <int BT>
 cudaError_t launch_contract_m(const KxDev& d, int sm_count, const double* f, const double* yd,
-                              double* part, int B, const int* mflag, cudaStream_t s)
+                              double* part, int B, const int* mflag, bool pdl, cudaStream_t s)
 {
-    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, mflag, s);
-    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, mflag, s);
-    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, mflag, s);
+    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, mflag, pdl, s);
+    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, mflag, pdl, s);
+    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, mflag, pdl, s);
 }
 
 }  // namespace
@@ -450,21 +459,20 @@ cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, c
 }
 
 cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
-                               double* part, int B, const int* mflag, cudaStream_t s)
+                               double* part, int B, const int* mflag, bool pdl, cudaStream_t s)
 {
     switch (kx_pick_bt(d.N, B)) {
-        case 1: return launch_contract_m<1>(d, sm_count, f, yd, part, B, mflag, s);
-        case 2: return launch_contract_m<2>(d, sm_count, f, yd, part, B, mflag, s);
-        case 4: return launch_contract_m<4>(d, sm_count, f, yd, part, B, mflag, s);
-        default: return launch_contract_m<8>(d, sm_count, f, yd, part, B, mflag, s);
+        case 1: return launch_contract_m<1>(d, sm_count, f, yd, part, B, mflag, pdl, s);
+        case 2: return launch_contract_m<2>(d, sm_count, f, yd, part, B, mflag, pdl, s);
+        case 4: return launch_contract_m<4>(d, sm_count, f, yd, part, B, mflag, pdl, s);
+        default: return launch_contract_m<8>(d, sm_count, f, yd, part, B, mflag, pdl, s);
     }
 }
 
 cudaError_t kx_launch_finish(const KxDev& d, const double* fin, const double* part, int B,
                              const KxStage& st, cudaStream_t s)
 {
-    k_finish<<<B, KX_CTA, 0, s>>>(d, fin, part, B, st);
-    return cudaGetLastError();
+    return kx_launch(k_finish, dim3(B), dim3(KX_CTA), 0, s, true, d, fin, part, B, st);
 }
 
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,

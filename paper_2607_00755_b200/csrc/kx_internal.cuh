@@ -46,38 +46,40 @@ struct KxDev {
     const double *exptab;     // [2^KX_EXP_BITS] 2^(k/2^KX_EXP_BITS)
 };
 
-// Tiled storage (KX_STORE_TILED), the operand of the DMMA contraction kernel (kx_tiled.cu).
+// Tiled storage (KX_STORE_TILED), the operands of the DMMA contraction kernel (kx_tiled.cu).
 //
-// Rows i are cut into tiles of KX_TI = 16.  Each tile has two "virtual tiles" of work, both of the form
-//     out[b, i] += sum_k X[b, k] * A[k, i]                      (k in quads of 4, quads in groups of 4)
-//   gain (vt = 2t):   k = (n, m) with n <= m;  A = W_inm + W_imn (0 where the triple is dropped for row i),
-//                     X = f_n f_m.  For fixed (tile, n) the m with any kept row form one interval: a "run",
-//                     padded to a multiple of 4.
-//   loss (vt = 2t+1): k = (j, c), c < Q;  A = M_c(i,j) = sum_{(n<=m) in bracket j of row i} Wsym T_c(2 omega_R - 1)
-//                     (Chebyshev moments of the bucket), X = a_c(b,j) = Chebyshev coefficients of the
-//                     degree-(Q-1) interpolant of omega -> f_j^(1-omega) f_(j+1)^omega (LOG) or the exact
-//                     two coefficients (LINEAR, Q = 2).
-// A group (4 quads) stores its 256 doubles in MMA-fragment order: [quad][row block rb][lane], the lane's
-// element being A[k = 4 quad + lane%4][i = 16 t + 8 rb + lane/4].  desc[quad] = xrow | srow << 20: the
-// row of XT holding X for k = 4 quad (rows xrow..xrow+3) and the row whose values scale it (f_n; the
-// ones row for loss quads).
+// Both terms have the form  out[b, i] += sum_k X[b, k] * A[k, i]  (k in quads of 4 = one DMMA.8x8x4).
+//
+//   gain:  rows i are cut into tiles of KX_TI = 16.  k = (n, m) with n <= m;  A = W_inm + W_imn (0 where the triple
+//          is dropped for row i), X = f_n f_m.  For fixed (tile, n) the m with any kept row form one interval: a
+//          "run", padded to a multiple of 4.  A group (4 quads) stores its 256 doubles in MMA-fragment order
+//          [quad][row block rb][lane], the lane's element being A[k = 4 quad + lane%4][i = 16 t + 8 rb + lane/4].
+//          desc[quad] = m0 | n << 20: the rows of f^T holding f_m for the quad (m0..m0+3) and the row that scales
+//          them (f_n; padding quads: 0 | ones_row << 20 with A = 0).  vtptr[t] = first group of tile t.
+//   loss:  k = (j, c), c < Q;  A = M_c(i,j) = sum_{(n<=m) in bracket j of row i} Wsym T_c(2 omega_R - 1)
+//          (Chebyshev moments of the bucket), X = a_c(b,j) = Chebyshev coefficients of the degree-(Q-1) interpolant
+//          of omega -> f_j^(1-omega) f_(j+1)^omega (LOG) or the exact two coefficients (LINEAR, Q = 2).  The operand
+//          is dense: AL[chunk kc][8-row block][quad][lane] holds A[k = 16 kc + 4 quad + lane%4][i = 8 block + lane/4],
+//          so that a chunk of 16 k for 256 consecutive rows (a "supertile") is one contiguous 32 KiB piece.
 struct KxTiled {
-    int NT;                   // number of tiles = ceil(N / 16)
+    int NT;                   // number of gain tiles = ceil(N / 16)
     int Q;                    // Chebyshev coefficients per bracket (LINEAR: 2)
-    int LQ;                   // loss quads per tile = ceil((N-1) Q / 4)
-    int LG;                   // loss groups per tile = ceil(LQ / 4)
+    int LC;                   // loss chunks of 16 k = ceil((N-1) Q / 16)
+    int NR8;                  // 8-row blocks = ceil(N / 8)
+    int RS;                   // 256-row supertiles = ceil(N / 256)
     int ones_row;             // = N: row of XT filled with 1
-    int loss_row0;            // = N + 1: first Chebyshev-coefficient row of XT
-    int xrows;                // rows of XT = loss_row0 + 16 LG
+    int loss_row0;            // = N + 4: first Chebyshev-coefficient row of XT (rows N+1..N+3 stay zero)
+    int xrows;                // rows of XT = loss_row0 + 16 LC
     int *trun_mlo;            // [NT*N] first m of the run (tile, n)
     unsigned *trun_q;         // [NT*N] quads of the run
     unsigned *trun_off;       // [NT*(N+1)] exclusive scan of trun_q inside the tile; [t*(N+1)+N] = quads of tile t
-    unsigned *vtptr;          // [2 NT + 1] exclusive scan of groups per virtual tile
-    double *A;                // [groups][256]
+    unsigned *vtptr;          // [NT + 1] exclusive scan of gain groups per tile
+    double *A;                // [groups][256]   gain operand
     unsigned *desc;           // [groups][4]
+    double *AL;               // [LC][NR8][128]  loss operand
     const double *dct;        // [Q*Q] (2 - delta_c0)/Q cos(c theta_q), theta_q = (2q+1) pi / (2Q)
     const double *nodes;      // [Q] omega_q = (1 + cos theta_q)/2
-    double flag_log2;         // log2(2 / Q!) - log2(eps_flag) ... see kx_tiled.cu k_xt
+    double flag_log2;         // log2(2 / Q!) ... see kx_tiled.cu k_xt
 };
 
 struct kx_handle_s {
@@ -90,13 +92,14 @@ struct kx_handle_s {
     int storage;              // KX_STORE_*
     bool tiled_ok;            // t.A / t.desc describe the current kinematics
     long long cap_groups;     // capacity of t.A / t.desc in groups
-    long long groups;         // host copy of vtptr[2 NT]
+    long long groups;         // host copy of vtptr[NT]
     int ws_xstride;           // columns of XT (batch capacity padded)
     double *XT;               // [t.xrows, ws_xstride] operand rows: f^T, ones, Chebyshev coefficients
     double *fmax;             // [wsB] max_i f[b,i]
     int *mflag;               // [wsB] member needs the exact streaming path (a bracket failed the error bound)
-    double *tpart;            // [tslots, ws_xstride, 16] partials of the DMMA kernel
-    long long tslots;
+    double *gpart;            // [8 sm_count + NT + 1, ws_xstride, 16]  gain partials of the DMMA kernel (one per warp and tile)
+    double *lpart;            // [sm_count + RS + 1, ws_xstride, 256] loss partials
+    int GG, GL;               // CTAs of the gain / loss role in the last launch of the DMMA kernel
     void *tiled_blob;         // one allocation holding the small tables of KxTiled
     bool nnz_stale;
     int chunk_for_B;          // the batch size taskptr was last built for (0 = none)
@@ -127,6 +130,27 @@ struct kx_handle_s {
         }                                                                                      \
     } while (0)
 
+// ---- programmatic dependent launch (PDL): a kernel launched with pdl = true may start while its predecessor in
+// the stream is still running; it calls kx_pdl_wait() before it touches anything the predecessor (or a kernel
+// before that) writes, and kx_pdl_trigger() as early as it likes to let its own successor start.  The first kernel
+// of every API call is launched with pdl = false, so calls never overlap each other.
+template <typename... KArgs, typename... Args>
+inline cudaError_t kx_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl,
+                             Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+#ifdef __CUDACC__
+__device__ __forceinline__ void kx_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void kx_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+
 // ---- launchers implemented in kx_build.cu
 cudaError_t kx_launch_kinematics(const KxDev& d, double m, cudaStream_t s);
 cudaError_t kx_launch_runs(const KxDev& d, cudaStream_t s);      // run table + scan + rowptr
@@ -150,16 +174,17 @@ struct KxStage {             // what the finishing kernel does after the reducti
     double *k1, *k2, *k3;
     double *ydnext;          // where to write yd of the next stage input (fused prep) or null
     // tiled path: partials of the DMMA kernel; members with mflag != 0 take the streaming partials instead
-    const double *tpart;     // [slots, xstride, 16] or null (streaming path only)
-    const unsigned *vtptr;
+    const double *gpart;     // [slots, xstride, 16] or null (streaming path only)
+    const double *lpart;     // [slots, xstride, 256]
+    const unsigned *vtptr;   // [NT + 1]
     const int *mflag;
-    int NT, nctas, xstride;
+    int NT, LC, RS, GW, GL, xstride;      // GW = gain workers (warps), GL = loss workers (CTAs)
     int *flag;
     int evolve;
 };
 cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, cudaStream_t s);
 cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
-                               double* part, int B, const int* mflag, cudaStream_t s);
+                               double* part, int B, const int* mflag, bool pdl, cudaStream_t s);
 cudaError_t kx_launch_finish(const KxDev& d, const double* f, const double* part, int B,
                              const KxStage& st, cudaStream_t s);
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
@@ -169,9 +194,9 @@ cudaError_t kx_launch_tile_runs(const KxDev& d, const KxTiled& t, cudaStream_t s
 cudaError_t kx_launch_tile_fill(const KxDev& d, const KxTiled& t, cudaStream_t s);     // A, desc (gain + loss)
 cudaError_t kx_launch_xt(const KxDev& d, const KxTiled& t, const double* f, double* yd, double* XT, int xstride,
                          double* fmax, int* mflag, int B, cudaStream_t s);
-cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, int G, const double* XT, int xstride,
-                           double* tpart, int B, cudaStream_t s);
+cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
+                           const double* XT, int xstride, double* gpart, double* lpart, int B, cudaStream_t s);
 int kx_xstride(int B);
-int kx_dmma_ctas(int sm_count, long long groups);
+void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long groups, int B, int* GG, int* GL);
 int kx_pick_bt(int N, int B);
 int kx_pick_chunk(long long nnz_est, int N, int B, int sm_count);

@@ -4,17 +4,26 @@
 //   nu[b,i]   = sum_j sum_{c<Q} M_c(i,j) a_c(b,j)   (loss_i = f_i nu_i)   eq. B.19-B.20, see
 //               kx_tiled_build.cu for the Chebyshev-moment form of the interpolated loss term and its error bound
 //
-// Both are out[b,i] += sum_k X[b,k] A[k,i] with A streamed once from HBM/L2 (cp.async ring per warp) and X read
-// from the small operand array XT (L1/L2 resident): X = f_n f_m for gain quads, X = a_c(b,j) for loss quads.
-// The products run on the FP64 tensor pipe: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), M = 8 members, N = 8 rows,
-// K = 4.  Work is cut into equal ranges of groups (4 quads = 2 KiB of A) per CTA; a range that crosses a
-// virtual-tile boundary produces one partial per piece, slot = CTA + virtual tile, and the finishing kernel
-// (kx_contract.cu) adds the partials of a tile in slot order: no atomics, bit-reproducible.
+// Both are out[b,i] += sum_k X[b,k] A[k,i] with A streamed once from HBM/L2 (cp.async) and X built from the small
+// operand array XT: X = f_n f_m for the gain, X = a_c(b,j) for the loss.  The products run on the FP64 tensor
+// pipe: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), M = 8 members, N = 8 rows, K = 4.  The CTAs of one launch are split
+// between the two terms in proportion to their work (see k_dmma); the finishing kernel (kx_contract.cu) adds the
+// partials: no atomics, bit-reproducible.
 //
 // Compiled with --fmad=false; fused multiply-adds are explicit.
 #include "kx_internal.cuh"
 
+#include <stdlib.h>
+
 namespace {
+
+// cost of one loss DMMA relative to one gain DMMA in the CTA split of k_dmma (the dense loss path needs fewer
+// operand loads per DMMA).  KX_LOSS_COST overrides it (tuning aid).
+double loss_cost()
+{
+    static const double v = [] { const char* e = getenv("KX_LOSS_COST"); const double x = e ? atof(e) : 0.0; return x > 0.0 ? x : 0.85; }();
+    return v;
+}
 
 // ---------------------------------------------------------------- per-member maximum, flag reset
 __global__ void __launch_bounds__(256) k_fmax(int N, const double* __restrict__ f, double* __restrict__ fmx,
@@ -58,6 +67,8 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
     const int N = d.N, Q = t.Q, j = blockIdx.x;
     const int bl = threadIdx.x & 63, ph = threadIdx.x >> 6;
     const bool logm = d.interp == KX_INTERP_LOG;
+    kx_pdl_trigger();
+    kx_pdl_wait();          // fmx and the reset of mflag come from k_fmax
     if (logm) {
         for (int k = threadIdx.x; k < Q * Q; k += 256) s_dct[k] = t.dct[k];
         if (threadIdx.x < Q) s_node[threadIdx.x] = t.nodes[threadIdx.x];
@@ -126,151 +137,304 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
 {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-constexpr int kStageBytes = KX_GROUP_DBL * 8 + 16;     // 2 KiB of A + 4 descriptors
+constexpr int kStageBytes = KX_GROUP_DBL * 8 + 16;     // gain ring stage: 2 KiB of A + 4 descriptors
+constexpr int kLossStages = 3;
+constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256 rows of AL ...
+__host__ __device__ constexpr int loss_stage_bytes(int NBT) { return kLossABytes + 16 * (NBT * 8 + 4) * 8; }   // ... + 16 k x members of X
 
+// One CTA per SM.  CTAs [0, GG) take equal ranges of gain groups, CTAs [GG, GG+GL) equal ranges of loss chunks.
+//
+// gain role: f^T of the CTA's 8 NBT members sits in shared memory (row stride 8 NBT + 4 doubles: the 4 x 8 fragment
+//   reads of a quad are bank-conflict free); every warp streams its own share of the groups through a private
+//   cp.async ring and holds a 16-row x 8 NBT-member accumulator (2 NBT DMMA per quad and fragment pair).
+//   The DMMAs of a run (fixed n) take X = f_m and accumulate into T; f_n multiplies T once, when the run ends.
+//   The ring keeps flowing across tile boundaries.
+// loss role: a dense GEMM.  The CTA stages chunks of 16 k (32 KiB of AL for 256 rows + the matching 16 rows of
+//   Chebyshev coefficients) through a 3-stage cp.async pipeline shared by all warps; warp w owns rows
+//   [32 w, 32 w + 32) x 8 NBT members (4 NBT DMMA per quad).
+// A range that crosses a tile (supertile) boundary produces one partial per piece, slot = worker + tile (a gain
+// worker is a warp, a loss worker a CTA); the finishing kernel adds the partials of a row in slot order: no
+// atomics, bit-reproducible.
 template <int NBT, int WARPS, int STAGES>
 __global__ void __launch_bounds__(WARPS * 32, 1)
-k_dmma(KxTiled t, const double* __restrict__ XT, int xstride, double* __restrict__ part)
+k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, const double* __restrict__ XT, int xstride,
+       double* __restrict__ gpart, double* __restrict__ lpart, int GG, int GL)
 {
     extern __shared__ __align__(16) unsigned char smem[];
+    constexpr int LD = NBT * 8 + 4;
+    constexpr int NTHR = WARPS * 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    unsigned char* ring = smem + (size_t)warp * STAGES * kStageBytes;
-    double* slab = reinterpret_cast<double*>(smem + (size_t)WARPS * STAGES * kStageBytes);   // [WARPS][NBT*8][16]
-
-    const unsigned Gtot = t.vtptr[2 * t.NT];
-    const unsigned nC = gridDim.x, c = blockIdx.x;
-    const unsigned g0 = (unsigned)((unsigned long long)c * Gtot / nC);
-    const unsigned g1 = (unsigned)((unsigned long long)(c + 1) * Gtot / nC);
+    const int krow = lane & 3, lr = lane >> 2;
     const int bcol0 = blockIdx.y * (NBT * 8);
-    const double* __restrict__ xcol = XT + bcol0 + (lane >> 2);   // + row * xstride + 8 bt
-    const int krow = lane & 3;
+    kx_pdl_trigger();
 
-    int vt = 0;
-    unsigned g = g0;
-    while (g < g1) {
-        while (t.vtptr[vt + 1] <= g) ++vt;
-        const unsigned pe = min(g1, t.vtptr[vt + 1]);
-        const unsigned len = pe - g, per = (len + WARPS - 1) / WARPS;
-        const unsigned wg0 = min(g + warp * per, pe), wg1 = min(wg0 + per, pe);
-        const unsigned n = wg1 - wg0;
+    if ((int)blockIdx.x < GG) {
+        // ------------------------------------------------------------ gain role: every warp is an independent worker
+        unsigned* s_vt = reinterpret_cast<unsigned*>(smem);                               // [NT + 1]
+        const int vtbytes = ((t.NT + 1) * 4 + 15) & ~15;
+        double* s_f = reinterpret_cast<double*>(smem + vtbytes);                          // [N + 4][LD]
+        unsigned char* ring = smem + vtbytes + (size_t)(N + 4) * LD * 8 + (size_t)warp * STAGES * kStageBytes;
 
-        double acc[NBT][2][2];
+        const unsigned NW = (unsigned)GG * WARPS, wk = blockIdx.x * WARPS + warp;
+        const unsigned g0 = (unsigned)((unsigned long long)wk * Gtot / NW);
+        const unsigned g1 = (unsigned)((unsigned long long)(wk + 1) * Gtot / NW);
+        const unsigned n = g1 - g0;
+        auto issue = [&](unsigned gi) {
+            const double* src = t.A + (size_t)(g0 + gi) * KX_GROUP_DBL;
+            unsigned char* dst = ring + (size_t)(gi % STAGES) * kStageBytes;
 #pragma unroll
-        for (int bt = 0; bt < NBT; ++bt) { acc[bt][0][0] = acc[bt][0][1] = acc[bt][1][0] = acc[bt][1][1] = 0.0; }
-
-        if (n > 0) {
-            auto issue = [&](unsigned grp) {
-                const double* src = t.A + (size_t)grp * KX_GROUP_DBL;
-                unsigned char* dst = ring + (size_t)((grp - wg0) % STAGES) * kStageBytes;
+            for (int k = 0; k < 4; ++k) cp_async16(dst + (k * 32 + lane) * 16, src + (k * 32 + lane) * 2);
+            if (lane == 0) cp_async16(dst + KX_GROUP_DBL * 8, t.desc + (size_t)(g0 + gi) * 4);
+        };
+        // The gain role reads only the caller's f and the tensor, nothing an earlier kernel of this call writes: under
+        // programmatic dependent launch it runs while the operand-preparation kernel is still at work.
+        // The tensor stream starts first; f^T and the tile table arrive while it is in flight.
 #pragma unroll
-                for (int k = 0; k < 4; ++k) cp_async16(dst + (k * 32 + lane) * 16, src + (k * 32 + lane) * 2);
-                if (lane == 0) cp_async16(dst + KX_GROUP_DBL * 8, t.desc + (size_t)grp * 4);
-            };
-#pragma unroll
-            for (int s = 0; s < STAGES - 1; ++s) {
-                if ((unsigned)s < n) issue(wg0 + s);
-                cp_async_commit();
-            }
-            // groups 0 and 1 must have landed before the first quad (X of quad q+1 is fetched during quad q)
-            cp_async_wait<STAGES - 3>();
-            __syncwarp();
-
-            double xn[NBT], sn[NBT];
-            unsigned srow_cur;
-            {
-                const unsigned dsc = *reinterpret_cast<const unsigned*>(ring + KX_GROUP_DBL * 8);
-                const unsigned xrow = dsc & 0xFFFFFu;
-                srow_cur = dsc >> 20;
-                const double* xr = xcol + (size_t)(xrow + krow) * xstride;
-                const double* sr = xcol + (size_t)srow_cur * xstride;
-#pragma unroll
-                for (int bt = 0; bt < NBT; ++bt) { xn[bt] = xr[8 * bt]; sn[bt] = sr[8 * bt]; }
-            }
-            double sc[NBT];
-#pragma unroll
-            for (int bt = 0; bt < NBT; ++bt) sc[bt] = sn[bt];
-
-            for (unsigned gi = 0; gi < n; ++gi) {
-                // refill the slot freed by group gi-1, then make sure groups gi and gi+1 are in shared memory
-                if (gi + STAGES - 1 < n) issue(wg0 + gi + STAGES - 1);
-                cp_async_commit();
-                cp_async_wait<STAGES - 2>();
-                __syncwarp();
-                const unsigned char* st = ring + (size_t)(gi % STAGES) * kStageBytes;
-                const double* wd = reinterpret_cast<const double*>(st);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    double xv[NBT];
-#pragma unroll
-                    for (int bt = 0; bt < NBT; ++bt) xv[bt] = xn[bt] * sc[bt];
-                    // prefetch X (and the scale row when it changes) of the next quad
-                    const bool more = (q < 3) || (gi + 1 < n);
-                    if (more) {
-                        const unsigned char* stn = (q < 3) ? st : ring + (size_t)((gi + 1) % STAGES) * kStageBytes;
-                        const unsigned dsc = *reinterpret_cast<const unsigned*>(stn + KX_GROUP_DBL * 8 + 4 * ((q + 1) & 3));
-                        const unsigned xrow = dsc & 0xFFFFFu, srow = dsc >> 20;
-                        const double* xr = xcol + (size_t)(xrow + krow) * xstride;
-#pragma unroll
-                        for (int bt = 0; bt < NBT; ++bt) xn[bt] = xr[8 * bt];
-                        if (srow != srow_cur) {
-                            srow_cur = srow;
-                            const double* sr = xcol + (size_t)srow * xstride;
-#pragma unroll
-                            for (int bt = 0; bt < NBT; ++bt) sn[bt] = sr[8 * bt];
-                        }
-                    }
-                    const double w0 = wd[q * 64 + lane], w1 = wd[q * 64 + 32 + lane];
-#pragma unroll
-                    for (int bt = 0; bt < NBT; ++bt) {
-                        dmma884(acc[bt][0][0], acc[bt][0][1], xv[bt], w0);
-                        dmma884(acc[bt][1][0], acc[bt][1][1], xv[bt], w1);
-                    }
-#pragma unroll
-                    for (int bt = 0; bt < NBT; ++bt) sc[bt] = sn[bt];
-                }
-                __syncwarp();     // every lane is done with this stage before it is refilled
-            }
-            cp_async_wait<0>();
+        for (int s = 0; s < STAGES - 1; ++s) {
+            if ((unsigned)s < n) issue(s);
+            cp_async_commit();
         }
+        // f^T: s_f[n][b] = f[bcol0 + b][n].  A warp moves blocks of 8 n x 4 members: 64-byte runs of f in, a
+        // bank-conflict-free 8 x 4 patch of s_f out (row stride LD = 4 mod 16 doubles).
+        {
+            const int nl = lane >> 2, bl = lane & 3;
+            const int nblk = (N + 7) >> 3, total = nblk * (NBT * 2);
+            for (int k0 = warp; k0 < total; k0 += 32 * WARPS) {
+                double v[32];
+#pragma unroll
+                for (int u = 0; u < 32; ++u) {
+                    const int k = k0 + u * WARPS;
+                    const int bq = k / nblk, nb_ = k - bq * nblk;
+                    const int nn = nb_ * 8 + nl, b = bcol0 + bq * 4 + bl;
+                    v[u] = (k < total && nn < N && b < B) ? __ldg(f + (size_t)b * N + nn) : 0.0;
+                }
+#pragma unroll
+                for (int u = 0; u < 32; ++u) {
+                    const int k = k0 + u * WARPS;
+                    const int bq = k / nblk, nb_ = k - bq * nblk;
+                    const int nn = nb_ * 8 + nl;
+                    if (k < total && nn < N) s_f[(size_t)nn * LD + bq * 4 + bl] = v[u];
+                }
+            }
+            for (int k = tid; k < 4 * LD; k += NTHR) s_f[(size_t)N * LD + k] = k < LD ? 1.0 : 0.0;     // ones row, 3 zero rows
+        }
+        for (int k = tid; k <= t.NT; k += NTHR) s_vt[k] = t.vtptr[k];
+        cp_async_wait<0>();
+        __syncthreads();
+        if (n == 0) { kx_pdl_wait(); return; }
 
-        // fixed-order reduction over the CTA's warps: lane holds out[b = 8 bt + lane/4][i = 8 rb + 2 (lane%4) + {0,1}]
+        const double* xcol = s_f + lr;                       // + row * LD + 8 bt
+        int vt = 0;
+        while (s_vt[vt + 1] <= g0) ++vt;
+        unsigned bnd = s_vt[vt + 1] - g0;                    // first group (relative) of the next tile
+
+        // acc: the tile's partial.  T: sum over the m of the current run (fixed n) of f_m A[(n,m), i]; when the run ends,
+        // acc += f_n T.  Lane holds out[b = 8 bt + lane/4][i = 8 rb + 2 (lane%4) + {0,1}], the same member b as its
+        // fragment of X, so f_n[b] scales its own accumulators.
+        double acc[NBT][2][2], T[NBT][2][2], sn[NBT];
 #pragma unroll
         for (int bt = 0; bt < NBT; ++bt)
 #pragma unroll
-            for (int rb = 0; rb < 2; ++rb)
-                *reinterpret_cast<double2*>(&slab[((size_t)warp * NBT * 8 + bt * 8 + (lane >> 2)) * 16 + rb * 8 + 2 * (lane & 3)]) =
-                    make_double2(acc[bt][rb][0], acc[bt][rb][1]);
-        __syncthreads();
-        double* dst = part + ((size_t)(c + vt) * xstride + bcol0) * 16;
-        for (int e = tid; e < NBT * 128; e += WARPS * 32) {
-            double s = 0.0;
+            for (int rb = 0; rb < 2; ++rb) { acc[bt][rb][0] = acc[bt][rb][1] = 0.0; T[bt][rb][0] = T[bt][rb][1] = 0.0; }
+        auto fold = [&]() {
 #pragma unroll
-            for (int w = 0; w < WARPS; ++w) s += slab[(size_t)w * NBT * 128 + e];
-            dst[e] = s;
+            for (int bt = 0; bt < NBT; ++bt)
+#pragma unroll
+                for (int rb = 0; rb < 2; ++rb) {
+                    acc[bt][rb][0] = fma(sn[bt], T[bt][rb][0], acc[bt][rb][0]);
+                    acc[bt][rb][1] = fma(sn[bt], T[bt][rb][1], acc[bt][rb][1]);
+                    T[bt][rb][0] = T[bt][rb][1] = 0.0;
+                }
+        };
+        // one partial per (worker, tile), slot = worker + tile
+        auto flush = [&](int tile) {
+            double* dst = gpart + ((size_t)(wk + tile) * xstride + bcol0 + lr) * 16 + 2 * krow;
+#pragma unroll
+            for (int bt = 0; bt < NBT; ++bt)
+#pragma unroll
+                for (int rb = 0; rb < 2; ++rb) {
+                    *reinterpret_cast<double2*>(dst + (size_t)bt * 128 + rb * 8) = make_double2(acc[bt][rb][0], acc[bt][rb][1]);
+                    acc[bt][rb][0] = acc[bt][rb][1] = 0.0;
+                }
+        };
+
+        // descriptors of the current group (dc) and the next one (dn) stay in registers: the f_m rows of a quad are
+        // requested a whole quad before they are used
+        uint4 dc = *reinterpret_cast<const uint4*>(ring + KX_GROUP_DBL * 8);
+        unsigned srow_cur = dc.x >> 20;
+        double xv[NBT];
+        {
+            const double* xr = xcol + (size_t)((dc.x & 0xFFFFFu) + krow) * LD;
+            const double* sr = xcol + (size_t)srow_cur * LD;
+#pragma unroll
+            for (int bt = 0; bt < NBT; ++bt) { sn[bt] = sr[8 * bt]; xv[bt] = xr[8 * bt]; }
         }
-        __syncthreads();
-        g = pe;
+
+        for (unsigned gi = 0; gi < n; ++gi) {
+            if (gi == bnd) {                                 // the range crosses into the next tile
+                fold();
+                flush(vt);
+                do { ++vt; } while (s_vt[vt + 1] - g0 <= gi);
+                bnd = s_vt[vt + 1] - g0;
+            }
+            // refill the slot freed by group gi-1, then make sure groups gi and gi+1 are in shared memory
+            if (gi + STAGES - 1 < n) issue(gi + STAGES - 1);
+            cp_async_commit();
+            cp_async_wait<STAGES - 2>();
+            __syncwarp();
+            const unsigned char* st = ring + (size_t)(gi % STAGES) * kStageBytes;
+            const double* wd = reinterpret_cast<const double*>(st) + lane;
+            const bool last_group = gi + 1 >= n;
+            uint4 dn = dc;
+            if (!last_group) dn = *reinterpret_cast<const uint4*>(ring + (size_t)((gi + 1) % STAGES) * kStageBytes + KX_GROUP_DBL * 8);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const unsigned dsc = q == 0 ? dc.y : (q == 1 ? dc.z : (q == 2 ? dc.w : dn.x));    // next quad
+                const bool more = (q < 3) || !last_group;
+                double xn[NBT];
+                {
+                    const double* xr = xcol + (size_t)((dsc & 0xFFFFFu) + krow) * LD;
+#pragma unroll
+                    for (int bt = 0; bt < NBT; ++bt) xn[bt] = xr[8 * bt];
+                }
+                const double w0 = wd[q * 64], w1 = wd[q * 64 + 32];
+#pragma unroll
+                for (int bt = 0; bt < NBT; ++bt) {
+                    dmma884(T[bt][0][0], T[bt][0][1], xv[bt], w0);
+                    dmma884(T[bt][1][0], T[bt][1][1], xv[bt], w1);
+                }
+                const unsigned srow = dsc >> 20;
+                if (more && srow != srow_cur) {              // the run (n) ends with this quad
+                    fold();
+                    srow_cur = srow;
+                    const double* sr = xcol + (size_t)srow * LD;
+#pragma unroll
+                    for (int bt = 0; bt < NBT; ++bt) sn[bt] = sr[8 * bt];
+                }
+#pragma unroll
+                for (int bt = 0; bt < NBT; ++bt) xv[bt] = xn[bt];
+            }
+            dc = dn;
+            __syncwarp();     // every lane is done with this stage before it is refilled
+        }
+        fold();
+        flush(vt);
+        kx_pdl_wait();        // the grid must not complete before the kernels it follows have
+        return;
+    }
+
+    // ---------------------------------------------------------------- loss role
+    {
+        constexpr int SB = loss_stage_bytes(NBT);
+        kx_pdl_wait();        // the Chebyshev coefficients in XT come from k_xt
+        const unsigned cl = blockIdx.x - GG;
+        const unsigned LC = (unsigned)t.LC;
+        const unsigned U = (unsigned)t.RS * LC;
+        const unsigned u0 = (unsigned)((unsigned long long)cl * U / (unsigned)GL);
+        const unsigned u1 = (unsigned)((unsigned long long)(cl + 1) * U / (unsigned)GL);
+        unsigned u = u0;
+        while (u < u1) {
+            const unsigned sp = u / LC;                                  // supertile
+            const unsigned ue = min(u1, (sp + 1) * LC);
+            const unsigned ka = u - sp * LC, n = ue - u;
+            const int nb = min(32, t.NR8 - 32 * (int)sp);                // 8-row blocks of this supertile
+            const int nbw = min(4, max(0, nb - 4 * warp));               // ... of this warp
+
+            auto issue = [&](unsigned kc, int slot) {
+                unsigned char* dstA = smem + (size_t)slot * SB;
+                const double* srcA = t.AL + ((size_t)kc * t.NR8 + 32 * sp) * 128;
+                for (int k = tid; k < nb * 64; k += NTHR) cp_async16(dstA + (size_t)k * 16, srcA + (size_t)k * 2);
+                double* dstX = reinterpret_cast<double*>(dstA + kLossABytes);
+                const double* srcX = XT + (size_t)(t.loss_row0 + 16 * kc) * xstride + bcol0;
+                for (int k = tid; k < 16 * NBT * 4; k += NTHR) {
+                    const int r = k / (NBT * 4), cc = k - r * (NBT * 4);
+                    cp_async16(dstX + (size_t)r * LD + 2 * cc, srcX + (size_t)r * xstride + 2 * cc);
+                }
+            };
+
+            double acc[4][NBT][2];
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int bt = 0; bt < NBT; ++bt) acc[r][bt][0] = acc[r][bt][1] = 0.0;
+
+#pragma unroll
+            for (int s = 0; s < kLossStages - 1; ++s) {
+                if ((unsigned)s < n) issue(ka + s, s);
+                cp_async_commit();
+            }
+            for (unsigned it = 0; it < n; ++it) {
+                cp_async_wait<kLossStages - 2>();        // this thread's copies of chunk `it` have landed
+                __syncthreads();                         // everyone's have; everyone is done with chunk it-1
+                if (it + kLossStages - 1 < n) issue(ka + it + kLossStages - 1, (int)((it + kLossStages - 1) % kLossStages));
+                cp_async_commit();
+                if (nbw > 0) {
+                    const double* sA = reinterpret_cast<const double*>(smem + (size_t)(it % kLossStages) * SB) + (size_t)warp * 512 + lane;
+                    const double* sX = reinterpret_cast<const double*>(smem + (size_t)(it % kLossStages) * SB + kLossABytes) + (size_t)krow * LD + lr;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        double xv[NBT];
+#pragma unroll
+                        for (int bt = 0; bt < NBT; ++bt) xv[bt] = sX[(size_t)(4 * q) * LD + 8 * bt];
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) {
+                            const double w = sA[(r * 4 + q) * 32];
+#pragma unroll
+                            for (int bt = 0; bt < NBT; ++bt) dmma884(acc[r][bt][0], acc[r][bt][1], xv[bt], w);
+                        }
+                    }
+                }
+            }
+            cp_async_wait<0>();
+            __syncthreads();              // the stages are free again for the next piece
+
+            double* dst = lpart + ((size_t)(cl + sp) * xstride + bcol0) * 256 + 32 * warp + 2 * krow;
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+                if (r < nbw)
+#pragma unroll
+                    for (int bt = 0; bt < NBT; ++bt)
+                        *reinterpret_cast<double2*>(dst + (size_t)(8 * bt + lr) * 256 + 8 * r) = make_double2(acc[r][bt][0], acc[r][bt][1]);
+            u = ue;
+        }
     }
 }
 
 template <int NBT, int WARPS, int STAGES>
-cudaError_t launch_dmma_t(const KxTiled& t, int G, const double* XT, int xstride, double* tpart, int B, cudaStream_t s)
+size_t dmma_smem(const KxTiled& t, int N)
 {
-    const size_t smem = (size_t)WARPS * STAGES * kStageBytes + (size_t)WARPS * NBT * 128 * 8;
+    const size_t gain = (size_t)(((t.NT + 1) * 4 + 15) & ~15) + (size_t)(N + 4) * (NBT * 8 + 4) * 8 + (size_t)WARPS * STAGES * kStageBytes;
+    const size_t loss = (size_t)kLossStages * loss_stage_bytes(NBT);
+    return gain > loss ? gain : loss;
+}
+
+template <int NBT, int WARPS, int STAGES>
+cudaError_t launch_dmma_t(const KxTiled& t, int N, unsigned Gtot, int GG, int GL, const double* f, const double* XT, int xstride,
+                          double* gpart, double* lpart, int B, cudaStream_t s)
+{
+    const size_t smem = dmma_smem<NBT, WARPS, STAGES>(t, N);
     cudaError_t e = cudaFuncSetAttribute(k_dmma<NBT, WARPS, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid(G, (B + NBT * 8 - 1) / (NBT * 8));
-    k_dmma<NBT, WARPS, STAGES><<<grid, WARPS * 32, smem, s>>>(t, XT, xstride, tpart);
-    return cudaGetLastError();
+    dim3 grid(GG + GL, (B + NBT * 8 - 1) / (NBT * 8));
+    return kx_launch(k_dmma<NBT, WARPS, STAGES>, grid, dim3(WARPS * 32), smem, s, true, t, N, B, Gtot, f, XT, xstride, gpart, lpart, GG, GL);
+}
+
+// member tiles (of 8) per CTA: limited by the batch and by the shared memory f^T of the gain role needs
+int dmma_nbt(int N, int B)
+{
+    int nbt = B <= 8 ? 1 : (B <= 16 ? 2 : (B <= 32 ? 4 : 8));
+    auto need = [&](int k) { return (size_t)(N + 4) * (k * 8 + 4) * 8 + (size_t)8 * (k <= 2 ? 8 : 4) * kStageBytes + 512; };
+    while (nbt > 1 && need(nbt) > 227u * 1024u) nbt >>= 1;
+    return nbt;
 }
 
 }  // namespace
 
-// columns of XT / tpart for a batch of B members: whole 8-member MMA tiles, whole CTA column groups
+// columns of XT / the partials for a batch of B members: whole 8-member MMA tiles, whole CTA column groups
 int kx_xstride(int B)
 {
     if (B <= 8) return 8;
@@ -279,27 +443,39 @@ int kx_xstride(int B)
     return ((B + 63) / 64) * 64;
 }
 
-int kx_dmma_ctas(int sm_count, long long groups)
+// CTAs per role.  Work in units of one gain group (8 DMMA per member tile): gain = groups, loss = LC * NR8 / 2.
+void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long groups, int B, int* GG, int* GL)
 {
-    long long g = groups / 8;
-    if (g < 1) g = 1;
-    return (int)(g < sm_count ? g : sm_count);
+    const int nbt = dmma_nbt(d.N, B);
+    const int ny = (B + nbt * 8 - 1) / (nbt * 8);
+    const double wg = (double)(groups > 0 ? groups : 1);
+    const double wl = 0.5 * (double)t.LC * (double)t.NR8 * loss_cost();
+    long long G = (long long)((wg + wl) / 8.0);
+    const long long cap = sm_count / ny > 2 ? sm_count / ny : 2;
+    if (G > cap) G = cap;
+    if (G < 2) G = 2;
+    int gl = (int)((double)G * wl / (wg + wl) + 0.5);
+    if (gl < 1) gl = 1;
+    if (gl > (int)G - 1) gl = (int)G - 1;
+    *GL = gl;
+    *GG = (int)G - gl;
 }
 
 cudaError_t kx_launch_xt(const KxDev& d, const KxTiled& t, const double* f, double* yd, double* XT, int xstride,
                          double* fmax, int* mflag, int B, cudaStream_t s)
 {
-    k_fmax<<<B, 256, 0, s>>>(d.N, f, fmax, mflag);
-    k_xt<<<d.N + 1, 256, 0, s>>>(d, t, f, reinterpret_cast<double2*>(yd), XT, xstride, fmax, mflag, B);
-    return cudaGetLastError();
+    k_fmax<<<B, 256, 0, s>>>(d.N, f, fmax, mflag);        // first kernel of the call: ordinary launch
+    return kx_launch(k_xt, dim3(d.N + 1), dim3(256), 0, s, true, d, t, f, reinterpret_cast<double2*>(yd), XT, xstride,
+                     (const double*)fmax, mflag, B);
 }
 
-cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, int G, const double* XT, int xstride,
-                           double* tpart, int B, cudaStream_t s)
+cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
+                           const double* XT, int xstride, double* gpart, double* lpart, int B, cudaStream_t s)
 {
-    (void)d;
-    if (B <= 8) return launch_dmma_t<1, 8, 8>(t, G, XT, xstride, tpart, B, s);
-    if (B <= 16) return launch_dmma_t<2, 8, 8>(t, G, XT, xstride, tpart, B, s);
-    if (B <= 32) return launch_dmma_t<4, 8, 4>(t, G, XT, xstride, tpart, B, s);
-    return launch_dmma_t<8, 8, 4>(t, G, XT, xstride, tpart, B, s);
+    switch (dmma_nbt(d.N, B)) {
+        case 1: return launch_dmma_t<1, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+        case 2: return launch_dmma_t<2, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+        case 4: return launch_dmma_t<4, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+        default: return launch_dmma_t<8, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+    }
 }

@@ -70,27 +70,16 @@ __global__ void __launch_bounds__(1024) k_tile_scan(KxDev d, KxTiled t)
     if (tid == N - 1) t.trun_off[tile * (N + 1) + N] = excl + cnt;
 }
 
-// groups per virtual tile -> vtptr; loss descriptors
+// gain groups per tile -> vtptr
 __global__ void k_vt_scan(KxDev d, KxTiled t)
 {
     if (threadIdx.x || blockIdx.x) return;
     unsigned run = 0;
     for (int tile = 0; tile < t.NT; ++tile) {
-        t.vtptr[2 * tile] = run;
+        t.vtptr[tile] = run;
         run += (t.trun_off[tile * (d.N + 1) + d.N] + 3u) >> 2;
-        t.vtptr[2 * tile + 1] = run;
-        run += (unsigned)t.LG;
     }
-    t.vtptr[2 * t.NT] = run;
-}
-
-__global__ void k_loss_desc(KxTiled t)
-{
-    const int lq = blockIdx.x * blockDim.x + threadIdx.x;
-    const int tile = blockIdx.y;
-    if (lq >= 4 * t.LG) return;
-    const size_t q = (size_t)t.vtptr[2 * tile + 1] * 4 + lq;
-    t.desc[q] = (unsigned)(t.loss_row0 + 4 * lq) | ((unsigned)t.ones_row << 20);
+    t.vtptr[t.NT] = run;
 }
 
 // ---------------------------------------------------------------- gain operand
@@ -102,7 +91,7 @@ __global__ void __launch_bounds__(256) k_pack_gain(KxDev d, KxTiled t)
     const unsigned* __restrict__ off = t.trun_off + (size_t)tile * (N + 1);
     const unsigned tq = off[N];                       // quads of this tile
     const unsigned nq = ((tq + 3u) >> 2) << 2;        // padded to whole groups
-    const size_t qbase = (size_t)t.vtptr[2 * tile] * 4;
+    const size_t qbase = (size_t)t.vtptr[tile] * 4;
     const double* __restrict__ K = d.K;
     const double* __restrict__ P = d.p;
     const double K0 = K[0], KN1 = K[N - 1];
@@ -146,11 +135,10 @@ __global__ void __launch_bounds__(128) k_cheb_moments(KxDev d, KxTiled t)
 {
     const int N = d.N;
     const int i = blockIdx.x;
-    const int tile = i / KX_TI, rb = (i % KX_TI) >> 3, ir = i & 7;
+    const int rb8 = i >> 3, ir = i & 7;
     const double* __restrict__ K = d.K;
     const double* __restrict__ P = d.p;
     const double K0 = K[0], KN1 = K[N - 1], Ki = K[i], pi_ = P[i];
-    const size_t qbase = (size_t)t.vtptr[2 * tile + 1] * 4;
     for (int j = threadIdx.x; j < N - 1; j += blockDim.x) {
         const double Kj = K[j], Kj1 = K[j + 1];
         const double inv = Kj1 - Kj;
@@ -202,7 +190,7 @@ __global__ void __launch_bounds__(128) k_cheb_moments(KxDev d, KxTiled t)
 #pragma unroll
         for (int c = 0; c < Q; ++c) {
             const int k = j * Q + c;
-            t.A[(qbase + (size_t)(k >> 2)) * 64 + rb * 32 + ir * 4 + (k & 3)] = M[c];
+            t.AL[(((size_t)(k >> 4) * t.NR8 + rb8) * 4 + ((k >> 2) & 3)) * 32 + ir * 4 + (k & 3)] = M[c];
         }
     }
 }
@@ -220,8 +208,6 @@ cudaError_t kx_launch_tile_runs(const KxDev& d, const KxTiled& t, cudaStream_t s
 
 cudaError_t kx_launch_tile_fill(const KxDev& d, const KxTiled& t, cudaStream_t s)
 {
-    dim3 gd((4 * t.LG + 127) / 128, t.NT);
-    k_loss_desc<<<gd, 128, 0, s>>>(t);
     int per_tile = (148 * 8 + t.NT - 1) / t.NT;
     dim3 gg(per_tile, t.NT);
     k_pack_gain<<<gg, 256, 0, s>>>(d, t);
