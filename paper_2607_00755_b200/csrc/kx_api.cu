@@ -97,9 +97,9 @@ void free_ws(kx_handle_s* h)
 {
     cudaFree(h->yd); cudaFree(h->part); cudaFree(h->fstage); cudaFree(h->k1); cudaFree(h->k2);
     cudaFree(h->k3); cudaFree(h->Cbuf); cudaFree(h->hostio);
-    cudaFree(h->XT); cudaFree(h->fmax); cudaFree(h->mflag); cudaFree(h->gpart); cudaFree(h->lpart);
+    cudaFree(h->XT); cudaFree(h->mstat); cudaFree(h->gpart); cudaFree(h->lpart);
     h->yd = h->part = h->fstage = h->k1 = h->k2 = h->k3 = h->Cbuf = h->hostio = nullptr;
-    h->XT = h->fmax = h->gpart = h->lpart = nullptr; h->mflag = nullptr;
+    h->XT = h->gpart = h->lpart = nullptr; h->mstat = nullptr;
     h->wsB = 0; h->ws_tasks = 0; h->ws_xstride = 0;
 }
 
@@ -125,9 +125,13 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
         const int xs = kx_xstride(nB);
         KX_CUDA(dalloc(&h->XT, (size_t)h->t.xrows * xs));
         KX_CUDA(cudaMemset(h->XT, 0, (size_t)h->t.xrows * xs * 8));      // padding rows stay zero for good
-        KX_CUDA(dalloc(&h->fmax, (size_t)nB));
-        KX_CUDA(dalloc(&h->mflag, (size_t)nB));
-        KX_CUDA(dalloc(&h->gpart, (size_t)(8 * h->sm_count + h->t.NT + 1) * xs * 16));
+        KX_CUDA(dalloc(&h->mstat, (size_t)nB * 2));
+        {
+            std::vector<long long> init((size_t)nB * 2);
+            for (int b = 0; b < nB; ++b) { init[2 * b] = (-0x7fffffffffffffffLL - 1); init[2 * b + 1] = 0; }
+            KX_CUDA(cudaMemcpy(h->mstat, init.data(), init.size() * 8, cudaMemcpyHostToDevice));
+        }
+        KX_CUDA(dalloc(&h->gpart, (size_t)(16 * h->sm_count + h->t.NT + 1) * xs * 16));
         KX_CUDA(dalloc(&h->lpart, (size_t)(h->sm_count + h->t.RS + 1) * xs * 256));
         h->ws_xstride = xs;
     }
@@ -198,21 +202,21 @@ kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bo
     if (use_tiled) {
         const int xs = h->ws_xstride;
         kx_dmma_split(h->d, h->t, h->sm_count, h->groups, B, &h->GG, &h->GL);
-        KX_CUDA(kx_launch_xt(h->d, h->t, f, h->yd, h->XT, xs, h->fmax, h->mflag, B, s));
+        KX_CUDA(kx_launch_xt(h->d, h->t, f, h->yd, h->XT, xs, h->mstat, B, s));
         if ((rc = prof_begin()) != KX_OK) return rc;
         KX_CUDA(kx_launch_dmma(h->d, h->t, h->groups, h->GG, h->GL, f, h->XT, xs, h->gpart, h->lpart, B, s));
         if ((rc = prof_end()) != KX_OK) return rc;
         if (h->d.interp == KX_INTERP_LOG)      // exact streaming path for flagged members only (LINEAR is exact)
-            KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, h->mflag, true, s));
+            KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, h->mstat, true, s));
         st->gpart = h->gpart; st->lpart = h->lpart; st->vtptr = h->t.vtptr;
-        st->mflag = h->d.interp == KX_INTERP_LOG ? h->mflag : nullptr;
-        st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS; st->GW = 8 * h->GG; st->GL = h->GL; st->xstride = xs;
+        st->mstat = h->d.interp == KX_INTERP_LOG ? h->mstat : nullptr;
+        st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS; st->GW = kx_dmma_workers(h->d.N, B) * h->GG; st->GL = h->GL; st->xstride = xs;
     } else {
         if (!have_yd) KX_CUDA(kx_launch_prep(h->d, f, h->yd, B, s));
         if ((rc = prof_begin()) != KX_OK) return rc;
         KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, nullptr, !have_yd, s));
         if ((rc = prof_end()) != KX_OK) return rc;
-        st->gpart = nullptr; st->lpart = nullptr; st->vtptr = nullptr; st->mflag = nullptr;
+        st->gpart = nullptr; st->lpart = nullptr; st->vtptr = nullptr; st->mstat = nullptr;
     }
     return KX_OK;
 }

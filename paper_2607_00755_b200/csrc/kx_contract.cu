@@ -66,7 +66,7 @@ enum { MODE_LOG_TAB = 0, MODE_LOG_LIBM = 1, MODE_LINEAR = 2 };
 template <int BT, int MODE>
 __global__ void __launch_bounds__(KX_CTA, 2)
 k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd,
-           double* __restrict__ part, int B, const int* __restrict__ mflag)
+           double* __restrict__ part, int B, const long long* __restrict__ mstat)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = d.N;
@@ -81,9 +81,9 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
     const int nb = min(BT, B - b0);
     kx_pdl_trigger();
     kx_pdl_wait();
-    if (mflag) {          // tiled path: only member groups holding a flagged member take the exact streaming path
-        int any = 0;
-        for (int b = 0; b < nb; ++b) any |= mflag[b0 + b];
+    if (mstat) {          // tiled path: only member groups holding a flagged member take the exact streaming path
+        bool any = false;
+        for (int b = 0; b < nb; ++b) any = any || kx_member_flagged(mstat, b0 + b);
         if (!any) return;
     }
 
@@ -221,7 +221,11 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
     const int N = d.N, tid = threadIdx.x, b = blockIdx.x;
     const double* fb = fin + (size_t)b * N;
     kx_pdl_wait();
-    const bool tiled = st.gpart != nullptr && !(st.mflag && st.mflag[b]);
+    const bool tiled = st.gpart != nullptr && !(st.mstat && kx_member_flagged(st.mstat, b));
+    if (st.mstat) {          // last reader of the member's statistics: reset them for the next call
+        __syncthreads();
+        if (tid == 0) { st.mstat[2 * b] = KX_MSTAT_NONE; st.mstat[2 * b + 1] = 0; }
+    }
 
     double C[kMaxPerThread], fi[kMaxPerThread], hi_[kMaxPerThread], Ei[kMaxPerThread], Ki[kMaxPerThread];
 #pragma unroll
@@ -403,7 +407,7 @@ k_moments(KxDev d, const double* __restrict__ f, double* n, double* rho, double*
 
 template <int BT, int MODE>
 cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, const double* yd,
-                              double* part, int B, const int* mflag, bool pdl, cudaStream_t s)
+                              double* part, int B, const long long* mstat, bool pdl, cudaStream_t s)
 {
     const int N = d.N;
     size_t smem = (size_t)BT * N * 24 + (size_t)(KX_CTA / 32) * 2 * BT * 8
@@ -418,16 +422,16 @@ cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, con
     int gx = (sm_count * occ + groups - 1) / groups;
     if (gx < 1) gx = 1;
     dim3 grid(gx, groups);
-    return kx_launch(k_contract<BT, MODE>, grid, dim3(KX_CTA), smem, s, pdl, d, f, reinterpret_cast<const double2*>(yd), part, B, mflag);
+    return kx_launch(k_contract<BT, MODE>, grid, dim3(KX_CTA), smem, s, pdl, d, f, reinterpret_cast<const double2*>(yd), part, B, mstat);
 }
 
 template <int BT>
 cudaError_t launch_contract_m(const KxDev& d, int sm_count, const double* f, const double* yd,
-                              double* part, int B, const int* mflag, bool pdl, cudaStream_t s)
+                              double* part, int B, const long long* mstat, bool pdl, cudaStream_t s)
 {
-    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, mflag, pdl, s);
-    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, mflag, pdl, s);
-    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, mflag, pdl, s);
+    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, mstat, pdl, s);
 }
 
 }  // namespace
@@ -459,13 +463,13 @@ cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, c
 }
 
 cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
-                               double* part, int B, const int* mflag, bool pdl, cudaStream_t s)
+                               double* part, int B, const long long* mstat, bool pdl, cudaStream_t s)
 {
     switch (kx_pick_bt(d.N, B)) {
-        case 1: return launch_contract_m<1>(d, sm_count, f, yd, part, B, mflag, pdl, s);
-        case 2: return launch_contract_m<2>(d, sm_count, f, yd, part, B, mflag, pdl, s);
-        case 4: return launch_contract_m<4>(d, sm_count, f, yd, part, B, mflag, pdl, s);
-        default: return launch_contract_m<8>(d, sm_count, f, yd, part, B, mflag, pdl, s);
+        case 1: return launch_contract_m<1>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+        case 2: return launch_contract_m<2>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+        case 4: return launch_contract_m<4>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+        default: return launch_contract_m<8>(d, sm_count, f, yd, part, B, mstat, pdl, s);
     }
 }
 

@@ -95,8 +95,8 @@ struct kx_handle_s {
     long long groups;         // host copy of vtptr[NT]
     int ws_xstride;           // columns of XT (batch capacity padded)
     double *XT;               // [t.xrows, ws_xstride] operand rows: f^T, ones, Chebyshev coefficients
-    double *fmax;             // [wsB] max_i f[b,i]
-    int *mflag;               // [wsB] member needs the exact streaming path (a bracket failed the error bound)
+    long long *mstat;         // [wsB][2] per member: ordered key of the largest interpolation-error term over the brackets,
+                              // bits of max_i |f_i| (see kx_member_flagged); reset by the finishing kernel
     double *gpart;            // [8 sm_count + NT + 1, ws_xstride, 16]  gain partials of the DMMA kernel (one per warp and tile)
     double *lpart;            // [sm_count + RS + 1, ws_xstride, 256] loss partials
     int GG, GL;               // CTAs of the gain / loss role in the last launch of the DMMA kernel
@@ -149,6 +149,26 @@ inline cudaError_t kx_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, si
 #ifdef __CUDACC__
 __device__ __forceinline__ void kx_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void kx_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// Per-member statistics of the tiled LOG path, accumulated with atomicMax by k_xt (order independent, so the
+// result is deterministic):  mstat[2b] = key(max over brackets j of  log2 max(f_j, f_j+1) + Q (log2 |ln(f_j+1/f_j)| - 2)
+// + log2(2/Q!)),  mstat[2b+1] = bits of max_i |f_i|.  key() maps doubles to integers of the same order.
+#define KX_MSTAT_NONE (-0x7fffffffffffffffLL - 1)
+__device__ __forceinline__ long long kx_dkey(double x)
+{
+    const long long b = __double_as_longlong(x);
+    return b >= 0 ? b : (b ^ 0x7fffffffffffffffLL);
+}
+// A member takes the exact streaming path when the interpolation error bound of some bracket,
+//     2 (|ln(f_(j+1)/f_j)|/4)^Q / Q! * max(f_j, f_(j+1)),   exceeds 1e-15 max_i f_i      (kx_tiled_build.cu)
+__device__ __forceinline__ bool kx_member_flagged(const long long* mstat, int b)
+{
+    const long long k = mstat[2 * b];
+    if (k == KX_MSTAT_NONE) return false;
+    const double lb = __longlong_as_double(k >= 0 ? k : (k ^ 0x7fffffffffffffffLL));
+    const double fm = __longlong_as_double(mstat[2 * b + 1]);
+    return lb - log2(fm) > -49.82892142331043;         // log2(1e-15)
+}
 #endif
 
 // ---- launchers implemented in kx_build.cu
@@ -173,18 +193,18 @@ struct KxStage {             // what the finishing kernel does after the reducti
     double *fstage;          // stage input written by this stage for the next one
     double *k1, *k2, *k3;
     double *ydnext;          // where to write yd of the next stage input (fused prep) or null
-    // tiled path: partials of the DMMA kernel; members with mflag != 0 take the streaming partials instead
+    // tiled path: partials of the DMMA kernel; flagged members (kx_member_flagged) take the streaming partials instead
     const double *gpart;     // [slots, xstride, 16] or null (streaming path only)
     const double *lpart;     // [slots, xstride, 256]
     const unsigned *vtptr;   // [NT + 1]
-    const int *mflag;
+    long long *mstat;        // [B][2] or null
     int NT, LC, RS, GW, GL, xstride;      // GW = gain workers (warps), GL = loss workers (CTAs)
     int *flag;
     int evolve;
 };
 cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, cudaStream_t s);
 cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
-                               double* part, int B, const int* mflag, bool pdl, cudaStream_t s);
+                               double* part, int B, const long long* mstat, bool pdl, cudaStream_t s);
 cudaError_t kx_launch_finish(const KxDev& d, const double* f, const double* part, int B,
                              const KxStage& st, cudaStream_t s);
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
@@ -193,10 +213,11 @@ cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n,
 cudaError_t kx_launch_tile_runs(const KxDev& d, const KxTiled& t, cudaStream_t s);     // runs, scans, vtptr
 cudaError_t kx_launch_tile_fill(const KxDev& d, const KxTiled& t, cudaStream_t s);     // A, desc (gain + loss)
 cudaError_t kx_launch_xt(const KxDev& d, const KxTiled& t, const double* f, double* yd, double* XT, int xstride,
-                         double* fmax, int* mflag, int B, cudaStream_t s);
+                         long long* mstat, int B, cudaStream_t s);
 cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
                            const double* XT, int xstride, double* gpart, double* lpart, int B, cudaStream_t s);
 int kx_xstride(int B);
+int kx_dmma_workers(int N, int B);     // gain workers (warps) per CTA of k_dmma
 void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long groups, int B, int* GG, int* GL);
 int kx_pick_bt(int N, int B);
 int kx_pick_chunk(long long nnz_est, int N, int B, int sm_count);

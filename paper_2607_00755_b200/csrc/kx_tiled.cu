@@ -25,41 +25,18 @@ double loss_cost()
     return v;
 }
 
-// ---------------------------------------------------------------- per-member maximum, flag reset
-__global__ void __launch_bounds__(256) k_fmax(int N, const double* __restrict__ f, double* __restrict__ fmx,
-                                              int* __restrict__ mflag)
-{
-    __shared__ double s_red[8];
-    const int b = blockIdx.x;
-    double v = 0.0;
-    for (int i = threadIdx.x; i < N; i += 256) v = fmax(v, fabs(f[(size_t)b * N + i]));
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double a = s_red[0];
-#pragma unroll
-        for (int w = 1; w < 8; ++w) a = fmax(a, s_red[w]);
-        fmx[b] = a;
-        mflag[b] = 0;
-    }
-}
-
 // ---------------------------------------------------------------- operand rows XT[row, b]
-//   rows 0..N-1        f^T                                   (gain: X = f_n f_m)
-//   row  N             1                                     (scale row of the loss quads)
-//   rows N+1+jQ+c      a_c(b,j), c < Q, j < N-1              (loss)
+//   rows loss_row0 + jQ + c    a_c(b,j), c < Q, j < N-1      (loss; the gain role of k_dmma reads f itself)
 // LOG:    g(omega_q) = 2^(y_j + omega_q (y_{j+1}-y_j)), y = log2 max(f, f_floor), at the Q Chebyshev nodes of [0,1];
 //         a_c = (2-delta_c0)/Q sum_q g(omega_q) cos(c theta_q)            (discrete Chebyshev transform)
 //         A member is flagged for the exact streaming path when, for some bracket,
-//             2 (|ln(f_{j+1}/f_j)|/4)^Q / Q! * max(f_j, f_{j+1}) > 1e-15 max_i f_i    (interpolation error bound)
+//             2 (|ln(f_{j+1}/f_j)|/4)^Q / Q! * max(f_j, f_{j+1}) > 1e-15 max_i f_i    (interpolation error bound);
+//         this kernel accumulates the two maxima per member (mstat, kx_internal.cuh), the consumers compare them.
 // LINEAR: a_0 = (f_j + f_{j+1})/2, a_1 = (f_{j+1} - f_j)/2 (exact).
 // Also writes yd[b,j] = (y_j, y_{j+1}-y_j) for the streaming kernel.
-// grid.x = N+1 (row j), 256 threads = 64 members x 4 coefficient phases.
+// grid.x = N (row j), 256 threads = 64 members x 4 coefficient phases.
 __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __restrict__ f, double2* __restrict__ yd,
-                                            double* __restrict__ XT, int xstride, const double* __restrict__ fmx,
-                                            int* __restrict__ mflag, int B)
+                                            double* __restrict__ XT, int xstride, long long* __restrict__ mstat, int B)
 {
     __shared__ double s_dct[KX_QMAX * KX_QMAX];
     __shared__ double s_node[KX_QMAX];
@@ -67,8 +44,7 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
     const int N = d.N, Q = t.Q, j = blockIdx.x;
     const int bl = threadIdx.x & 63, ph = threadIdx.x >> 6;
     const bool logm = d.interp == KX_INTERP_LOG;
-    kx_pdl_trigger();
-    kx_pdl_wait();          // fmx and the reset of mflag come from k_fmax
+    kx_pdl_trigger();       // first kernel of the call (ordinary launch): the contraction kernel may start right away
     if (logm) {
         for (int k = threadIdx.x; k < Q * Q; k += 256) s_dct[k] = t.dct[k];
         if (threadIdx.x < Q) s_node[threadIdx.x] = t.nodes[threadIdx.x];
@@ -77,16 +53,15 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
     for (int b0 = 0; b0 < B; b0 += 64) {
         const int b = b0 + bl;
         const bool act = b < B;
-        if (j == N) {
-            if (act && ph == 0) XT[(size_t)t.ones_row * xstride + b] = 1.0;
-            continue;
-        }
         double fj = 0.0, fj1 = 0.0;
         if (act) {
             fj = f[(size_t)b * N + j];
             fj1 = j + 1 < N ? f[(size_t)b * N + j + 1] : fj;
         }
-        if (act && ph == 0) XT[(size_t)j * xstride + b] = fj;
+        if (act && ph == 0) {
+            const long long fk = __double_as_longlong(fabs(fj));
+            if (fk > mstat[2 * b + 1]) atomicMax(mstat + 2 * b + 1, fk);
+        }
         if (!logm) {
             if (act && ph == 0) {
                 yd[(size_t)b * N + j] = make_double2(fj, fj1 - fj);
@@ -105,9 +80,9 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
             yd[(size_t)b * N + j] = make_double2(y0, dy);
             const double c = 0.6931471805599453 * fabs(dy);
             if (j < N - 1 && c > 0.0) {
-                // log2 of the bound relative to max f, against log2(1e-15)
-                const double lb = fmax(y0, y1) - log2(fmx[b]) + (double)Q * (log2(c) - 2.0) + t.flag_log2;
-                if (lb > -49.82892142331043) mflag[b] = 1;
+                // log2 of the bracket's error bound (log2 max_i f_i is subtracted by the consumers)
+                const long long lk = kx_dkey(fmax(y0, y1) + (double)Q * (log2(c) - 2.0) + t.flag_log2);
+                if (lk > mstat[2 * b]) atomicMax(mstat + 2 * b, lk);
             }
         }
         if (j >= N - 1) continue;       // uniform over the CTA
@@ -148,8 +123,9 @@ __host__ __device__ constexpr int loss_stage_bytes(int NBT) { return kLossABytes
 
 // One CTA per SM.  CTAs [0, GG) take equal ranges of gain groups, CTAs [GG, GG+GL) equal ranges of loss chunks.
 //
-// gain role: f^T of the CTA's 8 NBT members sits in shared memory (row stride 8 NBT + 4 doubles: the 4 x 8 fragment
-//   reads of a quad are bank-conflict free); every warp streams its own share of the groups through a private
+// gain role: the rows f[b, :] of the CTA's 8 NBT members sit in shared memory (row stride = 4 mod 16 doubles when
+//   N = 0 mod 16: the 8 members x 4 k fragment reads of a quad are bank-conflict free), copied straight from the
+//   caller's f; every warp streams its own share of the groups through a private
 //   cp.async ring and holds a 16-row x 8 NBT-member accumulator (2 NBT DMMA per quad and fragment pair).
 //   The DMMAs of a run (fixed n) take X = f_m and accumulate into T; f_n multiplies T once, when the run ends.
 //   The ring keeps flowing across tile boundaries.
@@ -176,8 +152,9 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
         // ------------------------------------------------------------ gain role: every warp is an independent worker
         unsigned* s_vt = reinterpret_cast<unsigned*>(smem);                               // [NT + 1]
         const int vtbytes = ((t.NT + 1) * 4 + 15) & ~15;
-        double* s_f = reinterpret_cast<double*>(smem + vtbytes);                          // [N + 4][LD]
-        unsigned char* ring = smem + vtbytes + (size_t)(N + 4) * LD * 8 + (size_t)warp * STAGES * kStageBytes;
+        const int LDN = (N + 7) & ~3;             // row stride of s_f: >= N + 4, = 0 mod 4; N = 0 mod 16 gives 4 mod 16
+        double* s_f = reinterpret_cast<double*>(smem + vtbytes);                          // [8 NBT][LDN]
+        unsigned char* ring = smem + vtbytes + (size_t)(NBT * 8) * LDN * 8 + (size_t)warp * STAGES * kStageBytes;
 
         const unsigned NW = (unsigned)GG * WARPS, wk = blockIdx.x * WARPS + warp;
         const unsigned g0 = (unsigned)((unsigned long long)wk * Gtot / NW);
@@ -198,36 +175,38 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
             if ((unsigned)s < n) issue(s);
             cp_async_commit();
         }
-        // f^T: s_f[n][b] = f[bcol0 + b][n].  A warp moves blocks of 8 n x 4 members: 64-byte runs of f in, a
-        // bank-conflict-free 8 x 4 patch of s_f out (row stride LD = 4 mod 16 doubles).
+        // s_f[b][n] = f[bcol0 + b][n], n < N; s_f[b][N] = 1 (the scale of padding quads), s_f[b][N+1..] = 0.  The rows of
+        // f are copied as they are (16-byte cp.async when N is even); members beyond B are zero.  Every CTA starts its
+        // walk somewhere else so that the CTAs do not all ask the same L2 lines at once.
         {
-            const int nl = lane >> 2, bl = lane & 3;
-            const int nblk = (N + 7) >> 3, total = nblk * (NBT * 2);
-            for (int k0 = warp; k0 < total; k0 += 32 * WARPS) {
-                double v[32];
-#pragma unroll
-                for (int u = 0; u < 32; ++u) {
-                    const int k = k0 + u * WARPS;
-                    const int bq = k / nblk, nb_ = k - bq * nblk;
-                    const int nn = nb_ * 8 + nl, b = bcol0 + bq * 4 + bl;
-                    v[u] = (k < total && nn < N && b < B) ? __ldg(f + (size_t)b * N + nn) : 0.0;
-                }
-#pragma unroll
-                for (int u = 0; u < 32; ++u) {
-                    const int k = k0 + u * WARPS;
-                    const int bq = k / nblk, nb_ = k - bq * nblk;
-                    const int nn = nb_ * 8 + nl;
-                    if (k < total && nn < N) s_f[(size_t)nn * LD + bq * 4 + bl] = v[u];
-                }
+            const int chunks = (N & 1) ? 0 : N >> 1;                   // 16-byte chunks per row
+            const int total = NBT * 8 * chunks;
+            const int rot = total ? (int)((blockIdx.x * 977u) % (unsigned)total) : 0;
+            for (int k0 = tid; k0 < total; k0 += NTHR) {
+                int k = k0 + rot;
+                if (k >= total) k -= total;
+                const int bb = k / chunks, cc = k - bb * chunks;
+                if (bcol0 + bb < B) cp_async16(s_f + (size_t)bb * LDN + 2 * cc, f + (size_t)(bcol0 + bb) * N + 2 * cc);
+                else *reinterpret_cast<double2*>(s_f + (size_t)bb * LDN + 2 * cc) = make_double2(0.0, 0.0);
             }
-            for (int k = tid; k < 4 * LD; k += NTHR) s_f[(size_t)N * LD + k] = k < LD ? 1.0 : 0.0;     // ones row, 3 zero rows
+            if (!chunks)
+                for (int k = tid; k < NBT * 8 * N; k += NTHR) {
+                    const int bb = k / N, nn = k - bb * N;
+                    s_f[(size_t)bb * LDN + nn] = bcol0 + bb < B ? __ldcg(f + (size_t)(bcol0 + bb) * N + nn) : 0.0;
+                }
+            for (int k = tid; k < NBT * 8 * (LDN - N); k += NTHR) {
+                const int bb = k / (LDN - N), cc = k - bb * (LDN - N);
+                s_f[(size_t)bb * LDN + N + cc] = cc == 0 ? 1.0 : 0.0;
+            }
         }
+        cp_async_commit();
         for (int k = tid; k <= t.NT; k += NTHR) s_vt[k] = t.vtptr[k];
         cp_async_wait<0>();
         __syncthreads();
         if (n == 0) { kx_pdl_wait(); return; }
 
-        const double* xcol = s_f + lr;                       // + row * LD + 8 bt
+        const double* xb = s_f + (size_t)lr * LDN + krow;    // + 8 bt LDN + column: the lane's member row of tile bt
+        const int LD8 = 8 * LDN;
         int vt = 0;
         while (s_vt[vt + 1] <= g0) ++vt;
         unsigned bnd = s_vt[vt + 1] - g0;                    // first group (relative) of the next tile
@@ -268,10 +247,10 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
         unsigned srow_cur = dc.x >> 20;
         double xv[NBT];
         {
-            const double* xr = xcol + (size_t)((dc.x & 0xFFFFFu) + krow) * LD;
-            const double* sr = xcol + (size_t)srow_cur * LD;
+            const double* xr = xb + (dc.x & 0xFFFFFu);
+            const double* sr = xb + srow_cur - krow;
 #pragma unroll
-            for (int bt = 0; bt < NBT; ++bt) { sn[bt] = sr[8 * bt]; xv[bt] = xr[8 * bt]; }
+            for (int bt = 0; bt < NBT; ++bt) { sn[bt] = sr[bt * LD8]; xv[bt] = xr[bt * LD8]; }
         }
 
         for (unsigned gi = 0; gi < n; ++gi) {
@@ -297,9 +276,9 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
                 const bool more = (q < 3) || !last_group;
                 double xn[NBT];
                 {
-                    const double* xr = xcol + (size_t)((dsc & 0xFFFFFu) + krow) * LD;
+                    const double* xr = xb + (dsc & 0xFFFFFu);
 #pragma unroll
-                    for (int bt = 0; bt < NBT; ++bt) xn[bt] = xr[8 * bt];
+                    for (int bt = 0; bt < NBT; ++bt) xn[bt] = xr[bt * LD8];
                 }
                 const double w0 = wd[q * 64], w1 = wd[q * 64 + 32];
 #pragma unroll
@@ -311,9 +290,9 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
                 if (more && srow != srow_cur) {              // the run (n) ends with this quad
                     fold();
                     srow_cur = srow;
-                    const double* sr = xcol + (size_t)srow * LD;
+                    const double* sr = xb + srow - krow;
 #pragma unroll
-                    for (int bt = 0; bt < NBT; ++bt) sn[bt] = sr[8 * bt];
+                    for (int bt = 0; bt < NBT; ++bt) sn[bt] = sr[bt * LD8];
                 }
 #pragma unroll
                 for (int bt = 0; bt < NBT; ++bt) xv[bt] = xn[bt];
@@ -330,6 +309,8 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
     // ---------------------------------------------------------------- loss role
     {
         constexpr int SB = loss_stage_bytes(NBT);
+        constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
+        static_assert(WARPS == 8 || WARPS == 16, "loss role: 8 or 16 warps");
         kx_pdl_wait();        // the Chebyshev coefficients in XT come from k_xt
         const unsigned cl = blockIdx.x - GG;
         const unsigned LC = (unsigned)t.LC;
@@ -342,7 +323,7 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
             const unsigned ue = min(u1, (sp + 1) * LC);
             const unsigned ka = u - sp * LC, n = ue - u;
             const int nb = min(32, t.NR8 - 32 * (int)sp);                // 8-row blocks of this supertile
-            const int nbw = min(4, max(0, nb - 4 * warp));               // ... of this warp
+            const int nbw = min(R8, max(0, nb - R8 * warp));             // ... of this warp
 
             auto issue = [&](unsigned kc, int slot) {
                 unsigned char* dstA = smem + (size_t)slot * SB;
@@ -356,9 +337,9 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
                 }
             };
 
-            double acc[4][NBT][2];
+            double acc[R8][NBT][2];
 #pragma unroll
-            for (int r = 0; r < 4; ++r)
+            for (int r = 0; r < R8; ++r)
 #pragma unroll
                 for (int bt = 0; bt < NBT; ++bt) acc[r][bt][0] = acc[r][bt][1] = 0.0;
 
@@ -373,7 +354,7 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
                 if (it + kLossStages - 1 < n) issue(ka + it + kLossStages - 1, (int)((it + kLossStages - 1) % kLossStages));
                 cp_async_commit();
                 if (nbw > 0) {
-                    const double* sA = reinterpret_cast<const double*>(smem + (size_t)(it % kLossStages) * SB) + (size_t)warp * 512 + lane;
+                    const double* sA = reinterpret_cast<const double*>(smem + (size_t)(it % kLossStages) * SB) + (size_t)warp * (R8 * 128) + lane;
                     const double* sX = reinterpret_cast<const double*>(smem + (size_t)(it % kLossStages) * SB + kLossABytes) + (size_t)krow * LD + lr;
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
@@ -381,7 +362,7 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
 #pragma unroll
                         for (int bt = 0; bt < NBT; ++bt) xv[bt] = sX[(size_t)(4 * q) * LD + 8 * bt];
 #pragma unroll
-                        for (int r = 0; r < 4; ++r) {
+                        for (int r = 0; r < R8; ++r) {
                             const double w = sA[(r * 4 + q) * 32];
 #pragma unroll
                             for (int bt = 0; bt < NBT; ++bt) dmma884(acc[r][bt][0], acc[r][bt][1], xv[bt], w);
@@ -392,9 +373,9 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
             cp_async_wait<0>();
             __syncthreads();              // the stages are free again for the next piece
 
-            double* dst = lpart + ((size_t)(cl + sp) * xstride + bcol0) * 256 + 32 * warp + 2 * krow;
+            double* dst = lpart + ((size_t)(cl + sp) * xstride + bcol0) * 256 + 8 * R8 * warp + 2 * krow;
 #pragma unroll
-            for (int r = 0; r < 4; ++r)
+            for (int r = 0; r < R8; ++r)
                 if (r < nbw)
 #pragma unroll
                     for (int bt = 0; bt < NBT; ++bt)
@@ -407,7 +388,7 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
 template <int NBT, int WARPS, int STAGES>
 size_t dmma_smem(const KxTiled& t, int N)
 {
-    const size_t gain = (size_t)(((t.NT + 1) * 4 + 15) & ~15) + (size_t)(N + 4) * (NBT * 8 + 4) * 8 + (size_t)WARPS * STAGES * kStageBytes;
+    const size_t gain = (size_t)(((t.NT + 1) * 4 + 15) & ~15) + (size_t)(NBT * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * STAGES * kStageBytes;
     const size_t loss = (size_t)kLossStages * loss_stage_bytes(NBT);
     return gain > loss ? gain : loss;
 }
@@ -424,15 +405,21 @@ cudaError_t launch_dmma_t(const KxTiled& t, int N, unsigned Gtot, int GG, int GL
 }
 
 // member tiles (of 8) per CTA: limited by the batch and by the shared memory f^T of the gain role needs
+int env_int(const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; }
+int kx_dmma_warps(int nbt) { static const int w16 = env_int("KX_W16", 0); return (nbt == 4 && w16) ? 16 : 8; }
 int dmma_nbt(int N, int B)
 {
+    static const int cap = env_int("KX_NBT_MAX", 8);
     int nbt = B <= 8 ? 1 : (B <= 16 ? 2 : (B <= 32 ? 4 : 8));
-    auto need = [&](int k) { return (size_t)(N + 4) * (k * 8 + 4) * 8 + (size_t)8 * (k <= 2 ? 8 : 4) * kStageBytes + 512; };
+    if (nbt > cap) nbt = cap;
+    auto need = [&](int k) { return (size_t)(k * 8) * ((N + 7) & ~3) * 8 + (size_t)kx_dmma_warps(k) * (k <= 2 ? 8 : (kx_dmma_warps(k) == 16 ? 3 : 4)) * kStageBytes + 512; };
     while (nbt > 1 && need(nbt) > 227u * 1024u) nbt >>= 1;
     return nbt;
 }
 
 }  // namespace
+
+int kx_dmma_workers(int N, int B) { return kx_dmma_warps(dmma_nbt(N, B)); }
 
 // columns of XT / the partials for a batch of B members: whole 8-member MMA tiles, whole CTA column groups
 int kx_xstride(int B)
@@ -462,11 +449,10 @@ void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long gro
 }
 
 cudaError_t kx_launch_xt(const KxDev& d, const KxTiled& t, const double* f, double* yd, double* XT, int xstride,
-                         double* fmax, int* mflag, int B, cudaStream_t s)
+                         long long* mstat, int B, cudaStream_t s)
 {
-    k_fmax<<<B, 256, 0, s>>>(d.N, f, fmax, mflag);        // first kernel of the call: ordinary launch
-    return kx_launch(k_xt, dim3(d.N + 1), dim3(256), 0, s, true, d, t, f, reinterpret_cast<double2*>(yd), XT, xstride,
-                     (const double*)fmax, mflag, B);
+    // first kernel of the call: ordinary launch
+    return kx_launch(k_xt, dim3(d.N), dim3(256), 0, s, false, d, t, f, reinterpret_cast<double2*>(yd), XT, xstride, mstat, B);
 }
 
 cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
@@ -475,7 +461,9 @@ cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, i
     switch (dmma_nbt(d.N, B)) {
         case 1: return launch_dmma_t<1, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
         case 2: return launch_dmma_t<2, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
-        case 4: return launch_dmma_t<4, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+        case 4:
+            if (kx_dmma_warps(4) == 16) return launch_dmma_t<4, 16, 3>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+            return launch_dmma_t<4, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
         default: return launch_dmma_t<8, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
     }
 }
