@@ -34,7 +34,12 @@ UNIT = "C[f]/s"
 WORKLOAD = "cfg3: N=256 log p/T in [1e-3,50], B=64 seeded bimodal f, |M|^2 ~ 1/(1+q^2/m_med^2)^2, m_med=0.5"
 # Algorithmic work of the dominant kernel k_dmma: one FMA (2 flop) per stored entry and member
 # for the gain, one per (i, bracket, Chebyshev coefficient) and member for the loss.  Padding of the tiled layout,
-# the f_n f_m products and the operand preparation are NOT counted.
+# the f_n scaling and the operand preparation are NOT counted.
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_dmma launch from the committed `ncu --set full` capture
+# (profiles/r01c_tiled_dmma.md); null for configurations that were not captured.
+NCU_TRAFFIC = {("log", 64): 65.04e6, ("linear", 64): 48.72e6}
+# kernels of one kx_collide on the tiled path: k_xt, k_dmma, k_contract (exact fallback, exits at once when no member is
+# flagged; LOG only), k_finish
 LOSS_NODES = {"log": 24, "linear": 2}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM; DMMA.8x8x4 runs at the same 37.2 TFLOP/s
 
@@ -86,11 +91,17 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def _inputs(rank: int, B: int):
-    c = kin.config(3, B=B)
-    if rank:   # every rank its own members: seeds 3000 + rank*B + b
-        c["f"] = np.stack([kin._random_bimodal(c["p"], 3000 + rank * B + b) for b in range(B)])
+def _inputs(rank: int, B: int, cfg: int = 3):
+    from paper_2607_00755_b200 import shard
+    c = kin.config(cfg, B=B)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank:   # every rank its own members: global member g has seed 1000*cfg + g
+        c["f"] = np.stack([kin._random_bimodal(c["p"], 1000 * cfg + int(g)) for g in shard.weak_member_ids(B, rank, world)])
     return c
+
+
+WORKLOADS = {3: WORKLOAD,
+             4: "cfg4: N=512 log p/T in [1e-3,100], seeded bimodal f, constant |M|^2 (not the headline: HBM-bound side measurement)"}
 
 
 def cpu_oracle(c, members: int, steps: int = 1, warmup: int = 0):
@@ -138,7 +149,9 @@ def main():
     ap.add_argument("--impl", default="kx", choices=["kx", "reference"])
     ap.add_argument("--mode", default="log", choices=["log", "linear"])
     ap.add_argument("--project", action="store_true", help="time the projected operator (App. C) instead of the raw one")
-    ap.add_argument("--batch", type=int, default=64)
+    ap.add_argument("--batch", type=int, default=None, help="members per GPU (default: 64 for cfg3, 8 for cfg4)")
+    ap.add_argument("--config", type=int, default=3, choices=[3, 4],
+                    help="3 = the headline workload; 4 = the N=512 small-batch workload (side measurement, HBM roofline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -164,8 +177,9 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    B, K, Wm = args.batch, args.steps, max(args.warmup, 3)
-    c = _inputs(rank, B)
+    B = args.batch if args.batch else (64 if args.config == 3 else 8)
+    K, Wm = args.steps, max(args.warmup, 3)
+    c = _inputs(rank, B, args.config)
     h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], device=local,
                   interp=kx.INTERP_LOG if args.mode == "log" else kx.INTERP_LINEAR)
     info = h.info()
@@ -228,10 +242,8 @@ def main():
     t_e2e = time.perf_counter() - t0
     clocks = sampler.stop()
 
-    times = torch.tensor([t_cold, t_warm, t_e2e, kern_ms * 1e-3], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    t_cold, t_warm, t_e2e, t_kern = [float(x) for x in times.cpu()]
+    from paper_2607_00755_b200 import shard
+    t_cold, t_warm, t_e2e, t_kern = shard.max_over_ranks([t_cold, t_warm, t_e2e, kern_ms * 1e-3], dist, dev)
     same = bool(torch.isfinite(C).all())
     if rank != 0:
         if dist is not None:
@@ -252,30 +264,40 @@ def main():
     peak = max(peak_nominal, probe["dmma"])
     flop = 2.0 * (nnz + Ngrid * (Ngrid - 1) * Q) * B
     ach = flop / kern_s / 1e12
-    roof = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-            "traffic": None, "kernel": "k_dmma<8,8,4> (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss)",
+    hbm_gbs = float(peaks.get("hbm_gbs", 6650.0))
+    t_hbm = info["tensor_bytes"] / (hbm_gbs * 1e9)
+    t_flop = flop / (peak * 1e12)
+    if t_hbm > t_flop:      # small batches: the tensor stream bounds the kernel (cfg4)
+        ach_gbs = info["tensor_bytes"] / kern_s / 1e9
+        roof_head = {"bound": "hbm", "achieved": ach_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": ach_gbs / hbm_gbs,
+                     "peak_source_hbm": f"{peak_src} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)", "tflops": ach}
+    else:
+        roof_head = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak}
+    roof = {**roof_head,
+            "traffic": NCU_TRAFFIC.get((args.mode, B)) if (not args.project and args.config == 3) else None,
+            "kernel": "k_dmma (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss)",
             "kernel_ms": kern_s * 1e3, "kernel_ms_l2_warm": kern_warm_ms / max(kern_warm_n, 1), "flop_per_launch": flop,
             "peak_source": f"FP64 tensor pipe: 148 SMs x 64 FMA/clk x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src}); "
                            f"probe in this run: DMMA {probe['dmma']:.1f}, DFMA {probe['dfma']:.1f} TFLOP/s",
             "peak_alt": {"value": float(peaks.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0,
                          "how": f"{peak_src} bf16_tflops x guide nominal ratio 45/2250"},
             "tensor_bytes_per_launch": info["tensor_bytes"],
-            "hbm_time_us_at_peak": info["tensor_bytes"] / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9) * 1e6}
+            "hbm_time_us_at_peak": t_hbm * 1e6, "tensor_time_us_at_peak": t_flop * 1e6}
     line = {
-        "metric": METRIC, "value": world * B * K / t_cold, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "metric": METRIC if args.config == 3 and B == 64 else f"C[f] evals/s (fp64, N={Ngrid}, B={B})", "value": shard.aggregate_rate(B, world, K, t_cold), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": t_cold / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "N": 256, "B_per_gpu": B, "mode": args.mode, "projected": bool(args.project),
+        "config": {"workload": WORKLOADS[args.config], "N": Ngrid, "B_per_gpu": B, "mode": args.mode, "projected": bool(args.project),
                    "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "storage": "tiled", "loss_nodes": Q, "l2": "flushed before every timed step (256 MiB write)",
                    "parallelism": f"independent batches x{world}" if world > 1 else "single GPU"},
         "value_l2_warm": world * B * K / t_warm, "ms_per_step_l2_warm": t_warm / K * 1e3,
         "calls_per_s": world * K / t_cold,
-        "e2e": {"value": world * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": B * 256 * 8,
-                "d2h_bytes_per_step": B * 256 * 8, "ms_per_step": t_e2e / K * 1e3},
-        "gpu_launches": (5 if args.mode == "log" else 4) * K, "clocks": clocks, "roofline": roof, "finite": same,
+        "e2e": {"value": world * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": B * Ngrid * 8,
+                "d2h_bytes_per_step": B * Ngrid * 8, "ms_per_step": t_e2e / K * 1e3},
+        "gpu_launches": (4 if args.mode == "log" else 3) * K, "clocks": clocks, "roofline": roof, "finite": same,
     }
-    if not args.no_cpu_baseline and world == 1:
-        cb = cpu_oracle(c, members=B, steps=3, warmup=1)
+    if not args.no_cpu_baseline and world == 1 and args.config == 3:
+        cb = cpu_oracle(c, members=B, steps=10, warmup=1)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
     else:
         line["cpu_baseline"] = None

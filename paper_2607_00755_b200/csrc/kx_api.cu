@@ -97,9 +97,9 @@ void free_ws(kx_handle_s* h)
 {
     cudaFree(h->yd); cudaFree(h->part); cudaFree(h->fstage); cudaFree(h->k1); cudaFree(h->k2);
     cudaFree(h->k3); cudaFree(h->Cbuf); cudaFree(h->hostio);
-    cudaFree(h->XT); cudaFree(h->mstat); cudaFree(h->gpart); cudaFree(h->lpart);
+    cudaFree(h->XT); cudaFree(h->mstat); cudaFree(h->gpart); cudaFree(h->lpart); cudaFree(h->gn);
     h->yd = h->part = h->fstage = h->k1 = h->k2 = h->k3 = h->Cbuf = h->hostio = nullptr;
-    h->XT = h->gpart = h->lpart = nullptr; h->mstat = nullptr;
+    h->XT = h->gpart = h->lpart = h->gn = nullptr; h->mstat = nullptr;
     h->wsB = 0; h->ws_tasks = 0; h->ws_xstride = 0;
 }
 
@@ -133,6 +133,7 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
         }
         KX_CUDA(dalloc(&h->gpart, (size_t)(16 * h->sm_count + h->t.NT + 1) * xs * 16));
         KX_CUDA(dalloc(&h->lpart, (size_t)(h->sm_count + h->t.RS + 1) * xs * 256));
+        KX_CUDA(dalloc(&h->gn, bn * 2));
         h->ws_xstride = xs;
     }
     h->wsB = nB; h->ws_tasks = need_tasks;
@@ -208,7 +209,7 @@ kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bo
         if ((rc = prof_end()) != KX_OK) return rc;
         if (h->d.interp == KX_INTERP_LOG)      // exact streaming path for flagged members only (LINEAR is exact)
             KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, h->mstat, true, s));
-        st->gpart = h->gpart; st->lpart = h->lpart; st->vtptr = h->t.vtptr;
+        st->gpart = h->gpart; st->lpart = h->lpart; st->gn = reinterpret_cast<double2*>(h->gn); st->vtptr = h->t.vtptr;
         st->mstat = h->d.interp == KX_INTERP_LOG ? h->mstat : nullptr;
         st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS; st->GW = kx_dmma_workers(h->d.N, B) * h->GG; st->GL = h->GL; st->xstride = xs;
     } else {
@@ -216,7 +217,7 @@ kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bo
         if ((rc = prof_begin()) != KX_OK) return rc;
         KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, nullptr, !have_yd, s));
         if ((rc = prof_end()) != KX_OK) return rc;
-        st->gpart = nullptr; st->lpart = nullptr; st->vtptr = nullptr; st->mstat = nullptr;
+        st->gpart = nullptr; st->lpart = nullptr; st->gn = nullptr; st->vtptr = nullptr; st->mstat = nullptr;
     }
     return KX_OK;
 }

@@ -210,6 +210,50 @@ __device__ __forceinline__ double block_max(double v, double* s_red)
     return a;
 }
 
+// ---------------------------------------------------------------- partials of the DMMA kernel -> (gain, nu)[b, i]
+// gain: tile = i/16, groups [a0,a1) of the tile were taken by the gain workers c0..c1 (equal ranges of the Gtot
+// groups), slot = c + tile.  loss: supertile = i/256, chunk units [sp LC, (sp+1) LC) of the RS LC units were taken by
+// the loss CTAs c0..c1, slot = c + sp.  A CTA adds the partials of 16 rows x 2 members; the slots of an output are
+// dealt to 8 threads (slot = first + part, step 8) and the 8 sums are added in part order: a fixed order,
+// bit-reproducible.
+__global__ void __launch_bounds__(256) k_reduce(int N, int B, KxStage st)
+{
+    __shared__ double s_g[8][32], s_l[8][32];
+    kx_pdl_trigger();
+    kx_pdl_wait();
+    const int tid = threadIdx.x, part = tid >> 5, o = tid & 31, il = o & 15, bl = o >> 4;
+    const int tile = blockIdx.x, b = blockIdx.y * 2 + bl, i = tile * 16 + il;
+    double g = 0.0, nu = 0.0;
+    if (b < B && i < N) {
+        const unsigned Gtot = st.vtptr[st.NT];
+        const unsigned a0 = st.vtptr[tile], a1 = st.vtptr[tile + 1];
+        if (a1 > a0) {
+            const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.GW - 1ull) / Gtot);
+            const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.GW - 1ull) / Gtot);
+            const double* src = st.gpart + ((size_t)tile * st.xstride + b) * 16 + il;
+#pragma unroll 4
+            for (unsigned c = c0 + part; c <= c1; c += 8) g += src[(size_t)c * st.xstride * 16];
+        }
+        const unsigned U = (unsigned)st.RS * (unsigned)st.LC;
+        const unsigned sp = (unsigned)i >> 8;
+        const unsigned l0 = sp * (unsigned)st.LC, l1 = l0 + (unsigned)st.LC;
+        const unsigned d0 = (unsigned)((((unsigned long long)l0 + 1ull) * (unsigned)st.GL - 1ull) / U);
+        const unsigned d1 = (unsigned)(((unsigned long long)l1 * (unsigned)st.GL - 1ull) / U);
+        const double* srl = st.lpart + ((size_t)sp * st.xstride + b) * 256 + (i & 255);
+#pragma unroll 4
+        for (unsigned c = d0 + part; c <= d1; c += 8) nu += srl[(size_t)c * st.xstride * 256];
+    }
+    s_g[part][o] = g;
+    s_l[part][o] = nu;
+    __syncthreads();
+    if (part == 0 && b < B && i < N) {
+        double G = s_g[0][o], L = s_l[0][o];
+#pragma unroll
+        for (int k = 1; k < 8; ++k) { G += s_g[k][o]; L += s_l[k][o]; }
+        st.gn[(size_t)b * N + i] = make_double2(G, L);
+    }
+}
+
 // ---------------------------------------------------------------- finishing kernel: one CTA per member b
 constexpr int kMaxPerThread = KX_MAX_N / KX_CTA;   // 4
 
@@ -235,30 +279,8 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
         if (i < N) {
             double g = 0.0, nu = 0.0;
             if (tiled) {
-                // partials of the DMMA kernel.  gain: tile = i/16, groups [a0,a1) of the tile were taken by the gain
-                // workers c0..c1 (equal ranges of the Gtot groups), slot = c + tile.  loss: supertile = i/256, chunk units
-                // [sp LC, (sp+1) LC) of the RS LC units were taken by the loss CTAs c0..c1, slot = c + sp.  Both are
-                // added in slot order.
-                {
-                    const unsigned Gtot = st.vtptr[st.NT];
-                    const int tile = i >> 4, il = i & 15;
-                    const unsigned a0 = st.vtptr[tile], a1 = st.vtptr[tile + 1];
-                    if (a1 > a0) {
-                        const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.GW - 1ull) / Gtot);
-                        const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.GW - 1ull) / Gtot);
-                        for (unsigned c = c0; c <= c1; ++c)
-                            g += st.gpart[((size_t)(c + tile) * st.xstride + b) * 16 + il];
-                    }
-                }
-                {
-                    const unsigned U = (unsigned)st.RS * (unsigned)st.LC;
-                    const unsigned sp = (unsigned)i >> 8, il = (unsigned)i & 255u;
-                    const unsigned a0 = sp * (unsigned)st.LC, a1 = a0 + (unsigned)st.LC;
-                    const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.GL - 1ull) / U);
-                    const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.GL - 1ull) / U);
-                    for (unsigned c = c0; c <= c1; ++c)
-                        nu += st.lpart[((size_t)(c + sp) * st.xstride + b) * 256 + il];
-                }
+                const double2 v = st.gn[(size_t)b * N + i];          // partials of the DMMA kernel, added by k_reduce
+                g = v.x; nu = v.y;
             } else {
                 const unsigned t0 = d.taskptr[i], t1 = d.taskptr[i + 1];
                 for (unsigned t = t0; t < t1; ++t) {
@@ -476,6 +498,10 @@ cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, co
 cudaError_t kx_launch_finish(const KxDev& d, const double* fin, const double* part, int B,
                              const KxStage& st, cudaStream_t s)
 {
+    if (st.gpart) {
+        cudaError_t e = kx_launch(k_reduce, dim3(st.NT, (B + 1) / 2), dim3(256), 0, s, true, d.N, B, st);
+        if (e != cudaSuccess) return e;
+    }
     return kx_launch(k_finish, dim3(B), dim3(KX_CTA), 0, s, true, d, fin, part, B, st);
 }
 

@@ -99,6 +99,7 @@ struct kx_handle_s {
                               // bits of max_i |f_i| (see kx_member_flagged); reset by the finishing kernel
     double *gpart;            // [8 sm_count + NT + 1, ws_xstride, 16]  gain partials of the DMMA kernel (one per warp and tile)
     double *lpart;            // [sm_count + RS + 1, ws_xstride, 256] loss partials
+    double *gn;               // [wsB, N, 2] (gain, nu) summed from the partials
     int GG, GL;               // CTAs of the gain / loss role in the last launch of the DMMA kernel
     void *tiled_blob;         // one allocation holding the small tables of KxTiled
     bool nnz_stale;
@@ -196,6 +197,7 @@ struct KxStage {             // what the finishing kernel does after the reducti
     // tiled path: partials of the DMMA kernel; flagged members (kx_member_flagged) take the streaming partials instead
     const double *gpart;     // [slots, xstride, 16] or null (streaming path only)
     const double *lpart;     // [slots, xstride, 256]
+    double2 *gn;             // [B, N] (gain, nu): the partials added up by k_reduce
     const unsigned *vtptr;   // [NT + 1]
     long long *mstat;        // [B][2] or null
     int NT, LC, RS, GW, GL, xstride;      // GW = gain workers (warps), GL = loss workers (CTAs)

@@ -13,17 +13,12 @@
 // Compiled with --fmad=false; fused multiply-adds are explicit.
 #include "kx_internal.cuh"
 
-#include <stdlib.h>
 
 namespace {
 
-// cost of one loss DMMA relative to one gain DMMA in the CTA split of k_dmma (the dense loss path needs fewer
-// operand loads per DMMA).  KX_LOSS_COST overrides it (tuning aid).
-double loss_cost()
-{
-    static const double v = [] { const char* e = getenv("KX_LOSS_COST"); const double x = e ? atof(e) : 0.0; return x > 0.0 ? x : 0.85; }();
-    return v;
-}
+// cost of one loss DMMA relative to one gain DMMA in the CTA split of k_dmma (measured on cfg3: the split that
+// makes both roles finish together)
+constexpr double kLossCost = 1.0;
 
 // ---------------------------------------------------------------- operand rows XT[row, b]
 //   rows loss_row0 + jQ + c    a_c(b,j), c < Q, j < N-1      (loss; the gain role of k_dmma reads f itself)
@@ -405,14 +400,11 @@ cudaError_t launch_dmma_t(const KxTiled& t, int N, unsigned Gtot, int GG, int GL
 }
 
 // member tiles (of 8) per CTA: limited by the batch and by the shared memory f^T of the gain role needs
-int env_int(const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; }
-int kx_dmma_warps(int nbt) { static const int w16 = env_int("KX_W16", 0); return (nbt == 4 && w16) ? 16 : 8; }
+int kx_dmma_warps(int nbt) { (void)nbt; return 8; }
 int dmma_nbt(int N, int B)
 {
-    static const int cap = env_int("KX_NBT_MAX", 8);
     int nbt = B <= 8 ? 1 : (B <= 16 ? 2 : (B <= 32 ? 4 : 8));
-    if (nbt > cap) nbt = cap;
-    auto need = [&](int k) { return (size_t)(k * 8) * ((N + 7) & ~3) * 8 + (size_t)kx_dmma_warps(k) * (k <= 2 ? 8 : (kx_dmma_warps(k) == 16 ? 3 : 4)) * kStageBytes + 512; };
+    auto need = [&](int k) { return (size_t)(k * 8) * ((N + 7) & ~3) * 8 + (size_t)kx_dmma_warps(k) * (k <= 2 ? 8 : 4) * kStageBytes + 512; };
     while (nbt > 1 && need(nbt) > 227u * 1024u) nbt >>= 1;
     return nbt;
 }
@@ -436,7 +428,7 @@ void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long gro
     const int nbt = dmma_nbt(d.N, B);
     const int ny = (B + nbt * 8 - 1) / (nbt * 8);
     const double wg = (double)(groups > 0 ? groups : 1);
-    const double wl = 0.5 * (double)t.LC * (double)t.NR8 * loss_cost();
+    const double wl = 0.5 * (double)t.LC * (double)t.NR8 * kLossCost;
     long long G = (long long)((wg + wl) / 8.0);
     const long long cap = sm_count / ny > 2 ? sm_count / ny : 2;
     if (G > cap) G = cap;
@@ -461,9 +453,7 @@ cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, i
     switch (dmma_nbt(d.N, B)) {
         case 1: return launch_dmma_t<1, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
         case 2: return launch_dmma_t<2, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
-        case 4:
-            if (kx_dmma_warps(4) == 16) return launch_dmma_t<4, 16, 3>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
-            return launch_dmma_t<4, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+        case 4: return launch_dmma_t<4, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
         default: return launch_dmma_t<8, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
     }
 }
