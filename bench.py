@@ -39,7 +39,7 @@ WORKLOAD = "cfg3: N=256 log p/T in [1e-3,50], B=64 seeded bimodal f, |M|^2 ~ 1/(
 # (profiles/r01c_tiled_dmma.md); null for configurations that were not captured.
 NCU_TRAFFIC = {("log", 64): 65.04e6, ("linear", 64): 48.72e6}
 # kernels of one kx_collide on the tiled path: k_xt, k_dmma, k_contract (exact fallback, exits at once when no member is
-# flagged; LOG only), k_finish
+# flagged; LOG only), k_reduce, k_finish
 LOSS_NODES = {"log": 24, "linear": 2}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM; DMMA.8x8x4 runs at the same 37.2 TFLOP/s
 
@@ -294,7 +294,7 @@ def main():
         "calls_per_s": world * K / t_cold,
         "e2e": {"value": world * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": B * Ngrid * 8,
                 "d2h_bytes_per_step": B * Ngrid * 8, "ms_per_step": t_e2e / K * 1e3},
-        "gpu_launches": (4 if args.mode == "log" else 3) * K, "clocks": clocks, "roofline": roof, "finite": same,
+        "gpu_launches": (5 if args.mode == "log" else 4) * K, "clocks": clocks, "roofline": roof, "finite": same,
     }
     if not args.no_cpu_baseline and world == 1 and args.config == 3:
         cb = cpu_oracle(c, members=B, steps=10, warmup=1)
