@@ -69,18 +69,13 @@ __global__ void k_runs(KxDev d)
     d.run_len[i * N + n] = len > 0 ? len : 0;
 }
 
-// exclusive scan of run_len[N*N] by ONE CTA of 1024 threads (N*N <= 2^20), then rowptr
-__global__ void __launch_bounds__(1024) k_scan_runs(KxDev d)
+// exclusive scan of run_len[N*N] in two coalesced passes, one CTA of 1024 threads per row i (N <= 1024):
+//   k_scan_rows: run_off[i,n] = sum_{n'<n} run_len[i,n'], row total -> taskptr[i] (scratch: k_tasks rebuilds taskptr later)
+//   k_scan_base: base_i = sum_{i'<i} total_i'; run_off[i,n] += base_i; rowptr[i] = base_i; run_off[N*N] = rowptr[N] = nnz
+__device__ __forceinline__ unsigned block_scan_1024(unsigned v, unsigned* s_warp, unsigned* total)
 {
-    __shared__ unsigned s_warp[32];
-    const int total = d.N * d.N;
-    const int per = (total + 1023) / 1024;
     const int t = threadIdx.x;
-    const int b0 = t * per, b1 = min(b0 + per, total);
-    unsigned sum = 0;
-    for (int k = b0; k < b1; ++k) sum += (unsigned)d.run_len[k];
-    // block exclusive scan of `sum`
-    unsigned v = sum;
+    const unsigned own = v;
     for (int o = 1; o < 32; o <<= 1) {
         unsigned u = __shfl_up_sync(0xffffffffu, v, o);
         if ((t & 31) >= o) v += u;
@@ -96,15 +91,35 @@ __global__ void __launch_bounds__(1024) k_scan_runs(KxDev d)
         s_warp[t] = w;
     }
     __syncthreads();
-    unsigned excl = v - sum + ((t >> 5) ? s_warp[(t >> 5) - 1] : 0u);
-    unsigned run = excl;
-    for (int k = b0; k < b1; ++k) {
-        d.run_off[k] = run;
-        run += (unsigned)d.run_len[k];
-    }
-    if (t == 1023) d.run_off[total] = s_warp[31];
-    __syncthreads();   // global writes of this CTA are visible to the CTA after the barrier
-    for (int i = t; i <= d.N; i += 1024) d.rowptr[i] = d.run_off[i * d.N];
+    *total = s_warp[31];
+    return v - own + ((t >> 5) ? s_warp[(t >> 5) - 1] : 0u);     // exclusive
+}
+
+__global__ void __launch_bounds__(1024) k_scan_rows(KxDev d)
+{
+    __shared__ unsigned s_warp[32];
+    const int i = blockIdx.x, t = threadIdx.x, N = d.N;
+    const unsigned len = t < N ? (unsigned)d.run_len[i * N + t] : 0u;
+    unsigned total;
+    const unsigned excl = block_scan_1024(len, s_warp, &total);
+    if (t < N) d.run_off[i * N + t] = excl;
+    if (t == 0) d.taskptr[i] = total;
+}
+
+__global__ void __launch_bounds__(1024) k_scan_base(KxDev d)
+{
+    __shared__ unsigned s_warp[32];
+    const int i = blockIdx.x, t = threadIdx.x, N = d.N;
+    const unsigned tot = t < N ? d.taskptr[t] : 0u;
+    unsigned all;
+    const unsigned excl = block_scan_1024(tot, s_warp, &all);      // thread t holds base_t
+    __shared__ unsigned s_base;
+    if (t == i) s_base = excl;
+    __syncthreads();
+    const unsigned base = s_base;
+    if (t < N) d.run_off[i * N + t] += base;
+    if (t == 0) d.rowptr[i] = base;
+    if (i == N - 1 && t == 0) { d.rowptr[N] = all; d.run_off[N * N] = all; }
 }
 
 // one warp per run (i,n); lanes over m.  Writes W (symmetrised), omega_R and n|m<<10|jL<<20.
@@ -183,7 +198,8 @@ cudaError_t kx_launch_runs(const KxDev& d, cudaStream_t s)
 {
     dim3 grid((d.N + 127) / 128, d.N);
     k_runs<<<grid, 128, 0, s>>>(d);
-    k_scan_runs<<<1, 1024, 0, s>>>(d);
+    k_scan_rows<<<d.N, 1024, 0, s>>>(d);
+    k_scan_base<<<d.N, 1024, 0, s>>>(d);
     return cudaGetLastError();
 }
 

@@ -169,3 +169,30 @@ def test_nonfinite_is_reported(torch_cuda):
         h.evolve(f, np.arange(6) * 1e200, method=kx.EULER)
     assert ei.value.status == 5
     h.close()
+
+
+def test_cfg5_full_size_invariants(torch_cuda):
+    """Config 5 at BASELINE size (N=256, S=1e4 RK4 steps, B=8, tensor rebuilt at each of the 4e4 stages): too long for
+    the oracle, so the properties that hold at any size are checked: the injected number is exact (sum_i h_i f_i = 6
+    for every member, reading D11), f stays finite, and the warmness <p^2>/<p>^2 falls monotonically with the
+    coupling from the collisionless value towards the non-relativistic thermal one (3 pi/8 = 1.178)."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    B, S = 8, 10_000
+    c = kin.config(5, B=B)
+    sch = kin.config5_schedule(c["p"], c["dp"], B=B, S=S)
+    h = kx.Handle(c["p"], c["dp"], c["m"])
+    f = _dev(torch, c["f"])
+    h.evolve(f, sch["tau"], method=kx.RK4, rate=sch["rate"], mass=sch["mass"], kappa=sch["kappa"],
+             G=_dev(torch, sch["G"]), amp=sch["amp"])
+    got = f.cpu().numpy()
+    assert np.isfinite(got).all()
+    hsum = (c["p"] ** 2 * c["dp"] * got).sum(axis=1)
+    injected = (sch["amp"] * np.diff(sch["tau"])[None, :]).sum()
+    assert abs(injected - 6.0) < 1e-12
+    assert np.abs(hsum / injected - 1).max() <= 1e-12
+    mo = h.moments(f).cpu().numpy()
+    warm = mo[3] / mo[2] ** 2
+    assert (np.diff(warm) < 0).all(), warm
+    assert 1.9 < warm[0] < 2.2 and 3 * np.pi / 8 < warm[-1] < 1.34, warm
+    h.close()
