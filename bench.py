@@ -36,8 +36,9 @@ WORKLOAD = "cfg3: N=256 log p/T in [1e-3,50], B=64 seeded bimodal f, |M|^2 ~ 1/(
 # for the gain, one per (i, bracket, Chebyshev coefficient) and member for the loss.  Padding of the tiled layout,
 # the f_n scaling and the operand preparation are NOT counted.
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_dmma launch from the committed `ncu --set full` capture
-# (profiles/r01c_tiled_dmma.md); null for configurations that were not captured.
-NCU_TRAFFIC = {("log", 64): 65.04e6, ("linear", 64): 48.72e6}
+# (profiles/r01c_tiled_dmma.md; LINEAR from the working capture of the same round); null for configurations that were
+# not captured.
+NCU_TRAFFIC = {("log", 64): 64.06e6, ("linear", 64): 48.72e6}
 # kernels of one kx_collide on the tiled path: k_xt, k_dmma, k_contract (exact fallback, exits at once when no member is
 # flagged; LOG only), k_reduce, k_finish
 LOSS_NODES = {"log": 24, "linear": 2}
@@ -250,6 +251,14 @@ def main():
             dist.destroy_process_group()
         return
 
+    # context for kernel_ms: what two CUDA events around an (almost) empty kernel measure on this box
+    tiny = torch.zeros(1, device=dev)
+    ev_over = []
+    for _ in range(20):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream); tiny.add_(1.0); e1.record(stream); e1.synchronize()
+        ev_over.append(e0.elapsed_time(e1))
+    ev_over_us = float(np.min(ev_over[3:])) * 1e3
     peaks, peak_src = _peaks()
     sm_max_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     nnz = info["nnz"]
@@ -276,7 +285,8 @@ def main():
     roof = {**roof_head,
             "traffic": NCU_TRAFFIC.get((args.mode, B)) if (not args.project and args.config == 3) else None,
             "kernel": "k_dmma (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss)",
-            "kernel_ms": kern_s * 1e3, "kernel_ms_l2_warm": kern_warm_ms / max(kern_warm_n, 1), "flop_per_launch": flop,
+            "kernel_ms": kern_s * 1e3, "kernel_ms_l2_warm": kern_warm_ms / max(kern_warm_n, 1),
+            "event_pair_around_empty_kernel_us": ev_over_us, "flop_per_launch": flop,
             "peak_source": f"FP64 tensor pipe: 148 SMs x 64 FMA/clk x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src}); "
                            f"probe in this run: DMMA {probe['dmma']:.1f}, DFMA {probe['dfma']:.1f} TFLOP/s",
             "peak_alt": {"value": float(peaks.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0,
