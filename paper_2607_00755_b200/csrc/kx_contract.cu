@@ -20,29 +20,6 @@
 
 namespace {
 
-// ---------------------------------------------------------------- exp2 for the LOG loss term
-// 2^t = 2^k * T[idx] * 2^r,  t = k + idx/256 + r, |r| <= 2^-9.  Adding 1.5*2^44 leaves round(256 t) in the
-// low mantissa bits (one DADD), T is a 256-entry table replicated 16x in shared memory so that the
-// 64-bit gather is bank-conflict free, 2^r = 1 + r q(r) with q the degree-3 Chebyshev interpolant of
-// (2^r-1)/r on |r| <= 1.01*2^-9 (polynomial error 5e-18), and 2^k is added to the exponent field by the
-// integer pipe.  FP64-pipe cost: 2 DADD + 1 DADD + 3 DFMA + 1 DMUL + 1 DFMA = 8.  Valid for
-// -1021 < t < 1023 (f_floor >= 1e-300 keeps t >= -997).
-__device__ __forceinline__ double kx_exp2_tab(double t, const double* __restrict__ tab_lane)
-{
-    const double MAG = 26388279066624.0;                 // 1.5 * 2^44
-    const double C1 = 0.6931471805599427, C2 = 0.24022650695910042,
-                 C3 = 0.05550411385340617, C4 = 0.009618129707037269;
-    double tm = t + MAG;
-    int nlo = __double2loint(tm);
-    double r = t - (tm - MAG);
-    double T = tab_lane[(nlo & ((1 << KX_EXP_BITS) - 1)) * KX_EXP_REP];
-    double q = fma(fma(fma(C4, r, C3), r, C2), r, C1);
-    double s = r * q;
-    double res = fma(T, s, T);
-    int hi = __double2hiint(res) + ((nlo >> KX_EXP_BITS) << 20);
-    return __hiloint2double(hi, __double2loint(res));
-}
-
 // ---------------------------------------------------------------- prep: (y_j, y_{j+1}-y_j) per (b, j)
 __device__ __forceinline__ double kx_yval(double f, int interp, double f_floor)
 {
@@ -139,7 +116,7 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
                 const double2 y = s_yd[b * N + j];
                 const double t = fma(omc, y.y, y.x);
                 double x;
-                if (MODE == MODE_LOG_TAB) x = kx_exp2_tab(t, tab_lane);
+                if (MODE == MODE_LOG_TAB) x = kx_exp2_tab<KX_EXP_REP>(t, tab_lane);
                 else if (MODE == MODE_LOG_LIBM) x = exp2(t);
                 else x = t;
                 l[b] = fma(Wc, x, l[b]);

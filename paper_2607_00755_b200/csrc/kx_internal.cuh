@@ -151,6 +151,31 @@ inline cudaError_t kx_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, si
 __device__ __forceinline__ void kx_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void kx_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// ---------------------------------------------------------------- exp2 for the LOG loss term
+// 2^t = 2^k * T[idx] * 2^r,  t = k + idx/256 + r, |r| <= 2^-9.  Adding 1.5*2^44 leaves round(256 t) in the
+// low mantissa bits (one DADD), T is a 256-entry table in shared memory (entry k at tab[k * STRIDE]; the streaming
+// kernel replicates it 16x so that its 64-bit gathers are bank-conflict free), 2^r = 1 + r q(r) with q the degree-3 Chebyshev interpolant of
+// (2^r-1)/r on |r| <= 1.01*2^-9 (polynomial error 5e-18), and 2^k is added to the exponent field by the
+// integer pipe.  FP64-pipe cost: 2 DADD + 1 DADD + 3 DFMA + 1 DMUL + 1 DFMA = 8.  Valid for
+// -1021 < t < 1023 (f_floor >= 1e-300 keeps t >= -997).
+template <int STRIDE>
+__device__ __forceinline__ double kx_exp2_tab(double t, const double* __restrict__ tab_lane)
+{
+    const double MAG = 26388279066624.0;                 // 1.5 * 2^44
+    const double C1 = 0.6931471805599427, C2 = 0.24022650695910042,
+                 C3 = 0.05550411385340617, C4 = 0.009618129707037269;
+    double tm = t + MAG;
+    int nlo = __double2loint(tm);
+    double r = t - (tm - MAG);
+    double T = tab_lane[(nlo & ((1 << KX_EXP_BITS) - 1)) * STRIDE];
+    double q = fma(fma(fma(C4, r, C3), r, C2), r, C1);
+    double s = r * q;
+    double res = fma(T, s, T);
+    int hi = __double2hiint(res) + ((nlo >> KX_EXP_BITS) << 20);
+    return __hiloint2double(hi, __double2loint(res));
+}
+
+
 // Per-member statistics of the tiled LOG path, accumulated with atomicMax by k_xt (order independent, so the
 // result is deterministic):  mstat[2b] = key(max over brackets j of  log2 max(f_j, f_j+1) + Q (log2 |ln(f_j+1/f_j)| - 2)
 // + log2(2/Q!)),  mstat[2b+1] = bits of max_i |f_i|.  key() maps doubles to integers of the same order.

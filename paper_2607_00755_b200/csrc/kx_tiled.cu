@@ -36,13 +36,17 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
     __shared__ double s_dct[KX_QMAX * KX_QMAX];
     __shared__ double s_node[KX_QMAX];
     __shared__ double s_G[KX_QMAX][64];
+    __shared__ double s_y[2][64];
+    __shared__ double s_tab[1 << KX_EXP_BITS];
     const int N = d.N, Q = t.Q, j = blockIdx.x;
+    const bool tab = d.exp_impl == KX_EXP_TABLE;
     const int bl = threadIdx.x & 63, ph = threadIdx.x >> 6;
     const bool logm = d.interp == KX_INTERP_LOG;
     kx_pdl_trigger();       // first kernel of the call (ordinary launch): the contraction kernel may start right away
     if (logm) {
         for (int k = threadIdx.x; k < Q * Q; k += 256) s_dct[k] = t.dct[k];
         if (threadIdx.x < Q) s_node[threadIdx.x] = t.nodes[threadIdx.x];
+        if (tab) s_tab[threadIdx.x] = d.exptab[threadIdx.x];          // 256 threads, 2^KX_EXP_BITS = 256 entries
     }
     __syncthreads();
     for (int b0 = 0; b0 < B; b0 += 64) {
@@ -68,8 +72,11 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
             }
             continue;
         }
-        const double y0 = log2(fmax(fj, d.f_floor));
-        const double y1 = log2(fmax(fj1, d.f_floor));
+        // one logarithm per thread: phase 0 takes f_j, phase 1 takes f_(j+1)
+        if (ph < 2) s_y[ph][bl] = log2(fmax(ph == 0 ? fj : fj1, d.f_floor));
+        __syncthreads();
+        const double y0 = s_y[0][bl];
+        const double y1 = j + 1 < N ? s_y[1][bl] : y0;
         const double dy = y1 - y0;
         if (act && ph == 0) {
             yd[(size_t)b * N + j] = make_double2(y0, dy);
@@ -80,14 +87,20 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
                 if (lk > mstat[2 * b]) atomicMax(mstat + 2 * b, lk);
             }
         }
-        if (j >= N - 1) continue;       // uniform over the CTA
-        for (int q = ph; q < Q; q += 4) s_G[q][bl] = exp2(fma(s_node[q], dy, y0));
+        if (j >= N - 1) { __syncthreads(); continue; }       // uniform over the CTA
+        if (tab) for (int q = ph; q < Q; q += 4) s_G[q][bl] = kx_exp2_tab<1>(fma(s_node[q], dy, y0), s_tab);
+        else for (int q = ph; q < Q; q += 4) s_G[q][bl] = exp2(fma(s_node[q], dy, y0));
         __syncthreads();
         if (act) {
             for (int c = ph; c < Q; c += 4) {
-                double a = 0.0;
-                for (int q = 0; q < Q; ++q) a = fma(s_dct[c * Q + q], s_G[q][bl], a);
-                XT[(size_t)(t.loss_row0 + j * Q + c) * xstride + b] = a;
+                double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;          // Q is a multiple of 4: four independent chains
+                for (int q = 0; q < Q; q += 4) {
+                    a0 = fma(s_dct[c * Q + q], s_G[q][bl], a0);
+                    a1 = fma(s_dct[c * Q + q + 1], s_G[q + 1][bl], a1);
+                    a2 = fma(s_dct[c * Q + q + 2], s_G[q + 2][bl], a2);
+                    a3 = fma(s_dct[c * Q + q + 3], s_G[q + 3][bl], a3);
+                }
+                XT[(size_t)(t.loss_row0 + j * Q + c) * xstride + b] = (a0 + a1) + (a2 + a3);
             }
         }
         __syncthreads();
