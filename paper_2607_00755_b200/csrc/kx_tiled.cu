@@ -20,6 +20,13 @@ namespace {
 // makes both roles finish together)
 constexpr double kLossCost = 1.0;
 
+// D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
 // ---------------------------------------------------------------- operand rows XT[row, b]
 //   rows loss_row0 + jQ + c    a_c(b,j), c < Q, j < N-1      (loss; the gain role of k_dmma reads f itself)
 // LOG:    g(omega_q) = 2^(y_j + omega_q (y_{j+1}-y_j)), y = log2 max(f, f_floor), at the Q Chebyshev nodes of [0,1];
@@ -33,9 +40,8 @@ constexpr double kLossCost = 1.0;
 __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __restrict__ f, double2* __restrict__ yd,
                                             double* __restrict__ XT, int xstride, long long* __restrict__ mstat, int B)
 {
-    __shared__ double s_dct[KX_QMAX * KX_QMAX];
     __shared__ double s_node[KX_QMAX];
-    __shared__ double s_G[KX_QMAX][64];
+    __shared__ double s_G[KX_QMAX][68];        // row stride 4 mod 16: the 4 x 8 fragment reads below are conflict free
     __shared__ double s_y[2][64];
     __shared__ double s_tab[1 << KX_EXP_BITS];
     const int N = d.N, Q = t.Q, j = blockIdx.x;
@@ -43,8 +49,16 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
     const int bl = threadIdx.x & 63, ph = threadIdx.x >> 6;
     const bool logm = d.interp == KX_INTERP_LOG;
     kx_pdl_trigger();       // first kernel of the call (ordinary launch): the contraction kernel may start right away
+    // the transform runs on the tensor pipe: a_c[b] = sum_q dct[c,q] G[q,b] is a (Q x Q) x (Q x 64) product, warp w takes
+    // members 8w..8w+7; its fragments of dct (lane: dct[8 ct + lane/4][4 ks + lane%4]) stay in registers
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double afr[KX_QMAX / 8][KX_QMAX / 4];
     if (logm) {
-        for (int k = threadIdx.x; k < Q * Q; k += 256) s_dct[k] = t.dct[k];
+#pragma unroll
+        for (int ct = 0; ct < KX_QMAX / 8; ++ct)
+#pragma unroll
+            for (int ks = 0; ks < KX_QMAX / 4; ++ks)
+                afr[ct][ks] = (8 * ct < Q && 4 * ks < Q) ? t.dct[(8 * ct + (lane >> 2)) * Q + 4 * ks + (lane & 3)] : 0.0;
         if (threadIdx.x < Q) s_node[threadIdx.x] = t.nodes[threadIdx.x];
         if (tab) s_tab[threadIdx.x] = d.exptab[threadIdx.x];          // 256 threads, 2^KX_EXP_BITS = 256 entries
     }
@@ -91,16 +105,27 @@ __global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __
         if (tab) for (int q = ph; q < Q; q += 4) s_G[q][bl] = kx_exp2_tab<1>(fma(s_node[q], dy, y0), s_tab);
         else for (int q = ph; q < Q; q += 4) s_G[q][bl] = exp2(fma(s_node[q], dy, y0));
         __syncthreads();
-        if (act) {
-            for (int c = ph; c < Q; c += 4) {
-                double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;          // Q is a multiple of 4: four independent chains
-                for (int q = 0; q < Q; q += 4) {
-                    a0 = fma(s_dct[c * Q + q], s_G[q][bl], a0);
-                    a1 = fma(s_dct[c * Q + q + 1], s_G[q + 1][bl], a1);
-                    a2 = fma(s_dct[c * Q + q + 2], s_G[q + 2][bl], a2);
-                    a3 = fma(s_dct[c * Q + q + 3], s_G[q + 3][bl], a3);
+        {
+            double D[KX_QMAX / 8][2];
+#pragma unroll
+            for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[ct][0] = D[ct][1] = 0.0;
+#pragma unroll
+            for (int ks = 0; ks < KX_QMAX / 4; ++ks) {
+                if (4 * ks < Q) {                                        // uniform
+                    const double g = s_G[4 * ks + (lane & 3)][8 * warp + (lane >> 2)];
+#pragma unroll
+                    for (int ct = 0; ct < KX_QMAX / 8; ++ct)
+                        if (8 * ct < Q) dmma884(D[ct][0], D[ct][1], afr[ct][ks], g);
                 }
-                XT[(size_t)(t.loss_row0 + j * Q + c) * xstride + b] = (a0 + a1) + (a2 + a3);
+            }
+            const int bw = b0 + 8 * warp + 2 * (lane & 3);                // lane holds a_c[bw], a_c[bw+1], c = 8 ct + lane/4
+#pragma unroll
+            for (int ct = 0; ct < KX_QMAX / 8; ++ct) {
+                if (8 * ct < Q) {
+                    double* dst = XT + (size_t)(t.loss_row0 + j * Q + 8 * ct + (lane >> 2)) * xstride + bw;
+                    if (bw + 1 < B) *reinterpret_cast<double2*>(dst) = make_double2(D[ct][0], D[ct][1]);
+                    else if (bw < B) dst[0] = D[ct][0];
+                }
             }
         }
         __syncthreads();
@@ -116,13 +141,6 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int NPEND>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(NPEND) : "memory"); }
-
-// D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
-__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
-{
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-        : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
 
 constexpr int kStageBytes = KX_GROUP_DBL * 8 + 16;     // gain ring stage: 2 KiB of A + 4 descriptors
 constexpr int kLossStages = 3;
