@@ -323,3 +323,29 @@ def test_tiled_batch_sizes(torch_cuda, oracle, B):
     C = h.collide(_dev(torch, c["f"])).cpu().numpy()
     assert _relerr(C, C0, g0) <= 2e-13
     h.close()
+
+
+def test_back_to_back_calls_are_ordered(torch_cuda):
+    """The kernels of one call overlap through programmatic dependent launch and every call reuses the handle's
+    workspaces (operand rows, partials, member statistics): calls enqueued back to back without a host sync must
+    give the bits of calls run one at a time, also when smooth and flagged (fallback) members alternate."""
+    torch = torch_cuda
+    c = kin.config(3, N=96, B=24)
+    h = _handle(c)
+    fa = c["f"].copy()
+    fb = c["f"][::-1].copy()
+    fb[3, c["p"] > 2.0] = 0.0            # one member that takes the exact streaming path
+    fb[10] *= 1e-120
+    da, db = _dev(torch, fa), _dev(torch, fb)
+    ref_a = h.collide(da, flags=1).clone()
+    torch.cuda.synchronize()
+    ref_b = h.collide(db, flags=1).clone()
+    torch.cuda.synchronize()
+    outs = [torch.empty_like(da) for _ in range(6)]
+    for rep in range(10):
+        for k, o in enumerate(outs):
+            h.collide(da if k % 2 == 0 else db, flags=1, out=o)
+        torch.cuda.synchronize()
+        for k, o in enumerate(outs):
+            assert torch.equal(o, ref_a if k % 2 == 0 else ref_b), (rep, k)
+    h.close()
