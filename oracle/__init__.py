@@ -46,6 +46,12 @@ def _load():
         _lib.okx_collide.argtypes = [C.c_int, C.c_int, _dp, _dp, _ip, _dp, C.c_int, C.c_double,
                                      _dp, _dp, _dp]
         _lib.okx_collide.restype = None
+        _lib.okx_collide_q.argtypes = [C.c_int, C.c_int, _dp, _dp, _ip, _dp, C.c_int, C.c_double, _dp, _dp, _dp]
+        _lib.okx_collide_q.restype = None
+        _lib.okx_evolve_q.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double,
+                                      C.c_double, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _dp, _dp, _dp, _dp,
+                                      C.c_int, C.c_int, _dp, _dp, _dp]
+        _lib.okx_evolve_q.restype = C.c_int
         _lib.okx_collide_rows.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double,
                                           C.c_double, _dp, C.c_int, _ip, C.c_int, C.c_double, _dp, _dp, _dp]
         _lib.okx_collide_rows.restype = None
@@ -111,6 +117,18 @@ def collide(T: Tables, f, interp=LOG, f_floor=1e-300):
     return g, l, c
 
 
+def collide_q(T: Tables, f, eta, f_floor=1e-300):
+    """Quantum-statistics operator (eq. 4.3 with B.20), eta = +1 Bose / -1 Fermi: returns gain, loss, C_raw [B,N]."""
+    assert eta in (1, -1)
+    f = _c(np.atleast_2d(f))
+    B, n = f.shape
+    assert n == T.N
+    g, l, c = np.empty((B, n)), np.empty((B, n)), np.empty((B, n))
+    _load().okx_collide_q(n, B, _d(f), _d(T.W), T.jL.ctypes.data_as(_ip), _d(T.wR), int(eta), float(f_floor),
+                          _d(g), _d(l), _d(c))
+    return g, l, c
+
+
 def collide_rows(p, dp, f, rows, *, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, interp=LOG, f_floor=1e-300):
     """O2-O9 for the selected rows i only (no stored tables): returns gain, loss, C_raw, each [B, len(rows)]."""
     p, dp = _c(p), _c(dp)
@@ -145,8 +163,9 @@ def moments(T: Tables, f):
 
 def evolve(p, dp, f, *, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, interp=LOG, f_floor=1e-300,
            eps_supp=1e-12, method=RK4, tau=None, rate=None, mass=None, kappa=None, project=True,
-           G=None, amp=None, want_diag=False):
-    """O12: fixed-step integration; returns f_final [B,N] (and diag [S,B,6] if want_diag)."""
+           G=None, amp=None, want_diag=False, eta=0):
+    """O12: fixed-step integration; returns f_final [B,N] (and diag [S,B,6] if want_diag).
+    eta = +1 / -1 integrates the quantum-statistics operator (collide_q) instead."""
     p, dp = _c(p), _c(dp)
     f = _c(np.atleast_2d(f)).copy()
     B, n = f.shape
@@ -159,10 +178,16 @@ def evolve(p, dp, f, *, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, interp=LOG, f_flo
     G = None if G is None else _c(np.atleast_2d(G))
     amp = None if amp is None else _c(np.atleast_2d(amp))
     diag = np.zeros((S, B, 6)) if want_diag else None
-    rc = _load().okx_evolve(n, B, _d(p), _d(dp), float(m), float(g_chi), float(M2_0), float(m_med),
-                            int(interp), float(f_floor), float(eps_supp), _d(f), int(method), S,
-                            _d(tau), _d(rate), _d(mass), _d(kappa), int(bool(project)), nsrc,
-                            _d(G), _d(amp), _d(diag))
+    if eta:
+        rc = _load().okx_evolve_q(int(eta), n, B, _d(p), _d(dp), float(m), float(g_chi), float(M2_0), float(m_med),
+                                  float(f_floor), float(eps_supp), _d(f), int(method), S,
+                                  _d(tau), _d(rate), _d(mass), _d(kappa), int(bool(project)), nsrc,
+                                  _d(G), _d(amp), _d(diag))
+    else:
+        rc = _load().okx_evolve(n, B, _d(p), _d(dp), float(m), float(g_chi), float(M2_0), float(m_med),
+                                int(interp), float(f_floor), float(eps_supp), _d(f), int(method), S,
+                                _d(tau), _d(rate), _d(mass), _d(kappa), int(bool(project)), nsrc,
+                                _d(G), _d(amp), _d(diag))
     assert rc == 0
     return (f, diag) if want_diag else f
 

@@ -170,6 +170,41 @@ void okx_collide(int N, int B, const double *f, const double *W, const int32_t *
         }
 }
 
+/* ---- Quantum-statistics operator: the full Lambda_inm of eq. 4.3,
+ *     Lambda = f_n f_m (1 + eta f_i)(1 + eta f_j~) - f_i f_j~ (1 + eta f_n)(1 + eta f_m),
+ * eta = +1 (Bose-Einstein), -1 (Fermi-Dirac); one species, so eta_i = eta_n = eta_m = eta_j~ = eta.
+ * Off-grid occupation by eq. B.20: y_k = ln(f_k / (1 + eta f_k)), y_j~ = w_L y_L + w_R y_R,
+ * f_j~ = e^y / (1 - eta e^y); f_k is floored at f_floor inside the logarithm (reading D8).
+ * gain_i = sum W f_n f_m (1+eta f_i)(1+eta f_j~), loss_i = f_i sum W f_j~ (1+eta f_n)(1+eta f_m), C = gain - loss. */
+void okx_collide_q(int N, int B, const double *f, const double *W, const int32_t *jL, const double *wR,
+                   int eta, double f_floor, double *gain, double *loss, double *C)
+{
+#pragma omp parallel for collapse(2) schedule(dynamic)
+    for (int b = 0; b < B; ++b)
+        for (int i = 0; i < N; ++i) {
+            const double *fb = f + (size_t)b * N;
+            const long double e = (long double)eta, fi = fb[i];
+            long double g = 0.0L, l = 0.0L;
+            for (int n = 0; n < N; ++n)
+                for (int mm = 0; mm < N; ++mm) {
+                    size_t idx = ((size_t)i * N + n) * N + mm;
+                    int j = jL[idx];
+                    if (j < 0) continue;
+                    double oR = wR[idx], oL = 1.0 - oR;
+                    double fL = fmax(fb[j], f_floor), fR = fmax(fb[j + 1], f_floor);
+                    double yL = log(fL / (1.0 + eta * fL)), yR = log(fR / (1.0 + eta * fR));
+                    double ey = exp(oL * yL + oR * yR);
+                    long double fj = (long double)ey / (1.0L - e * (long double)ey);
+                    long double fn = fb[n], fm = fb[mm], w = W[idx];
+                    g += w * fn * fm * (1.0L + e * fi) * (1.0L + e * fj);
+                    l += w * fi * fj * (1.0L + e * fn) * (1.0L + e * fm);
+                }
+            if (gain) gain[(size_t)b * N + i] = (double)g;
+            if (loss) loss[(size_t)b * N + i] = (double)l;
+            if (C) C[(size_t)b * N + i] = (double)(g - l);
+        }
+}
+
 /* ---- O2-O9 for SELECTED rows i only, without storing the tables: the same per-triple code (okx_triple) and the
  * same accumulation as okx_collide, used to sample the operator at sizes where the dense N^3 tables are too
  * slow to build (N = 512).  rows[nrows]; outputs are [B, nrows]. */
@@ -294,7 +329,7 @@ void okx_moments(int N, const double *f, const double *p, const double *h, const
  * diag: NULL or [S,B,6] = eps_N, eps_E, R_N, R_E (of the step's first stage), n, rho (after the step). */
 typedef struct {
     int N; const double *p, *dp; double m, g_chi, M2_0, m_med; int interp; double f_floor, eps_supp;
-    double *W; int32_t *jL; double *wR; double *E, *K, *h; double cur_m;
+    double *W; int32_t *jL; double *wR; double *E, *K, *h; double cur_m; int eta;
 } okx_ctx;
 
 static void okx_rhs(okx_ctx *c, const double *f, double mass, int use_mass, double kR, int project,
@@ -307,7 +342,8 @@ static void okx_rhs(okx_ctx *c, const double *f, double mass, int use_mass, doub
         c->cur_m = mass;
     }
     double *Craw = malloc(sizeof(double) * N), *Cp = malloc(sizeof(double) * N);
-    okx_collide(N, 1, f, c->W, c->jL, c->wR, c->interp, c->f_floor, NULL, NULL, Craw);
+    if (c->eta) okx_collide_q(N, 1, f, c->W, c->jL, c->wR, c->eta, c->f_floor, NULL, NULL, Craw);
+    else okx_collide(N, 1, f, c->W, c->jL, c->wR, c->interp, c->f_floor, NULL, NULL, Craw);
     if (project) okx_project(N, f, Craw, c->h, c->E, c->K, c->eps_supp, Cp, diag4);
     else { memcpy(Cp, Craw, sizeof(double) * N); if (diag4) okx_project(N, f, Craw, c->h, c->E, c->K, c->eps_supp, Craw, diag4); }
     for (int i = 0; i < N; ++i) {
@@ -318,7 +354,7 @@ static void okx_rhs(okx_ctx *c, const double *f, double mass, int use_mass, doub
     free(Craw); free(Cp);
 }
 
-int okx_evolve(int N, int B, const double *p, const double *dp, double m, double g_chi,
+static int okx_evolve_impl(int eta, int N, int B, const double *p, const double *dp, double m, double g_chi,
                double M2_0, double m_med, int interp, double f_floor, double eps_supp,
                double *f, int method, int S, const double *tau, const double *rate,
                const double *mass, const double *kappa, int project,
@@ -328,6 +364,7 @@ int okx_evolve(int N, int B, const double *p, const double *dp, double m, double
     okx_ctx c = { N, p, dp, m, g_chi, M2_0, m_med, interp, f_floor, eps_supp,
                   malloc(sizeof(double) * N3), malloc(sizeof(int32_t) * N3), malloc(sizeof(double) * N3),
                   malloc(sizeof(double) * N), malloc(sizeof(double) * N), malloc(sizeof(double) * N), m };
+    c.eta = eta;
     okx_build(N, p, dp, m, g_chi, M2_0, m_med, c.W, c.jL, c.wR);
     okx_kinematics(N, p, dp, m, c.E, c.K, c.h);
     double *k1 = malloc(sizeof(double) * N), *k2 = malloc(sizeof(double) * N), *k3 = malloc(sizeof(double) * N),
@@ -399,6 +436,27 @@ int okx_evolve(int N, int B, const double *p, const double *dp, double m, double
     free(k1); free(k2); free(k3); free(k4); free(ft); free(ampk);
     free(c.W); free(c.jL); free(c.wR); free(c.E); free(c.K); free(c.h);
     return 0;
+}
+
+int okx_evolve(int N, int B, const double *p, const double *dp, double m, double g_chi,
+               double M2_0, double m_med, int interp, double f_floor, double eps_supp,
+               double *f, int method, int S, const double *tau, const double *rate,
+               const double *mass, const double *kappa, int project,
+               int nsrc, const double *G, const double *amp, double *diag)
+{
+    return okx_evolve_impl(0, N, B, p, dp, m, g_chi, M2_0, m_med, interp, f_floor, eps_supp, f, method, S, tau, rate,
+                           mass, kappa, project, nsrc, G, amp, diag);
+}
+
+/* the same integrators with the quantum-statistics operator okx_collide_q (eta = +1 / -1) */
+int okx_evolve_q(int eta, int N, int B, const double *p, const double *dp, double m, double g_chi,
+                 double M2_0, double m_med, double f_floor, double eps_supp,
+                 double *f, int method, int S, const double *tau, const double *rate,
+                 const double *mass, const double *kappa, int project,
+                 int nsrc, const double *G, const double *amp, double *diag)
+{
+    return okx_evolve_impl(eta, N, B, p, dp, m, g_chi, M2_0, m_med, 0, f_floor, eps_supp, f, method, S, tau, rate,
+                           mass, kappa, project, nsrc, G, amp, diag);
 }
 
 /* ---- Pin helper (P9), NOT on the evaluate path: the reduced kernel F(p_i,p_n,p_m) by the

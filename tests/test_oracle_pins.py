@@ -364,3 +364,57 @@ def test_collide_rows_equals_full_tables(oracle, cfg, interp):
     gr, lr, Cr = oracle.collide_rows(c["p"], c["dp"], c["f"], rows, m=c["m"], g_chi=c["g_chi"], M2_0=c["M2_0"],
                                      m_med=c["m_med"], interp=interp)
     assert np.array_equal(gr, g[:, rows]) and np.array_equal(lr, l[:, rows]) and np.array_equal(Cr, C[:, rows])
+
+
+# ------------------------------------------------------------------ quantum-statistics operator
+@pytest.mark.parametrize("eta,mu,Tchi", [(1, 0.0, 1.0), (1, -0.4, 0.7), (-1, 0.5, 1.0), (-1, 2.0, 0.3)])
+def test_Q1_quantum_thermal_fixed_point(oracle, eta, mu, Tchi):
+    """Fig. 11: N=96, T/m=1, mu=0 Bose-Einstein; the raw operator vanishes at round-off because
+    y = ln(f/(1+eta f)) = (mu-E)/T is linear in E (eq. B.20).  Same for Fermi-Dirac and other (T, mu)."""
+    p = kin.log_grid(96, 1e-3, 1e2)
+    dp = kin.trapezoid_widths(p)
+    T = oracle.Tables(p, dp, 1.0)
+    f = 1.0 / (np.exp((T.E - mu) / Tchi) - eta)
+    g, l, C = oracle.collide_q(T, f, eta)
+    assert np.abs(C).max() <= 1e-13 * np.abs(g).max()
+    # a distribution that is NOT of that form does not vanish (the test has teeth)
+    g2, l2, C2 = oracle.collide_q(T, f * (1.0 - 0.3 * np.sin(p) ** 2), eta)
+    assert np.abs(C2).max() >= 1e-4 * np.abs(g2).max()
+
+
+@pytest.mark.parametrize("eta", [1, -1])
+def test_Q2_dilute_limit_is_the_classical_operator(oracle, eta):
+    """eq. 2.6: for f << 1 the quantum factors drop out; the difference is O(f) relative."""
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    for eps in (1e-4, 1e-7):
+        f = eps * c["f"]
+        g0, l0, C0 = oracle.collide(T, f, oracle.LOG)
+        g, l, C = oracle.collide_q(T, f, eta)
+        rel = np.abs(C - C0).max() / np.abs(g0).max()
+        assert rel <= 20.0 * eps * np.abs(c["f"]).max(), (eps, rel)
+        assert rel >= 1e-3 * eps            # and it is there: the quantum terms are not silently dropped
+
+
+@pytest.mark.parametrize("eta", [1, -1])
+def test_Q3_quantum_conservation_and_H_theorem_on_exact_grid(oracle, eta):
+    """On the massless uniform grid of pin P4 every j~ is on-grid, Lambda is antisymmetric under (i,j~)<->(n,m) and
+    h_i W_inm is symmetric, so the RAW quantum operator conserves number and energy at round-off and the discrete
+    entropy production  -sum_i h_i C_i ln(f_i/(1+eta f_i))  is >= 0 (a wrong sign or a dropped factor breaks one)."""
+    N = 40
+    p = 0.25 * np.arange(1, N + 1)
+    dp = np.full(N, 0.25)
+    T = oracle.Tables(p, dp, 0.0)
+    rng = np.random.default_rng(77)
+    f = (0.4 + 0.3 * rng.uniform(size=N)) * np.exp(-0.5 * (p - 3.0) ** 2) + 0.05 * np.exp(-p / 4)
+    if eta == -1:
+        assert f.max() < 1.0
+    g, l, C = oracle.collide_q(T, f, eta)
+    h = T.h
+    assert abs((h * C[0]).sum()) <= 1e-13 * (h * np.abs(C[0])).sum()
+    assert abs((h * T.E * C[0]).sum()) <= 1e-13 * (h * T.E * np.abs(C[0])).sum()
+    sigma = -(h * C[0] * np.log(f / (1.0 + eta * f))).sum()
+    assert sigma > 0.0
+    # eta enters: Bose enhancement and Pauli blocking move the operator in opposite directions from the classical one
+    g0, l0, C0 = oracle.collide(T, f, oracle.LOG)
+    assert np.abs(C[0] - C0[0]).max() > 1e-3 * np.abs(g0).max()
