@@ -7,6 +7,7 @@
  *   index map         E_j~ = E_n+E_m-E_i, bracket j_L and weight omega_R            eq. 4.4, B.19
  *   kernel tensor     W_inm = dp_n dp_m F_inm / (2 E_i g_chi)                        eq. 4.7, B.15-B.17
  *   operator          C_i = sum_{n,m} W_inm (f_n f_m - f_i f_j~)                     eq. 4.6 with eq. 2.6
+ *                     or with the quantum factors of eq. 4.3 for KX_STAT_BOSE / KX_STAT_FERMI
  *   interpolation     f_j~ = exp(w_L ln f_L + w_R ln f_R)  (LOG)  or  w_L f_L + w_R f_R (LINEAR)   eq. B.20
  *   projection        C^proj = C^raw - xi_i (alpha + beta E_i)                       App. C, eq. C.2-C.8
  *   moments           n = g/(2 pi^2) sum h f, rho = g/(2 pi^2) sum h E f             eq. B.2
@@ -63,6 +64,13 @@ typedef enum {
 /* exp used by the LOG loss term */
 #define KX_EXP_TABLE 0        /* 128-entry table + degree-4 polynomial, <= 1 ulp-level error (default) */
 #define KX_EXP_LIBM  1        /* CUDA math library exp2() */
+/* quantum statistics of the species (eq. 4.3): Lambda_inm = f_n f_m (1+eta f_i)(1+eta f_j~)
+ * - f_i f_j~ (1+eta f_n)(1+eta f_m), off-grid occupation through y = ln(f/(1+eta f)) (eq. B.20).
+ * eta != 0 needs KX_INTERP_LOG and is evaluated by the exact streaming kernel (the operator is no longer bilinear);
+ * Fermi-Dirac needs 0 <= f < 1. */
+#define KX_STAT_CLASSICAL 0   /* Maxwell-Boltzmann, the dilute limit of eq. 2.6 (default) */
+#define KX_STAT_BOSE      1
+#define KX_STAT_FERMI   (-1)
 /* flags of kx_collide / kx_evolve */
 #define KX_PROJECT 1u         /* apply the two-moment projection of App. C */
 #define KX_DIAG    2u         /* kx_evolve: fill ctl->diag */
@@ -84,7 +92,7 @@ typedef struct {
     int32_t precision;   /* KX_FP64      */
     int32_t exp_impl;    /* KX_EXP_*     */
     int32_t loss_nodes;  /* KX_STORE_TILED + LOG: Chebyshev nodes per bracket, 8|16|24|32; 0 = default (24) */
-    int32_t reserved;    /* must be 0 */
+    int32_t statistics;  /* KX_STAT_*: eta = 0 | +1 | -1 */
     double  f_floor;     /* y = ln max(f, f_floor), reading D8; must be >= 1e-300 and > 0 */
     double  eps_supp;    /* support threshold of eq. C.4, reading D9 */
 } kx_opts_t;
@@ -103,7 +111,8 @@ kx_status_t kx_set_mass(kx_handle_t h, double m, void* stream);
  * In place (C == f) is not allowed. */
 kx_status_t kx_collide(kx_handle_t h, const double* f, double* C, int32_t B, uint32_t flags, void* stream);
 
-/* a4, a5 separately: gain[b,i] = sum W f_n f_m, loss[b,i] = f_i sum W f_j~ (DEVICE [B,N]; either may be NULL). */
+/* a4, a5 separately: gain[b,i] = sum W f_n f_m, loss[b,i] = f_i sum W f_j~ (DEVICE [B,N]; either may be NULL);
+ * with statistics: gain = sum W f_n f_m (1+eta f_i)(1+eta f_j~), loss = f_i sum W f_j~ (1+eta f_n)(1+eta f_m). */
 kx_status_t kx_collide_parts(kx_handle_t h, const double* f, double* gain, double* loss, int32_t B, void* stream);
 
 /* General form: any of C, gain, loss, diag may be NULL.  diag: DEVICE [B,4] = eps_N, eps_E (eq. C.1,

@@ -4,9 +4,9 @@ C ABI of include/kx.h (libkx.so); this package is the thin ctypes binding (argum
 There is no CPU fallback: importing works anywhere, every call needs an sm_100 GPU.
 """
 from .kx import (Handle, KxError, build_library, library_path, exported_symbols,
-                 INTERP_LOG, INTERP_LINEAR, EXP_TABLE, EXP_LIBM, STORE_SYM_ROWS, STORE_TILED, PROJECT, DIAG,
+                 INTERP_LOG, INTERP_LINEAR, EXP_TABLE, EXP_LIBM, STORE_SYM_ROWS, STORE_TILED, STAT_CLASSICAL, STAT_BOSE, STAT_FERMI, PROJECT, DIAG,
                  EULER, HEUN, RK4)
 
 __all__ = ["Handle", "KxError", "build_library", "library_path", "exported_symbols",
-           "INTERP_LOG", "INTERP_LINEAR", "EXP_TABLE", "EXP_LIBM", "STORE_SYM_ROWS", "STORE_TILED", "PROJECT", "DIAG",
+           "INTERP_LOG", "INTERP_LINEAR", "EXP_TABLE", "EXP_LIBM", "STORE_SYM_ROWS", "STORE_TILED", "STAT_CLASSICAL", "STAT_BOSE", "STAT_FERMI", "PROJECT", "DIAG",
            "EULER", "HEUN", "RK4"]

@@ -114,7 +114,7 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
     free_ws(h);
     const size_t bn = (size_t)nB * h->d.N;
     KX_CUDA(dalloc(&h->yd, bn * 2));
-    KX_CUDA(dalloc(&h->part, (size_t)need_tasks * nB * 2));
+    KX_CUDA(dalloc(&h->part, (size_t)need_tasks * nB * 4));      // 2 sums per (task, member); 4 with quantum statistics
     KX_CUDA(dalloc(&h->fstage, bn));
     KX_CUDA(dalloc(&h->k1, bn));
     KX_CUDA(dalloc(&h->k2, bn));
@@ -297,6 +297,15 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         return KX_ERR_INVALID_ARG;
     }
     if (o.interp != KX_INTERP_LOG && o.interp != KX_INTERP_LINEAR) { g_build_err = "unknown interpolation"; return KX_ERR_INVALID_ARG; }
+    if (o.statistics != KX_STAT_CLASSICAL && o.statistics != KX_STAT_BOSE && o.statistics != KX_STAT_FERMI) {
+        g_build_err = "statistics must be 0 (classical), +1 (Bose) or -1 (Fermi)";
+        return KX_ERR_INVALID_ARG;
+    }
+    if (o.statistics != KX_STAT_CLASSICAL && o.interp != KX_INTERP_LOG) {
+        g_build_err = "quantum statistics need KX_INTERP_LOG (eq. B.20)";
+        return KX_ERR_UNSUPPORTED;
+    }
+    if (o.statistics != KX_STAT_CLASSICAL) o.storage = KX_STORE_SYM_ROWS;     // evaluated by the exact streaming kernel
     if (o.exp_impl != KX_EXP_TABLE && o.exp_impl != KX_EXP_LIBM) { g_build_err = "unknown exp_impl"; return KX_ERR_INVALID_ARG; }
     if (!(o.f_floor >= 1e-300) || !(o.eps_supp >= 0.0)) { g_build_err = "need f_floor >= 1e-300 and eps_supp >= 0"; return KX_ERR_INVALID_ARG; }
 
@@ -322,7 +331,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     KxDev& d = h->d;
     d = KxDev{};
     h->t = KxTiled{};
-    d.N = N; d.interp = o.interp; d.exp_impl = o.exp_impl; d.chunk = 0;
+    d.N = N; d.interp = o.interp; d.exp_impl = o.exp_impl; d.eta = o.statistics; d.chunk = 0;
     d.m = sp->m; d.g_chi = sp->g_chi; d.M2_0 = msq->M2_0; d.m_med = msq->m_med;
     d.f_floor = o.f_floor; d.eps_supp = o.eps_supp;
     cudaStream_t s = (cudaStream_t)stream;

@@ -21,9 +21,12 @@
 namespace {
 
 // ---------------------------------------------------------------- prep: (y_j, y_{j+1}-y_j) per (b, j)
-__device__ __forceinline__ double kx_yval(double f, int interp, double f_floor)
+// y of eq. B.20 in base 2: log2(f / (1 + eta f)), f floored (reading D8); LINEAR interpolation works on f itself
+__device__ __forceinline__ double kx_yval(double f, int interp, double f_floor, int eta)
 {
-    return interp == KX_INTERP_LOG ? log2(fmax(f, f_floor)) : f;
+    if (interp != KX_INTERP_LOG) return f;
+    const double ff = fmax(f, f_floor);
+    return eta == 0 ? log2(ff) : log2(ff / (1.0 + (double)eta * ff));
 }
 
 __global__ void k_prep(KxDev d, const double* __restrict__ f, double2* __restrict__ yd, int B)
@@ -32,15 +35,18 @@ __global__ void k_prep(KxDev d, const double* __restrict__ f, double2* __restric
     int b = blockIdx.y;
     if (j >= d.N) return;
     const double* fb = f + (size_t)b * d.N;
-    double y0 = kx_yval(fb[j], d.interp, d.f_floor);
-    double y1 = (j + 1 < d.N) ? kx_yval(fb[j + 1], d.interp, d.f_floor) : y0;
+    double y0 = kx_yval(fb[j], d.interp, d.f_floor, d.eta);
+    double y1 = (j + 1 < d.N) ? kx_yval(fb[j + 1], d.interp, d.f_floor, d.eta) : y0;
     yd[(size_t)b * d.N + j] = make_double2(y0, y1 - y0);
 }
 
 // ---------------------------------------------------------------- contraction
 enum { MODE_LOG_TAB = 0, MODE_LOG_LIBM = 1, MODE_LINEAR = 2 };
 
-template <int BT, int MODE>
+// QS = 1: quantum statistics (eq. 4.3).  With x = f_j~ = e^y / (1 - eta e^y) four sums per (row, member) are kept,
+//   G1 = sum W f_n f_m,  L1 = sum W x,  G2 = sum W f_n f_m x,  L2 = sum W x (f_n + f_m),
+// from which  gain = (1 + eta f_i)(G1 + eta G2),  loss = f_i (L1 + eta L2 + G2)   (eta^2 = 1; k_finish).
+template <int BT, int MODE, int QS>
 __global__ void __launch_bounds__(KX_CTA, 2)
 k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd,
            double* __restrict__ part, int B, const long long* __restrict__ mstat)
@@ -49,8 +55,9 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
     const int N = d.N;
     double2* s_yd = reinterpret_cast<double2*>(smem_raw);                 // [BT][N]
     double* s_f = reinterpret_cast<double*>(s_yd + (size_t)BT * N);       // [BT][N]
-    double* s_red = s_f + (size_t)BT * N;                                 // [8][2*BT]
-    double* s_tab = s_red + (KX_CTA / 32) * 2 * BT;                       // [256][16] (MODE_LOG_TAB)
+    constexpr int NV = QS ? 4 : 2;                                         // sums per (row, member)
+    double* s_red = s_f + (size_t)BT * N;                                 // [8][NV*BT]
+    double* s_tab = s_red + (KX_CTA / 32) * NV * BT;                       // [256][16] (MODE_LOG_TAB)
     unsigned* s_tp = reinterpret_cast<unsigned*>(s_tab + (MODE == MODE_LOG_TAB ? (KX_EXP_REP << KX_EXP_BITS) : 0)); // [N+1]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -95,9 +102,10 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
         const unsigned e0 = r0 + (task - s_tp[i]) * chunk;
         const unsigned e1 = min(e0 + chunk, r1);
 
-        double g[BT], l[BT];
+        double g[BT], l[BT], g2[QS ? BT : 1], l2[QS ? BT : 1];
 #pragma unroll
-        for (int b = 0; b < BT; ++b) { g[b] = 0.0; l[b] = 0.0; }
+        for (int b = 0; b < BT; ++b) { g[b] = 0.0; l[b] = 0.0; if (QS) { g2[b] = 0.0; l2[b] = 0.0; } }
+        const double eta = (double)d.eta;
 
         unsigned e = e0 + tid;
         double W = 0.0, om = 0.0;
@@ -111,7 +119,8 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
             const int n = pkc & 1023, m = (pkc >> 10) & 1023, j = pkc >> 20;
 #pragma unroll
             for (int b = 0; b < BT; ++b) {
-                const double pn = s_f[b * N + n] * s_f[b * N + m];
+                const double fn = s_f[b * N + n], fm = s_f[b * N + m];
+                const double pn = fn * fm;
                 g[b] = fma(Wc, pn, g[b]);
                 const double2 y = s_yd[b * N + j];
                 const double t = fma(omc, y.y, y.x);
@@ -119,7 +128,14 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
                 if (MODE == MODE_LOG_TAB) x = kx_exp2_tab<KX_EXP_REP>(t, tab_lane);
                 else if (MODE == MODE_LOG_LIBM) x = exp2(t);
                 else x = t;
-                l[b] = fma(Wc, x, l[b]);
+                if (QS) {
+                    const double wf = Wc * (x / (1.0 - eta * x));       // W f_j~, eq. B.20
+                    l[b] += wf;
+                    g2[b] = fma(wf, pn, g2[b]);
+                    l2[b] = fma(wf, fn + fm, l2[b]);
+                } else {
+                    l[b] = fma(Wc, x, l[b]);
+                }
             }
         }
         // fixed-order reduction: xor butterfly inside the warp, then warps 0..7 in order
@@ -129,22 +145,27 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
             for (int o = 16; o > 0; o >>= 1) {
                 g[b] += __shfl_xor_sync(0xffffffffu, g[b], o);
                 l[b] += __shfl_xor_sync(0xffffffffu, l[b], o);
+                if (QS) {
+                    g2[b] += __shfl_xor_sync(0xffffffffu, g2[b], o);
+                    l2[b] += __shfl_xor_sync(0xffffffffu, l2[b], o);
+                }
             }
         }
         if (lane == 0) {
 #pragma unroll
             for (int b = 0; b < BT; ++b) {
-                s_red[warp * 2 * BT + 2 * b] = g[b];
-                s_red[warp * 2 * BT + 2 * b + 1] = l[b];
+                s_red[warp * NV * BT + NV * b] = g[b];
+                s_red[warp * NV * BT + NV * b + 1] = l[b];
+                if (QS) { s_red[warp * NV * BT + NV * b + 2] = g2[b]; s_red[warp * NV * BT + NV * b + 3] = l2[b]; }
             }
         }
         __syncthreads();
-        if (tid < 2 * BT) {
+        if (tid < NV * BT) {
             double acc = 0.0;
 #pragma unroll
-            for (int w = 0; w < KX_CTA / 32; ++w) acc += s_red[w * 2 * BT + tid];
-            const int b = tid >> 1;
-            if (b < nb) part[((size_t)task * B + (b0 + b)) * 2 + (tid & 1)] = acc;
+            for (int w = 0; w < KX_CTA / 32; ++w) acc += s_red[w * NV * BT + tid];
+            const int b = tid / NV;
+            if (b < nb) part[((size_t)task * B + (b0 + b)) * NV + (tid % NV)] = acc;
         }
         __syncthreads();
     }
@@ -254,18 +275,26 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
         const int i = tid + q * KX_CTA;
         C[q] = 0.0; fi[q] = 0.0; hi_[q] = 0.0; Ei[q] = 0.0; Ki[q] = 0.0;
         if (i < N) {
-            double g = 0.0, nu = 0.0;
+            double g = 0.0, nu = 0.0, gq2 = 0.0, lq2 = 0.0;
             if (tiled) {
                 const double2 v = st.gn[(size_t)b * N + i];          // partials of the DMMA kernel, added by k_reduce
                 g = v.x; nu = v.y;
             } else {
                 const unsigned t0 = d.taskptr[i], t1 = d.taskptr[i + 1];
+                const int nv = d.eta ? 4 : 2;
                 for (unsigned t = t0; t < t1; ++t) {
-                    g += part[((size_t)t * B + b) * 2];
-                    nu += part[((size_t)t * B + b) * 2 + 1];
+                    const double* pp = part + ((size_t)t * B + b) * nv;
+                    g += pp[0];
+                    nu += pp[1];
+                    if (d.eta) { gq2 += pp[2]; lq2 += pp[3]; }
                 }
             }
             fi[q] = fb[i];
+            if (d.eta) {                                          // eq. 4.3 from the four sums (see k_contract)
+                const double eta = (double)d.eta;
+                g = (1.0 + eta * fi[q]) * (g + eta * gq2);
+                nu = nu + eta * lq2 + gq2;
+            }
             C[q] = fma(-fi[q], nu, g);                            // a6
             hi_[q] = d.h[i]; Ei[q] = d.E[i]; Ki[q] = d.K[i];
             if (st.gain) st.gain[(size_t)b * N + i] = g;
@@ -366,7 +395,7 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
             else { next = f0 + (dt / 6.0) * (st.k1[o] + 2.0 * st.k2[o] + 2.0 * st.k3[o] + k); st.f[o] = next; }
         }
         if (!isfinite(next)) bad = true;
-        s_y[i] = kx_yval(next, d.interp, d.f_floor);
+        s_y[i] = kx_yval(next, d.interp, d.f_floor, d.eta);
     }
     if (bad) atomicOr(st.flag, 1);
     __syncthreads();
@@ -404,33 +433,37 @@ k_moments(KxDev d, const double* __restrict__ f, double* n, double* rho, double*
     }
 }
 
-template <int BT, int MODE>
+template <int BT, int MODE, int QS>
 cudaError_t launch_contract_t(const KxDev& d, int sm_count, const double* f, const double* yd,
                               double* part, int B, const long long* mstat, bool pdl, cudaStream_t s)
 {
     const int N = d.N;
-    size_t smem = (size_t)BT * N * 24 + (size_t)(KX_CTA / 32) * 2 * BT * 8
+    size_t smem = (size_t)BT * N * 24 + (size_t)(KX_CTA / 32) * (QS ? 4 : 2) * BT * 8
                 + (MODE == MODE_LOG_TAB ? (size_t)(KX_EXP_REP << KX_EXP_BITS) * 8 : 0) + (size_t)(N + 1) * 4;
-    cudaError_t e = cudaFuncSetAttribute(k_contract<BT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_contract<BT, MODE, QS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_contract<BT, MODE>, KX_CTA, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_contract<BT, MODE, QS>, KX_CTA, smem);
     if (e != cudaSuccess) return e;
     if (occ < 1) occ = 1;
     const int groups = (B + BT - 1) / BT;
     int gx = (sm_count * occ + groups - 1) / groups;
     if (gx < 1) gx = 1;
     dim3 grid(gx, groups);
-    return kx_launch(k_contract<BT, MODE>, grid, dim3(KX_CTA), smem, s, pdl, d, f, reinterpret_cast<const double2*>(yd), part, B, mstat);
+    return kx_launch(k_contract<BT, MODE, QS>, grid, dim3(KX_CTA), smem, s, pdl, d, f, reinterpret_cast<const double2*>(yd), part, B, mstat);
 }
 
 template <int BT>
 cudaError_t launch_contract_m(const KxDev& d, int sm_count, const double* f, const double* yd,
                               double* part, int B, const long long* mstat, bool pdl, cudaStream_t s)
 {
-    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR>(d, sm_count, f, yd, part, B, mstat, pdl, s);
-    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM>(d, sm_count, f, yd, part, B, mstat, pdl, s);
-    return launch_contract_t<BT, MODE_LOG_TAB>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+    if (d.eta) {         // quantum statistics: LOG interpolation only (checked in kx_build)
+        if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM, 1>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+        return launch_contract_t<BT, MODE_LOG_TAB, 1>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+    }
+    if (d.interp == KX_INTERP_LINEAR) return launch_contract_t<BT, MODE_LINEAR, 0>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+    if (d.exp_impl == KX_EXP_LIBM) return launch_contract_t<BT, MODE_LOG_LIBM, 0>(d, sm_count, f, yd, part, B, mstat, pdl, s);
+    return launch_contract_t<BT, MODE_LOG_TAB, 0>(d, sm_count, f, yd, part, B, mstat, pdl, s);
 }
 
 }  // namespace

@@ -25,6 +25,7 @@ struct KxDev {
     int N;
     int interp;          // KX_INTERP_*
     int exp_impl;        // KX_EXP_*
+    int eta;             // KX_STAT_*: 0, +1 (Bose), -1 (Fermi)
     int chunk;           // entries per contraction task
     double m, g_chi, M2_0, m_med, f_floor, eps_supp;
     // grid and kinematics [N]
