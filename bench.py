@@ -151,6 +151,10 @@ def main():
     ap.add_argument("--mode", default="log", choices=["log", "linear"])
     ap.add_argument("--project", action="store_true", help="time the projected operator (App. C) instead of the raw one")
     ap.add_argument("--batch", type=int, default=None, help="members per GPU (default: 64 for cfg3, 8 for cfg4)")
+    ap.add_argument("--storage", default="tiled", choices=["tiled", "rows"],
+                    help="rows = the exact streaming kernel alone (one exp per entry and member): FP64-ALU roofline")
+    ap.add_argument("--statistics", default="classical", choices=["classical", "bose", "fermi"],
+                    help="quantum statistics of eq. 4.3 (side measurement; streaming kernel, FP64-ALU roofline)")
     ap.add_argument("--config", type=int, default=3, choices=[3, 4],
                     help="3 = the headline workload; 4 = the N=512 small-batch workload (side measurement, HBM roofline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -181,8 +185,13 @@ def main():
     B = args.batch if args.batch else (64 if args.config == 3 else 8)
     K, Wm = args.steps, max(args.warmup, 3)
     c = _inputs(rank, B, args.config)
+    stat = {"classical": kx.STAT_CLASSICAL, "bose": kx.STAT_BOSE, "fermi": kx.STAT_FERMI}[args.statistics]
+    streaming = args.storage == "rows" or stat != 0
+    if stat != 0:    # occupations of order one, Fermi below 1: where the quantum factors matter
+        c["f"] = c["f"] / np.abs(c["f"]).max(axis=1, keepdims=True) * (0.8 if stat < 0 else 2.5)
     h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], device=local,
-                  interp=kx.INTERP_LOG if args.mode == "log" else kx.INTERP_LINEAR)
+                  interp=kx.INTERP_LOG if args.mode == "log" else kx.INTERP_LINEAR,
+                  storage=kx.STORE_SYM_ROWS if streaming else kx.STORE_TILED, statistics=stat)
     info = h.info()
     dev = torch.device("cuda", local)
     f = torch.tensor(c["f"], dtype=torch.float64, device=dev)
@@ -282,9 +291,19 @@ def main():
                      "peak_source_hbm": f"{peak_src} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)", "tflops": ach}
     else:
         roof_head = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak}
+    if streaming:
+        # k_contract: FP64-pipe instructions per (entry, member) counted in the SASS of the inner loop (DESIGN.md
+        # section 5): 12 classical LOG, 3 LINEAR, 33 with quantum statistics; peak = 148 SMs x 64 FP64 lanes x max clock
+        c_inst = 33 if stat != 0 else (12 if args.mode == "log" else 3)
+        ach_inst = nnz * B * c_inst / kern_s / 1e12
+        peak_inst = SM_COUNT * FP64_LANES_PER_SM * sm_max_hz / 1e12
+        roof_head = {"bound": "alu", "achieved": ach_inst, "peak": peak_inst, "unit": "T FP64 inst/s",
+                     "frac": ach_inst / peak_inst, "fp64_inst_per_entry_member": c_inst}
+        flop = float(nnz) * B * c_inst
     roof = {**roof_head,
-            "traffic": NCU_TRAFFIC.get((args.mode, B)) if (not args.project and args.config == 3) else None,
-            "kernel": "k_dmma (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss)",
+            "traffic": NCU_TRAFFIC.get((args.mode, B)) if (not args.project and args.config == 3 and not streaming) else None,
+            "kernel": ("k_contract (exact streaming kernel: gather, exp2, FMA per entry and member)" if streaming
+                       else "k_dmma (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss)"),
             "kernel_ms": kern_s * 1e3, "kernel_ms_l2_warm": kern_warm_ms / max(kern_warm_n, 1),
             "event_pair_around_empty_kernel_us": ev_over_us, "flop_per_launch": flop,
             "peak_source": f"FP64 tensor pipe: 148 SMs x 64 FMA/clk x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src}); "
@@ -294,17 +313,17 @@ def main():
             "tensor_bytes_per_launch": info["tensor_bytes"],
             "hbm_time_us_at_peak": t_hbm * 1e6, "tensor_time_us_at_peak": t_flop * 1e6}
     line = {
-        "metric": METRIC if args.config == 3 and B == 64 else f"C[f] evals/s (fp64, N={Ngrid}, B={B})", "value": shard.aggregate_rate(B, world, K, t_cold), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "metric": METRIC if args.config == 3 and B == 64 and stat == 0 else f"C[f] evals/s (fp64, N={Ngrid}, B={B})", "value": shard.aggregate_rate(B, world, K, t_cold), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": t_cold / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config], "N": Ngrid, "B_per_gpu": B, "mode": args.mode, "projected": bool(args.project),
-                   "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "storage": "tiled", "loss_nodes": Q, "l2": "flushed before every timed step (256 MiB write)",
+        "config": {"workload": WORKLOADS[args.config], "N": Ngrid, "B_per_gpu": B, "mode": args.mode, "statistics": args.statistics, "projected": bool(args.project),
+                   "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "storage": "rows (streaming)" if streaming else "tiled", "loss_nodes": Q, "l2": "flushed before every timed step (256 MiB write)",
                    "parallelism": f"independent batches x{world}" if world > 1 else "single GPU"},
         "value_l2_warm": world * B * K / t_warm, "ms_per_step_l2_warm": t_warm / K * 1e3,
         "calls_per_s": world * K / t_cold,
         "e2e": {"value": world * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": B * Ngrid * 8,
                 "d2h_bytes_per_step": B * Ngrid * 8, "ms_per_step": t_e2e / K * 1e3},
-        "gpu_launches": (5 if args.mode == "log" else 4) * K, "clocks": clocks, "roofline": roof, "finite": same,
+        "gpu_launches": (3 if streaming else (5 if args.mode == "log" else 4)) * K, "clocks": clocks, "roofline": roof, "finite": same,
     }
     if not args.no_cpu_baseline and world == 1 and args.config == 3:
         cb = cpu_oracle(c, members=B, steps=10, warmup=1)
