@@ -151,6 +151,9 @@ def main():
     ap.add_argument("--mode", default="log", choices=["log", "linear"])
     ap.add_argument("--project", action="store_true", help="time the projected operator (App. C) instead of the raw one")
     ap.add_argument("--batch", type=int, default=None, help="members per GPU (default: 64 for cfg3, 8 for cfg4)")
+    ap.add_argument("--flush", default="write+read", choices=["write", "write+read"],
+                    help="L2 flush before every timed step: a 256 MiB write, optionally followed by a 256 MiB read that "
+                         "leaves L2 holding clean lines (default)")
     ap.add_argument("--storage", default="tiled", choices=["tiled", "rows"],
                     help="rows = the exact streaming kernel alone (one exp per entry and member): FP64-ALU roofline")
     ap.add_argument("--statistics", default="classical", choices=["classical", "bose", "fermi"],
@@ -198,13 +201,22 @@ def main():
     C = torch.empty_like(f)
     flags = kx.PROJECT if args.project else 0
     flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)    # 256 MiB > 126 MB L2
+    flush_rd = torch.zeros(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)
+    flush_sink = torch.zeros(1, dtype=torch.float64, device=dev)
+
+    def flush_l2():
+        """Write 256 MiB (evicts everything), then read another 256 MiB so that L2 is left holding CLEAN lines: the
+        write-back of the flusher's own dirty lines would otherwise be charged to the kernels that follow."""
+        flush.zero_()
+        if args.flush == "write+read":
+            flush_sink.copy_(flush_rd.sum(dim=0, keepdim=True))
     stream = torch.cuda.current_stream()
 
     def step():
         h.collide(f, flags=flags, out=C)
 
     for _ in range(Wm):
-        flush.zero_()
+        flush_l2()
         step()
     barrier()
 
@@ -215,7 +227,7 @@ def main():
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     barrier()
     for k in range(K):
-        flush.zero_()
+        flush_l2()
         ev[k][0].record(stream)
         step()
         ev[k][1].record(stream)
@@ -317,7 +329,7 @@ def main():
         "ms_per_step": t_cold / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config], "N": Ngrid, "B_per_gpu": B, "mode": args.mode, "statistics": args.statistics, "projected": bool(args.project),
-                   "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "storage": "rows (streaming)" if streaming else "tiled", "loss_nodes": Q, "l2": "flushed before every timed step (256 MiB write)",
+                   "nnz": nnz, "tensor_bytes": info["tensor_bytes"], "storage": "rows (streaming)" if streaming else "tiled", "loss_nodes": Q, "l2": "flushed before every timed step (256 MiB write" + (", then a 256 MiB read so that no dirty lines are left)" if args.flush == "write+read" else ")"),
                    "parallelism": f"independent batches x{world}" if world > 1 else "single GPU"},
         "value_l2_warm": world * B * K / t_warm, "ms_per_step_l2_warm": t_warm / K * 1e3,
         "calls_per_s": world * K / t_cold,
