@@ -7,6 +7,8 @@ from __future__ import annotations
 
 import ctypes as C
 import os
+import subprocess
+import warnings
 
 import numpy as np
 
@@ -82,6 +84,12 @@ def _load():
         return _lib
     if not os.path.exists(_build.LIB):
         _build.build()
+    elif _build.needs_build():       # a source is newer than the library: never run a stale build silently
+        try:
+            _build.build()
+        except (OSError, subprocess.CalledProcessError) as e:
+            warnings.warn(f"libkx.so is older than its sources and could not be rebuilt ({e}); loading it as it is",
+                          RuntimeWarning)
     lib = C.CDLL(_build.LIB)
     vp, i32, u32, i64p = C.c_void_p, C.c_int32, C.c_uint32, C.POINTER(C.c_int64)
     lib.kx_build.argtypes = [C.POINTER(_Grid), C.POINTER(_Species), C.POINTER(_Msq), C.POINTER(_Opts),
