@@ -156,6 +156,37 @@ typedef struct {
 kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
                       const kx_evolve_t* ctl, void* stream);
 
+/* Adaptive Heun integration in u = ln a (Sec. 4.2; settings of PAPER.md:474), static kinematic mass:
+ *     df/du = kappa_b R(u) C[f] + sum_s amp_s G_s,   R(u) = rate0 exp(rate_slope (u - u0))        (eq. 4.9)
+ * Every attempted step is an Euler predictor f_P = f + du k1 and the Heun corrector f_H = f + du (k1 + k2)/2 (two
+ * operator evaluations); err = max_{b,i} |f_H - f_P| / (atol + rtol max(|f|, |f_H|)) over the whole batch; the step is
+ * accepted iff err <= 1, and du <- du clamp(safety / sqrt(err), 0.2, 5), du <= u1 - u (reading D15).
+ * Error norm, accept/reject and the step-size update run on the device; the host only enqueues attempts (in chunks of
+ * 8, reading the controller state between chunks) until u reaches u1 or max_steps attempts were made. */
+typedef struct {
+    double u0, u1;         /* integration interval, u1 > u0 */
+    double du0;            /* first step (1e-4) */
+    double rtol, atol;     /* 1e-2 and 2e-8 */
+    double safety;         /* 0.9 */
+    double rate0, rate_slope;
+    const double* kappa;   /* HOST [B] per-member coupling multiplier; NULL => 1 */
+    const double* amp;     /* HOST [src->nsrc] constant source rates per unit u (src->amp is not used); NULL => no sources */
+    int32_t max_steps;     /* attempted steps at most (> 0) */
+    uint32_t flags;        /* KX_PROJECT */
+} kx_adaptive_t;
+
+typedef struct {
+    double u, du;          /* where the integration stopped, the step it would take next */
+    int64_t accepted, rejected;
+    int32_t done;          /* 1 iff u reached u1 */
+} kx_adaptive_result_t;
+
+/* f: DEVICE [B,N] in/out; src: only nsrc and G are read (may be NULL); result: HOST (may be NULL).  Synchronises.
+ * KX_ERR_NONFINITE if f left the finite range; KX_ERR_UNSUPPORTED on a handle whose mass was changed is not raised:
+ * the current tensor is used throughout. */
+kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
+                               const kx_adaptive_t* ctl, kx_adaptive_result_t* result, void* stream);
+
 /* Number of stored (i, n<=m) entries, bytes of tensor data one kx_collide streams (the tiled operand when
  * it is in use, else 20 bytes per entry), grid size.
  * Synchronises the device.  Any output pointer may be NULL. */

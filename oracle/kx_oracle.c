@@ -459,6 +459,59 @@ int okx_evolve_q(int eta, int N, int B, const double *p, const double *dp, doubl
                            mass, kappa, project, nsrc, G, amp, diag);
 }
 
+/* ---- Adaptive Heun in u = ln a (Sec. 4.2: "first computes an Euler predictor and then corrects it
+ * using the average of the slopes at the beginning and end of the step. The difference between the predictor and
+ * corrected value provides a local error estimate used to adjust the step size"; settings rtol, atol, du0, safety of
+ * PAPER.md:474).  df/du = kappa_b R(u) C[f] + sum_s amp_s G_s, R(u) = rate0 exp(slope (u - u0)), static mass.
+ * Controller (the paper does not print it; reading D15): err = max_{b,i} |f_H - f_P| / (atol + rtol
+ * max(|f|, |f_H|)) over the whole batch; accept iff err <= 1; du <- du clamp(safety / sqrt(max(err, 1e-10)), 0.2, 5);
+ * du <= u1 - u; stop when u1 - u <= 1e-14 max(|u1|, 1).  out = {u, du, accepted, rejected, done}. */
+int okx_evolve_adaptive(int eta, int N, int B, const double *p, const double *dp, double m, double g_chi,
+                        double M2_0, double m_med, double f_floor, double eps_supp, double *f,
+                        double u0, double u1, double du0, double rtol, double atol, double safety,
+                        double rate0, double slope, const double *kappa, int project,
+                        int nsrc, const double *G, const double *amp, int max_steps, double *out)
+{
+    size_t N3 = (size_t)N * N * N;
+    okx_ctx c = { N, p, dp, m, g_chi, M2_0, m_med, 0, f_floor, eps_supp,
+                  malloc(sizeof(double) * N3), malloc(sizeof(int32_t) * N3), malloc(sizeof(double) * N3),
+                  malloc(sizeof(double) * N), malloc(sizeof(double) * N), malloc(sizeof(double) * N), m };
+    c.eta = eta;
+    okx_build(N, p, dp, m, g_chi, M2_0, m_med, c.W, c.jL, c.wR);
+    okx_kinematics(N, p, dp, m, c.E, c.K, c.h);
+    double *k1 = malloc(sizeof(double) * N), *k2 = malloc(sizeof(double) * N);
+    double *fP = malloc(sizeof(double) * N), *fH = malloc(sizeof(double) * (size_t)B * N);
+    double u = u0, du = du0 < u1 - u0 ? du0 : u1 - u0;
+    long acc = 0, rej = 0;
+    int done = 0;
+    for (int step = 0; step < max_steps && !done; ++step) {
+        double err = 0.0;
+        for (int b = 0; b < B; ++b) {
+            double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+            okx_rhs(&c, fb, m, 0, kb * rate0 * exp(slope * (u - u0)), project, nsrc, G, amp, k1, NULL);
+            for (int i = 0; i < N; ++i) fP[i] = fb[i] + du * k1[i];                        /* Euler predictor */
+            okx_rhs(&c, fP, m, 0, kb * rate0 * exp(slope * (u + du - u0)), project, nsrc, G, amp, k2, NULL);
+            for (int i = 0; i < N; ++i) {
+                double fh = fb[i] + 0.5 * du * (k1[i] + k2[i]);                             /* Heun corrector */
+                fH[(size_t)b * N + i] = fh;
+                double e = fabs(fh - fP[i]) / (atol + rtol * fmax(fabs(fb[i]), fabs(fh)));
+                if (!(e <= err)) err = isfinite(e) ? e : INFINITY;
+            }
+        }
+        int ok = err <= 1.0;
+        double fac = safety / sqrt(fmax(err, 1e-10));
+        if (!(fac == fac)) fac = 0.2;
+        fac = fmin(fmax(fac, 0.2), 5.0);
+        if (ok) { memcpy(f, fH, sizeof(double) * (size_t)B * N); u += du; ++acc; } else ++rej;
+        du *= fac;
+        if (u1 - u <= 1e-14 * fmax(fabs(u1), 1.0)) { done = 1; u = u1; }
+        else if (du > u1 - u) du = u1 - u;
+    }
+    out[0] = u; out[1] = du; out[2] = (double)acc; out[3] = (double)rej; out[4] = (double)done;
+    free(c.W); free(c.jL); free(c.wR); free(c.E); free(c.K); free(c.h); free(k1); free(k2); free(fP); free(fH);
+    return 0;
+}
+
 /* ---- Pin helper (P9), NOT on the evaluate path: the reduced kernel F(p_i,p_n,p_m) by the
  * mu-quadrature of eq. B.5-B.12, nodes/weights supplied by the caller.
  * If m_med > 0 the integrand carries |M|^2(t(mu)), t = 2m^2-2E_iE_n+2p_ip_n mu (reading D5). */

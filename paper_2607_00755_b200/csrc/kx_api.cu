@@ -266,6 +266,7 @@ void kx_destroy(kx_handle_t h)
         cudaFree(h->dev_blob);
         cudaFree(h->tiled_blob);
         cudaFree(h->t.AL);
+        cudaFree(h->adapt);
         for (auto& ev : h->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     }
     delete h;
@@ -578,6 +579,79 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
     KX_CUDA(cudaMemcpyAsync(&flag, h->flag, 4, cudaMemcpyDeviceToHost, s));
     KX_CUDA(cudaStreamSynchronize(s));
     if (flag) { h->err = "kx_evolve: f became non-finite"; return KX_ERR_NONFINITE; }
+    return KX_OK;
+}
+
+kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
+                               const kx_adaptive_t* ctl, kx_adaptive_result_t* result, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    kx_status_t rc = check_batch(h, f, B);
+    if (rc != KX_OK) return rc;
+    if (!ctl || !(ctl->u1 > ctl->u0) || !(ctl->du0 > 0.0) || !(ctl->rtol >= 0.0) || !(ctl->atol >= 0.0) ||
+        !(ctl->rtol + ctl->atol > 0.0) || !(ctl->safety > 0.0 && ctl->safety <= 1.0) || ctl->max_steps < 1 ||
+        !isfinite(ctl->rate0) || !isfinite(ctl->rate_slope)) {
+        h->err = "kx_evolve_adaptive: need u1 > u0, du0 > 0, rtol, atol >= 0 (not both 0), 0 < safety <= 1, max_steps >= 1";
+        return KX_ERR_INVALID_ARG;
+    }
+    const int nsrc = (src && ctl->amp) ? src->nsrc : 0;
+    if (nsrc < 0 || nsrc > KX_MAX_SRC || (nsrc > 0 && !src->G)) { h->err = "bad source description"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const int N = h->d.N;
+    if ((rc = ensure_ws(h, B)) != KX_OK) return rc;
+    if (!h->adapt) KX_CUDA(cudaMalloc((void**)&h->adapt, sizeof(KxAdapt)));
+    double* kappa_d = nullptr;
+    if (ctl->kappa) {
+        kappa_d = h->Cbuf + (size_t)h->wsB * N;
+        KX_CUDA(cudaMemcpyAsync(kappa_d, ctl->kappa, (size_t)B * 8, cudaMemcpyHostToDevice, s));
+    }
+    KxAdapt init = {};
+    init.u = ctl->u0;
+    init.du = ctl->du0 < ctl->u1 - ctl->u0 ? ctl->du0 : ctl->u1 - ctl->u0;
+    init.errkey = 0;                 // key of +0.0
+    KX_CUDA(cudaMemcpyAsync(h->adapt, &init, sizeof init, cudaMemcpyHostToDevice, s));
+    KX_CUDA(cudaMemsetAsync(h->flag, 0, 4, s));
+    const bool use_tiled = h->storage == KX_STORE_TILED;
+    if (use_tiled && (rc = ensure_tiled(h, s)) != KX_OK) return rc;
+    if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
+
+    KxAdapt state = init;
+    int attempts = 0;
+    while (attempts < ctl->max_steps && !state.done) {
+        const int chunk = ctl->max_steps - attempts < 8 ? ctl->max_steps - attempts : 8;
+        for (int a = 0; a < chunk; ++a) {
+            for (int stg = 0; stg < 2; ++stg) {
+                const double* fin = stg == 0 ? f : h->fstage;
+                KxStage st = {};
+                if ((rc = launch_eval(h, fin, B, /*have_yd=*/stg == 1 && !use_tiled, use_tiled, &st, s)) != KX_OK) return rc;
+                st.flags = ctl->flags & KX_PROJECT;
+                st.diag_stride = 6;
+                st.evolve = 1; st.rk_method = KX_HEUN_ADAPT; st.rk_stage = stg;
+                st.kappa = kappa_d;
+                st.nsrc = nsrc; st.G = nsrc ? src->G : nullptr;
+                for (int q = 0; q < nsrc; ++q) st.amp[q] = ctl->amp[q];
+                st.f = f; st.fstage = h->fstage; st.k1 = h->k1; st.k2 = h->k2; st.k3 = h->k3;
+                st.ydnext = (!use_tiled && stg == 0) ? h->yd : nullptr;
+                st.flag = h->flag;
+                st.ad = h->adapt; st.ad_u0 = ctl->u0; st.ad_rate0 = ctl->rate0; st.ad_slope = ctl->rate_slope;
+                st.ad_rtol = ctl->rtol; st.ad_atol = ctl->atol;
+                KX_CUDA(kx_launch_finish(h->d, fin, h->part, B, st, s));
+            }
+            KX_CUDA(kx_launch_adapt_step(h->d, f, h->k2, B, h->adapt, ctl->u1, ctl->safety, h->flag, s));
+        }
+        attempts += chunk;
+        KX_CUDA(cudaMemcpyAsync(&state, h->adapt, sizeof state, cudaMemcpyDeviceToHost, s));
+        KX_CUDA(cudaStreamSynchronize(s));
+    }
+    int flag = 0;
+    KX_CUDA(cudaMemcpyAsync(&flag, h->flag, 4, cudaMemcpyDeviceToHost, s));
+    KX_CUDA(cudaStreamSynchronize(s));
+    if (result) {
+        result->u = state.u; result->du = state.du;
+        result->accepted = state.accepted; result->rejected = state.rejected; result->done = state.done;
+    }
+    if (flag) { h->err = "kx_evolve_adaptive: f became non-finite"; return KX_ERR_NONFINITE; }
     return KX_OK;
 }
 

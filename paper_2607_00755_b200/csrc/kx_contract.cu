@@ -369,9 +369,15 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
     if (!st.evolve) return;
 
     // ---- a8: k = kappa_b R C + sum_s amp_s G_s, then the Runge-Kutta bookkeeping of this stage
-    const double kR = (st.kappa ? st.kappa[b] : 1.0) * st.rate;
-    const double dt = st.dt;
+    double rate = st.rate, dt = st.dt;
+    if (st.rk_method == KX_HEUN_ADAPT) {      // step and rate from the device controller (kx_evolve_adaptive)
+        const double u = st.ad->u;
+        dt = st.ad->du;
+        rate = st.ad_rate0 * exp(st.ad_slope * ((st.rk_stage == 0 ? u : u + dt) - st.ad_u0));
+    }
+    const double kR = (st.kappa ? st.kappa[b] : 1.0) * rate;
     bool bad = false;
+    double errmax = 0.0;
 #pragma unroll
     for (int q = 0; q < kMaxPerThread; ++q) {
         const int i = tid + q * KX_CTA;
@@ -388,6 +394,14 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
         } else if (st.rk_method == KX_HEUN) {
             if (st.rk_stage == 0) { st.k1[o] = k; next = f0 + dt * k; st.fstage[o] = next; }
             else { next = f0 + 0.5 * dt * (st.k1[o] + k); st.f[o] = next; }
+        } else if (st.rk_method == KX_HEUN_ADAPT) {
+            if (st.rk_stage == 0) { st.k1[o] = k; next = f0 + dt * k; st.fstage[o] = next; }      // Euler predictor
+            else {                                                                                  // Heun corrector, kept aside
+                next = f0 + 0.5 * dt * (st.k1[o] + k);
+                st.k2[o] = next;
+                const double e = fabs(next - st.fstage[o]) / (st.ad_atol + st.ad_rtol * fmax(fabs(f0), fabs(next)));
+                errmax = isfinite(e) ? fmax(errmax, e) : INFINITY;
+            }
         } else {
             if (st.rk_stage == 0) { st.k1[o] = k; next = f0 + 0.5 * dt * k; st.fstage[o] = next; }
             else if (st.rk_stage == 1) { st.k2[o] = k; next = f0 + 0.5 * dt * k; st.fstage[o] = next; }
@@ -397,7 +411,11 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
         if (!isfinite(next)) bad = true;
         s_y[i] = kx_yval(next, d.interp, d.f_floor, d.eta);
     }
-    if (bad) atomicOr(st.flag, 1);
+    if (bad && st.rk_method != KX_HEUN_ADAPT) atomicOr(st.flag, 1);      // a rejected attempt may overflow harmlessly
+    if (st.rk_method == KX_HEUN_ADAPT && st.rk_stage == 1) {
+        const double e = block_max(errmax, s_red);                         // order independent: deterministic
+        if (tid == 0) atomicMax(&st.ad->errkey, kx_dkey(e));
+    }
     __syncthreads();
     if (st.ydnext) {
         double2* ydn = reinterpret_cast<double2*>(st.ydnext) + (size_t)b * N;
@@ -406,6 +424,43 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
             ydn[i] = make_double2(y0, y1 - y0);
         }
     }
+}
+
+// ---------------------------------------------------------------- adaptive Heun: accept / reject, controller update
+// k_adapt_accept: one CTA per member; every CTA reads the same error norm and takes the same decision.
+__global__ void __launch_bounds__(KX_CTA) k_adapt_accept(int N, double* __restrict__ f, const double* __restrict__ fnew,
+                                                         const KxAdapt* __restrict__ ad, int* __restrict__ flag)
+{
+    if (ad->done) return;
+    const long long k = ad->errkey;
+    const double err = __longlong_as_double(k >= 0 ? k : (k ^ 0x7fffffffffffffffLL));
+    if (!(err <= 1.0)) return;                                   // rejected (also when err is inf / nan)
+    bool bad = false;
+    for (int i = threadIdx.x; i < N; i += KX_CTA) {
+        const double v = fnew[(size_t)blockIdx.x * N + i];
+        f[(size_t)blockIdx.x * N + i] = v;
+        if (!isfinite(v)) bad = true;
+    }
+    if (bad) atomicOr(flag, 1);
+}
+
+// k_adapt_ctrl: one thread.  du <- du clamp(safety / sqrt(err), 0.2, 5); accepted: u <- u + du_old, du <= u1 - u.
+__global__ void k_adapt_ctrl(KxAdapt* ad, double u1, double safety)
+{
+    if (ad->done) return;
+    const long long k = ad->errkey;
+    const double err = __longlong_as_double(k >= 0 ? k : (k ^ 0x7fffffffffffffffLL));
+    const bool ok = err <= 1.0;
+    double fac = safety / sqrt(fmax(err, 1e-10));
+    if (!(fac == fac)) fac = 0.2;                                // nan error: shrink
+    fac = fmin(fmax(fac, 0.2), 5.0);
+    double u = ad->u, du = ad->du;
+    if (ok) { u += du; ad->accepted += 1; } else { ad->rejected += 1; }
+    du *= fac;
+    if (u1 - u <= 1e-14 * fmax(fabs(u1), 1.0)) { ad->done = 1; u = u1; }
+    else if (du > u1 - u) du = u1 - u;
+    ad->u = u; ad->du = du;
+    ad->errkey = kx_dkey(0.0);
 }
 
 // ---------------------------------------------------------------- a9: moments, eq. B.2
@@ -513,6 +568,14 @@ cudaError_t kx_launch_finish(const KxDev& d, const double* fin, const double* pa
         if (e != cudaSuccess) return e;
     }
     return kx_launch(k_finish, dim3(B), dim3(KX_CTA), 0, s, true, d, fin, part, B, st);
+}
+
+cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, int B, KxAdapt* ad, double u1, double safety,
+                                 int* flag, cudaStream_t s)
+{
+    k_adapt_accept<<<B, KX_CTA, 0, s>>>(d.N, f, fnew, ad, flag);
+    k_adapt_ctrl<<<1, 1, 0, s>>>(ad, u1, safety);
+    return cudaGetLastError();
 }
 
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,

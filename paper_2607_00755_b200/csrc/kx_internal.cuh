@@ -83,6 +83,7 @@ struct KxTiled {
     double flag_log2;         // log2(2 / Q!) ... see kx_tiled.cu k_xt
 };
 
+struct KxAdapt;
 struct kx_handle_s {
     KxDev d;
     int device;
@@ -113,6 +114,7 @@ struct kx_handle_s {
     double *fstage, *k1, *k2, *k3, *Cbuf;   // [wsB, N] evolve buffers
     double *hostio;           // [wsB, N] x2 staging for kx_collide_host
     int *flag;                // device non-finite flag
+    KxAdapt *adapt;           // device controller state of kx_evolve_adaptive
     void *dev_blob;           // one allocation holding the [N]-sized arrays
     bool profiling;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;
@@ -205,6 +207,14 @@ cudaError_t kx_launch_fill(const KxDev& d, cudaStream_t s);      // W, omega, nm
 cudaError_t kx_launch_tasks(const KxDev& d, int chunk, cudaStream_t s);
 
 // ---- launchers implemented in kx_contract.cu
+// controller state of kx_evolve_adaptive, on the device
+struct KxAdapt {
+    double u, du;
+    long long errkey;        // ordered key (kx_dkey) of the largest scaled error of the attempt, atomicMax over the CTAs
+    long long accepted, rejected;
+    int done;
+};
+
 struct KxStage {             // what the finishing kernel does after the reduction
     unsigned flags;          // KX_PROJECT
     double *C, *gain, *loss, *diag;       // outputs of kx_collide_ex (any may be null); diag stride 4
@@ -229,12 +239,18 @@ struct KxStage {             // what the finishing kernel does after the reducti
     int NT, LC, RS, GW, GL, xstride;      // GW = gain workers (warps), GL = loss workers (CTAs)
     int *flag;
     int evolve;
+    // adaptive Heun (rk_method == KX_HEUN_ADAPT): dt and the rate come from the device controller state
+    KxAdapt *ad;
+    double ad_u0, ad_rate0, ad_slope, ad_rtol, ad_atol;
 };
+#define KX_HEUN_ADAPT 3      // internal: Euler predictor / Heun corrector with the error norm of kx_evolve_adaptive
 cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, cudaStream_t s);
 cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
                                double* part, int B, const long long* mstat, bool pdl, cudaStream_t s);
 cudaError_t kx_launch_finish(const KxDev& d, const double* f, const double* part, int B,
                              const KxStage& st, cudaStream_t s);
+cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, int B, KxAdapt* ad, double u1, double safety,
+                                 int* flag, cudaStream_t s);      // accept/reject + controller update
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
                               double* p1, double* p2, int stride, cudaStream_t s);
 // ---- tiled path (kx_tiled_build.cu, kx_tiled.cu)

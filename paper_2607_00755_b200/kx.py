@@ -61,9 +61,20 @@ class _Evolve(C.Structure):
                 ("kappa", _dp), ("flags", C.c_uint32), ("diag", C.c_void_p)]
 
 
+class _Adaptive(C.Structure):
+    _fields_ = [("u0", C.c_double), ("u1", C.c_double), ("du0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double),
+                ("safety", C.c_double), ("rate0", C.c_double), ("rate_slope", C.c_double), ("kappa", _dp), ("amp", _dp),
+                ("max_steps", C.c_int32), ("flags", C.c_uint32)]
+
+
+class _AdaptiveResult(C.Structure):
+    _fields_ = [("u", C.c_double), ("du", C.c_double), ("accepted", C.c_int64), ("rejected", C.c_int64),
+                ("done", C.c_int32)]
+
+
 # every symbol include/kx.h declares
 SYMBOLS = ["kx_build", "kx_set_mass", "kx_collide", "kx_collide_parts", "kx_collide_ex",
-           "kx_collide_host", "kx_moments", "kx_evolve", "kx_info", "kx_tensor_export",
+           "kx_collide_host", "kx_moments", "kx_evolve", "kx_evolve_adaptive", "kx_info", "kx_tensor_export",
            "kx_kinematics_export", "kx_profile", "kx_profile_read", "kx_probe_flops", "kx_last_error", "kx_destroy", "kx_version"]
 
 _lib = None
@@ -101,6 +112,8 @@ def _load():
     lib.kx_collide_host.argtypes = [vp, vp, vp, i32, u32, vp]
     lib.kx_moments.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp]
     lib.kx_evolve.argtypes = [vp, vp, i32, C.POINTER(_Source), C.POINTER(_Evolve), vp]
+    lib.kx_evolve_adaptive.argtypes = [vp, vp, i32, C.POINTER(_Source), C.POINTER(_Adaptive),
+                                       C.POINTER(_AdaptiveResult), vp]
     lib.kx_info.argtypes = [vp, i64p, i64p, C.POINTER(i32)]
     lib.kx_tensor_export.argtypes = [vp, C.c_int64, i64p, _dp, _dp, C.POINTER(C.c_uint32)]
     lib.kx_kinematics_export.argtypes = [vp, _dp, _dp, _dp]
@@ -275,6 +288,31 @@ class Handle:
         self._check(self._lib.kx_evolve(self._h, _dev(f), B, C.byref(src) if src is not None else None,
                                         C.byref(ctl), _stream(stream)))
         return diag
+
+    def evolve_adaptive(self, f, u0, u1, *, du0=1e-4, rtol=1e-2, atol=2e-8, safety=0.9, rate0=1.0, rate_slope=0.0,
+                        kappa=None, project=True, G=None, amp=None, max_steps=100000, stream=None):
+        """kx_evolve_adaptive: adaptive Heun in u (Sec. 4.2); f [B,N] in place; returns dict(u, du, accepted,
+        rejected, done)."""
+        B = self._batch(f)
+        kappa = None if kappa is None else _f64(kappa)
+        if kappa is not None and kappa.size != B:
+            raise ValueError("kappa must have B entries")
+        src = None
+        if G is not None and amp is not None:
+            if G.dim() != 2 or G.shape[1] != self.N:
+                raise ValueError("G must be [nsrc, N]")
+            amp = _f64(amp)
+            if amp.shape != (G.shape[0],):
+                raise ValueError("amp must be [nsrc]")
+            src = _Source(int(G.shape[0]), _dev(G), None)
+        else:
+            amp = None
+        ctl = _Adaptive(float(u0), float(u1), float(du0), float(rtol), float(atol), float(safety), float(rate0),
+                        float(rate_slope), _ptr(kappa), _ptr(amp), int(max_steps), PROJECT if project else 0)
+        res = _AdaptiveResult()
+        self._check(self._lib.kx_evolve_adaptive(self._h, _dev(f), B, C.byref(src) if src is not None else None,
+                                                 C.byref(ctl), C.byref(res), _stream(stream)))
+        return dict(u=res.u, du=res.du, accepted=int(res.accepted), rejected=int(res.rejected), done=bool(res.done))
 
     def profile(self, enable=True):
         self._check(self._lib.kx_profile(self._h, int(bool(enable))))

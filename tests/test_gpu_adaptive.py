@@ -1,0 +1,92 @@
+"""kx_evolve_adaptive (adaptive Heun of Sec. 4.2) against the oracle's integrator: the same
+accepted / rejected counts, the same final u and f, on the tensor-core path, the streaming path and with Bose statistics."""
+import numpy as np
+import pytest
+
+import kx_inputs as kin
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    return torch
+
+
+def _dev(torch, a):
+    return torch.tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda")
+
+
+def _nu(oracle, T, f):
+    g, l, C = oracle.collide(T, f, oracle.LOG)
+    return float((l / np.where(f > 0, f, 1.0)).max())
+
+
+@pytest.mark.parametrize("storage", ["tiled", "rows"])
+def test_adaptive_parity_cfg1(torch_cuda, oracle, storage):
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    nu = _nu(oracle, T, c["f"])
+    kw = dict(u0=0.0, u1=6.0 / nu, du0=2.0 / nu, rtol=1e-3, atol=1e-12)
+    f_ref, info_ref = oracle.evolve_adaptive(c["p"], c["dp"], c["f"], **kw)
+    assert info_ref["rejected"] >= 1          # the first step is too long: the reject path is exercised
+    h = kx.Handle(c["p"], c["dp"], c["m"], storage=kx.STORE_TILED if storage == "tiled" else kx.STORE_SYM_ROWS)
+    f = _dev(torch, c["f"])
+    info = h.evolve_adaptive(f, **kw)
+    assert (info["accepted"], info["rejected"], info["done"]) == (info_ref["accepted"], info_ref["rejected"], True)
+    assert abs(info["u"] - info_ref["u"]) <= 1e-12 * abs(info_ref["u"])
+    assert abs(info["du"] - info_ref["du"]) <= 1e-8 * abs(info_ref["du"])
+    assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-10 * np.abs(f_ref).max()
+    h.close()
+
+
+def test_adaptive_batch_sources_rate_kappa(torch_cuda, oracle):
+    """A batch with per-member couplings, two sources and an exponential rate; one common step for all members."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    B = 5
+    c = kin.config(3, N=64, B=B)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    nu = _nu(oracle, T, c["f"])
+    G = np.stack([np.exp(-0.5 * (c["p"] - 3.0) ** 2), np.exp(-0.5 * ((c["p"] - 8.0) / 2.0) ** 2)])
+    amp = np.array([0.02, 0.01]) * nu
+    kappa = np.array([0.0, 0.3, 1.0, 2.0, 0.1])
+    kw = dict(u0=0.5, u1=0.5 + 3.0 / nu, du0=0.05 / nu, rtol=1e-2, atol=2e-8, rate0=1.0, rate_slope=0.2 * nu)
+    f_ref, info_ref = oracle.evolve_adaptive(c["p"], c["dp"], c["f"], m=c["m"], M2_0=c["M2_0"], m_med=c["m_med"],
+                                             kappa=kappa, G=G, amp=amp, **kw)
+    h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    f = _dev(torch, c["f"])
+    info = h.evolve_adaptive(f, kappa=kappa, G=_dev(torch, G), amp=amp, **kw)
+    assert (info["accepted"], info["rejected"], info["done"]) == (info_ref["accepted"], info_ref["rejected"], True)
+    assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-10 * np.abs(f_ref).max()
+    h.close()
+
+
+def test_adaptive_bose_and_step_budget(torch_cuda, oracle):
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(1)
+    f0 = c["f"] / np.abs(c["f"]).max() * 2.0
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    g, l, C = oracle.collide_q(T, f0, 1)
+    nu = float((l[0] / f0[0]).max())
+    kw = dict(u0=0.0, u1=4.0 / nu, du0=0.05 / nu, rtol=1e-3, atol=1e-12)
+    f_ref, info_ref = oracle.evolve_adaptive(c["p"], c["dp"], f0, eta=1, **kw)
+    h = kx.Handle(c["p"], c["dp"], c["m"], statistics=kx.STAT_BOSE)
+    f = _dev(torch, f0)
+    info = h.evolve_adaptive(f, **kw)
+    assert (info["accepted"], info["rejected"]) == (info_ref["accepted"], info_ref["rejected"])
+    assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-10 * np.abs(f_ref).max()
+    # a step budget that is too small stops early, says so, and leaves a state the oracle reproduces
+    f = _dev(torch, f0)
+    info = h.evolve_adaptive(f, max_steps=5, **kw)
+    f_ref5, info_ref5 = oracle.evolve_adaptive(c["p"], c["dp"], f0, eta=1, max_steps=5, **kw)
+    assert not info["done"] and info["accepted"] + info["rejected"] == 5
+    assert abs(info["u"] - info_ref5["u"]) <= 1e-12 * abs(info_ref5["u"])
+    assert np.abs(f.cpu().numpy() - f_ref5).max() <= 1e-11 * np.abs(f_ref5).max()
+    h.close()

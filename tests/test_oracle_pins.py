@@ -418,3 +418,44 @@ def test_Q3_quantum_conservation_and_H_theorem_on_exact_grid(oracle, eta):
     # eta enters: Bose enhancement and Pauli blocking move the operator in opposite directions from the classical one
     g0, l0, C0 = oracle.collide(T, f, oracle.LOG)
     assert np.abs(C[0] - C0[0]).max() > 1e-3 * np.abs(g0).max()
+
+
+# ------------------------------------------------------------------ adaptive Heun
+def test_A1_adaptive_heun_converges_to_rk4(oracle):
+    """The adaptive Heun solution approaches a fine fixed-step RK4 solution as rtol -> 0, the error scales with the
+    tolerance (second-order local estimate) and tighter tolerances take more steps; a first step far too large is rejected."""
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    g, l, C = oracle.collide(T, c["f"], oracle.LOG)
+    nu = float((l[0] / c["f"][0]).max())
+    u1 = 20.0 / nu
+    ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.RK4, tau=np.linspace(0.0, u1, 2001))
+    errs, steps = [], []
+    for rtol in (1e-3, 1e-4, 1e-5):
+        f, info = oracle.evolve_adaptive(c["p"], c["dp"], c["f"], u0=0.0, u1=u1, du0=0.01 / nu, rtol=rtol, atol=1e-3 * rtol * 1e-6)
+        assert info["done"] and abs(info["u"] - u1) <= 1e-12 * u1
+        errs.append(np.abs(f - ref).max() / np.abs(ref).max())
+        steps.append(info["accepted"])
+    assert errs[0] < 1e-3 and errs[2] < 1e-5
+    assert 3.0 < errs[0] / errs[1] < 30.0 and 3.0 < errs[1] / errs[2] < 30.0
+    assert steps[0] < steps[1] < steps[2]
+    f, info = oracle.evolve_adaptive(c["p"], c["dp"], c["f"], u0=0.0, u1=u1, du0=5.0 / nu, rtol=1e-3, atol=1e-12)
+    assert info["rejected"] >= 2 and info["done"]
+    # number and energy are conserved along the way (projected operator)
+    m0, m1 = oracle.moments(T, c["f"]), oracle.moments(T, f)
+    assert np.allclose(m0[:, :2], m1[:, :2], rtol=1e-11, atol=0)
+
+
+def test_A2_adaptive_heun_sources_only_closed_form(oracle):
+    """kappa = 0: df/du = sum_s amp_s G_s is constant, Heun is exact, the error estimate is 0, every step is accepted and
+    grows by the maximal factor 5: n steps with du0 (5^n - 1)/4 >= u1 - u0, and f = f0 + (u1-u0) sum amp G exactly."""
+    c = kin.config(1)
+    N = c["p"].size
+    G = np.stack([np.exp(-0.5 * (c["p"] - 3.0) ** 2), np.exp(-0.5 * ((c["p"] - 6.0) / 2.0) ** 2)])
+    amp = np.array([0.3, 0.05])
+    u0, u1, du0 = 1.0, 4.0, 1e-4
+    f, info = oracle.evolve_adaptive(c["p"], c["dp"], c["f"], u0=u0, u1=u1, du0=du0, kappa=np.zeros(1), G=G, amp=amp)
+    n = int(np.ceil(np.log(4.0 * (u1 - u0) / du0 + 1.0) / np.log(5.0)))
+    assert info["accepted"] == n and info["rejected"] == 0 and info["done"]
+    want = c["f"] + (u1 - u0) * (amp[:, None] * G).sum(axis=0)[None, :]
+    assert np.abs(f - want).max() <= 1e-13 * np.abs(want).max()
