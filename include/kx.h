@@ -156,6 +156,14 @@ typedef struct {
 kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
                       const kx_evolve_t* ctl, void* stream);
 
+/* Monoenergetic source (eq. 3.7): deposition of delta(p - p0) on the grid for the handle's current mass
+ * (PAPER.md:171).  With p_L <= p0 <= p_R the neighbouring grid points and the energy-linear fractions
+ * alpha_R = (E_0 - E_L)/(E_R - E_L), alpha_L = 1 - alpha_R, the shape G_L = alpha_L / h_L, G_R = alpha_R / h_R (0 elsewhere)
+ * has sum_i h_i G_i = 1 and sum_i h_i E_i G_i = E_0 exactly: used as a row of kx_source_t.G with amp = (2 pi^2/g_chi) x
+ * (injected number per unit tau), it reproduces the injected number and energy rates of eq. B.2 exactly.
+ * G: DEVICE [N].  KX_ERR_INVALID_ARG unless p[0] <= p0 <= p[N-1].  Asynchronous. */
+kx_status_t kx_delta_source(kx_handle_t h, double p0, double* G, void* stream);
+
 /* Adaptive Heun integration in u = ln a (Sec. 4.2; settings of PAPER.md:474), static kinematic mass:
  *     df/du = kappa_b R(u) C[f] + sum_s amp_s G_s,   R(u) = rate0 exp(rate_slope (u - u0))        (eq. 4.9)
  * Every attempted step is an Euler predictor f_P = f + du k1 and the Heun corrector f_H = f + du (k1 + k2)/2 (two

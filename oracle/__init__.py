@@ -55,6 +55,8 @@ def _load():
         _lib.okx_evolve_adaptive.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp] + [C.c_double] * 6 + [_dp] + \
             [C.c_double] * 8 + [_dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp]
         _lib.okx_evolve_adaptive.restype = C.c_int
+        _lib.okx_delta_source.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_double, _dp]
+        _lib.okx_delta_source.restype = C.c_int
         _lib.okx_collide_rows.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double,
                                           C.c_double, _dp, C.c_int, _ip, C.c_int, C.c_double, _dp, _dp, _dp]
         _lib.okx_collide_rows.restype = None
@@ -213,6 +215,15 @@ def evolve_adaptive(p, dp, f, *, u0, u1, du0=1e-4, rtol=1e-2, atol=2e-8, safety=
                                      _d(kappa), int(bool(project)), nsrc, _d(G), _d(amp), int(max_steps), _d(out))
     assert rc == 0
     return f, dict(u=out[0], du=out[1], accepted=int(out[2]), rejected=int(out[3]), done=bool(out[4]))
+
+
+def delta_source(p, dp, m, p0):
+    """Grid deposition of a monoenergetic source at p0: G [N] with sum h G = 1, sum h E G = E_0."""
+    p, dp = _c(p), _c(dp)
+    G = np.empty(p.size)
+    rc = _load().okx_delta_source(p.size, _d(p), _d(dp), float(m), float(p0), _d(G))
+    assert rc == 0, "p0 outside the grid"
+    return G
 
 
 def F_quadrature(pi, pn, pm, m, M2_0, m_med, mu, wmu):

@@ -459,6 +459,23 @@ int okx_evolve_q(int eta, int N, int B, const double *p, const double *dp, doubl
                            mass, kappa, project, nsrc, G, amp, diag);
 }
 
+/* ---- Monoenergetic source (eq. 3.7) deposited on the grid: "split between the two
+ * neighboring grid points q_L < q_0 < q_R using the energy-linear deposition fractions alpha_R = (E_0 - E_L)/(E_R - E_L)
+ * and alpha_L = 1 - alpha_R ... normalized so that the discrete zeroth and energy moments reproduce exactly the injected
+ * particle-number and energy rates": G_L = alpha_L/h_L, G_R = alpha_R/h_R, so sum h G = 1 and sum h E G = E_0. */
+int okx_delta_source(int N, const double *p, const double *dp, double m, double p0, double *G)
+{
+    if (!(p0 >= p[0] && p0 <= p[N - 1])) return 1;
+    int L = 0;
+    for (int j = 0; j <= N - 2; ++j) if (p[j] <= p0) L = j;        /* largest L <= N-2 with p_L <= p0 */
+    double EL = sqrt(p[L] * p[L] + m * m), ER = sqrt(p[L + 1] * p[L + 1] + m * m), E0 = sqrt(p0 * p0 + m * m);
+    double aR = (E0 - EL) / (ER - EL);
+    for (int i = 0; i < N; ++i) G[i] = 0.0;
+    G[L] = (1.0 - aR) / (p[L] * p[L] * dp[L]);
+    G[L + 1] = aR / (p[L + 1] * p[L + 1] * dp[L + 1]);
+    return 0;
+}
+
 /* ---- Adaptive Heun in u = ln a (Sec. 4.2: "first computes an Euler predictor and then corrects it
  * using the average of the slopes at the beginning and end of the step. The difference between the predictor and
  * corrected value provides a local error estimate used to adjust the step size"; settings rtol, atol, du0, safety of

@@ -326,6 +326,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     kx_handle_s* h = new (std::nothrow) kx_handle_s();
     if (!h) { g_build_err = "out of host memory"; return KX_ERR_ALLOC; }
     h->device = device;
+    h->p_lo = grid->p[0]; h->p_hi = grid->p[N - 1];
     h->sm_count = prop.multiProcessorCount;
     h->nnz_stale = true;
     h->storage = o.storage;
@@ -579,6 +580,15 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
     KX_CUDA(cudaMemcpyAsync(&flag, h->flag, 4, cudaMemcpyDeviceToHost, s));
     KX_CUDA(cudaStreamSynchronize(s));
     if (flag) { h->err = "kx_evolve: f became non-finite"; return KX_ERR_NONFINITE; }
+    return KX_OK;
+}
+
+kx_status_t kx_delta_source(kx_handle_t h, double p0, double* G, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    if (!G || !(p0 >= h->p_lo && p0 <= h->p_hi)) { h->err = "kx_delta_source: G is NULL or p0 outside the grid"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    KX_CUDA(kx_launch_delta_source(h->d, p0, G, (cudaStream_t)stream));
     return KX_OK;
 }
 

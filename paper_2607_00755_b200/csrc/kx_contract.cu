@@ -463,6 +463,27 @@ __global__ void k_adapt_ctrl(KxAdapt* ad, double u1, double safety)
     ad->errkey = kx_dkey(0.0);
 }
 
+// ---------------------------------------------------------------- monoenergetic source deposition
+__global__ void __launch_bounds__(KX_CTA) k_delta_source(KxDev d, double p0, double* __restrict__ G)
+{
+    __shared__ int s_L;
+    const int N = d.N;
+    if (threadIdx.x == 0) {            // largest L <= N-2 with p_L <= p0
+        int lo = 0, hi = N - 2;
+        while (lo < hi) {
+            int mid = (lo + hi + 1) >> 1;
+            if (d.p[mid] <= p0) lo = mid; else hi = mid - 1;
+        }
+        s_L = lo;
+    }
+    __syncthreads();
+    const int L = s_L;
+    const double E0 = sqrt(p0 * p0 + d.m * d.m);
+    const double aR = (E0 - d.E[L]) / (d.E[L + 1] - d.E[L]);      // energy-linear deposition fractions
+    for (int i = threadIdx.x; i < N; i += KX_CTA)
+        G[i] = i == L ? (1.0 - aR) / d.h[L] : (i == L + 1 ? aR / d.h[L + 1] : 0.0);
+}
+
 // ---------------------------------------------------------------- a9: moments, eq. B.2
 __global__ void __launch_bounds__(KX_CTA)
 k_moments(KxDev d, const double* __restrict__ f, double* n, double* rho, double* p1, double* p2, int stride)
@@ -575,6 +596,12 @@ cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, 
 {
     k_adapt_accept<<<B, KX_CTA, 0, s>>>(d.N, f, fnew, ad, flag);
     k_adapt_ctrl<<<1, 1, 0, s>>>(ad, u1, safety);
+    return cudaGetLastError();
+}
+
+cudaError_t kx_launch_delta_source(const KxDev& d, double p0, double* G, cudaStream_t s)
+{
+    k_delta_source<<<1, KX_CTA, 0, s>>>(d, p0, G);
     return cudaGetLastError();
 }
 

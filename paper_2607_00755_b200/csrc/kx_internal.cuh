@@ -115,6 +115,7 @@ struct kx_handle_s {
     double *hostio;           // [wsB, N] x2 staging for kx_collide_host
     int *flag;                // device non-finite flag
     KxAdapt *adapt;           // device controller state of kx_evolve_adaptive
+    double p_lo, p_hi;        // host copies of p[0], p[N-1]
     void *dev_blob;           // one allocation holding the [N]-sized arrays
     bool profiling;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;
@@ -251,6 +252,7 @@ cudaError_t kx_launch_finish(const KxDev& d, const double* f, const double* part
                              const KxStage& st, cudaStream_t s);
 cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, int B, KxAdapt* ad, double u1, double safety,
                                  int* flag, cudaStream_t s);      // accept/reject + controller update
+cudaError_t kx_launch_delta_source(const KxDev& d, double p0, double* G, cudaStream_t s);
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
                               double* p1, double* p2, int stride, cudaStream_t s);
 // ---- tiled path (kx_tiled_build.cu, kx_tiled.cu)

@@ -74,7 +74,7 @@ class _AdaptiveResult(C.Structure):
 
 # every symbol include/kx.h declares
 SYMBOLS = ["kx_build", "kx_set_mass", "kx_collide", "kx_collide_parts", "kx_collide_ex",
-           "kx_collide_host", "kx_moments", "kx_evolve", "kx_evolve_adaptive", "kx_info", "kx_tensor_export",
+           "kx_collide_host", "kx_moments", "kx_evolve", "kx_evolve_adaptive", "kx_delta_source", "kx_info", "kx_tensor_export",
            "kx_kinematics_export", "kx_profile", "kx_profile_read", "kx_probe_flops", "kx_last_error", "kx_destroy", "kx_version"]
 
 _lib = None
@@ -114,6 +114,7 @@ def _load():
     lib.kx_evolve.argtypes = [vp, vp, i32, C.POINTER(_Source), C.POINTER(_Evolve), vp]
     lib.kx_evolve_adaptive.argtypes = [vp, vp, i32, C.POINTER(_Source), C.POINTER(_Adaptive),
                                        C.POINTER(_AdaptiveResult), vp]
+    lib.kx_delta_source.argtypes = [vp, C.c_double, vp, vp]
     lib.kx_info.argtypes = [vp, i64p, i64p, C.POINTER(i32)]
     lib.kx_tensor_export.argtypes = [vp, C.c_int64, i64p, _dp, _dp, C.POINTER(C.c_uint32)]
     lib.kx_kinematics_export.argtypes = [vp, _dp, _dp, _dp]
@@ -313,6 +314,13 @@ class Handle:
         self._check(self._lib.kx_evolve_adaptive(self._h, _dev(f), B, C.byref(src) if src is not None else None,
                                                  C.byref(ctl), C.byref(res), _stream(stream)))
         return dict(u=res.u, du=res.du, accepted=int(res.accepted), rejected=int(res.rejected), done=bool(res.done))
+
+    def delta_source(self, p0, stream=None):
+        """kx_delta_source: shape [N] of a monoenergetic source at p0 for the current mass."""
+        import torch
+        G = torch.empty(self.N, dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._lib.kx_delta_source(self._h, float(p0), C.c_void_p(G.data_ptr()), _stream(stream)))
+        return G
 
     def profile(self, enable=True):
         self._check(self._lib.kx_profile(self._h, int(bool(enable))))

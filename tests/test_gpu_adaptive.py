@@ -90,3 +90,32 @@ def test_adaptive_bose_and_step_budget(torch_cuda, oracle):
     assert abs(info["u"] - info_ref5["u"]) <= 1e-12 * abs(info_ref5["u"])
     assert np.abs(f.cpu().numpy() - f_ref5).max() <= 1e-11 * np.abs(f_ref5).max()
     h.close()
+
+
+@pytest.mark.parametrize("m", [0.0, 1.0, 300.0])
+def test_delta_source_parity_and_injection(torch_cuda, oracle, m):
+    """kx_delta_source against the oracle, element by element, also after kx_set_mass; used as a source of
+    kx_evolve it injects exactly the prescribed number and energy per step."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    p = kin.log_grid(48, 1e-2, 50.0)
+    dp = kin.trapezoid_widths(p)
+    h = kx.Handle(p, dp, 2.0)
+    h.set_mass(m)
+    E, K, hw = oracle.kinematics(p, dp, m)
+    for p0 in (p[0], 0.37, p[20], 11.0, p[-1]):
+        G = h.delta_source(p0).cpu().numpy()
+        G0 = oracle.delta_source(p, dp, m, p0)
+        assert np.abs(G - G0).max() <= 1e-13 * np.abs(G0).max()
+    with pytest.raises(kx.KxError):
+        h.delta_source(2.0 * p[-1])
+    # sources only (kappa = 0): 10 Euler steps inject 10 * amp * dtau particles of energy E_0 each
+    p0 = 3.3
+    G = h.delta_source(p0)
+    f = torch.zeros((1, p.size), dtype=torch.float64, device="cuda")
+    tau = np.linspace(0.0, 1.0, 11)
+    h.evolve(f, tau, method=kx.EULER, kappa=np.zeros(1), G=G[None, :].contiguous(), amp=np.full((1, 10), 0.7), project=False)
+    got = f.cpu().numpy()[0]
+    assert abs((hw * got).sum() - 0.7) <= 1e-14
+    assert abs((hw * E * got).sum() - 0.7 * np.sqrt(p0 * p0 + m * m)) <= 1e-13 * (1.0 + m)
+    h.close()

@@ -459,3 +459,29 @@ def test_A2_adaptive_heun_sources_only_closed_form(oracle):
     assert info["accepted"] == n and info["rejected"] == 0 and info["done"]
     want = c["f"] + (u1 - u0) * (amp[:, None] * G).sum(axis=0)[None, :]
     assert np.abs(f - want).max() <= 1e-13 * np.abs(want).max()
+
+
+# ------------------------------------------------------------------ monoenergetic source deposition (8(f) item 4)
+@pytest.mark.parametrize("m", [0.0, 1.0, 300.0])
+def test_S1_delta_source_moments_exact(oracle, m):
+    """the deposited source reproduces the injected number and energy exactly; it sits on the two
+    neighbours of p0, with the whole weight on a grid point when p0 hits one; the fractions are linear in ENERGY."""
+    p = kin.log_grid(64, 1e-3, 1e2)
+    dp = kin.trapezoid_widths(p)
+    E, K, h = oracle.kinematics(p, dp, m)
+    for p0 in (p[0], 0.5 * (p[10] + p[11]), p[30] * 1.0000001, 7.3, p[-1]):
+        G = oracle.delta_source(p, dp, m, p0)
+        E0 = np.sqrt(p0 * p0 + m * m)
+        assert abs((h * G).sum() - 1.0) <= 1e-14
+        assert abs((h * E * G).sum() - E0) <= 1e-13 * E0
+        nz = np.nonzero(G)[0]
+        assert 1 <= nz.size <= 2 and (nz.size == 1 or nz[1] == nz[0] + 1)
+        assert p[nz[0]] <= p0 <= p[min(nz[0] + 1, p.size - 1)]
+        assert (G >= 0).all()
+    G = oracle.delta_source(p, dp, m, p[17])
+    assert np.count_nonzero(G) == 1 and G[17] == 1.0 / h[17]
+    # not linear in momentum: at the momentum midpoint the right fraction differs from 1/2 for a massive species
+    if m == 1.0:
+        j = 40
+        G = oracle.delta_source(p, dp, m, 0.5 * (p[j] + p[j + 1]))
+        assert abs(h[j + 1] * G[j + 1] - 0.5) > 1e-3
