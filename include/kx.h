@@ -85,7 +85,7 @@ typedef struct { int32_t n; const double* p; const double* dp; } kx_grid_t;
 typedef struct { double m; double g_chi; } kx_species_t;
 /* |M|^2 = M2_0 (m_med <= 0: contact, eq. B.17) or M2_0 / (1 + (-t)/m_med^2)^2, t = (p_i-p_n)^2 (reading D5) */
 typedef struct { double M2_0; double m_med; } kx_msq_t;
-/* Options; pass NULL for the defaults {LOG, TILED, FP64, EXP_TABLE, 0, 0, 1e-300, 1e-12} */
+/* Options; pass NULL for the defaults {LOG, TILED, FP64, EXP_TABLE, 0, 0, 0, 0, 1e-300, 1e-12} */
 typedef struct {
     int32_t interp;      /* KX_INTERP_*  */
     int32_t storage;     /* KX_STORE_*   */
@@ -93,6 +93,10 @@ typedef struct {
     int32_t exp_impl;    /* KX_EXP_*     */
     int32_t loss_nodes;  /* KX_STORE_TILED + LOG: Chebyshev nodes per bracket, 8|16|24|32; 0 = default (24) */
     int32_t statistics;  /* KX_STAT_*: eta = 0 | +1 | -1 */
+    int32_t n_mu;        /* 0 (default): analytic reduced kernel, eq. B.17 / reading D5.  > 0: the numerical angular kernel
+                            F_inm of eq. B.4-B.12 with n_mu Gauss-Legendre nodes in mu = cos(p_i, p_n),
+                            |M|^2 evaluated at t(mu) (O(n_mu N^3) build); n_mu <= 4096 */
+    int32_t reserved;    /* must be 0 */
     double  f_floor;     /* y = ln max(f, f_floor), reading D8; must be >= 1e-300 and > 0 */
     double  eps_supp;    /* support threshold of eq. C.4, reading D9 */
 } kx_opts_t;

@@ -57,6 +57,9 @@ def _load():
         _lib.okx_evolve_adaptive.restype = C.c_int
         _lib.okx_delta_source.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_double, _dp]
         _lib.okx_delta_source.restype = C.c_int
+        _lib.okx_requadrature.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int,
+                                          _dp, _dp, _dp, _ip]
+        _lib.okx_requadrature.restype = None
         _lib.okx_collide_rows.argtypes = [C.c_int, C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double,
                                           C.c_double, _dp, C.c_int, _ip, C.c_int, C.c_double, _dp, _dp, _dp]
         _lib.okx_collide_rows.restype = None
@@ -99,7 +102,9 @@ def kinematics(p, dp, m):
 class Tables:
     """Dense W[i,n,m], jL[i,n,m] (-1 = dropped), wR[i,n,m] from the quadruple loop (O2-O7)."""
 
-    def __init__(self, p, dp, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0):
+    def __init__(self, p, dp, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, n_mu=0):
+        """n_mu > 0: W from the numerical angular kernel (eq. B.5-B.12) with n_mu Gauss-Legendre nodes
+        (numpy.polynomial.legendre.leggauss) instead of the analytic kernel of eq. B.17."""
         self.p, self.dp = _c(p), _c(dp)
         self.m, self.g_chi, self.M2_0, self.m_med = float(m), float(g_chi), float(M2_0), float(m_med)
         n = self.N = self.p.size
@@ -109,6 +114,11 @@ class Tables:
         self.kept = _load().okx_build(n, _d(self.p), _d(self.dp), self.m, self.g_chi, self.M2_0,
                                       self.m_med, _d(self.W), self.jL.ctypes.data_as(_ip), _d(self.wR))
         self.E, self.K, self.h = kinematics(self.p, self.dp, self.m)
+        if n_mu:
+            mu, wmu = np.polynomial.legendre.leggauss(int(n_mu))
+            mu, wmu = _c(mu), _c(wmu)
+            _load().okx_requadrature(n, _d(self.p), _d(self.dp), self.m, self.g_chi, self.M2_0, self.m_med, int(n_mu),
+                                     _d(mu), _d(wmu), _d(self.W), self.jL.ctypes.data_as(_ip))
 
 
 def collide(T: Tables, f, interp=LOG, f_floor=1e-300):

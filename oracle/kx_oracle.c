@@ -578,3 +578,21 @@ double okx_F_closed(double pi_, double pn, double pm, double m, double M2_0, dou
     const double pi3 = (double)(OKX_PI * OKX_PI * OKX_PI);
     return (1.0 / (64.0 * pi3 * pi_)) * (pn * pm / (En * Em)) * J;
 }
+
+/* ---- Numerical angular kernel: replace the analytic F of every KEPT triple by the
+ * mu-quadrature of eq. B.5-B.12 (okx_F_quadrature above): W_inm = dp_n dp_m F_inm / (2 E_i g_chi), eq. 4.7.  The index
+ * map (jL, omega_R) is untouched: it is fixed by energy conservation alone. */
+void okx_requadrature(int N, const double *p, const double *dp, double m, double g_chi, double M2_0, double m_med,
+                      int nmu, const double *mu, const double *wmu, double *W, const int32_t *jL)
+{
+#pragma omp parallel for schedule(dynamic)
+    for (int i = 0; i < N; ++i) {
+        double Ei = sqrt(p[i] * p[i] + m * m);
+        for (int n = 0; n < N; ++n)
+            for (int mm = 0; mm < N; ++mm) {
+                size_t idx = ((size_t)i * N + n) * N + mm;
+                if (jL[idx] < 0) continue;
+                W[idx] = dp[n] * dp[mm] / (2.0 * Ei * g_chi) * okx_F_quadrature(p[i], p[n], p[mm], m, M2_0, m_med, nmu, mu, wmu);
+            }
+    }
+}

@@ -267,6 +267,7 @@ void kx_destroy(kx_handle_t h)
         cudaFree(h->tiled_blob);
         cudaFree(h->t.AL);
         cudaFree(h->adapt);
+        cudaFree(h->gl);
         for (auto& ev : h->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     }
     delete h;
@@ -288,7 +289,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     }
     if (!(sp->m >= 0.0) || !(sp->g_chi > 0.0) || !isfinite(sp->m)) { g_build_err = "need m >= 0 and g_chi > 0"; return KX_ERR_INVALID_ARG; }
     if (!isfinite(msq->M2_0) || !isfinite(msq->m_med)) { g_build_err = "non-finite |M|^2 parameters"; return KX_ERR_INVALID_ARG; }
-    kx_opts_t o = {KX_INTERP_LOG, KX_STORE_TILED, KX_FP64, KX_EXP_TABLE, 0, 0, 1e-300, 1e-12};
+    kx_opts_t o = {KX_INTERP_LOG, KX_STORE_TILED, KX_FP64, KX_EXP_TABLE, 0, 0, 0, 0, 1e-300, 1e-12};
     if (opts) o = *opts;
     if (o.loss_nodes == 0) o.loss_nodes = 24;
     if (o.precision != KX_FP64) { g_build_err = "fp32 mode is not implemented"; return KX_ERR_UNSUPPORTED; }
@@ -307,6 +308,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         return KX_ERR_UNSUPPORTED;
     }
     if (o.statistics != KX_STAT_CLASSICAL) o.storage = KX_STORE_SYM_ROWS;     // evaluated by the exact streaming kernel
+    if (o.n_mu < 0 || o.n_mu > 4096 || o.reserved != 0) { g_build_err = "n_mu must be in [0, 4096] and reserved 0"; return KX_ERR_INVALID_ARG; }
     if (o.exp_impl != KX_EXP_TABLE && o.exp_impl != KX_EXP_LIBM) { g_build_err = "unknown exp_impl"; return KX_ERR_INVALID_ARG; }
     if (!(o.f_floor >= 1e-300) || !(o.eps_supp >= 0.0)) { g_build_err = "need f_floor >= 1e-300 and eps_supp >= 0"; return KX_ERR_INVALID_ARG; }
 
@@ -370,6 +372,33 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         KX_CUDA(cudaMemcpyAsync(DP, grid->dp, (size_t)N * 8, cudaMemcpyHostToDevice, s));
         KX_CUDA(cudaMemcpyAsync(tab, t.data(), t.size() * 8, cudaMemcpyHostToDevice, s));
         KX_CUDA(cudaMemsetAsync(h->flag, 0, 4, s));
+        if (o.n_mu > 0) {
+            // Gauss-Legendre nodes and weights on [-1,1] (constants, not data dependent): Newton on P_n in long double
+            const int n = o.n_mu;
+            std::vector<double> gl(2 * (size_t)n);
+            const long double pi = 3.14159265358979323846264338327950288L;
+            for (int k = 0; k < n; ++k) {
+                long double x = cosl(pi * (k + 0.75L) / (n + 0.5L)), dpn = 1.0L;
+                for (int it = 0; it < 100; ++it) {
+                    long double p0 = 1.0L, p1 = x;
+                    for (int j = 2; j <= n; ++j) { long double p2 = ((2 * j - 1) * x * p1 - (j - 1) * p0) / j; p0 = p1; p1 = p2; }
+                    if (n == 1) { p0 = 1.0L; p1 = x; }
+                    dpn = n * (x * p1 - p0) / (x * x - 1.0L);
+                    const long double dx = p1 / dpn;
+                    x -= dx;
+                    if (fabsl(dx) < 1e-19L) break;
+                }
+                long double p0 = 1.0L, p1 = x;
+                for (int j = 2; j <= n; ++j) { long double p2 = ((2 * j - 1) * x * p1 - (j - 1) * p0) / j; p0 = p1; p1 = p2; }
+                dpn = n * (x * p1 - p0) / (x * x - 1.0L);
+                gl[n - 1 - k] = (double)x;                                   // ascending
+                gl[(size_t)n + n - 1 - k] = (double)(2.0L / ((1.0L - x * x) * dpn * dpn));
+            }
+            KX_CUDA(cudaMalloc((void**)&h->gl, gl.size() * 8));
+            KX_CUDA(cudaMemcpyAsync(h->gl, gl.data(), gl.size() * 8, cudaMemcpyHostToDevice, s));
+            KX_CUDA(cudaStreamSynchronize(s));
+            d.n_mu = n; d.gl_mu = h->gl; d.gl_w = h->gl + n;
+        }
         KX_CUDA(kx_launch_kinematics(d, d.m, s));
         KX_CUDA(kx_launch_runs(d, s));
         unsigned nnz = 0;

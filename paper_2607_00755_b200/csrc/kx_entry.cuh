@@ -67,6 +67,43 @@ static __device__ double kx_J(double a, double b, double dK, double M2_0, double
 }
 
 
+// Numerical reduced kernel F(p_i, p_n, p_m) of eq. B.4-B.12: Gauss-Legendre quadrature over
+// mu = cos(p_i, p_n); for every node the nu-integral is analytic (B.11) between the roots of the quadratic B.8-B.10
+// clipped to [-1,1]; |M|^2 is evaluated at t(mu) = 2 m^2 - 2 E_i E_n + 2 p_i p_n mu (reading D5).
+static __device__ double kx_F_quad(const KxDev& d, double pi_, double pn, double pm)
+{
+    const double m = d.m;
+    const double Ei = sqrt(pi_ * pi_ + m * m), En = sqrt(pn * pn + m * m), Em = sqrt(pm * pm + m * m);
+    double acc = 0.0;
+    for (int q = 0; q < d.n_mu; ++q) {
+        const double u = d.gl_mu[q];
+        const double A0 = m * m + En * Em - En * Ei - Em * Ei + pi_ * pn * u;      // B.5
+        const double A1 = pi_ * pm - pn * pm * u;                                    // B.6
+        const double K2 = pn * pn * pm * pm * (1.0 - u * u);                         // B.7
+        const double a = -(K2 + A1 * A1), b = -2.0 * A0 * A1, c = K2 - A0 * A0;      // B.8
+        const double disc = b * b - 4.0 * a * c;
+        if (!(disc > 0.0) || !(a < 0.0)) continue;
+        const double sq = sqrt(disc);
+        const double r1 = (-b + sq) / (2.0 * a), r2 = (-b - sq) / (2.0 * a);         // B.10
+        const double lo = fmin(r1, r2), hi = fmax(r1, r2);
+        if (hi <= -1.0 || lo >= 1.0) continue;
+        const double vm = fmax(lo, -1.0), vp = fmin(hi, 1.0);
+        const double am = fmax(-1.0, fmin(1.0, (2.0 * a * vm + b) / sq));
+        const double ap = fmax(-1.0, fmin(1.0, (2.0 * a * vp + b) / sq));
+        const double I = (asin(am) - asin(ap)) / sqrt(-a);                           // B.11
+        double M2 = d.M2_0;
+        if (d.m_med > 0.0) {
+            const double t = 2.0 * m * m - 2.0 * Ei * En + 2.0 * pi_ * pn * u;
+            const double dd = 1.0 + (-t) / (d.m_med * d.m_med);
+            M2 = d.M2_0 / (dd * dd);
+        }
+        acc += d.gl_w[q] * I * M2;
+    }
+    const double twopi = 2.0 * kPi;
+    const double pref = 1.0 / (4.0 * (twopi * twopi) * (twopi * twopi)) * (pn * pm) * (pn * pm) / (En * Em);   // B.12
+    return pref * acc;
+}
+
 // K~ of a KEPT triple, snapped into the domain (reading D4)                       eq. 4.4
 __device__ __forceinline__ double kx_Kt(double Kn, double Km, double Ki, double K0, double KN1)
 {
@@ -80,6 +117,12 @@ __device__ __forceinline__ double kx_Wsym(const KxDev& d, const double* __restri
                                           double pref_in)
 {
     const double pm = P[m];
+    if (d.n_mu > 0) {      // numerical angular kernel: W = dp_n dp_m F_inm / (2 E_i g_chi), both orderings       eq. 4.7
+        const double Ei = sqrt(pi_ * pi_ + d.m * d.m);
+        double F = kx_F_quad(d, pi_, pn, pm);
+        if (m != n) F += kx_F_quad(d, pi_, pm, pn);
+        return d.dp[n] * d.dp[m] / (2.0 * Ei * d.g_chi) * F;
+    }
     const double pj = sqrt(Kt * (Kt + 2.0 * d.m));   // eq. 4.4
     // eq. B.15-B.16
     double J = kx_J(fmax(fabs(pi_ - pn), fabs(pm - pj)), fmin(pi_ + pn, pm + pj), Ki - Kn, d.M2_0, d.m_med);

@@ -26,6 +26,8 @@ struct KxDev {
     int interp;          // KX_INTERP_*
     int exp_impl;        // KX_EXP_*
     int eta;             // KX_STAT_*: 0, +1 (Bose), -1 (Fermi)
+    int n_mu;            // > 0: numerical angular kernel with n_mu Gauss-Legendre nodes (gl_mu, gl_w)
+    const double *gl_mu, *gl_w;
     int chunk;           // entries per contraction task
     double m, g_chi, M2_0, m_med, f_floor, eps_supp;
     // grid and kinematics [N]
@@ -116,6 +118,7 @@ struct kx_handle_s {
     int *flag;                // device non-finite flag
     KxAdapt *adapt;           // device controller state of kx_evolve_adaptive
     double p_lo, p_hi;        // host copies of p[0], p[N-1]
+    double *gl;               // device [2 n_mu]: Gauss-Legendre nodes and weights (n_mu > 0)
     void *dev_blob;           // one allocation holding the [N]-sized arrays
     bool profiling;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;

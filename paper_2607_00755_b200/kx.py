@@ -48,7 +48,7 @@ class _Msq(C.Structure):
 
 class _Opts(C.Structure):
     _fields_ = [("interp", C.c_int32), ("storage", C.c_int32), ("precision", C.c_int32),
-                ("exp_impl", C.c_int32), ("loss_nodes", C.c_int32), ("statistics", C.c_int32),
+                ("exp_impl", C.c_int32), ("loss_nodes", C.c_int32), ("statistics", C.c_int32), ("n_mu", C.c_int32), ("reserved", C.c_int32),
                 ("f_floor", C.c_double), ("eps_supp", C.c_double)]
 
 
@@ -168,7 +168,7 @@ class Handle:
     """kx_build: kinematics, index map and kernel tensor on the device for one (grid, species, |M|^2)."""
 
     def __init__(self, p, dp, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, *, interp=INTERP_LOG,
-                 exp_impl=EXP_TABLE, storage=STORE_TILED, loss_nodes=0, statistics=STAT_CLASSICAL, f_floor=1e-300,
+                 exp_impl=EXP_TABLE, storage=STORE_TILED, loss_nodes=0, statistics=STAT_CLASSICAL, n_mu=0, f_floor=1e-300,
                  eps_supp=1e-12, device=0, stream=None):
         import torch
         if not torch.cuda.is_available():
@@ -184,7 +184,7 @@ class Handle:
         grid = _Grid(self.N, _ptr(p), _ptr(dp))
         sp = _Species(float(m), float(g_chi))
         msq = _Msq(float(M2_0), float(m_med))
-        opts = _Opts(int(interp), int(storage), FP64, int(exp_impl), int(loss_nodes), int(statistics), float(f_floor),
+        opts = _Opts(int(interp), int(storage), FP64, int(exp_impl), int(loss_nodes), int(statistics), int(n_mu), 0, float(f_floor),
                      float(eps_supp))
         with torch.cuda.device(self.device):
             rc = lib.kx_build(C.byref(grid), C.byref(sp), C.byref(msq), C.byref(opts), self.device,

@@ -97,3 +97,33 @@ def test_quantum_rejects_linear_interpolation(torch_cuda):
         kx.Handle(c["p"], c["dp"], c["m"], statistics=1, interp=kx.INTERP_LINEAR)
     with pytest.raises(kx.KxError):
         kx.Handle(c["p"], c["dp"], c["m"], statistics=2)
+
+
+@pytest.mark.parametrize("cfg,N,n_mu", [(1, None, 48), (3, 40, 32)])
+def test_numerical_angular_kernel_parity(torch_cuda, oracle, cfg, N, n_mu):
+    """n_mu > 0: the device builder evaluates F_inm by the Gauss-Legendre quadrature of eq.
+    B.5-B.12; entries and operator against the oracle's quadrature tables (its nodes come from numpy, the library's from
+    its own Newton iteration), on the streaming and the tensor-core storage."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(cfg, N=N, B=3)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], n_mu=n_mu)
+    n = T.N
+    Wsym = T.W + np.transpose(T.W, (0, 2, 1))
+    Wsym[:, np.arange(n), np.arange(n)] = T.W[:, np.arange(n), np.arange(n)]
+    g0, l0, C0 = oracle.collide(T, c["f"], oracle.LOG)
+    scale = np.abs(g0).max(axis=1, keepdims=True)
+    for storage in (kx.STORE_SYM_ROWS, kx.STORE_TILED):
+        h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], n_mu=n_mu, storage=storage)
+        ex = h.tensor_export()
+        rowptr, W, nn, mm = ex["rowptr"], ex["W"], ex["n"], ex["m"]
+        i_of = np.repeat(np.arange(n), np.diff(rowptr))
+        # tolerance: B.11 takes asin at arguments clipped to +-1, where an ulp of the argument moves the result by
+        # sqrt(ulp) ~ 1e-8 of a node's weight (DESIGN.md section 14); measured 4e-10
+        assert np.abs(W - Wsym[i_of, nn, mm]).max() <= 1e-8 * np.abs(Wsym).max()
+        C = h.collide(_dev(torch, c["f"])).cpu().numpy()
+        assert (np.abs(C - C0) / scale).max() <= 1e-8
+        h.close()
+    # and it is the quadrature, not the analytic kernel
+    T0 = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    assert np.abs(T.W - T0.W).max() > 1e-5 * np.abs(T0.W).max()

@@ -485,3 +485,23 @@ def test_S1_delta_source_moments_exact(oracle, m):
         j = 40
         G = oracle.delta_source(p, dp, m, 0.5 * (p[j] + p[j + 1]))
         assert abs(h[j + 1] * G[j + 1] - 0.5) > 1e-3
+
+
+# ------------------------------------------------------------------ numerical angular kernel (8(f) item 3)
+@pytest.mark.parametrize("cfg,N", [(1, None), (3, 40)])
+def test_K1_numerical_kernel_converges_to_analytic(oracle, cfg, N):
+    """for |M|^2 = const (and for the t-channel form of D5) the mu-quadrature of eq. B.5-B.12 reproduces
+    the analytic kernel; the tables built with n_mu nodes approach the analytic ones like 1/n_mu (kinks of the integrand),
+    and so does the operator.  The index map is the same."""
+    c = kin.config(cfg, N=N, B=1)
+    T0 = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T0, c["f"], oracle.LOG)
+    devW, devC = [], []
+    for n_mu in (64, 512, 4096):
+        T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], n_mu=n_mu)
+        assert np.array_equal(T.jL, T0.jL) and np.array_equal(T.wR, T0.wR)
+        devW.append(np.abs(T.W - T0.W).max() / np.abs(T0.W).max())
+        g, l, C = oracle.collide(T, c["f"], oracle.LOG)
+        devC.append(np.abs(C - C0).max() / np.abs(g0).max())
+    assert devW[0] < 0.15 and devW[2] < 2e-3 and devW[0] > 3 * devW[1] > 9 * devW[2]
+    assert devC[2] < 2e-4 and devC[0] > 3 * devC[2]
