@@ -218,33 +218,40 @@ __global__ void __launch_bounds__(256) k_reduce(int N, int B, KxStage st)
 {
     __shared__ double s_g[8][32], s_l[8][32];
     kx_pdl_trigger();
-    kx_pdl_wait();
     const int tid = threadIdx.x, part = tid >> 5, o = tid & 31, il = o & 15, bl = o >> 4;
     const int tile = blockIdx.x, b = blockIdx.y * 2 + bl, i = tile * 16 + il;
-    double g = 0.0, nu = 0.0;
-    if (b < B && i < N) {
+    const bool on = b < B && i < N;
+    // everything that does not depend on the contraction kernel happens before the wait: the slot ranges
+    unsigned c0 = 1, c1 = 0, d0 = 1, d1 = 0;
+    const double* src = nullptr;
+    const double* srl = nullptr;
+    if (on) {
         const unsigned Gtot = st.vtptr[st.NT];
         const unsigned a0 = st.vtptr[tile], a1 = st.vtptr[tile + 1];
         if (a1 > a0) {
-            const unsigned c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.GW - 1ull) / Gtot);
-            const unsigned c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.GW - 1ull) / Gtot);
-            const double* src = st.gpart + ((size_t)tile * st.xstride + b) * 16 + il;
-#pragma unroll 4
-            for (unsigned c = c0 + part; c <= c1; c += 8) g += src[(size_t)c * st.xstride * 16];
+            c0 = (unsigned)((((unsigned long long)a0 + 1ull) * (unsigned)st.GW - 1ull) / Gtot);
+            c1 = (unsigned)(((unsigned long long)a1 * (unsigned)st.GW - 1ull) / Gtot);
         }
+        src = st.gpart + ((size_t)tile * st.xstride + b) * 16 + il;
         const unsigned U = (unsigned)st.RS * (unsigned)st.LC;
         const unsigned sp = (unsigned)i >> 8;
         const unsigned l0 = sp * (unsigned)st.LC, l1 = l0 + (unsigned)st.LC;
-        const unsigned d0 = (unsigned)((((unsigned long long)l0 + 1ull) * (unsigned)st.GL - 1ull) / U);
-        const unsigned d1 = (unsigned)(((unsigned long long)l1 * (unsigned)st.GL - 1ull) / U);
-        const double* srl = st.lpart + ((size_t)sp * st.xstride + b) * 256 + (i & 255);
+        d0 = (unsigned)((((unsigned long long)l0 + 1ull) * (unsigned)st.GL - 1ull) / U);
+        d1 = (unsigned)(((unsigned long long)l1 * (unsigned)st.GL - 1ull) / U);
+        srl = st.lpart + ((size_t)sp * st.xstride + b) * 256 + (i & 255);
+    }
+    kx_pdl_wait();
+    double g = 0.0, nu = 0.0;
+    if (on) {
+#pragma unroll 4
+        for (unsigned c = c0 + part; c <= c1; c += 8) g += src[(size_t)c * st.xstride * 16];
 #pragma unroll 4
         for (unsigned c = d0 + part; c <= d1; c += 8) nu += srl[(size_t)c * st.xstride * 256];
     }
     s_g[part][o] = g;
     s_l[part][o] = nu;
     __syncthreads();
-    if (part == 0 && b < B && i < N) {
+    if (part == 0 && on) {
         double G = s_g[0][o], L = s_l[0][o];
 #pragma unroll
         for (int k = 1; k < 8; ++k) { G += s_g[k][o]; L += s_l[k][o]; }
@@ -262,6 +269,14 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
     __shared__ double s_y[KX_MAX_N];
     const int N = d.N, tid = threadIdx.x, b = blockIdx.x;
     const double* fb = fin + (size_t)b * N;
+    // inputs that no kernel of this call writes (the stage input, the kinematics) are fetched before the wait
+    double C[kMaxPerThread], fi[kMaxPerThread], hi_[kMaxPerThread], Ei[kMaxPerThread], Ki[kMaxPerThread];
+#pragma unroll
+    for (int q = 0; q < kMaxPerThread; ++q) {
+        const int i = tid + q * KX_CTA;
+        C[q] = 0.0; fi[q] = 0.0; hi_[q] = 0.0; Ei[q] = 0.0; Ki[q] = 0.0;
+        if (i < N) { fi[q] = fb[i]; hi_[q] = d.h[i]; Ei[q] = d.E[i]; Ki[q] = d.K[i]; }
+    }
     kx_pdl_wait();
     const bool tiled = st.gpart != nullptr && !(st.mstat && kx_member_flagged(st.mstat, b));
     if (st.mstat) {          // last reader of the member's statistics: reset them for the next call
@@ -269,11 +284,9 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
         if (tid == 0) { st.mstat[2 * b] = KX_MSTAT_NONE; st.mstat[2 * b + 1] = 0; }
     }
 
-    double C[kMaxPerThread], fi[kMaxPerThread], hi_[kMaxPerThread], Ei[kMaxPerThread], Ki[kMaxPerThread];
 #pragma unroll
     for (int q = 0; q < kMaxPerThread; ++q) {
         const int i = tid + q * KX_CTA;
-        C[q] = 0.0; fi[q] = 0.0; hi_[q] = 0.0; Ei[q] = 0.0; Ki[q] = 0.0;
         if (i < N) {
             double g = 0.0, nu = 0.0, gq2 = 0.0, lq2 = 0.0;
             if (tiled) {
@@ -289,14 +302,12 @@ k_finish(KxDev d, const double* __restrict__ fin, const double* __restrict__ par
                     if (d.eta) { gq2 += pp[2]; lq2 += pp[3]; }
                 }
             }
-            fi[q] = fb[i];
             if (d.eta) {                                          // eq. 4.3 from the four sums (see k_contract)
                 const double eta = (double)d.eta;
                 g = (1.0 + eta * fi[q]) * (g + eta * gq2);
                 nu = nu + eta * lq2 + gq2;
             }
             C[q] = fma(-fi[q], nu, g);                            // a6
-            hi_[q] = d.h[i]; Ei[q] = d.E[i]; Ki[q] = d.K[i];
             if (st.gain) st.gain[(size_t)b * N + i] = g;
             if (st.loss) st.loss[(size_t)b * N + i] = fi[q] * nu;
         }

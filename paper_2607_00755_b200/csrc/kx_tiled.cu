@@ -337,7 +337,7 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
         constexpr int SB = loss_stage_bytes(NBT);
         constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
         static_assert(WARPS == 8 || WARPS == 16, "loss role: 8 or 16 warps");
-        kx_pdl_wait();        // the Chebyshev coefficients in XT come from k_xt
+        bool waited = false;  // the Chebyshev coefficients in XT come from k_xt: griddepcontrol.wait before the first X copy
         const unsigned cl = blockIdx.x - GG;
         const unsigned LC = (unsigned)t.LC;
         const unsigned U = (unsigned)t.RS * LC;
@@ -351,17 +351,20 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
             const int nb = min(32, t.NR8 - 32 * (int)sp);                // 8-row blocks of this supertile
             const int nbw = min(R8, max(0, nb - R8 * warp));             // ... of this warp
 
-            auto issue = [&](unsigned kc, int slot) {
+            auto issueA = [&](unsigned kc, int slot) {          // the tensor: does not depend on any kernel of this call
                 unsigned char* dstA = smem + (size_t)slot * SB;
                 const double* srcA = t.AL + ((size_t)kc * t.NR8 + 32 * sp) * 128;
                 for (int k = tid; k < nb * 64; k += NTHR) cp_async16(dstA + (size_t)k * 16, srcA + (size_t)k * 2);
-                double* dstX = reinterpret_cast<double*>(dstA + kLossABytes);
+            };
+            auto issueX = [&](unsigned kc, int slot) {          // the coefficients written by k_xt
+                double* dstX = reinterpret_cast<double*>(smem + (size_t)slot * SB + kLossABytes);
                 const double* srcX = XT + (size_t)(t.loss_row0 + 16 * kc) * xstride + bcol0;
                 for (int k = tid; k < 16 * NBT * 4; k += NTHR) {
                     const int r = k / (NBT * 4), cc = k - r * (NBT * 4);
                     cp_async16(dstX + (size_t)r * LD + 2 * cc, srcX + (size_t)r * xstride + 2 * cc);
                 }
             };
+            auto issue = [&](unsigned kc, int slot) { issueA(kc, slot); issueX(kc, slot); };
 
             double acc[R8][NBT][2];
 #pragma unroll
@@ -369,9 +372,14 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
 #pragma unroll
                 for (int bt = 0; bt < NBT; ++bt) acc[r][bt][0] = acc[r][bt][1] = 0.0;
 
+            // prologue: the tensor chunks are requested before the wait on the operand-preparation kernel
+#pragma unroll
+            for (int s = 0; s < kLossStages - 1; ++s)
+                if ((unsigned)s < n) issueA(ka + s, s);
+            if (!waited) { kx_pdl_wait(); waited = true; }
 #pragma unroll
             for (int s = 0; s < kLossStages - 1; ++s) {
-                if ((unsigned)s < n) issue(ka + s, s);
+                if ((unsigned)s < n) issueX(ka + s, s);
                 cp_async_commit();
             }
             for (unsigned it = 0; it < n; ++it) {
@@ -408,6 +416,7 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
                         *reinterpret_cast<double2*>(dst + (size_t)(8 * bt + lr) * 256 + 8 * r) = make_double2(acc[r][bt][0], acc[r][bt][1]);
             u = ue;
         }
+        if (!waited) kx_pdl_wait();
     }
 }
 
