@@ -207,8 +207,10 @@ kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bo
         if ((rc = prof_begin()) != KX_OK) return rc;
         KX_CUDA(kx_launch_dmma(h->d, h->t, h->groups, h->GG, h->GL, f, h->XT, xs, h->gpart, h->lpart, B, s));
         if ((rc = prof_end()) != KX_OK) return rc;
-        if (h->d.interp == KX_INTERP_LOG)      // exact streaming path for flagged members only (LINEAR is exact)
-            KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, h->mstat, true, s));
+        // exact streaming path for flagged members only (LINEAR is exact): launched by kx_launch_finish after k_reduce,
+        // so that its launch and its flag check hide behind the reduction instead of following the contraction
+        st->fb_f = nullptr;
+        if (h->d.interp == KX_INTERP_LOG) { st->fb_sm_count = h->sm_count; st->fb_f = f; st->fb_yd = h->yd; st->fb_part = h->part; }
         st->gpart = h->gpart; st->lpart = h->lpart; st->gn = reinterpret_cast<double2*>(h->gn); st->vtptr = h->t.vtptr;
         st->mstat = h->d.interp == KX_INTERP_LOG ? h->mstat : nullptr;
         st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS; st->GW = kx_dmma_workers(h->d.N, B) * h->GG; st->GL = h->GL; st->xstride = xs;

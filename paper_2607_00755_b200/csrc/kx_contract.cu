@@ -598,6 +598,10 @@ cudaError_t kx_launch_finish(const KxDev& d, const double* fin, const double* pa
     if (st.gpart) {
         cudaError_t e = kx_launch(k_reduce, dim3(st.NT, (B + 1) / 2), dim3(256), 0, s, true, d.N, B, st);
         if (e != cudaSuccess) return e;
+        if (st.fb_f) {
+            e = kx_launch_contract(d, st.fb_sm_count, st.fb_f, st.fb_yd, st.fb_part, B, st.mstat, true, s);
+            if (e != cudaSuccess) return e;
+        }
     }
     return kx_launch(k_finish, dim3(B), dim3(KX_CTA), 0, s, true, d, fin, part, B, st);
 }

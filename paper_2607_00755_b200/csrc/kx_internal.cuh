@@ -243,6 +243,10 @@ struct KxStage {             // what the finishing kernel does after the reducti
     int NT, LC, RS, GW, GL, xstride;      // GW = gain workers (warps), GL = loss workers (CTAs)
     int *flag;
     int evolve;
+    // tiled LOG path: the exact fallback kernel (gated per member group) is launched between k_reduce and k_finish
+    int fb_sm_count;
+    const double *fb_f, *fb_yd;
+    double *fb_part;
     // adaptive Heun (rk_method == KX_HEUN_ADAPT): dt and the rate come from the device controller state
     KxAdapt *ad;
     double ad_u0, ad_rate0, ad_slope, ad_rtol, ad_atol;
