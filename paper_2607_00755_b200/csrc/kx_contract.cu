@@ -243,10 +243,18 @@ __global__ void __launch_bounds__(256) k_reduce(int N, int B, KxStage st)
     kx_pdl_wait();
     double g = 0.0, nu = 0.0;
     if (on) {
-#pragma unroll 4
+        // all loads of an output are in flight together: the first 8 loss partials are requested before the gain loop
+        double vl[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const unsigned c = d0 + part + 8u * (unsigned)u;
+            vl[u] = c <= d1 ? srl[(size_t)c * st.xstride * 256] : 0.0;
+        }
+#pragma unroll 8
         for (unsigned c = c0 + part; c <= c1; c += 8) g += src[(size_t)c * st.xstride * 16];
-#pragma unroll 4
-        for (unsigned c = d0 + part; c <= d1; c += 8) nu += srl[(size_t)c * st.xstride * 256];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) nu += vl[u];
+        for (unsigned c = d0 + part + 64u; c <= d1; c += 8) nu += srl[(size_t)c * st.xstride * 256];
     }
     s_g[part][o] = g;
     s_l[part][o] = nu;
