@@ -305,8 +305,8 @@ def main():
         roof_head = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak}
     if streaming:
         # k_contract: FP64-pipe instructions per (entry, member) counted in the SASS of the inner loop (DESIGN.md
-        # section 5): 12 classical LOG, 3 LINEAR, 33 with quantum statistics; peak = 148 SMs x 64 FP64 lanes x max clock
-        c_inst = 33 if stat != 0 else (12 if args.mode == "log" else 3)
+        # section 5): 12 classical LOG, 3 LINEAR, 22 with quantum statistics; peak = 148 SMs x 64 FP64 lanes x max clock
+        c_inst = 22 if stat != 0 else (12 if args.mode == "log" else 3)
         ach_inst = nnz * B * c_inst / kern_s / 1e12
         peak_inst = SM_COUNT * FP64_LANES_PER_SM * sm_max_hz / 1e12
         roof_head = {"bound": "alu", "achieved": ach_inst, "peak": peak_inst, "unit": "T FP64 inst/s",

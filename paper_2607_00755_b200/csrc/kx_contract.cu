@@ -129,7 +129,16 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
                 else if (MODE == MODE_LOG_LIBM) x = exp2(t);
                 else x = t;
                 if (QS) {
-                    const double wf = Wc * (x / (1.0 - eta * x));       // W f_j~, eq. B.20
+                    // W f_j~, eq. B.20: x / (1 - eta x) with the reciprocal from the hardware estimate (2^-23) and two
+                    // Newton steps (2^-46, 2^-92: full double precision) instead of the IEEE division sequence
+                    const double dn = fma(-eta, x, 1.0);
+                    double rc;
+                    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(dn));
+                    double er = fma(-dn, rc, 1.0);
+                    rc = fma(rc, er, rc);
+                    er = fma(-dn, rc, 1.0);
+                    rc = fma(rc, er, rc);
+                    const double wf = Wc * (x * rc);
                     l[b] += wf;
                     g2[b] = fma(wf, pn, g2[b]);
                     l2[b] = fma(wf, fn + fm, l2[b]);
