@@ -349,3 +349,28 @@ def test_back_to_back_calls_are_ordered(torch_cuda):
         for k, o in enumerate(outs):
             assert torch.equal(o, ref_a if k % 2 == 0 else ref_b), (rep, k)
     h.close()
+
+
+def test_collide_max_grid_sampled_rows(torch_cuda, oracle):
+    """The ABI's largest grid, N = 1024 (n, m, j_L packed 10 bits each; 2.8 GB tiled operand), B = 3, mediator |M|^2:
+    sampled rows against the oracle, conservation of the projected operator, and the packed index limits."""
+    torch = torch_cuda
+    N, B = 1024, 3
+    p = kin.log_grid(N, 1e-3, 100.0)
+    dp = kin.trapezoid_widths(p)
+    f = np.stack([kin._random_bimodal(p, 9000 + b) for b in range(B)])
+    rows = np.array([0, 1, 15, 16, 255, 256, 511, 777, 1008, 1022, 1023])
+    g0, l0, C0 = oracle.collide_rows(p, dp, f, rows, m=1.0, M2_0=1.0, m_med=0.5)
+    c = dict(p=p, dp=dp, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.5)
+    h = _handle(c)
+    fd = _dev(torch, f)
+    o = h.collide_ex(fd, flags=0, want=("C", "gain", "loss"))
+    gmax = np.abs(o["gain"].cpu().numpy()).max(axis=1, keepdims=True)
+    for key, ref in (("gain", g0), ("loss", l0), ("C", C0)):
+        assert (np.abs(o[key].cpu().numpy()[:, rows] - ref) / gmax).max() <= TOL, key
+    E, K, hw = h.kinematics_export()
+    Cp = h.collide(fd, flags=1).cpu().numpy()
+    Craw = o["C"].cpu().numpy()
+    assert (np.abs((hw * Cp).sum(axis=1)) <= 1e-13 * (hw * np.abs(Craw)).sum(axis=1)).all()
+    assert (np.abs((hw * E * Cp).sum(axis=1)) <= 1e-13 * (hw * E * np.abs(Craw)).sum(axis=1)).all()
+    h.close()
