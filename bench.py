@@ -321,7 +321,9 @@ def main():
             "peak_source": f"FP64 tensor pipe: 148 SMs x 64 FMA/clk x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src}); "
                            f"probe in this run: DMMA {probe['dmma']:.1f}, DFMA {probe['dfma']:.1f} TFLOP/s",
             "peak_alt": {"value": float(peaks.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0,
-                         "how": f"{peak_src} bf16_tflops x guide nominal ratio 45/2250"},
+                         "how": f"{peak_src} bf16_tflops x guide nominal ratio 45/2250 (the rule for a contraction in another "
+                                "dtype); `peak` is the stricter figure the DMMA probe reaches",
+                         "frac": ach / (float(peaks.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0)},
             "tensor_bytes_per_launch": info["tensor_bytes"],
             "hbm_time_us_at_peak": t_hbm * 1e6, "tensor_time_us_at_peak": t_flop * 1e6}
     line = {
