@@ -140,6 +140,11 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
     return KX_OK;
 }
 
+// Integrators on small problems are bound by kernel launches, not by work: below this many (entry, member) pairs per
+// operator evaluation the exact streaming path (2 kernels per stage) beats the tensor-core path (5 kernels per stage);
+// measured: cfg1 12 vs 21 us per stage, cfg2 16 vs 23 us, N=256 B=4 76 vs 33 us.
+constexpr long long kSmallProblem = 1500000;
+
 long long nnz_estimate(const kx_handle_s* h)
 {
     if (!h->nnz_stale) return h->nnz;
@@ -560,7 +565,7 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
     bool have_yd = false;            // yd already holds the current stage input (written by the last finish)
     // a static tensor is evaluated through the tiled (DMMA) operand; with a mass schedule every stage has new
     // kinematics, and re-deriving the Chebyshev moments per stage costs more than the exact streaming path
-    const bool use_tiled = h->storage == KX_STORE_TILED && !ctl->mass;
+    const bool use_tiled = h->storage == KX_STORE_TILED && !ctl->mass && nnz_estimate(h) * B > kSmallProblem;
     if (use_tiled && (rc = ensure_tiled(h, s)) != KX_OK) return rc;
 
     for (int k = 0; k < S; ++k) {
@@ -653,7 +658,7 @@ kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_sou
     init.errkey = 0;                 // key of +0.0
     KX_CUDA(cudaMemcpyAsync(h->adapt, &init, sizeof init, cudaMemcpyHostToDevice, s));
     KX_CUDA(cudaMemsetAsync(h->flag, 0, 4, s));
-    const bool use_tiled = h->storage == KX_STORE_TILED;
+    const bool use_tiled = h->storage == KX_STORE_TILED && nnz_estimate(h) * B > kSmallProblem;
     if (use_tiled && (rc = ensure_tiled(h, s)) != KX_OK) return rc;
     if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
 

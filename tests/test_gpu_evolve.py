@@ -196,3 +196,27 @@ def test_cfg5_full_size_invariants(torch_cuda):
     assert (np.diff(warm) < 0).all(), warm
     assert 1.9 < warm[0] < 2.2 and 3 * np.pi / 8 < warm[-1] < 1.34, warm
     h.close()
+
+
+@pytest.mark.parametrize("method", ["HEUN", "RK4"])
+def test_evolve_tensor_core_path_batch(torch_cuda, oracle, method):
+    """A batch large enough (nnz x B > 1.5e6 entry-member pairs) that kx_evolve keeps the tensor-core path for its stages
+    (small problems are routed to the two-kernel streaming path): static mass, per-member couplings, mediator |M|^2."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    B = 6
+    c = kin.config(3, N=96, B=B)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    assert int((T.jL >= 0).sum()) // 2 * B > 1_500_000
+    g, l, C = oracle.collide(T, c["f"], oracle.LOG)
+    nu = float((l / np.where(c["f"] > 0, c["f"], 1.0)).max())
+    tau = np.arange(7) * (0.4 / nu)
+    kappa = np.linspace(0.2, 1.5, B)
+    meth = dict(HEUN=(oracle.HEUN, kx.HEUN), RK4=(oracle.RK4, kx.RK4))[method]
+    f_ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], M2_0=c["M2_0"], m_med=c["m_med"], method=meth[0], tau=tau,
+                          kappa=kappa)
+    h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    f = _dev(torch, c["f"])
+    h.evolve(f, tau, method=meth[1], kappa=kappa)
+    assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-10 * np.abs(f_ref).max()
+    h.close()
