@@ -22,7 +22,7 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  kx_collide*,
  *     kx_moments and kx_set_mass only enqueue work on it and return without synchronising, except
  *     that the first call with a larger batch B than seen before grows the handle's workspace
- *     (cudaMalloc, implicit sync).  kx_build, kx_evolve, kx_collide_host and kx_tensor_export
+ *     (cudaMalloc, implicit sync).  kx_build, kx_evolve, kx_evolve_adaptive, kx_collide_host and kx_tensor_export
  *     synchronise the stream before returning.
  *   - The handle owns the kernel tensor and all workspaces.  One host thread at a time per handle.
  *   - There is no CPU fallback: every entry point fails with KX_ERR_CUDA when no sm_100 device
@@ -56,13 +56,13 @@ typedef enum {
                                  evaluated by the streaming kernel, one exp per (entry, member) in LOG mode */
 #define KX_STORE_TILED    1   /* default: SYM_ROWS plus the 16-row tiled operand of the FP64 tensor-core (DMMA)
                                  contraction: gain as (n<=m) x members GEMM, LOG loss through the Chebyshev moments
-                                 of each (i, bracket) bucket (DESIGN.md section 4); members with a bracket whose
+                                 of each (i, bracket) bucket (DESIGN.md section 5); members with a bracket whose
                                  interpolation error bound exceeds 1e-15 max f fall back to the streaming kernel */
 /* precision */
 #define KX_FP64 0
 #define KX_FP32 1             /* not implemented: KX_ERR_UNSUPPORTED */
 /* exp used by the LOG loss term */
-#define KX_EXP_TABLE 0        /* 128-entry table + degree-4 polynomial, <= 1 ulp-level error (default) */
+#define KX_EXP_TABLE 0        /* 256-entry table x degree-4 polynomial of the remainder, <= 2 ulp (default) */
 #define KX_EXP_LIBM  1        /* CUDA math library exp2() */
 /* quantum statistics of the species (eq. 4.3): Lambda_inm = f_n f_m (1+eta f_i)(1+eta f_j~)
  * - f_i f_j~ (1+eta f_n)(1+eta f_m), off-grid occupation through y = ln(f/(1+eta f)) (eq. B.20).
