@@ -66,8 +66,8 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
     kx_pdl_trigger();
     kx_pdl_wait();
     if (mstat) {          // tiled path: only member groups holding a flagged member take the exact streaming path
-        bool any = false;
-        for (int b = 0; b < nb; ++b) any = any || kx_member_flagged(mstat, b0 + b);
+        // one member per thread and one vote: a single round trip to the statistics instead of one per member
+        const int any = __syncthreads_or(tid < nb && kx_member_flagged(mstat, b0 + tid));
         if (!any) return;
     }
 
