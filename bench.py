@@ -39,8 +39,8 @@ WORKLOAD = "cfg3: N=256 log p/T in [1e-3,50], B=64 seeded bimodal f, |M|^2 ~ 1/(
 # (profiles/r01c_tiled_dmma.md; LINEAR from the working capture of the same round); null for configurations that were
 # not captured.
 NCU_TRAFFIC = {("log", 64): 64.85e6, ("linear", 64): 48.72e6}
-# kernels of one kx_collide on the tiled path: k_xt, k_dmma, k_contract (exact fallback, exits at once when no member is
-# flagged; LOG only), k_reduce, k_finish
+# kernels of one kx_collide on the tiled path: k_dmma, k_reduce, k_contract (exact fallback, exits at once when no member
+# is flagged; LOG only), k_finish
 LOSS_NODES = {"log": 24, "linear": 2}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM; DMMA.8x8x4 runs at the same 37.2 TFLOP/s
 
@@ -315,7 +315,7 @@ def main():
     roof = {**roof_head,
             "traffic": NCU_TRAFFIC.get((args.mode, B)) if (not args.project and args.config == 3 and not streaming) else None,
             "kernel": ("k_contract (exact streaming kernel: gather, exp2, FMA per entry and member)" if streaming
-                       else "k_dmma (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss)"),
+                       else "k_dmma (FP64 DMMA.8x8x4: gain + Chebyshev-moment loss, coefficients computed in the kernel)"),
             "kernel_ms": kern_s * 1e3, "kernel_ms_l2_warm": kern_warm_ms / max(kern_warm_n, 1),
             "event_pair_around_empty_kernel_us": ev_over_us, "flop_per_launch": flop,
             "peak_source": f"FP64 tensor pipe: 148 SMs x 64 FMA/clk x 2 x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm, {peak_src}); "
@@ -337,7 +337,7 @@ def main():
         "calls_per_s": world * K / t_cold,
         "e2e": {"value": world * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": B * Ngrid * 8,
                 "d2h_bytes_per_step": B * Ngrid * 8, "ms_per_step": t_e2e / K * 1e3},
-        "gpu_launches": (3 if streaming else (5 if args.mode == "log" else 4)) * K, "clocks": clocks, "roofline": roof, "finite": same,
+        "gpu_launches": (3 if streaming else (4 if args.mode == "log" else 3)) * K, "clocks": clocks, "roofline": roof, "finite": same,
     }
     if not args.no_cpu_baseline and world == 1 and args.config == 3:
         cb = cpu_oracle(c, members=B, steps=10, warmup=1)

@@ -97,9 +97,9 @@ void free_ws(kx_handle_s* h)
 {
     cudaFree(h->yd); cudaFree(h->part); cudaFree(h->fstage); cudaFree(h->k1); cudaFree(h->k2);
     cudaFree(h->k3); cudaFree(h->Cbuf); cudaFree(h->hostio);
-    cudaFree(h->XT); cudaFree(h->mstat); cudaFree(h->gpart); cudaFree(h->lpart); cudaFree(h->gn);
+    cudaFree(h->mstat); cudaFree(h->gpart); cudaFree(h->lpart); cudaFree(h->gn);
     h->yd = h->part = h->fstage = h->k1 = h->k2 = h->k3 = h->Cbuf = h->hostio = nullptr;
-    h->XT = h->gpart = h->lpart = h->gn = nullptr; h->mstat = nullptr;
+    h->gpart = h->lpart = h->gn = nullptr; h->mstat = nullptr;
     h->wsB = 0; h->ws_tasks = 0; h->ws_xstride = 0;
 }
 
@@ -123,8 +123,6 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
     KX_CUDA(dalloc(&h->hostio, bn * 2));
     if (h->storage == KX_STORE_TILED) {
         const int xs = kx_xstride(nB);
-        KX_CUDA(dalloc(&h->XT, (size_t)h->t.xrows * xs));
-        KX_CUDA(cudaMemset(h->XT, 0, (size_t)h->t.xrows * xs * 8));      // padding rows stay zero for good
         KX_CUDA(dalloc(&h->mstat, (size_t)nB * 2));
         {
             std::vector<long long> init((size_t)nB * 2);
@@ -208,14 +206,13 @@ kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bo
     if (use_tiled) {
         const int xs = h->ws_xstride;
         kx_dmma_split(h->d, h->t, h->sm_count, h->groups, B, &h->GG, &h->GL);
-        KX_CUDA(kx_launch_xt(h->d, h->t, f, h->yd, h->XT, xs, h->mstat, B, s));
         if ((rc = prof_begin()) != KX_OK) return rc;
-        KX_CUDA(kx_launch_dmma(h->d, h->t, h->groups, h->GG, h->GL, f, h->XT, xs, h->gpart, h->lpart, B, s));
+        KX_CUDA(kx_launch_dmma(h->d, h->t, h->groups, h->GG, h->GL, f, h->mstat, xs, h->gpart, h->lpart, B, s));
         if ((rc = prof_end()) != KX_OK) return rc;
         // exact streaming path for flagged members only (LINEAR is exact): launched by kx_launch_finish after k_reduce,
         // so that its launch and its flag check hide behind the reduction instead of following the contraction
         st->fb_f = nullptr;
-        if (h->d.interp == KX_INTERP_LOG) { st->fb_sm_count = h->sm_count; st->fb_f = f; st->fb_yd = h->yd; st->fb_part = h->part; }
+        if (h->d.interp == KX_INTERP_LOG) { st->fb_sm_count = h->sm_count; st->fb_f = f; st->fb_yd = nullptr; st->fb_part = h->part; }
         st->gpart = h->gpart; st->lpart = h->lpart; st->gn = reinterpret_cast<double2*>(h->gn); st->vtptr = h->t.vtptr;
         st->mstat = h->d.interp == KX_INTERP_LOG ? h->mstat : nullptr;
         st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS; st->GW = kx_dmma_workers(h->d.N, B) * h->GG; st->GL = h->GL; st->xstride = xs;
@@ -423,9 +420,6 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
             t.LC = ((N - 1) * t.Q + 15) / 16;
             t.NR8 = (N + 7) / 8;
             t.RS = (N + 255) / 256;
-            t.ones_row = N;
-            t.loss_row0 = N + 4;
-            t.xrows = t.loss_row0 + 16 * t.LC;
             // loss operand: fixed size; the padding (k >= (N-1) Q, rows >= N) stays zero for good
             KX_CUDA(dalloc(&t.AL, (size_t)t.LC * t.NR8 * 128));
             KX_CUDA(cudaMemsetAsync(t.AL, 0, (size_t)t.LC * t.NR8 * 128 * 8, s));

@@ -74,8 +74,14 @@ k_contract(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd
     for (int k = tid; k < BT * N; k += KX_CTA) {
         int b = k / N, j = k - b * N;
         if (b < nb) {
-            s_yd[k] = yd[(size_t)(b0 + b) * N + j];
-            s_f[k] = f[(size_t)(b0 + b) * N + j];
+            const double fv = f[(size_t)(b0 + b) * N + j];
+            if (yd) s_yd[k] = yd[(size_t)(b0 + b) * N + j];
+            else {        // fallback of the tiled path: no prepared y, computed here (k_prep's arithmetic)
+                const double y0 = kx_yval(fv, d.interp, d.f_floor, d.eta);
+                const double y1 = j + 1 < N ? kx_yval(f[(size_t)(b0 + b) * N + j + 1], d.interp, d.f_floor, d.eta) : y0;
+                s_yd[k] = make_double2(y0, y1 - y0);
+            }
+            s_f[k] = fv;
         } else {                                  // ragged last group: harmless values, results discarded
             s_yd[k] = make_double2(0.0, 0.0);
             s_f[k] = 0.0;

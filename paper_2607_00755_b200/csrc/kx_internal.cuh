@@ -58,7 +58,7 @@ struct KxDev {
 //          "run", padded to a multiple of 4.  A group (4 quads) stores its 256 doubles in MMA-fragment order
 //          [quad][row block rb][lane], the lane's element being A[k = 4 quad + lane%4][i = 16 t + 8 rb + lane/4].
 //          desc[quad] = m0 | n << 20: the rows of f^T holding f_m for the quad (m0..m0+3) and the row that scales
-//          them (f_n; padding quads: 0 | ones_row << 20 with A = 0).  vtptr[t] = first group of tile t.
+//          them (f_n; padding quads: 0 | N << 20, the column of ones, with A = 0).  vtptr[t] = first group of tile t.
 //   loss:  k = (j, c), c < Q;  A = M_c(i,j) = sum_{(n<=m) in bracket j of row i} Wsym T_c(2 omega_R - 1)
 //          (Chebyshev moments of the bucket), X = a_c(b,j) = Chebyshev coefficients of the degree-(Q-1) interpolant
 //          of omega -> f_j^(1-omega) f_(j+1)^omega (LOG) or the exact two coefficients (LINEAR, Q = 2).  The operand
@@ -70,9 +70,6 @@ struct KxTiled {
     int LC;                   // loss chunks of 16 k = ceil((N-1) Q / 16)
     int NR8;                  // 8-row blocks = ceil(N / 8)
     int RS;                   // 256-row supertiles = ceil(N / 256)
-    int ones_row;             // = N: row of XT filled with 1
-    int loss_row0;            // = N + 4: first Chebyshev-coefficient row of XT (rows N+1..N+3 stay zero)
-    int xrows;                // rows of XT = loss_row0 + 16 LC
     int *trun_mlo;            // [NT*N] first m of the run (tile, n)
     unsigned *trun_q;         // [NT*N] quads of the run
     unsigned *trun_off;       // [NT*(N+1)] exclusive scan of trun_q inside the tile; [t*(N+1)+N] = quads of tile t
@@ -82,7 +79,7 @@ struct KxTiled {
     double *AL;               // [LC][NR8][128]  loss operand
     const double *dct;        // [Q*Q] (2 - delta_c0)/Q cos(c theta_q), theta_q = (2q+1) pi / (2Q)
     const double *nodes;      // [Q] omega_q = (1 + cos theta_q)/2
-    double flag_log2;         // log2(2 / Q!) ... see kx_tiled.cu k_xt
+    double flag_log2;         // log2(2 / Q!) ... see the loss role of k_dmma (kx_tiled.cu)
 };
 
 struct KxAdapt;
@@ -97,8 +94,7 @@ struct kx_handle_s {
     bool tiled_ok;            // t.A / t.desc describe the current kinematics
     long long cap_groups;     // capacity of t.A / t.desc in groups
     long long groups;         // host copy of vtptr[NT]
-    int ws_xstride;           // columns of XT (batch capacity padded)
-    double *XT;               // [t.xrows, ws_xstride] operand rows: f^T, ones, Chebyshev coefficients
+    int ws_xstride;           // members per partial slot (batch capacity padded)
     long long *mstat;         // [wsB][2] per member: ordered key of the largest interpolation-error term over the brackets,
                               // bits of max_i |f_i| (see kx_member_flagged); reset by the finishing kernel
     double *gpart;            // [8 sm_count + NT + 1, ws_xstride, 16]  gain partials of the DMMA kernel (one per warp and tile)
@@ -183,7 +179,7 @@ __device__ __forceinline__ double kx_exp2_tab(double t, const double* __restrict
 }
 
 
-// Per-member statistics of the tiled LOG path, accumulated with atomicMax by k_xt (order independent, so the
+// Per-member statistics of the tiled LOG path, accumulated with atomicMax by the loss role of k_dmma (order independent, so the
 // result is deterministic):  mstat[2b] = key(max over brackets j of  log2 max(f_j, f_j+1) + Q (log2 |ln(f_j+1/f_j)| - 2)
 // + log2(2/Q!)),  mstat[2b+1] = bits of max_i |f_i|.  key() maps doubles to integers of the same order.
 #define KX_MSTAT_NONE (-0x7fffffffffffffffLL - 1)
@@ -265,10 +261,8 @@ cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n,
 // ---- tiled path (kx_tiled_build.cu, kx_tiled.cu)
 cudaError_t kx_launch_tile_runs(const KxDev& d, const KxTiled& t, cudaStream_t s);     // runs, scans, vtptr
 cudaError_t kx_launch_tile_fill(const KxDev& d, const KxTiled& t, cudaStream_t s);     // A, desc (gain + loss)
-cudaError_t kx_launch_xt(const KxDev& d, const KxTiled& t, const double* f, double* yd, double* XT, int xstride,
-                         long long* mstat, int B, cudaStream_t s);
 cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
-                           const double* XT, int xstride, double* gpart, double* lpart, int B, cudaStream_t s);
+                           long long* mstat, int xstride, double* gpart, double* lpart, int B, cudaStream_t s);
 int kx_xstride(int B);
 int kx_dmma_workers(int N, int B);     // gain workers (warps) per CTA of k_dmma
 void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long groups, int B, int* GG, int* GL);

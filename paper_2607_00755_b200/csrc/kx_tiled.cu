@@ -4,8 +4,8 @@
 //   nu[b,i]   = sum_j sum_{c<Q} M_c(i,j) a_c(b,j)   (loss_i = f_i nu_i)   eq. B.19-B.20, see
 //               kx_tiled_build.cu for the Chebyshev-moment form of the interpolated loss term and its error bound
 //
-// Both are out[b,i] += sum_k X[b,k] A[k,i] with A streamed once from HBM/L2 (cp.async) and X built from the small
-// operand array XT: X = f_n f_m for the gain, X = a_c(b,j) for the loss.  The products run on the FP64 tensor
+// Both are out[b,i] += sum_k X[b,k] A[k,i] with A streamed once from HBM/L2 (cp.async) and X built in shared memory
+// from the caller's f: X = f_n f_m for the gain, X = a_c(b,j) for the loss.  The products run on the FP64 tensor
 // pipe: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), M = 8 members, N = 8 rows, K = 4.  The CTAs of one launch are split
 // between the two terms in proportion to their work (see k_dmma); the finishing kernel (kx_contract.cu) adds the
 // partials: no atomics, bit-reproducible.
@@ -13,123 +13,17 @@
 // Compiled with --fmad=false; fused multiply-adds are explicit.
 #include "kx_internal.cuh"
 
-
 namespace {
 
 // cost of one loss DMMA relative to one gain DMMA in the CTA split of k_dmma (measured on cfg3: the split that
-// makes both roles finish together)
-constexpr double kLossCost = 1.0;
+// makes both roles finish together; the loss CTAs also compute their Chebyshev coefficients first)
+constexpr double kLossCost = 1.3;
 
 // D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
 {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
         : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-// ---------------------------------------------------------------- operand rows XT[row, b]
-//   rows loss_row0 + jQ + c    a_c(b,j), c < Q, j < N-1      (loss; the gain role of k_dmma reads f itself)
-// LOG:    g(omega_q) = 2^(y_j + omega_q (y_{j+1}-y_j)), y = log2 max(f, f_floor), at the Q Chebyshev nodes of [0,1];
-//         a_c = (2-delta_c0)/Q sum_q g(omega_q) cos(c theta_q)            (discrete Chebyshev transform)
-//         A member is flagged for the exact streaming path when, for some bracket,
-//             2 (|ln(f_{j+1}/f_j)|/4)^Q / Q! * max(f_j, f_{j+1}) > 1e-15 max_i f_i    (interpolation error bound);
-//         this kernel accumulates the two maxima per member (mstat, kx_internal.cuh), the consumers compare them.
-// LINEAR: a_0 = (f_j + f_{j+1})/2, a_1 = (f_{j+1} - f_j)/2 (exact).
-// Also writes yd[b,j] = (y_j, y_{j+1}-y_j) for the streaming kernel.
-// grid.x = N (row j), 256 threads = 64 members x 4 coefficient phases.
-__global__ void __launch_bounds__(256) k_xt(KxDev d, KxTiled t, const double* __restrict__ f, double2* __restrict__ yd,
-                                            double* __restrict__ XT, int xstride, long long* __restrict__ mstat, int B)
-{
-    __shared__ double s_node[KX_QMAX];
-    __shared__ double s_G[KX_QMAX][68];        // row stride 4 mod 16: the 4 x 8 fragment reads below are conflict free
-    __shared__ double s_y[2][64];
-    __shared__ double s_tab[1 << KX_EXP_BITS];
-    const int N = d.N, Q = t.Q, j = blockIdx.x;
-    const bool tab = d.exp_impl == KX_EXP_TABLE;
-    const int bl = threadIdx.x & 63, ph = threadIdx.x >> 6;
-    const bool logm = d.interp == KX_INTERP_LOG;
-    kx_pdl_trigger();       // first kernel of the call (ordinary launch): the contraction kernel may start right away
-    // the transform runs on the tensor pipe: a_c[b] = sum_q dct[c,q] G[q,b] is a (Q x Q) x (Q x 64) product, warp w takes
-    // members 8w..8w+7; its fragments of dct (lane: dct[8 ct + lane/4][4 ks + lane%4]) stay in registers
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double afr[KX_QMAX / 8][KX_QMAX / 4];
-    if (logm) {
-#pragma unroll
-        for (int ct = 0; ct < KX_QMAX / 8; ++ct)
-#pragma unroll
-            for (int ks = 0; ks < KX_QMAX / 4; ++ks)
-                afr[ct][ks] = (8 * ct < Q && 4 * ks < Q) ? t.dct[(8 * ct + (lane >> 2)) * Q + 4 * ks + (lane & 3)] : 0.0;
-        if (threadIdx.x < Q) s_node[threadIdx.x] = t.nodes[threadIdx.x];
-        if (tab) s_tab[threadIdx.x] = d.exptab[threadIdx.x];          // 256 threads, 2^KX_EXP_BITS = 256 entries
-    }
-    __syncthreads();
-    for (int b0 = 0; b0 < B; b0 += 64) {
-        const int b = b0 + bl;
-        const bool act = b < B;
-        double fj = 0.0, fj1 = 0.0;
-        if (act) {
-            fj = f[(size_t)b * N + j];
-            fj1 = j + 1 < N ? f[(size_t)b * N + j + 1] : fj;
-        }
-        if (act && ph == 0) {
-            const long long fk = __double_as_longlong(fabs(fj));
-            if (fk > mstat[2 * b + 1]) atomicMax(mstat + 2 * b + 1, fk);
-        }
-        if (!logm) {
-            if (act && ph == 0) {
-                yd[(size_t)b * N + j] = make_double2(fj, fj1 - fj);
-                if (j < N - 1) {
-                    double* row = XT + (size_t)(t.loss_row0 + 2 * j) * xstride + b;
-                    row[0] = 0.5 * (fj + fj1);
-                    row[xstride] = 0.5 * (fj1 - fj);
-                }
-            }
-            continue;
-        }
-        // one logarithm per thread: phase 0 takes f_j, phase 1 takes f_(j+1)
-        if (ph < 2) s_y[ph][bl] = log2(fmax(ph == 0 ? fj : fj1, d.f_floor));
-        __syncthreads();
-        const double y0 = s_y[0][bl];
-        const double y1 = j + 1 < N ? s_y[1][bl] : y0;
-        const double dy = y1 - y0;
-        if (act && ph == 0) {
-            yd[(size_t)b * N + j] = make_double2(y0, dy);
-            const double c = 0.6931471805599453 * fabs(dy);
-            if (j < N - 1 && c > 0.0) {
-                // log2 of the bracket's error bound (log2 max_i f_i is subtracted by the consumers)
-                const long long lk = kx_dkey(fmax(y0, y1) + (double)Q * (log2(c) - 2.0) + t.flag_log2);
-                if (lk > mstat[2 * b]) atomicMax(mstat + 2 * b, lk);
-            }
-        }
-        if (j >= N - 1) { __syncthreads(); continue; }       // uniform over the CTA
-        if (tab) for (int q = ph; q < Q; q += 4) s_G[q][bl] = kx_exp2_tab<1>(fma(s_node[q], dy, y0), s_tab);
-        else for (int q = ph; q < Q; q += 4) s_G[q][bl] = exp2(fma(s_node[q], dy, y0));
-        __syncthreads();
-        {
-            double D[KX_QMAX / 8][2];
-#pragma unroll
-            for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[ct][0] = D[ct][1] = 0.0;
-#pragma unroll
-            for (int ks = 0; ks < KX_QMAX / 4; ++ks) {
-                if (4 * ks < Q) {                                        // uniform
-                    const double g = s_G[4 * ks + (lane & 3)][8 * warp + (lane >> 2)];
-#pragma unroll
-                    for (int ct = 0; ct < KX_QMAX / 8; ++ct)
-                        if (8 * ct < Q) dmma884(D[ct][0], D[ct][1], afr[ct][ks], g);
-                }
-            }
-            const int bw = b0 + 8 * warp + 2 * (lane & 3);                // lane holds a_c[bw], a_c[bw+1], c = 8 ct + lane/4
-#pragma unroll
-            for (int ct = 0; ct < KX_QMAX / 8; ++ct) {
-                if (8 * ct < Q) {
-                    double* dst = XT + (size_t)(t.loss_row0 + j * Q + 8 * ct + (lane >> 2)) * xstride + bw;
-                    if (bw + 1 < B) *reinterpret_cast<double2*>(dst) = make_double2(D[ct][0], D[ct][1]);
-                    else if (bw < B) dst[0] = D[ct][0];
-                }
-            }
-        }
-        __syncthreads();
-    }
 }
 
 // ---------------------------------------------------------------- the contraction
@@ -144,8 +38,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 constexpr int kStageBytes = KX_GROUP_DBL * 8 + 16;     // gain ring stage: 2 KiB of A + 4 descriptors
 constexpr int kLossStages = 3;
-constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256 rows of AL ...
-__host__ __device__ constexpr int loss_stage_bytes(int NBT) { return kLossABytes + 16 * (NBT * 8 + 4) * 8; }   // ... + 16 k x members of X
+constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256 rows of AL
 
 // One CTA per SM.  CTAs [0, GG) take equal ranges of gain groups, CTAs [GG, GG+GL) equal ranges of loss chunks.
 //
@@ -155,16 +48,18 @@ __host__ __device__ constexpr int loss_stage_bytes(int NBT) { return kLossABytes
 //   cp.async ring and holds a 16-row x 8 NBT-member accumulator (2 NBT DMMA per quad and fragment pair).
 //   The DMMAs of a run (fixed n) take X = f_m and accumulate into T; f_n multiplies T once, when the run ends.
 //   The ring keeps flowing across tile boundaries.
-// loss role: a dense GEMM.  The CTA stages chunks of 16 k (32 KiB of AL for 256 rows + the matching 16 rows of
-//   Chebyshev coefficients) through a 3-stage cp.async pipeline shared by all warps; warp w owns rows
-//   [32 w, 32 w + 32) x 8 NBT members (4 NBT DMMA per quad).
+// loss role: a dense GEMM.  The CTA first computes the Chebyshev coefficients a_c(b,j) of its own share of k = (j,c)
+//   rows straight into shared memory (window by window if the share does not fit): exp2 at the Chebyshev nodes, then
+//   the discrete Chebyshev transform on the tensor pipe; it also accumulates the per-member statistics that route a
+//   member to the exact fallback.  Then warp w streams its rows [32 w, 32 w + 32) of AL through a private 3-stage
+//   cp.async ring (4 KiB per chunk of 16 k) and multiplies them with the resident coefficients (4 NBT DMMA per quad).
 // A range that crosses a tile (supertile) boundary produces one partial per piece, slot = worker + tile (a gain
 // worker is a warp, a loss worker a CTA); the finishing kernel adds the partials of a row in slot order: no
 // atomics, bit-reproducible.
 template <int NBT, int WARPS, int STAGES>
 __global__ void __launch_bounds__(WARPS * 32, 1)
-k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, const double* __restrict__ XT, int xstride,
-       double* __restrict__ gpart, double* __restrict__ lpart, int GG, int GL)
+k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, long long* __restrict__ mstat,
+       int xstride, double* __restrict__ gpart, double* __restrict__ lpart, int GG, int GL, int WC)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int LD = NBT * 8 + 4;
@@ -334,10 +229,137 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
 
     // ---------------------------------------------------------------- loss role
     {
-        constexpr int SB = loss_stage_bytes(NBT);
         constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
-        static_assert(WARPS == 8 || WARPS == 16, "loss role: 8 or 16 warps");
-        bool waited = false;  // the Chebyshev coefficients in XT come from k_xt: griddepcontrol.wait before the first X copy
+        static_assert(WARPS == 8, "loss role: 8 warps (the coefficient pass maps warp <-> member tile)");
+        constexpr int JB = 4;                     // brackets per coefficient pass: 256 threads = JB x 64 members
+        const int N_ = N, Q = t.Q;
+        const bool logm = dk.interp == KX_INTERP_LOG, tab = dk.exp_impl == KX_EXP_TABLE;
+        // shared memory: [A stages | scratch of the coefficient passes] [X window] [dct fragments, nodes, exp2 table]
+        unsigned char* sStage = smem;
+        double* sXw = reinterpret_cast<double*>(smem + (size_t)kLossStages * kLossABytes);          // [WC*16][LD]
+        double* s_afr = sXw + (size_t)WC * 16 * LD;                                                 // [(Q/8)(Q/4)][32]
+        double* s_node = s_afr + (KX_QMAX / 8) * (KX_QMAX / 4) * 32;                                // [QMAX]
+        double* s_tab = s_node + KX_QMAX;                                                           // [256]
+        double* s_G = reinterpret_cast<double*>(smem);                                              // [JB][Q][68] (aliases the stages)
+        if (logm) {
+            for (int k = tid; k < (Q / 8) * (Q / 4) * 32; k += NTHR) {
+                const int ln = k & 31, fr = k >> 5, ct = fr / (Q / 4), ks = fr - ct * (Q / 4);
+                s_afr[k] = t.dct[(8 * ct + (ln >> 2)) * Q + 4 * ks + (ln & 3)];
+            }
+            if (tid < Q) s_node[tid] = t.nodes[tid];
+            if (tab) for (int k = tid; k < (1 << KX_EXP_BITS); k += NTHR) s_tab[k] = dk.exptab[k];
+        }
+        __syncthreads();
+
+        // Chebyshev coefficients a_c(b, j) of the window's k = (j, c) rows, k in [K0, K0 + 16 wn), straight into shared
+        // memory.  LOG: g(omega_q) = 2^(y_j + omega_q (y_(j+1) - y_j)) at the Q
+        // Chebyshev nodes, then the discrete Chebyshev transform as a (Q x Q) x (Q x 8 NBT) product on the tensor pipe;
+        // LINEAR: a_0 = (f_j + f_(j+1))/2, a_1 = (f_(j+1) - f_j)/2.  Also the member statistics (flags) of kx_internal.cuh.
+        auto build_window = [&](unsigned K0, unsigned wn) {
+            const unsigned K1 = K0 + 16u * wn;
+            const int jlo = (int)(K0 / (unsigned)Q);
+            const int jhi = min((int)((K1 - 1u) / (unsigned)Q), N_ - 2);
+            // rows beyond the last bracket are padding: zero
+            {
+                const unsigned kpad = (unsigned)(N_ - 1) * (unsigned)Q;
+                for (unsigned k = max(K0, kpad) + (unsigned)warp; k < K1; k += WARPS)
+                    for (int c2 = lane; c2 < LD; c2 += 32) sXw[(size_t)(k - K0) * LD + c2] = 0.0;
+            }
+            const int jj = tid >> 6, bl = tid & 63;
+            if (!logm) {          // LINEAR: two exact coefficients per bracket, no transform: one flat loop
+                const int total = (jhi - jlo + 1) * 64;
+                for (int i0 = tid; i0 < total; i0 += 8 * NTHR) {          // 16 independent loads in flight per thread
+                    double v0[8], v1[8];
+#pragma unroll
+                    for (int u2 = 0; u2 < 8; ++u2) {
+                        const int idx = i0 + u2 * NTHR, j = jlo + (idx >> 6), bm = idx & 63, b = bcol0 + bm;
+                        const bool ok = idx < total && bm < NBT * 8 && b < B;
+                        v0[u2] = ok ? __ldcg(f + (size_t)b * N_ + j) : 0.0;
+                        v1[u2] = ok ? __ldcg(f + (size_t)b * N_ + j + 1) : 0.0;
+                    }
+#pragma unroll
+                    for (int u2 = 0; u2 < 8; ++u2) {
+                        const int idx = i0 + u2 * NTHR, j = jlo + (idx >> 6), bm = idx & 63;
+                        if (idx < total && bm < NBT * 8) {
+                            const unsigned k = (unsigned)j * 2u;
+                            if (k >= K0 && k < K1) sXw[(size_t)(k - K0) * LD + bm] = 0.5 * (v0[u2] + v1[u2]);
+                            if (k + 1 >= K0 && k + 1 < K1) sXw[(size_t)(k + 1 - K0) * LD + bm] = 0.5 * (v1[u2] - v0[u2]);
+                        }
+                    }
+                }
+                __syncthreads();
+                return;
+            }
+            // the f values of a pass are requested one pass ahead
+            auto fetch = [&](int j0, double& a0, double& a1) {
+                const int j = j0 + jj, b = bcol0 + bl;
+                a0 = 0.0; a1 = 0.0;
+                if (j <= jhi && bl < NBT * 8 && b < B) { a0 = __ldcg(f + (size_t)b * N_ + j); a1 = __ldcg(f + (size_t)b * N_ + j + 1); }
+            };
+            double fnx0, fnx1;
+            fetch(jlo, fnx0, fnx1);
+            for (int j0 = jlo; j0 <= jhi; j0 += JB) {
+                const int j = j0 + jj;
+                const bool valid = j <= jhi && bl < NBT * 8;
+                const int b = bcol0 + bl;
+                const double fj = fnx0, fj1 = fnx1;
+                if (j0 + JB <= jhi) fetch(j0 + JB, fnx0, fnx1);
+                if (valid && b < B) atomicMax(mstat + 2 * b + 1, __double_as_longlong(fmax(fabs(fj), fabs(fj1))));
+                if (valid) {
+                    const double y0 = log2(fmax(fj, dk.f_floor)), y1 = log2(fmax(fj1, dk.f_floor)), dy = y1 - y0;
+                    const double cabs = 0.6931471805599453 * fabs(dy);
+                    // log2 of the bracket's error bound (log2 max_i f_i is subtracted by the consumers); the atomics return
+                    // nothing, so nobody waits for them
+                    if (b < B && cabs > 0.0)
+                        atomicMax(mstat + 2 * b, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
+                    double* g = s_G + (size_t)jj * KX_QMAX * 68 + bl;
+                    if (tab) for (int q = 0; q < Q; ++q) g[q * 68] = kx_exp2_tab<1>(fma(s_node[q], dy, y0), s_tab);
+                    else for (int q = 0; q < Q; ++q) g[q * 68] = exp2(fma(s_node[q], dy, y0));
+                }
+                __syncthreads();
+                // transform: warp w takes member tile w of every bracket of the pass
+                if (warp < NBT) {
+                    // JB x (Q/8) independent accumulator chains: the DMMA latency of one hides behind the others
+                    double D[JB][KX_QMAX / 8][2];
+#pragma unroll
+                    for (int j2 = 0; j2 < JB; ++j2)
+#pragma unroll
+                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[j2][ct][0] = D[j2][ct][1] = 0.0;
+                    const double* g = s_G + (size_t)krow * 68 + 8 * warp + lr;
+#pragma unroll
+                    for (int ks = 0; ks < KX_QMAX / 4; ++ks) {
+                        if (4 * ks < Q) {
+                            double afr[KX_QMAX / 8];
+#pragma unroll
+                            for (int ct = 0; ct < KX_QMAX / 8; ++ct) afr[ct] = 8 * ct < Q ? s_afr[(ct * (Q / 4) + ks) * 32 + lane] : 0.0;
+#pragma unroll
+                            for (int j2 = 0; j2 < JB; ++j2) {
+                                const double gv = g[(size_t)j2 * KX_QMAX * 68 + (4 * ks) * 68];
+#pragma unroll
+                                for (int ct = 0; ct < KX_QMAX / 8; ++ct)
+                                    if (8 * ct < Q) dmma884(D[j2][ct][0], D[j2][ct][1], afr[ct], gv);
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int j2 = 0; j2 < JB; ++j2) {
+                        if (j0 + j2 <= jhi) {
+#pragma unroll
+                            for (int ct = 0; ct < KX_QMAX / 8; ++ct) {
+                                if (8 * ct < Q) {
+                                    const unsigned k = (unsigned)(j0 + j2) * (unsigned)Q + 8u * ct + (unsigned)lr;
+                                    if (k >= K0 && k < K1)
+                                        *reinterpret_cast<double2*>(sXw + (size_t)(k - K0) * LD + 8 * warp + 2 * krow) = make_double2(D[j2][ct][0], D[j2][ct][1]);
+                                }
+                            }
+                        }
+                    }
+                }
+                __syncthreads();
+            }
+            __syncthreads();
+        };
+
         const unsigned cl = blockIdx.x - GG;
         const unsigned LC = (unsigned)t.LC;
         const unsigned U = (unsigned)t.RS * LC;
@@ -351,20 +373,17 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
             const int nb = min(32, t.NR8 - 32 * (int)sp);                // 8-row blocks of this supertile
             const int nbw = min(R8, max(0, nb - R8 * warp));             // ... of this warp
 
-            auto issueA = [&](unsigned kc, int slot) {          // the tensor: does not depend on any kernel of this call
-                unsigned char* dstA = smem + (size_t)slot * SB;
-                const double* srcA = t.AL + ((size_t)kc * t.NR8 + 32 * sp) * 128;
-                for (int k = tid; k < nb * 64; k += NTHR) cp_async16(dstA + (size_t)k * 16, srcA + (size_t)k * 2);
-            };
-            auto issueX = [&](unsigned kc, int slot) {          // the coefficients written by k_xt
-                double* dstX = reinterpret_cast<double*>(smem + (size_t)slot * SB + kLossABytes);
-                const double* srcX = XT + (size_t)(t.loss_row0 + 16 * kc) * xstride + bcol0;
-                for (int k = tid; k < 16 * NBT * 4; k += NTHR) {
-                    const int r = k / (NBT * 4), cc = k - r * (NBT * 4);
-                    cp_async16(dstX + (size_t)r * LD + 2 * cc, srcX + (size_t)r * xstride + 2 * cc);
+            // every warp streams its own rows of the tensor (4 KiB per chunk: 4 eight-row blocks) through a private
+            // cp.async ring: no CTA-wide barrier inside a window
+            unsigned char* wring = sStage + (size_t)warp * (kLossStages * kLossABytes / WARPS);
+            constexpr int kWStage = kLossABytes / WARPS;                  // 4 KiB
+            auto issue = [&](unsigned kc, int slot) {
+                if (nbw > 0) {
+                    const double* srcA = t.AL + ((size_t)kc * t.NR8 + 32 * sp + R8 * warp) * 128;
+                    unsigned char* dstA = wring + (size_t)slot * kWStage;
+                    for (int k = lane; k < nbw * 64; k += 32) cp_async16(dstA + (size_t)k * 16, srcA + (size_t)k * 2);
                 }
             };
-            auto issue = [&](unsigned kc, int slot) { issueA(kc, slot); issueX(kc, slot); };
 
             double acc[R8][NBT][2];
 #pragma unroll
@@ -372,40 +391,40 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
 #pragma unroll
                 for (int bt = 0; bt < NBT; ++bt) acc[r][bt][0] = acc[r][bt][1] = 0.0;
 
-            // prologue: the tensor chunks are requested before the wait on the operand-preparation kernel
+            for (unsigned w0 = 0; w0 < n; w0 += (unsigned)WC) {
+                const unsigned wn = min((unsigned)WC, n - w0), kw = ka + w0;
+                build_window(16u * kw, wn);          // ends with a barrier: the scratch (= the rings) is free again
 #pragma unroll
-            for (int s = 0; s < kLossStages - 1; ++s)
-                if ((unsigned)s < n) issueA(ka + s, s);
-            if (!waited) { kx_pdl_wait(); waited = true; }
+                for (int s2 = 0; s2 < kLossStages - 1; ++s2) {
+                    if ((unsigned)s2 < wn) issue(kw + s2, s2);
+                    cp_async_commit();
+                }
+                for (unsigned it = 0; it < wn; ++it) {
+                    if (it + kLossStages - 1 < wn) issue(kw + it + kLossStages - 1, (int)((it + kLossStages - 1) % kLossStages));
+                    cp_async_commit();
+                    cp_async_wait<kLossStages - 1>();        // chunk `it` of this warp has landed
+                    __syncwarp();
+                    if (nbw > 0) {
+                        const double* sA = reinterpret_cast<const double*>(wring + (size_t)(it % kLossStages) * kWStage) + lane;
+                        const double* sX = sXw + (size_t)(16 * it + krow) * LD + lr;
 #pragma unroll
-            for (int s = 0; s < kLossStages - 1; ++s) {
-                if ((unsigned)s < n) issueX(ka + s, s);
-                cp_async_commit();
-            }
-            for (unsigned it = 0; it < n; ++it) {
-                cp_async_wait<kLossStages - 2>();        // this thread's copies of chunk `it` have landed
-                __syncthreads();                         // everyone's have; everyone is done with chunk it-1
-                if (it + kLossStages - 1 < n) issue(ka + it + kLossStages - 1, (int)((it + kLossStages - 1) % kLossStages));
-                cp_async_commit();
-                if (nbw > 0) {
-                    const double* sA = reinterpret_cast<const double*>(smem + (size_t)(it % kLossStages) * SB) + (size_t)warp * (R8 * 128) + lane;
-                    const double* sX = reinterpret_cast<const double*>(smem + (size_t)(it % kLossStages) * SB + kLossABytes) + (size_t)krow * LD + lr;
+                        for (int q = 0; q < 4; ++q) {
+                            double xv[NBT];
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        double xv[NBT];
+                            for (int bt = 0; bt < NBT; ++bt) xv[bt] = sX[(size_t)(4 * q) * LD + 8 * bt];
 #pragma unroll
-                        for (int bt = 0; bt < NBT; ++bt) xv[bt] = sX[(size_t)(4 * q) * LD + 8 * bt];
+                            for (int r = 0; r < R8; ++r) {
+                                const double w = sA[(r * 4 + q) * 32];
 #pragma unroll
-                        for (int r = 0; r < R8; ++r) {
-                            const double w = sA[(r * 4 + q) * 32];
-#pragma unroll
-                            for (int bt = 0; bt < NBT; ++bt) dmma884(acc[r][bt][0], acc[r][bt][1], xv[bt], w);
+                                for (int bt = 0; bt < NBT; ++bt) dmma884(acc[r][bt][0], acc[r][bt][1], xv[bt], w);
+                            }
                         }
                     }
+                    __syncwarp();                            // the stage is refilled two iterations from now
                 }
+                cp_async_wait<0>();
+                __syncthreads();              // the rings are free again (next window's scratch, next piece)
             }
-            cp_async_wait<0>();
-            __syncthreads();              // the stages are free again for the next piece
 
             double* dst = lpart + ((size_t)(cl + sp) * xstride + bcol0) * 256 + 8 * R8 * warp + 2 * krow;
 #pragma unroll
@@ -416,27 +435,41 @@ k_dmma(KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, con
                         *reinterpret_cast<double2*>(dst + (size_t)(8 * bt + lr) * 256 + 8 * r) = make_double2(acc[r][bt][0], acc[r][bt][1]);
             u = ue;
         }
-        if (!waited) kx_pdl_wait();
     }
 }
 
+constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + ((KX_QMAX / 8) * (KX_QMAX / 4) * 32 + KX_QMAX + (1 << KX_EXP_BITS)) * 8;
+
+// chunks of 16 k whose Chebyshev coefficients a loss CTA keeps in shared memory at a time: its whole share if it fits
+int loss_window(const KxTiled& t, int GL, int nbt)
+{
+    const long long U = (long long)t.RS * t.LC;
+    const long long share = (U + GL - 1) / GL + 1;
+    const long long fit = (long long)((227u * 1024u - kLossFixedBytes) / ((size_t)16 * (nbt * 8 + 4) * 8));
+    long long wc = share < fit ? share : fit;
+    return (int)(wc < 1 ? 1 : wc);
+}
+
 template <int NBT, int WARPS, int STAGES>
-size_t dmma_smem(const KxTiled& t, int N)
+size_t dmma_smem(const KxTiled& t, int N, int WC)
 {
     const size_t gain = (size_t)(((t.NT + 1) * 4 + 15) & ~15) + (size_t)(NBT * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * STAGES * kStageBytes;
-    const size_t loss = (size_t)kLossStages * loss_stage_bytes(NBT);
+    const size_t loss = kLossFixedBytes + (size_t)WC * 16 * (NBT * 8 + 4) * 8;
     return gain > loss ? gain : loss;
 }
 
 template <int NBT, int WARPS, int STAGES>
-cudaError_t launch_dmma_t(const KxTiled& t, int N, unsigned Gtot, int GG, int GL, const double* f, const double* XT, int xstride,
-                          double* gpart, double* lpart, int B, cudaStream_t s)
+cudaError_t launch_dmma_t(const KxDev& d, const KxTiled& t, unsigned Gtot, int GG, int GL, const double* f, long long* mstat,
+                          int xstride, double* gpart, double* lpart, int B, cudaStream_t s)
 {
-    const size_t smem = dmma_smem<NBT, WARPS, STAGES>(t, N);
+    const int WC = loss_window(t, GL, NBT);
+    const size_t smem = dmma_smem<NBT, WARPS, STAGES>(t, d.N, WC);
     cudaError_t e = cudaFuncSetAttribute(k_dmma<NBT, WARPS, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid(GG + GL, (B + NBT * 8 - 1) / (NBT * 8));
-    return kx_launch(k_dmma<NBT, WARPS, STAGES>, grid, dim3(WARPS * 32), smem, s, true, t, N, B, Gtot, f, XT, xstride, gpart, lpart, GG, GL);
+    // first kernel of the call: ordinary launch
+    return kx_launch(k_dmma<NBT, WARPS, STAGES>, grid, dim3(WARPS * 32), smem, s, false, d, t, d.N, B, Gtot, f, mstat, xstride,
+                     gpart, lpart, GG, GL, WC);
 }
 
 // member tiles (of 8) per CTA: limited by the batch and by the shared memory f^T of the gain role needs
@@ -453,7 +486,7 @@ int dmma_nbt(int N, int B)
 
 int kx_dmma_workers(int N, int B) { return kx_dmma_warps(dmma_nbt(N, B)); }
 
-// columns of XT / the partials for a batch of B members: whole 8-member MMA tiles, whole CTA column groups
+// columns of the partials for a batch of B members: whole 8-member MMA tiles, whole CTA column groups
 int kx_xstride(int B)
 {
     if (B <= 8) return 8;
@@ -480,20 +513,13 @@ void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long gro
     *GG = (int)G - gl;
 }
 
-cudaError_t kx_launch_xt(const KxDev& d, const KxTiled& t, const double* f, double* yd, double* XT, int xstride,
-                         long long* mstat, int B, cudaStream_t s)
-{
-    // first kernel of the call: ordinary launch
-    return kx_launch(k_xt, dim3(d.N), dim3(256), 0, s, false, d, t, f, reinterpret_cast<double2*>(yd), XT, xstride, mstat, B);
-}
-
 cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
-                           const double* XT, int xstride, double* gpart, double* lpart, int B, cudaStream_t s)
+                           long long* mstat, int xstride, double* gpart, double* lpart, int B, cudaStream_t s)
 {
     switch (dmma_nbt(d.N, B)) {
-        case 1: return launch_dmma_t<1, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
-        case 2: return launch_dmma_t<2, 8, 8>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
-        case 4: return launch_dmma_t<4, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
-        default: return launch_dmma_t<8, 8, 4>(t, d.N, (unsigned)groups, GG, GL, f, XT, xstride, gpart, lpart, B, s);
+        case 1: return launch_dmma_t<1, 8, 8>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
+        case 2: return launch_dmma_t<2, 8, 8>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
+        case 4: return launch_dmma_t<4, 8, 4>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
+        default: return launch_dmma_t<8, 8, 4>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
     }
 }

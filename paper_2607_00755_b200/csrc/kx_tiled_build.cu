@@ -12,7 +12,8 @@
 //     2 (|ln(f_(j+1)/f_j)| / 4)^Q / Q! * max(f_j, f_(j+1))
 // so sum_e W_e g(omega_e) = sum_c a_c M_c(i,j) up to that bound: N^3 B exponentials become an N^2 Q B contraction.
 // Brackets whose bound is not negligible are evaluated exactly by the streaming kernel (kx_contract.cu); the
-// decision is taken per member in k_xt (kx_tiled.cu).  LINEAR interpolation is the exact case Q = 2.
+// decision is taken per member from the statistics the loss role of k_dmma accumulates (kx_tiled.cu).  LINEAR
+// interpolation is the exact case Q = 2.
 //
 // Compiled with --fmad=false; fused multiply-adds are explicit.
 #include "kx_internal.cuh"
@@ -100,7 +101,7 @@ __global__ void __launch_bounds__(256) k_pack_gain(KxDev d, KxTiled t)
         const unsigned q = w >> 1;
         const int rb = (int)(w & 1u);
         double W = 0.0;
-        unsigned desc = (unsigned)t.ones_row << 20;   // padding quad: X row 0 scaled by the ones row, A = 0
+        unsigned desc = (unsigned)N << 20;            // padding quad: f_m columns 0..3 scaled by the ones column N, A = 0
         if (q < tq) {
             int lo = 0, hi = N - 1;                   // the run: off[n] <= q < off[n+1]
             while (lo < hi) {
