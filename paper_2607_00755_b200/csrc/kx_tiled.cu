@@ -231,7 +231,10 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
     {
         constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
         static_assert(WARPS == 8, "loss role: 8 warps (the coefficient pass maps warp <-> member tile)");
-        constexpr int JB = 4;                     // brackets per coefficient pass: 256 threads = JB x 64 members
+        constexpr int MB = NBT * 8;               // members of this CTA
+        // brackets per coefficient pass: 256 threads = JB brackets x MB members, as many as the scratch holds at Q = 32
+        constexpr int JB = NBT == 1 ? 16 : 256 / MB;
+        constexpr int GS = MB + 4;                // row stride of the node values: 4 mod 8, conflict-free fragment reads
         const int N_ = N, Q = t.Q;
         const bool logm = dk.interp == KX_INTERP_LOG, tab = dk.exp_impl == KX_EXP_TABLE;
         // shared memory: [A stages | scratch of the coefficient passes] [X window] [dct fragments, nodes, exp2 table]
@@ -240,7 +243,8 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
         double* s_afr = sXw + (size_t)WC * 16 * LD;                                                 // [(Q/8)(Q/4)][32]
         double* s_node = s_afr + (KX_QMAX / 8) * (KX_QMAX / 4) * 32;                                // [QMAX]
         double* s_tab = s_node + KX_QMAX;                                                           // [256]
-        double* s_G = reinterpret_cast<double*>(smem);                                              // [JB][Q][68] (aliases the stages)
+        double* s_G = reinterpret_cast<double*>(smem);                                              // [JB][Q][GS] (aliases the stages)
+        static_assert((size_t)JB * KX_QMAX * GS * 8 <= (size_t)kLossStages * kLossABytes, "coefficient scratch must fit the stages");
         if (logm) {
             for (int k = tid; k < (Q / 8) * (Q / 4) * 32; k += NTHR) {
                 const int ln = k & 31, fr = k >> 5, ct = fr / (Q / 4), ks = fr - ct * (Q / 4);
@@ -265,22 +269,22 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
                 for (unsigned k = max(K0, kpad) + (unsigned)warp; k < K1; k += WARPS)
                     for (int c2 = lane; c2 < LD; c2 += 32) sXw[(size_t)(k - K0) * LD + c2] = 0.0;
             }
-            const int jj = tid >> 6, bl = tid & 63;
+            const int jj = tid / MB, bl = tid % MB;
             if (!logm) {          // LINEAR: two exact coefficients per bracket, no transform: one flat loop
-                const int total = (jhi - jlo + 1) * 64;
+                const int total = (jhi - jlo + 1) * MB;
                 for (int i0 = tid; i0 < total; i0 += 8 * NTHR) {          // 16 independent loads in flight per thread
                     double v0[8], v1[8];
 #pragma unroll
                     for (int u2 = 0; u2 < 8; ++u2) {
-                        const int idx = i0 + u2 * NTHR, j = jlo + (idx >> 6), bm = idx & 63, b = bcol0 + bm;
-                        const bool ok = idx < total && bm < NBT * 8 && b < B;
+                        const int idx = i0 + u2 * NTHR, j = jlo + idx / MB, bm = idx % MB, b = bcol0 + bm;
+                        const bool ok = idx < total && b < B;
                         v0[u2] = ok ? __ldcg(f + (size_t)b * N_ + j) : 0.0;
                         v1[u2] = ok ? __ldcg(f + (size_t)b * N_ + j + 1) : 0.0;
                     }
 #pragma unroll
                     for (int u2 = 0; u2 < 8; ++u2) {
-                        const int idx = i0 + u2 * NTHR, j = jlo + (idx >> 6), bm = idx & 63;
-                        if (idx < total && bm < NBT * 8) {
+                        const int idx = i0 + u2 * NTHR, j = jlo + idx / MB, bm = idx % MB;
+                        if (idx < total) {
                             const unsigned k = (unsigned)j * 2u;
                             if (k >= K0 && k < K1) sXw[(size_t)(k - K0) * LD + bm] = 0.5 * (v0[u2] + v1[u2]);
                             if (k + 1 >= K0 && k + 1 < K1) sXw[(size_t)(k + 1 - K0) * LD + bm] = 0.5 * (v1[u2] - v0[u2]);
@@ -294,13 +298,13 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
             auto fetch = [&](int j0, double& a0, double& a1) {
                 const int j = j0 + jj, b = bcol0 + bl;
                 a0 = 0.0; a1 = 0.0;
-                if (j <= jhi && bl < NBT * 8 && b < B) { a0 = __ldcg(f + (size_t)b * N_ + j); a1 = __ldcg(f + (size_t)b * N_ + j + 1); }
+                if (jj < JB && j <= jhi && b < B) { a0 = __ldcg(f + (size_t)b * N_ + j); a1 = __ldcg(f + (size_t)b * N_ + j + 1); }
             };
             double fnx0, fnx1;
             fetch(jlo, fnx0, fnx1);
             for (int j0 = jlo; j0 <= jhi; j0 += JB) {
                 const int j = j0 + jj;
-                const bool valid = j <= jhi && bl < NBT * 8;
+                const bool valid = jj < JB && j <= jhi;
                 const int b = bcol0 + bl;
                 const double fj = fnx0, fj1 = fnx1;
                 if (j0 + JB <= jhi) fetch(j0 + JB, fnx0, fnx1);
@@ -312,20 +316,24 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
                     // nothing, so nobody waits for them
                     if (b < B && cabs > 0.0)
                         atomicMax(mstat + 2 * b, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
-                    double* g = s_G + (size_t)jj * KX_QMAX * 68 + bl;
-                    if (tab) for (int q = 0; q < Q; ++q) g[q * 68] = kx_exp2_tab<1>(fma(s_node[q], dy, y0), s_tab);
-                    else for (int q = 0; q < Q; ++q) g[q * 68] = exp2(fma(s_node[q], dy, y0));
+                    double* g = s_G + (size_t)jj * Q * GS + bl;
+                    if (tab) for (int q = 0; q < Q; ++q) g[q * GS] = kx_exp2_tab<1>(fma(s_node[q], dy, y0), s_tab);
+                    else for (int q = 0; q < Q; ++q) g[q * GS] = exp2(fma(s_node[q], dy, y0));
                 }
                 __syncthreads();
-                // transform: warp w takes member tile w of every bracket of the pass
-                if (warp < NBT) {
-                    // JB x (Q/8) independent accumulator chains: the DMMA latency of one hides behind the others
-                    double D[JB][KX_QMAX / 8][2];
+                // transform: a task is (bracket of the pass, member tile); the 8 warps take 32 tasks at a time, 4 each, with
+                // 4 x (Q/8) independent accumulator chains so that the DMMA latency of one hides behind the others
+                for (int base = 0; base < JB * NBT; base += 32) {
+                    double D[4][KX_QMAX / 8][2];
+                    int tj[4], tm[4];
 #pragma unroll
-                    for (int j2 = 0; j2 < JB; ++j2)
+                    for (int u2 = 0; u2 < 4; ++u2) {
+                        const int idx = base + warp + 8 * u2;
+                        tj[u2] = idx < JB * NBT ? idx / NBT : -1;
+                        tm[u2] = idx % NBT;
 #pragma unroll
-                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[j2][ct][0] = D[j2][ct][1] = 0.0;
-                    const double* g = s_G + (size_t)krow * 68 + 8 * warp + lr;
+                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[u2][ct][0] = D[u2][ct][1] = 0.0;
+                    }
 #pragma unroll
                     for (int ks = 0; ks < KX_QMAX / 4; ++ks) {
                         if (4 * ks < Q) {
@@ -333,23 +341,25 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
 #pragma unroll
                             for (int ct = 0; ct < KX_QMAX / 8; ++ct) afr[ct] = 8 * ct < Q ? s_afr[(ct * (Q / 4) + ks) * 32 + lane] : 0.0;
 #pragma unroll
-                            for (int j2 = 0; j2 < JB; ++j2) {
-                                const double gv = g[(size_t)j2 * KX_QMAX * 68 + (4 * ks) * 68];
+                            for (int u2 = 0; u2 < 4; ++u2) {
+                                if (tj[u2] >= 0) {          // uniform over the warp
+                                    const double gv = s_G[((size_t)tj[u2] * Q + 4 * ks + krow) * GS + 8 * tm[u2] + lr];
 #pragma unroll
-                                for (int ct = 0; ct < KX_QMAX / 8; ++ct)
-                                    if (8 * ct < Q) dmma884(D[j2][ct][0], D[j2][ct][1], afr[ct], gv);
+                                    for (int ct = 0; ct < KX_QMAX / 8; ++ct)
+                                        if (8 * ct < Q) dmma884(D[u2][ct][0], D[u2][ct][1], afr[ct], gv);
+                                }
                             }
                         }
                     }
 #pragma unroll
-                    for (int j2 = 0; j2 < JB; ++j2) {
-                        if (j0 + j2 <= jhi) {
+                    for (int u2 = 0; u2 < 4; ++u2) {
+                        if (tj[u2] >= 0 && j0 + tj[u2] <= jhi) {
 #pragma unroll
                             for (int ct = 0; ct < KX_QMAX / 8; ++ct) {
                                 if (8 * ct < Q) {
-                                    const unsigned k = (unsigned)(j0 + j2) * (unsigned)Q + 8u * ct + (unsigned)lr;
+                                    const unsigned k = (unsigned)(j0 + tj[u2]) * (unsigned)Q + 8u * ct + (unsigned)lr;
                                     if (k >= K0 && k < K1)
-                                        *reinterpret_cast<double2*>(sXw + (size_t)(k - K0) * LD + 8 * warp + 2 * krow) = make_double2(D[j2][ct][0], D[j2][ct][1]);
+                                        *reinterpret_cast<double2*>(sXw + (size_t)(k - K0) * LD + 8 * tm[u2] + 2 * krow) = make_double2(D[u2][ct][0], D[u2][ct][1]);
                                 }
                             }
                         }
