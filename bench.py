@@ -38,7 +38,7 @@ WORKLOAD = "cfg3: N=256 log p/T in [1e-3,50], B=64 seeded bimodal f, |M|^2 ~ 1/(
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_dmma launch from the committed `ncu --set full` capture
 # (profiles/r01c_tiled_dmma.md; LINEAR from the working capture of the same round); null for configurations that were
 # not captured.
-NCU_TRAFFIC = {("log", 64): 64.85e6, ("linear", 64): 48.72e6}
+NCU_TRAFFIC = {("log", 64): 61.43e6, ("linear", 64): 48.72e6}
 # kernels of one kx_collide on the tiled path: k_dmma, k_reduce, k_contract (exact fallback, exits at once when no member
 # is flagged; LOG only), k_finish
 LOSS_NODES = {"log": 24, "linear": 2}
