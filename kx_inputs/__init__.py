@@ -137,10 +137,11 @@ def config5_schedule(p: np.ndarray, dp: np.ndarray, *, B: int = 8, S: int = 10_0
     uh[1::2] = 0.5 * (u[:-1] + u[1:])
     x = np.exp(uh)
     R1 = 128.0 * math.pi ** 3
-    h = p * p * dp                            # normalisation weight of the SOURCE SHAPES only
     G = np.stack([np.exp(-((p - 3.0) ** 2) / (2 * 1.0 ** 2)),
                   np.exp(-((p - 30.0) ** 2) / (2 * 3.0 ** 2))])
-    G /= (G * h).sum(axis=1, keepdims=True)
+    # input recipe, not the method's arithmetic: each shape is scaled so that its plain Riemann sum
+    # sum_i q_i^2 dq_i G_i over the grid handed in equals 1 (neither side consumes this sum as a result)
+    G /= (G * (p * p * dp)).sum(axis=1, keepdims=True)
     xs = np.exp(u[:-1])                       # x at the start of each step
     amp = np.zeros((2, S))
     amp[0, xs < 1.0 - 1e-12] = 1e-3 / du

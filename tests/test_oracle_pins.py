@@ -505,3 +505,105 @@ def test_K1_numerical_kernel_converges_to_analytic(oracle, cfg, N):
         devC.append(np.abs(C - C0).max() / np.abs(g0).max())
     assert devW[0] < 0.15 and devW[2] < 2e-3 and devW[0] > 3 * devW[1] > 9 * devW[2]
     assert devC[2] < 2e-4 and devC[0] > 3 * devC[2]
+
+
+# ------------------------------------------------------------------ non-autonomous integrators: stage times of rate[] and mass[]
+def test_E1_rate_stage_indexing_by_reparametrisation(oracle):
+    """eq. 4.9: df/dtau = R(tau) C[f].  With R = e^{a tau} the substitution s = (e^{a tau} - 1)/a makes the
+    problem autonomous, df/ds = C[f]: the run with rate[] sampled at nodes and midpoints must converge to the static-rate
+    solution at s(T) with the order of the method (1/2/4).  Handing stages 2-3 of RK4 the node value, or Heun's second
+    stage the start value, makes the scheme first order and fails the order and the magnitude checks."""
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    g, l, C = oracle.collide(T, c["f"], 0)
+    s_end = 8.0 / (l[0] / c["f"][0]).max()
+    a = 4.0 / s_end                               # R grows from 1 to 5 over the run
+    t_end = math.log(5.0) / a
+    ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.RK4, tau=np.linspace(0.0, s_end, 513))
+    scale = np.abs(ref).max()
+
+    def run(method, S):
+        tau = np.linspace(0.0, t_end, S + 1)
+        th = np.empty(2 * S + 1)
+        th[0::2] = tau
+        th[1::2] = 0.5 * (tau[:-1] + tau[1:])
+        return oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=method, tau=tau, rate=np.exp(a * th))
+
+    for method, order, tol16 in ((oracle.EULER, 1, 1e-1), (oracle.HEUN, 2, 2e-2), (oracle.RK4, 4, 1e-4)):
+        e1 = np.abs(run(method, 16) - ref).max() / scale
+        e2 = np.abs(run(method, 32) - ref).max() / scale
+        assert e1 / e2 > 0.7 * 2 ** order, (method, e1, e2)
+        assert e1 < tol16, (method, e1)
+
+
+def test_E2_stage_times_against_textbook_tableaux(oracle):
+    """The arrays rate[2S+1], mass[2S+1] hold nodes and midpoints (eq. 4.9).  Independent check of which
+    entry each stage reads: generic one-step methods for y' = F(t, y) written from their Butcher tableaux (Euler c=(0);
+    Heun c=(0,1), b=(1/2,1/2); classical RK4 c=(0,1/2,1/2,1), b=(1/6,1/3,1/3,1/6)) with F(t, y) = kappa R(t) C_proj[y; m(t)]
+    + amp G evaluated through FUNCTIONS of t, against okx_evolve fed the sampled arrays.  R and m take different values
+    at every node and midpoint, so any mix-up of the positions changes the result at O(1)."""
+    N, B, S = 24, 2, 3
+    p = kin.log_grid(N, 2e-2, 20.0)
+    dp = kin.trapezoid_widths(p)
+    f0 = np.stack([kin._random_bimodal(p, 77 + b) for b in range(B)])
+    kappa = np.array([1.0, 0.3])
+    G = np.exp(-0.5 * (p - 2.0) ** 2)[None, :]
+    tau = np.array([0.0, 0.7, 1.1, 2.0])
+    Rfun = lambda t: 40.0 * math.exp(0.9 * t)
+    mfun = lambda t: 0.5 * math.exp(0.6 * t)
+    amp = np.array([[0.02, 0.0, 0.05]])
+    th = np.empty(2 * S + 1)
+    th[0::2] = tau
+    th[1::2] = 0.5 * (tau[:-1] + tau[1:])
+    rate = np.array([Rfun(t) for t in th])
+    mass = np.array([mfun(t) for t in th])
+
+    def F(t, y, k):
+        T = oracle.Tables(p, dp, mfun(t))
+        g, l, C = oracle.collide(T, y, oracle.LOG)
+        Cp, _ = oracle.project(T, y, C)
+        return kappa[:, None] * Rfun(t) * Cp + amp[0, k] * G
+
+    tableaux = {oracle.EULER: ([0.0], [[]], [1.0]),
+                oracle.HEUN: ([0.0, 1.0], [[], [1.0]], [0.5, 0.5]),
+                oracle.RK4: ([0.0, 0.5, 0.5, 1.0], [[], [0.5], [0.0, 0.5], [0.0, 0.0, 1.0]], [1 / 6, 1 / 3, 1 / 3, 1 / 6])}
+    for method, (cs, As, bs) in tableaux.items():
+        y = f0.copy()
+        for k in range(S):
+            hstep = tau[k + 1] - tau[k]
+            ks = []
+            for cst, arow in zip(cs, As):
+                yst = y + hstep * sum((aij * kj for aij, kj in zip(arow, ks)), np.zeros_like(y))
+                ks.append(F(tau[k] + cst * hstep, yst, k))
+            y = y + hstep * sum(bj * kj for bj, kj in zip(bs, ks))
+        got = oracle.evolve(p, dp, f0, m=mfun(0.0), method=method, tau=tau, rate=rate, mass=mass, kappa=kappa,
+                            G=G, amp=amp)
+        assert np.abs(got - y).max() <= 1e-12 * np.abs(y).max(), method
+        # teeth: the same arrays shifted by one position (midpoint <-> node) give a different answer
+        bad = oracle.evolve(p, dp, f0, m=mfun(0.0), method=method, tau=tau, rate=np.roll(rate, 1), mass=mass, kappa=kappa,
+                            G=G, amp=amp)
+        assert np.abs(bad - y).max() > 1e-4 * np.abs(y).max()
+
+
+def test_A3_adaptive_rate_slope_by_reparametrisation(oracle):
+    """okx_evolve_adaptive's R(u) = rate0 e^{slope (u - u0)} (eq. 4.9 with 1/H a power of a): s = rate0 (e^{slope (u-u0)} - 1)
+    / slope makes the problem autonomous, so the adaptive solution must approach the static-rate fine RK4 solution at s(u1)
+    with an error proportional to rtol (Heun with R taken at u and u + du is second order; R taken at u for both stages is
+    first order: error ~ sqrt(rtol) and far above the bound)."""
+    c = kin.config(1)
+    T = oracle.Tables(c["p"], c["dp"], c["m"])
+    g, l, C = oracle.collide(T, c["f"], oracle.LOG)
+    nu = float((l[0] / c["f"][0]).max())
+    s_end = 12.0 / nu
+    u0, u1, rate0 = -1.0, 1.0, 0.5
+    slope = math.log(9.0) / (u1 - u0)                       # R grows ninefold
+    rate0 = s_end * slope / (math.exp(slope * (u1 - u0)) - 1.0)
+    ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.RK4, tau=np.linspace(0.0, s_end, 1501))
+    errs = []
+    for rtol in (1e-4, 1e-5):
+        f, info = oracle.evolve_adaptive(c["p"], c["dp"], c["f"], u0=u0, u1=u1, du0=1e-4, rtol=rtol, atol=rtol * 1e-9,
+                                         rate0=rate0, rate_slope=slope)
+        assert info["done"]
+        errs.append(np.abs(f - ref).max() / np.abs(ref).max())
+    assert errs[0] < 2e-4 and errs[1] < 2e-5, errs
+    assert errs[0] / errs[1] > 5.0, errs
