@@ -14,16 +14,24 @@
  *   time stepping     df/dtau = kappa_b R(tau) C^proj[f; m(tau)] + sum_s amp_s G_s   eq. 4.9
  *
  * Conventions
- *   - Every function returns kx_status_t (KX_OK = 0).  No exceptions, no abort(), no global state.
- *     kx_last_error(h) returns a handle-owned, NUL-terminated description of the last failure.
+ *   - Every function returns kx_status_t (KX_OK = 0).  No exceptions, no abort(), no state shared between handles.
+ *     kx_last_error(h) returns a handle-owned, NUL-terminated description of the last failure; kx_last_error(NULL)
+ *     returns the calling thread's last kx_build failure (thread-local: there is no handle to own it).
  *   - Pointers are marked HOST or DEVICE.  DEVICE pointers are caller-owned allocations on the
  *     handle's device (e.g. torch.Tensor.data_ptr()), 16-byte aligned, row-major [B,N] fp64.
  *     HOST arrays are read during the call and may be freed afterwards.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  kx_collide*,
- *     kx_moments and kx_set_mass only enqueue work on it and return without synchronising, except
- *     that the first call with a larger batch B than seen before grows the handle's workspace
- *     (cudaMalloc, implicit sync).  kx_build, kx_evolve, kx_evolve_adaptive, kx_collide_host and kx_tensor_export
+ *     kx_moments and kx_set_mass only enqueue work on it and return without synchronising, with two
+ *     exceptions: (1) the first call with a larger batch B than seen before grows the handle's workspace
+ *     (cudaMalloc, implicit sync) -- kx_reserve(h, B) does that ahead of time; (2) on a KX_STORE_TILED handle
+ *     the first kx_collide* / kx_evolve* after kx_set_mass (or after a mass-schedule kx_evolve) rebuilds the
+ *     tiled operand, which synchronises the stream and may reallocate it; the first kx_set_mass itself
+ *     synchronises and reallocates the row storage to N^2 (N+1)/2 entries (every triple may be kept at
+ *     another mass).  kx_build, kx_evolve, kx_evolve_adaptive, kx_collide_host and kx_tensor_export
  *     synchronise the stream before returning.
+ *   - One operator evaluation is one cooperative kernel launch (all of its CTAs are resident at once and
+ *     meet at a grid barrier); run other work on the same device in the same stream or expect it to
+ *     serialise with the evaluation.
  *   - The handle owns the kernel tensor and all workspaces.  One host thread at a time per handle.
  *   - There is no CPU fallback: every entry point fails with KX_ERR_CUDA when no sm_100 device
  *     is usable.
@@ -41,10 +49,10 @@ typedef struct kx_handle_s* kx_handle_t;
 
 typedef enum {
     KX_OK = 0,
-    KX_ERR_INVALID_ARG = 1,   /* null pointer, N<4 or N>1024, non-monotone grid, dp<=0, B<1, misaligned pointer */
+    KX_ERR_INVALID_ARG = 1,   /* null pointer, N<4, non-monotone grid, dp<=0, B<1, misaligned pointer */
     KX_ERR_ALLOC = 2,         /* host or device allocation failed */
     KX_ERR_CUDA = 3,          /* CUDA runtime error (message in kx_last_error) */
-    KX_ERR_UNSUPPORTED = 4,   /* option not implemented (fp32 mode) */
+    KX_ERR_UNSUPPORTED = 4,   /* option not implemented (fp32 mode); N > 1024 (n, m, j_L are packed 10 bits each) */
     KX_ERR_NONFINITE = 5      /* kx_evolve produced a NaN/Inf in f */
 } kx_status_t;
 
@@ -212,11 +220,27 @@ kx_status_t kx_tensor_export(kx_handle_t h, int64_t cap, int64_t* rowptr, double
 /* Copy the device kinematics to HOST arrays of length N (any may be NULL): E_i, K_i, h_i. */
 kx_status_t kx_kinematics_export(kx_handle_t h, double* E, double* K, double* hw);
 
-/* Measurement aid (bench.py): while enabled, every launch of the contraction kernel (a4/a5, the dominant kernel)
+/* Allocate the workspaces, the task table and (KX_STORE_TILED) the launch plan for batches of up to B members now, so
+ * that later kx_collide* calls with B' <= B only enqueue work (no cudaMalloc, no synchronisation). */
+kx_status_t kx_reserve(kx_handle_t h, int32_t B, void* stream);
+
+/* KX_STORE_TILED + LOG: number of (member, evaluation) pairs that took the exact fallback (their Chebyshev error bound
+ * was not negligible, or f held an Inf/NaN) since the last call; resets the counter.  Synchronises the device. */
+kx_status_t kx_fallback_members(kx_handle_t h, int64_t* count);
+
+/* Measurement aid (bench.py): while enabled, every launch of the evaluation kernel (a4-a8, the dominant kernel)
  * is bracketed by two CUDA events recorded on the caller's stream.  kx_profile_read synchronises the device,
  * returns the summed kernel time in milliseconds and the number of launches since the last read, and resets. */
 kx_status_t kx_profile(kx_handle_t h, int32_t enable);
 kx_status_t kx_profile_read(kx_handle_t h, double* contract_ms, int64_t* launches);
+
+/* Measurement aid (bench.py): while enabled, the evaluation kernel writes %globaltimer stamps (ns) of its phases, one
+ * row of 32 slots per CTA (160 rows): 0 entry, 1 prologue done, 2 partials written, 3 grid barrier passed, 4 exact
+ * fallback done, 5 finishing phase done, 8..15 end of each gain warp's stream (tensor-core path).  kx_trace_read copies
+ * the stamps of the launches since the last read (later launches overwrite earlier ones) to HOST stamps[160*32],
+ * zero = not written, and clears them.  Synchronises the device. */
+kx_status_t kx_trace(kx_handle_t h, int32_t enable);
+kx_status_t kx_trace_read(kx_handle_t h, uint64_t* stamps);
 
 /* Measurement aid (bench.py): peak FP64 throughput of `device` in TFLOP/s, register-resident chains without memory
  * traffic.  kind 0 = DFMA (plain FP64 pipe), 1 = DMMA.8x8x4 (FP64 tensor pipe, the instruction of the tiled

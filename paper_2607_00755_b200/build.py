@@ -14,10 +14,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkx.so")
 SOURCES = ["kx_api.cu", "kx_build.cu", "kx_contract.cu", "kx_tiled_build.cu", "kx_tiled.cu", "kx_probe.cu"]
-HEADERS = [os.path.join(CSRC, "kx_internal.cuh"), os.path.join(CSRC, "kx_entry.cuh"), os.path.join(HERE, "..", "include", "kx.h")]
+HEADERS = [os.path.join(CSRC, "kx_internal.cuh"), os.path.join(CSRC, "kx_entry.cuh"), os.path.join(CSRC, "kx_device.cuh"), os.path.join(HERE, "..", "include", "kx.h")]
 # --fmad=false: validity decisions, omega and the Runge-Kutta updates must not depend on implicit FMA
 # contraction; the hot loops call fma() explicitly.
-NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+NVCC_FLAGS = ["-O3", "-std=c++17", "--threads", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--fmad=false", "-Xcompiler", "-fPIC", "-shared"]
 
 

@@ -9,7 +9,7 @@
 
 namespace {
 
-std::string g_build_err;
+thread_local std::string g_build_err;     // last kx_build failure of the calling thread (there is no handle yet)
 
 struct DeviceGuard {
     int prev = -1;
@@ -61,35 +61,24 @@ kx_status_t alloc_tiled(kx_handle_s* h, long long groups)
     return KX_OK;
 }
 
-// upper bound of the groups of the tiled storage for ANY mass: every (n <= m) pair in every tile
-inline long long tiled_groups_bound(const kx_handle_s* h)
-{
-    const long long N = h->d.N, NT = h->t.NT;
-    const long long quads_per_tile = (N * (N + 1) / 2 + 3) / 4 + N;     // each run rounds up by < 1 quad
-    return NT * ((quads_per_tile + 3) / 4);
-}
-
-// a2-a3 in the tiled layout for the current kinematics (the run table of kx_launch_runs must be current)
-kx_status_t build_tiled(kx_handle_s* h, cudaStream_t s, bool may_sync)
+// a2-a3 in the tiled layout for the current kinematics (the run table of kx_launch_runs must be current).
+// Synchronises the stream (the group count decides the allocation) and may reallocate the gain operand.
+kx_status_t build_tiled(kx_handle_s* h, cudaStream_t s)
 {
     KX_CUDA(kx_launch_tile_runs(h->d, h->t, s));
-    if (may_sync) {
-        unsigned g = 0;
-        KX_CUDA(cudaMemcpyAsync(&g, h->t.vtptr + h->t.NT, 4, cudaMemcpyDeviceToHost, s));
-        KX_CUDA(cudaStreamSynchronize(s));
-        h->groups = g;
-        if (h->cap_groups < (long long)g) {
-            kx_status_t rc = alloc_tiled(h, g);
-            if (rc != KX_OK) return rc;
-        }
-    } else if (h->cap_groups < tiled_groups_bound(h)) {
-        h->err = "internal: tiled capacity too small for an asynchronous rebuild";
-        return KX_ERR_ALLOC;
+    h->vt_host.assign((size_t)h->t.NT + 1, 0u);
+    KX_CUDA(cudaMemcpyAsync(h->vt_host.data(), h->t.vtptr, ((size_t)h->t.NT + 1) * 4, cudaMemcpyDeviceToHost, s));
+    KX_CUDA(cudaStreamSynchronize(s));
+    const unsigned g = h->vt_host[h->t.NT];
+    h->groups = g;
+    if (h->cap_groups < (long long)g) {
+        kx_status_t rc = alloc_tiled(h, g);
+        if (rc != KX_OK) return rc;
     }
-    const long long used = may_sync ? h->groups : h->cap_groups;
-    KX_CUDA(cudaMemsetAsync(h->t.A, 0, (size_t)used * KX_GROUP_DBL * 8, s));
+    KX_CUDA(cudaMemsetAsync(h->t.A, 0, (size_t)h->groups * KX_GROUP_DBL * 8, s));
     KX_CUDA(kx_launch_tile_fill(h->d, h->t, s));
     h->tiled_ok = true;
+    h->plan_B = 0;
     return KX_OK;
 }
 
@@ -97,9 +86,9 @@ void free_ws(kx_handle_s* h)
 {
     cudaFree(h->yd); cudaFree(h->part); cudaFree(h->fstage); cudaFree(h->k1); cudaFree(h->k2);
     cudaFree(h->k3); cudaFree(h->Cbuf); cudaFree(h->hostio);
-    cudaFree(h->mstat); cudaFree(h->gpart); cudaFree(h->lpart); cudaFree(h->gn);
+    cudaFree(h->mstat); cudaFree(h->gpart); cudaFree(h->lpart);
     h->yd = h->part = h->fstage = h->k1 = h->k2 = h->k3 = h->Cbuf = h->hostio = nullptr;
-    h->gpart = h->lpart = h->gn = nullptr; h->mstat = nullptr;
+    h->gpart = h->lpart = nullptr; h->mstat = nullptr;
     h->wsB = 0; h->ws_tasks = 0; h->ws_xstride = 0;
 }
 
@@ -123,16 +112,16 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
     KX_CUDA(dalloc(&h->hostio, bn * 2));
     if (h->storage == KX_STORE_TILED) {
         const int xs = kx_xstride(nB);
-        KX_CUDA(dalloc(&h->mstat, (size_t)nB * 2));
+        KX_CUDA(dalloc(&h->mstat, (size_t)nB * 4));           // two buffers, used alternately (launch parity)
         {
-            std::vector<long long> init((size_t)nB * 2);
-            for (int b = 0; b < nB; ++b) { init[2 * b] = (-0x7fffffffffffffffLL - 1); init[2 * b + 1] = 0; }
+            std::vector<long long> init((size_t)nB * 4);
+            for (int b = 0; b < 2 * nB; ++b) { init[2 * b] = (-0x7fffffffffffffffLL - 1); init[2 * b + 1] = 0; }
             KX_CUDA(cudaMemcpy(h->mstat, init.data(), init.size() * 8, cudaMemcpyHostToDevice));
         }
-        KX_CUDA(dalloc(&h->gpart, (size_t)(16 * h->sm_count + h->t.NT + 1) * xs * 16));
+        KX_CUDA(dalloc(&h->gpart, (size_t)(h->sm_count + h->t.NT + 1) * xs * 16));
         KX_CUDA(dalloc(&h->lpart, (size_t)(h->sm_count + h->t.RS + 1) * xs * 256));
-        KX_CUDA(dalloc(&h->gn, bn * 2));
         h->ws_xstride = xs;
+        h->plan_B = 0;
     }
     h->wsB = nB; h->ws_tasks = need_tasks;
     return KX_OK;
@@ -178,15 +167,14 @@ kx_status_t rebuild(kx_handle_s* h, double m, cudaStream_t s)
 kx_status_t ensure_tiled(kx_handle_s* h, cudaStream_t s)
 {
     if (h->storage != KX_STORE_TILED || h->tiled_ok) return KX_OK;
-    return build_tiled(h, s, true);
+    return build_tiled(h, s);
 }
 
-// one evaluation of a4-a5 into the partial buffers; returns through *st the fields the finishing kernel needs
-kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bool use_tiled, KxStage* st,
-                        cudaStream_t s)
+// One operator evaluation (a4-a8) = ONE cooperative kernel: the caller has filled the outputs and the Runge-Kutta fields
+// of *st; this adds the path's buffers, the barrier epoch and the trace pointer and launches.
+kx_status_t launch_step(kx_handle_s* h, const double* f, int B, bool have_yd, bool use_tiled, KxStage* st, cudaStream_t s)
 {
-    auto prof_begin = [&]() -> kx_status_t {
-        if (!h->profiling) return KX_OK;
+    if (h->profiling) {
         if (h->prof_used == h->prof_events.size()) {
             cudaEvent_t a, b;
             KX_CUDA(cudaEventCreate(&a));
@@ -194,34 +182,35 @@ kx_status_t launch_eval(kx_handle_s* h, const double* f, int B, bool have_yd, bo
             h->prof_events.emplace_back(a, b);
         }
         KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].first, s));
-        return KX_OK;
-    };
-    auto prof_end = [&]() -> kx_status_t {
-        if (!h->profiling) return KX_OK;
+    }
+    st->part = h->part;
+    st->bar = h->bar;
+    st->fb_count = h->bar + 2;
+    h->epoch += 2;                   // two barrier epochs per launch
+    st->epoch = h->epoch;
+    st->trace = h->tracing ? h->trace : nullptr;
+    if (use_tiled) {
+        if (h->plan_B != B) {
+            kx_dmma_plan(h->d, h->t, h->sm_count, h->vt_host.data(), B, &h->plan);
+            h->plan_B = B;
+        }
+        const int par = (int)((h->epoch >> 1) & 1u);
+        st->gpart = h->gpart; st->lpart = h->lpart; st->xstride = h->ws_xstride;
+        st->mstat = nullptr; st->mstat_next = nullptr; st->mstat_cap = 0;
+        if (h->d.interp == KX_INTERP_LOG) {      // LINEAR is exact: no statistics, no fallback
+            st->mstat = h->mstat + (size_t)par * h->wsB * 2;
+            st->mstat_next = h->mstat + (size_t)(1 - par) * h->wsB * 2;
+            st->mstat_cap = h->wsB;
+        }
+        st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS;
+        KX_CUDA(kx_launch_dmma(h->d, h->t, h->plan, f, B, *st, s));
+    } else {
+        st->gpart = nullptr; st->lpart = nullptr; st->mstat = nullptr; st->mstat_next = nullptr;
+        KX_CUDA(kx_launch_stream(h->d, h->sm_count, f, have_yd ? h->yd : nullptr, B, *st, s));
+    }
+    if (h->profiling) {
         KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].second, s));
         h->prof_used++;
-        return KX_OK;
-    };
-    kx_status_t rc;
-    if (use_tiled) {
-        const int xs = h->ws_xstride;
-        kx_dmma_split(h->d, h->t, h->sm_count, h->groups, B, &h->GG, &h->GL);
-        if ((rc = prof_begin()) != KX_OK) return rc;
-        KX_CUDA(kx_launch_dmma(h->d, h->t, h->groups, h->GG, h->GL, f, h->mstat, xs, h->gpart, h->lpart, B, s));
-        if ((rc = prof_end()) != KX_OK) return rc;
-        // exact streaming path for flagged members only (LINEAR is exact): launched by kx_launch_finish after k_reduce,
-        // so that its launch and its flag check hide behind the reduction instead of following the contraction
-        st->fb_f = nullptr;
-        if (h->d.interp == KX_INTERP_LOG) { st->fb_sm_count = h->sm_count; st->fb_f = f; st->fb_yd = nullptr; st->fb_part = h->part; }
-        st->gpart = h->gpart; st->lpart = h->lpart; st->gn = reinterpret_cast<double2*>(h->gn); st->vtptr = h->t.vtptr;
-        st->mstat = h->d.interp == KX_INTERP_LOG ? h->mstat : nullptr;
-        st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS; st->GW = kx_dmma_workers(h->d.N, B) * h->GG; st->GL = h->GL; st->xstride = xs;
-    } else {
-        if (!have_yd) KX_CUDA(kx_launch_prep(h->d, f, h->yd, B, s));
-        if ((rc = prof_begin()) != KX_OK) return rc;
-        KX_CUDA(kx_launch_contract(h->d, h->sm_count, f, h->yd, h->part, B, nullptr, !have_yd, s));
-        if ((rc = prof_end()) != KX_OK) return rc;
-        st->gpart = nullptr; st->lpart = nullptr; st->gn = nullptr; st->vtptr = nullptr; st->mstat = nullptr;
     }
     return KX_OK;
 }
@@ -243,12 +232,10 @@ kx_status_t collide_impl(kx_handle_s* h, const double* f, double* C, double* gai
     if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
     if ((rc = ensure_tiled(h, s)) != KX_OK) return rc;
     KxStage st = {};
-    if ((rc = launch_eval(h, f, B, false, h->storage == KX_STORE_TILED, &st, s)) != KX_OK) return rc;
     st.flags = flags & KX_PROJECT;
     st.C = C; st.gain = gain; st.loss = loss; st.diag = diag; st.diag_stride = 4;
     st.evolve = 0;
-    KX_CUDA(kx_launch_finish(h->d, f, h->part, B, st, s));
-    return KX_OK;
+    return launch_step(h, f, B, false, h->storage == KX_STORE_TILED, &st, s);
 }
 
 }  // namespace
@@ -271,6 +258,8 @@ void kx_destroy(kx_handle_t h)
         cudaFree(h->tiled_blob);
         cudaFree(h->t.AL);
         cudaFree(h->adapt);
+        cudaFree(h->bar);
+        cudaFree(h->trace);
         cudaFree(h->gl);
         for (auto& ev : h->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     }
@@ -283,7 +272,8 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     if (out) *out = nullptr;
     if (!grid || !sp || !msq || !out || !grid->p || !grid->dp) { g_build_err = "null argument"; return KX_ERR_INVALID_ARG; }
     const int N = grid->n;
-    if (N < 4 || N > KX_MAX_N) { g_build_err = "N must be in [4, 1024]"; return KX_ERR_INVALID_ARG; }
+    if (N < 4) { g_build_err = "N must be at least 4"; return KX_ERR_INVALID_ARG; }
+    if (N > KX_MAX_N) { g_build_err = "N > 1024 is not supported (n, m, j_L are packed 10 bits each)"; return KX_ERR_UNSUPPORTED; }
     for (int i = 0; i < N; ++i) {
         if (!(grid->p[i] > 0.0) || !(grid->dp[i] > 0.0) || !isfinite(grid->p[i]) || !isfinite(grid->dp[i]) ||
             (i > 0 && !(grid->p[i] > grid->p[i - 1]))) {
@@ -376,6 +366,9 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         KX_CUDA(cudaMemcpyAsync(DP, grid->dp, (size_t)N * 8, cudaMemcpyHostToDevice, s));
         KX_CUDA(cudaMemcpyAsync(tab, t.data(), t.size() * 8, cudaMemcpyHostToDevice, s));
         KX_CUDA(cudaMemsetAsync(h->flag, 0, 4, s));
+        KX_CUDA(cudaMalloc((void**)&h->bar, 16));
+        KX_CUDA(cudaMemsetAsync(h->bar, 0, 16, s));
+        KX_CUDA(kx_dmma_configure());
         if (o.n_mu > 0) {
             // Gauss-Legendre nodes and weights on [-1,1] (constants, not data dependent): Newton on P_n in long double
             const int n = o.n_mu;
@@ -448,7 +441,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
             t.flag_log2 = (double)lf;
             KX_CUDA(cudaMemcpyAsync(dd, tab.data(), tab.size() * 8, cudaMemcpyHostToDevice, s));
             KX_CUDA(cudaStreamSynchronize(s));
-            kx_status_t rc2 = build_tiled(h, s, true);
+            kx_status_t rc2 = build_tiled(h, s);
             if (rc2 != KX_OK) return rc2;
             KX_CUDA(cudaStreamSynchronize(s));
         }
@@ -581,7 +574,6 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
             if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
             const double* fin = stg == 0 ? f : h->fstage;
             KxStage st = {};
-            if ((rc = launch_eval(h, fin, B, have_yd, use_tiled, &st, s)) != KX_OK) return rc;
             st.flags = ctl->flags & KX_PROJECT;
             st.diag = (diag && stg == 0) ? ctl->diag + (size_t)k * B * 6 : nullptr;
             st.diag_stride = 6;
@@ -591,7 +583,7 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
             for (int q = 0; q < nsrc; ++q) st.amp[q] = src->amp[(size_t)q * S + k];
             st.f = f; st.fstage = h->fstage; st.k1 = h->k1; st.k2 = h->k2; st.k3 = h->k3;
             st.ydnext = use_tiled ? nullptr : h->yd; st.flag = h->flag;
-            KX_CUDA(kx_launch_finish(h->d, fin, h->part, B, st, s));
+            if ((rc = launch_step(h, fin, B, have_yd, use_tiled, &st, s)) != KX_OK) return rc;
             have_yd = !use_tiled;
         }
         if (diag) {
@@ -664,7 +656,6 @@ kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_sou
             for (int stg = 0; stg < 2; ++stg) {
                 const double* fin = stg == 0 ? f : h->fstage;
                 KxStage st = {};
-                if ((rc = launch_eval(h, fin, B, /*have_yd=*/stg == 1 && !use_tiled, use_tiled, &st, s)) != KX_OK) return rc;
                 st.flags = ctl->flags & KX_PROJECT;
                 st.diag_stride = 6;
                 st.evolve = 1; st.rk_method = KX_HEUN_ADAPT; st.rk_stage = stg;
@@ -676,7 +667,7 @@ kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_sou
                 st.flag = h->flag;
                 st.ad = h->adapt; st.ad_u0 = ctl->u0; st.ad_rate0 = ctl->rate0; st.ad_slope = ctl->rate_slope;
                 st.ad_rtol = ctl->rtol; st.ad_atol = ctl->atol;
-                KX_CUDA(kx_launch_finish(h->d, fin, h->part, B, st, s));
+                if ((rc = launch_step(h, fin, B, /*have_yd=*/stg == 1 && !use_tiled, use_tiled, &st, s)) != KX_OK) return rc;
             }
             KX_CUDA(kx_launch_adapt_step(h->d, f, h->k2, B, h->adapt, ctl->u1, ctl->safety, h->flag, s));
         }
@@ -692,6 +683,58 @@ kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_sou
         result->accepted = state.accepted; result->rejected = state.rejected; result->done = state.done;
     }
     if (flag) { h->err = "kx_evolve_adaptive: f became non-finite"; return KX_ERR_NONFINITE; }
+    return KX_OK;
+}
+
+kx_status_t kx_reserve(kx_handle_t h, int32_t B, void* stream)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    if (B < 1) { h->err = "kx_reserve: B < 1"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    kx_status_t rc = ensure_ws(h, B);
+    if (rc != KX_OK) return rc;
+    if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
+    if ((rc = ensure_tiled(h, s)) != KX_OK) return rc;
+    if (h->storage == KX_STORE_TILED && h->plan_B != B) {
+        kx_dmma_plan(h->d, h->t, h->sm_count, h->vt_host.data(), B, &h->plan);
+        h->plan_B = B;
+    }
+    return KX_OK;
+}
+
+kx_status_t kx_fallback_members(kx_handle_t h, int64_t* count)
+{
+    if (!h || !count) return KX_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    KX_CUDA(cudaDeviceSynchronize());
+    unsigned v = 0;
+    KX_CUDA(cudaMemcpy(&v, h->bar + 2, 4, cudaMemcpyDeviceToHost));
+    KX_CUDA(cudaMemset(h->bar + 2, 0, 4));
+    *count = (int64_t)v;
+    return KX_OK;
+}
+
+kx_status_t kx_trace(kx_handle_t h, int32_t enable)
+{
+    if (!h) return KX_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    if (enable && !h->trace) {
+        KX_CUDA(cudaMalloc((void**)&h->trace, (size_t)KX_TRACE_CTAS * KX_TRACE_SLOTS * 8));
+        KX_CUDA(cudaMemset(h->trace, 0, (size_t)KX_TRACE_CTAS * KX_TRACE_SLOTS * 8));
+    }
+    h->tracing = enable != 0;
+    return KX_OK;
+}
+
+kx_status_t kx_trace_read(kx_handle_t h, uint64_t* stamps)
+{
+    if (!h || !stamps) return KX_ERR_INVALID_ARG;
+    if (!h->trace) { h->err = "kx_trace_read: tracing was never enabled"; return KX_ERR_INVALID_ARG; }
+    DeviceGuard guard(h->device);
+    KX_CUDA(cudaDeviceSynchronize());
+    KX_CUDA(cudaMemcpy(stamps, h->trace, (size_t)KX_TRACE_CTAS * KX_TRACE_SLOTS * 8, cudaMemcpyDeviceToHost));
+    KX_CUDA(cudaMemset(h->trace, 0, (size_t)KX_TRACE_CTAS * KX_TRACE_SLOTS * 8));
     return KX_OK;
 }
 

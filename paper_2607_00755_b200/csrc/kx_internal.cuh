@@ -19,6 +19,9 @@
 #define KX_TI         16       // rows i per tile of the tiled (DMMA) storage: two 8-row MMA blocks
 #define KX_QMAX       32       // largest number of Chebyshev nodes of the compressed LOG loss term
 #define KX_GROUP_DBL  256      // doubles of tensor data per group: 4 quads x 2 row blocks x 32 lanes
+#define KX_TRACE_CTAS  160      // clock-stamp trace (kx_trace): CTAs x slots of 8 bytes
+#define KX_TRACE_SLOTS 32
+#define KX_FB_BT      4        // members per group of the exact fallback inside the DMMA kernel
 
 // Device-side view of a handle: plain pointers, passed by value to every kernel.
 struct KxDev {
@@ -82,6 +85,20 @@ struct KxTiled {
     double flag_log2;         // log2(2 / Q!) ... see the loss role of k_dmma (kx_tiled.cu)
 };
 
+// Plan of one launch of the DMMA kernel (made on the host by kx_dmma_plan, passed by value).
+//   CTAs [0, GG) take the gain role, [GG, GG + GL) the loss role.  Gain warp w (global index = CTA * 8 + warp) works on
+//   ONE tile: the warps [wstart[t], wstart[t+1]) share the groups of tile t in equal contiguous ranges (a warp never
+//   crosses a tile, so a CTA adds the accumulators of its warps in shared memory and writes one partial per tile it
+//   touches, slot = CTA + tile).  Warps beyond wstart[NT] are idle.
+#define KX_MAX_NT 64
+struct KxPlan {
+    int nbt;                  // member tiles (of 8) per pass
+    int GG, GL;               // CTAs per role
+    int WC;                   // chunks of 16 k whose Chebyshev coefficients a loss CTA holds at a time
+    unsigned wstart[KX_MAX_NT + 1];
+    unsigned vt[KX_MAX_NT + 1];      // copy of vtptr: first group of every tile
+};
+
 struct KxAdapt;
 struct kx_handle_s {
     KxDev d;
@@ -95,12 +112,17 @@ struct kx_handle_s {
     long long cap_groups;     // capacity of t.A / t.desc in groups
     long long groups;         // host copy of vtptr[NT]
     int ws_xstride;           // members per partial slot (batch capacity padded)
-    long long *mstat;         // [wsB][2] per member: ordered key of the largest interpolation-error term over the brackets,
-                              // bits of max_i |f_i| (see kx_member_flagged); reset by the finishing kernel
-    double *gpart;            // [8 sm_count + NT + 1, ws_xstride, 16]  gain partials of the DMMA kernel (one per warp and tile)
-    double *lpart;            // [sm_count + RS + 1, ws_xstride, 256] loss partials
-    double *gn;               // [wsB, N, 2] (gain, nu) summed from the partials
-    int GG, GL;               // CTAs of the gain / loss role in the last launch of the DMMA kernel
+    long long *mstat;         // [2][wsB][2] per member, double-buffered by launch parity: ordered key of the largest
+                              // interpolation-error term over the brackets, bits of max_i |f_i| (see kx_member_flagged)
+    double *gpart;            // [sm_count + NT + 1, ws_xstride, 16]  gain partials of the DMMA kernel (one per CTA and tile)
+    double *lpart;            // [sm_count + RS + 1, ws_xstride, 256] loss partials (one per CTA and supertile)
+    std::vector<unsigned> vt_host;   // host copy of vtptr [NT + 1] (the plan of the DMMA kernel is made on the host)
+    KxPlan plan;              // role split and warp -> tile map of the DMMA kernel for batch plan_B
+    int plan_B;               // 0 = no plan
+    unsigned *bar;            // device [4]: grid barrier of the fused kernels (arrival count, released epoch), fallback count
+    unsigned epoch;           // launch serial number of the fused kernels (two barrier epochs per launch)
+    unsigned long long *trace;       // device [KX_TRACE_CTAS][KX_TRACE_SLOTS] clock stamps of the last fused launch, or null
+    bool tracing;
     void *tiled_blob;         // one allocation holding the small tables of KxTiled
     bool nnz_stale;
     int chunk_for_B;          // the batch size taskptr was last built for (0 = none)
@@ -134,25 +156,22 @@ struct kx_handle_s {
         }                                                                                      \
     } while (0)
 
-// ---- programmatic dependent launch (PDL): a kernel launched with pdl = true may start while its predecessor in
-// the stream is still running; it calls kx_pdl_wait() before it touches anything the predecessor (or a kernel
-// before that) writes, and kx_pdl_trigger() as early as it likes to let its own successor start.  The first kernel
-// of every API call is launched with pdl = false, so calls never overlap each other.
+// ---- cooperative launch: every CTA of the grid is resident at the same time, so the grid barrier of the fused
+// kernels (kx_device.cuh) cannot deadlock.  The launch fails (cudaErrorCooperativeLaunchTooLarge) instead of hanging
+// if the grid does not fit.
 template <typename... KArgs, typename... Args>
-inline cudaError_t kx_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl,
-                             Args&&... args)
+inline cudaError_t kx_launch_coop(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                  Args&&... args)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
     cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 #ifdef __CUDACC__
-__device__ __forceinline__ void kx_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void kx_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ---------------------------------------------------------------- exp2 for the LOG loss term
 // 2^t = 2^k * T[idx] * 2^r,  t = k + idx/256 + r, |r| <= 2^-9.  Adding 1.5*2^44 leaves round(256 t) in the
@@ -189,15 +208,7 @@ __device__ __forceinline__ long long kx_dkey(double x)
     return b >= 0 ? b : (b ^ 0x7fffffffffffffffLL);
 }
 // A member takes the exact streaming path when the interpolation error bound of some bracket,
-//     2 (|ln(f_(j+1)/f_j)|/4)^Q / Q! * max(f_j, f_(j+1)),   exceeds 1e-15 max_i f_i      (kx_tiled_build.cu)
-__device__ __forceinline__ bool kx_member_flagged(const long long* mstat, int b)
-{
-    const long long k = mstat[2 * b];
-    if (k == KX_MSTAT_NONE) return false;
-    const double lb = __longlong_as_double(k >= 0 ? k : (k ^ 0x7fffffffffffffffLL));
-    const double fm = __longlong_as_double(mstat[2 * b + 1]);
-    return lb - log2(fm) > -49.82892142331043;         // log2(1e-15)
-}
+//     2 (|ln(f_(j+1)/f_j)|/4)^Q / Q! * max(f_j, f_(j+1)),   exceeds 1e-15 max_i f_i      (kxd::member_flagged, kx_device.cuh)
 #endif
 
 // ---- launchers implemented in kx_build.cu
@@ -230,28 +241,28 @@ struct KxStage {             // what the finishing kernel does after the reducti
     double *fstage;          // stage input written by this stage for the next one
     double *k1, *k2, *k3;
     double *ydnext;          // where to write yd of the next stage input (fused prep) or null
-    // tiled path: partials of the DMMA kernel; flagged members (kx_member_flagged) take the streaming partials instead
-    const double *gpart;     // [slots, xstride, 16] or null (streaming path only)
-    const double *lpart;     // [slots, xstride, 256]
-    double2 *gn;             // [B, N] (gain, nu): the partials added up by k_reduce
-    const unsigned *vtptr;   // [NT + 1]
-    long long *mstat;        // [B][2] or null
-    int NT, LC, RS, GW, GL, xstride;      // GW = gain workers (warps), GL = loss workers (CTAs)
+    // tiled path: partials of the DMMA phase; flagged members (kx_member_flagged) take the streaming partials instead
+    double *gpart;           // [slots, xstride, 16] or null (streaming path only)
+    double *lpart;           // [slots, xstride, 256]
+    long long *mstat;        // this launch's member statistics [B][2], or null (LINEAR: no fallback)
+    long long *mstat_next;   // the other buffer: reset (all mstat_cap members) by the finishing phase for the next launch
+    int mstat_cap;
+    int NT, LC, RS, xstride;
     int *flag;
     int evolve;
-    // tiled LOG path: the exact fallback kernel (gated per member group) is launched between k_reduce and k_finish
-    int fb_sm_count;
-    const double *fb_f, *fb_yd;
-    double *fb_part;
+    double *part;            // [tasks, B, 2 or 4] partials of the exact streaming contraction
+    // grid barrier of the fused kernels (kx_device.cuh) and the optional clock-stamp trace
+    unsigned *bar;
+    unsigned epoch;
+    unsigned long long *trace;
+    unsigned *fb_count;      // device counter: members evaluated by the exact fallback (kx_fallback_count)
     // adaptive Heun (rk_method == KX_HEUN_ADAPT): dt and the rate come from the device controller state
     KxAdapt *ad;
     double ad_u0, ad_rate0, ad_slope, ad_rtol, ad_atol;
 };
 #define KX_HEUN_ADAPT 3      // internal: Euler predictor / Heun corrector with the error norm of kx_evolve_adaptive
-cudaError_t kx_launch_prep(const KxDev& d, const double* f, double* yd, int B, cudaStream_t s);
-cudaError_t kx_launch_contract(const KxDev& d, int sm_count, const double* f, const double* yd,
-                               double* part, int B, const long long* mstat, bool pdl, cudaStream_t s);
-cudaError_t kx_launch_finish(const KxDev& d, const double* f, const double* part, int B,
+// one operator evaluation on the exact streaming path: y = log2 f, contraction, grid barrier, finishing phase: ONE kernel
+cudaError_t kx_launch_stream(const KxDev& d, int sm_count, const double* f, const double* yd, int B,
                              const KxStage& st, cudaStream_t s);
 cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, int B, KxAdapt* ad, double u1, double safety,
                                  int* flag, cudaStream_t s);      // accept/reject + controller update
@@ -261,10 +272,11 @@ cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n,
 // ---- tiled path (kx_tiled_build.cu, kx_tiled.cu)
 cudaError_t kx_launch_tile_runs(const KxDev& d, const KxTiled& t, cudaStream_t s);     // runs, scans, vtptr
 cudaError_t kx_launch_tile_fill(const KxDev& d, const KxTiled& t, cudaStream_t s);     // A, desc (gain + loss)
-cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
-                           long long* mstat, int xstride, double* gpart, double* lpart, int B, cudaStream_t s);
+// one operator evaluation on the tensor-core path: DMMA phase, grid barrier, (exact fallback, barrier,) finishing phase
+cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B,
+                           const KxStage& st, cudaStream_t s);
+cudaError_t kx_dmma_configure(); // shared-memory attributes of every instantiation (once per process)
 int kx_xstride(int B);
-int kx_dmma_workers(int N, int B);     // gain workers (warps) per CTA of k_dmma
-void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long groups, int B, int* GG, int* GL);
+void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned* vt_host, int B, KxPlan* plan);
 int kx_pick_bt(int N, int B);
 int kx_pick_chunk(long long nnz_est, int N, int B, int sm_count);

@@ -1,23 +1,31 @@
-// kx_tiled.cu -- steps a4-a5 as one FP64 tensor-core contraction over the tiled storage (KX_STORE_TILED).
+// kx_tiled.cu -- one operator evaluation on the tensor-core path (KX_STORE_TILED) as ONE cooperative kernel:
 //
-//   gain[b,i] = sum_{n<=m} (W_inm + W_imn) f_n f_m                        eq. 4.6 with 2.6
-//   nu[b,i]   = sum_j sum_{c<Q} M_c(i,j) a_c(b,j)   (loss_i = f_i nu_i)   eq. B.19-B.20, see
-//               kx_tiled_build.cu for the Chebyshev-moment form of the interpolated loss term and its error bound
+//   DMMA phase       gain[b,i] = sum_{n<=m} (W_inm + W_imn) f_n f_m                 eq. 4.6 with 2.6
+//                    nu[b,i]   = sum_j sum_{c<Q} M_c(i,j) a_c(b,j)  (loss_i = f_i nu_i)   eq. B.19-B.20,
+//                    see kx_tiled_build.cu for the Chebyshev-moment form of the interpolated loss term and its error bound
+//   grid barrier
+//   [exact fallback  members whose interpolation error bound is not negligible are evaluated by the streaming contraction
+//                    (kxd::contract_group), spread over the whole grid; second grid barrier.  Normally skipped.]
+//   finishing phase  a6-a8 (kxd::finish_member): CTA b adds the partials of member b in a fixed order, raw operator,
+//                    projection, diagnostics, fused Runge-Kutta stage
 //
-// Both are out[b,i] += sum_k X[b,k] A[k,i] with A streamed once from HBM/L2 (cp.async) and X built in shared memory
-// from the caller's f: X = f_n f_m for the gain, X = a_c(b,j) for the loss.  The products run on the FP64 tensor
-// pipe: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), M = 8 members, N = 8 rows, K = 4.  The CTAs of one launch are split
-// between the two terms in proportion to their work (see k_dmma); the finishing kernel (kx_contract.cu) adds the
-// partials: no atomics, bit-reproducible.
+// Both contractions are out[b,i] += sum_k X[b,k] A[k,i] with A streamed once from HBM/L2 (cp.async) and X built in shared
+// memory from the caller's f: X = f_n f_m for the gain, X = a_c(b,j) for the loss.  The products run on the FP64 tensor
+// pipe: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), M = 8 members, N = 8 rows, K = 4.  The CTAs (one per SM) are split between
+// the two terms in proportion to their work (kx_dmma_plan).  No atomics on data: bit-reproducible.
 //
 // Compiled with --fmad=false; fused multiply-adds are explicit.
-#include "kx_internal.cuh"
+#include "kx_device.cuh"
+
+#include <vector>
 
 namespace {
 
-// cost of one loss DMMA relative to one gain DMMA in the CTA split of k_dmma (measured on cfg3: the split that
-// makes both roles finish together; the loss CTAs also compute their Chebyshev coefficients first)
-constexpr double kLossCost = 1.3;
+using namespace kxd;
+
+// cost of one loss DMMA relative to one gain DMMA in the CTA split (the loss CTAs also compute their Chebyshev
+// coefficients first; calibrated with the clock-stamp trace on cfg3 so that both roles reach the barrier together)
+constexpr double kLossCost = 1.22;
 
 // D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
@@ -26,7 +34,6 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
         : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// ---------------------------------------------------------------- the contraction
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -36,110 +43,107 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int NPEND>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(NPEND) : "memory"); }
 
+constexpr int WARPS = kDmmaWarps;
+constexpr int NTHR = WARPS * 32;
+static_assert(NTHR == KX_CTA, "the finishing phase and the exact fallback run with 256 threads");
 constexpr int kStageBytes = KX_GROUP_DBL * 8 + 16;     // gain ring stage: 2 KiB of A + 4 descriptors
 constexpr int kLossStages = 3;
 constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256 rows of AL
 
-// One CTA per SM.  CTAs [0, GG) take equal ranges of gain groups, CTAs [GG, GG+GL) equal ranges of loss chunks.
-//
-// gain role: the rows f[b, :] of the CTA's 8 NBT members sit in shared memory (row stride = 4 mod 16 doubles when
-//   N = 0 mod 16: the 8 members x 4 k fragment reads of a quad are bank-conflict free), copied straight from the
-//   caller's f; every warp streams its own share of the groups through a private
-//   cp.async ring and holds a 16-row x 8 NBT-member accumulator (2 NBT DMMA per quad and fragment pair).
-//   The DMMAs of a run (fixed n) take X = f_m and accumulate into T; f_n multiplies T once, when the run ends.
-//   The ring keeps flowing across tile boundaries.
-// loss role: a dense GEMM.  The CTA first computes the Chebyshev coefficients a_c(b,j) of its own share of k = (j,c)
-//   rows straight into shared memory (window by window if the share does not fit): exp2 at the Chebyshev nodes, then
-//   the discrete Chebyshev transform on the tensor pipe; it also accumulates the per-member statistics that route a
-//   member to the exact fallback.  Then warp w streams its rows [32 w, 32 w + 32) of AL through a private 3-stage
-//   cp.async ring (4 KiB per chunk of 16 k) and multiplies them with the resident coefficients (4 NBT DMMA per quad).
-// A range that crosses a tile (supertile) boundary produces one partial per piece, slot = worker + tile (a gain
-// worker is a warp, a loss worker a CTA); the finishing kernel adds the partials of a row in slot order: no
-// atomics, bit-reproducible.
-template <int NBT, int WARPS, int STAGES>
-__global__ void __launch_bounds__(WARPS * 32, 1)
-k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restrict__ f, long long* __restrict__ mstat,
-       int xstride, double* __restrict__ gpart, double* __restrict__ lpart, int GG, int GL, int WC)
+// ---------------------------------------------------------------- gain role
+// The rows f[b, :] of the pass's 8 NBT members sit in shared memory (row stride = 4 mod 16 doubles when N = 0 mod 16: the
+// 8 members x 4 k fragment reads of a quad are bank-conflict free), copied straight from the caller's f.  Every warp is
+// an independent worker: it streams its own contiguous share of ONE tile's groups (plan.wstart) through a private
+// cp.async ring and holds a 16-row x 8 NBT-member accumulator (2 NBT DMMA per quad and fragment pair).  The DMMAs of a
+// run (fixed n) take X = f_m and accumulate into T; f_n multiplies T once, when the run ends.  When all warps are done
+// they leave their accumulators in shared memory and the CTA adds those of the same tile in warp order: one partial per
+// (CTA, tile), slot = CTA + tile.
+template <int NBT, int STAGES>
+__device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, int N, int B, int bcol0,
+                                          const double* __restrict__ f, int xstride, double* __restrict__ gpart,
+                                          unsigned char* smem, int* s_wtile, unsigned long long* trace)
 {
-    extern __shared__ __align__(16) unsigned char smem[];
-    constexpr int LD = NBT * 8 + 4;
-    constexpr int NTHR = WARPS * 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int krow = lane & 3, lr = lane >> 2;
-    const int bcol0 = blockIdx.y * (NBT * 8);
-    kx_pdl_trigger();
+    const int LDN = (N + 7) & ~3;             // row stride of s_f: >= N + 4, = 0 mod 4; N = 0 mod 16 gives 4 mod 16
+    double* s_f = reinterpret_cast<double*>(smem);                                    // [8 NBT][LDN]
+    unsigned char* ring = smem + (size_t)(NBT * 8) * LDN * 8 + (size_t)warp * STAGES * kStageBytes;
 
-    if ((int)blockIdx.x < GG) {
-        // ------------------------------------------------------------ gain role: every warp is an independent worker
-        unsigned* s_vt = reinterpret_cast<unsigned*>(smem);                               // [NT + 1]
-        const int vtbytes = ((t.NT + 1) * 4 + 15) & ~15;
-        const int LDN = (N + 7) & ~3;             // row stride of s_f: >= N + 4, = 0 mod 4; N = 0 mod 16 gives 4 mod 16
-        double* s_f = reinterpret_cast<double*>(smem + vtbytes);                          // [8 NBT][LDN]
-        unsigned char* ring = smem + vtbytes + (size_t)(NBT * 8) * LDN * 8 + (size_t)warp * STAGES * kStageBytes;
-
-        const unsigned NW = (unsigned)GG * WARPS, wk = blockIdx.x * WARPS + warp;
-        const unsigned g0 = (unsigned)((unsigned long long)wk * Gtot / NW);
-        const unsigned g1 = (unsigned)((unsigned long long)(wk + 1) * Gtot / NW);
-        const unsigned n = g1 - g0;
-        auto issue = [&](unsigned gi) {
-            const double* src = t.A + (size_t)(g0 + gi) * KX_GROUP_DBL;
-            unsigned char* dst = ring + (size_t)(gi % STAGES) * kStageBytes;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) cp_async16(dst + (k * 32 + lane) * 16, src + (k * 32 + lane) * 2);
-            if (lane == 0) cp_async16(dst + KX_GROUP_DBL * 8, t.desc + (size_t)(g0 + gi) * 4);
-        };
-        // The gain role reads only the caller's f and the tensor, nothing an earlier kernel of this call writes: under
-        // programmatic dependent launch it runs while the operand-preparation kernel is still at work.
-        // The tensor stream starts first; f^T and the tile table arrive while it is in flight.
-#pragma unroll
-        for (int s = 0; s < STAGES - 1; ++s) {
-            if ((unsigned)s < n) issue(s);
-            cp_async_commit();
+    // this warp's tile and its share of the tile's groups
+    const unsigned wk = blockIdx.x * WARPS + warp;
+    int tile = -1;
+    unsigned g0 = 0, n = 0;
+    if (wk < plan.wstart[t.NT]) {
+        int lo = 0, hi = t.NT - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (plan.wstart[mid] <= wk) lo = mid; else hi = mid - 1;
         }
-        // s_f[b][n] = f[bcol0 + b][n], n < N; s_f[b][N] = 1 (the scale of padding quads), s_f[b][N+1..] = 0.  The rows of
-        // f are copied as they are (16-byte cp.async when N is even); members beyond B are zero.  Every CTA starts its
-        // walk somewhere else so that the CTAs do not all ask the same L2 lines at once.
-        {
-            const int chunks = (N & 1) ? 0 : N >> 1;                   // 16-byte chunks per row
-            const int total = NBT * 8 * chunks;
-            const int rot = total ? (int)((blockIdx.x * 977u) % (unsigned)total) : 0;
-            for (int k0 = tid; k0 < total; k0 += NTHR) {
-                int k = k0 + rot;
-                if (k >= total) k -= total;
-                const int bb = k / chunks, cc = k - bb * chunks;
-                if (bcol0 + bb < B) cp_async16(s_f + (size_t)bb * LDN + 2 * cc, f + (size_t)(bcol0 + bb) * N + 2 * cc);
-                else *reinterpret_cast<double2*>(s_f + (size_t)bb * LDN + 2 * cc) = make_double2(0.0, 0.0);
-            }
-            if (!chunks)
-                for (int k = tid; k < NBT * 8 * N; k += NTHR) {
-                    const int bb = k / N, nn = k - bb * N;
-                    s_f[(size_t)bb * LDN + nn] = bcol0 + bb < B ? __ldcg(f + (size_t)(bcol0 + bb) * N + nn) : 0.0;
-                }
-            for (int k = tid; k < NBT * 8 * (LDN - N); k += NTHR) {
-                const int bb = k / (LDN - N), cc = k - bb * (LDN - N);
-                s_f[(size_t)bb * LDN + N + cc] = cc == 0 ? 1.0 : 0.0;
-            }
-        }
+        tile = lo;
+        const unsigned w0 = plan.wstart[tile], wt = plan.wstart[tile + 1] - w0, r = wk - w0;
+        const unsigned a0 = plan.vt[tile], gt = plan.vt[tile + 1] - a0;
+        g0 = a0 + (unsigned)((unsigned long long)r * gt / wt);
+        n = a0 + (unsigned)((unsigned long long)(r + 1) * gt / wt) - g0;
+    }
+    auto issue = [&](unsigned gi) {
+        const double* src = t.A + (size_t)(g0 + gi) * KX_GROUP_DBL;
+        unsigned char* dst = ring + (size_t)(gi % STAGES) * kStageBytes;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) cp_async16(dst + (k * 32 + lane) * 16, src + (k * 32 + lane) * 2);
+        if (lane == 0) cp_async16(dst + KX_GROUP_DBL * 8, t.desc + (size_t)(g0 + gi) * 4);
+    };
+    // the tensor stream starts first; f arrives while it is in flight
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if ((unsigned)s < n) issue(s);
         cp_async_commit();
-        for (int k = tid; k <= t.NT; k += NTHR) s_vt[k] = t.vtptr[k];
-        cp_async_wait<0>();
-        __syncthreads();
-        if (n == 0) { kx_pdl_wait(); return; }
+    }
+    // s_f[b][n] = f[bcol0 + b][n], n < N; s_f[b][N] = 1 (the scale of padding quads), s_f[b][N+1..] = 0.  The rows of
+    // f are copied as they are (16-byte cp.async when N is even); members beyond B are zero.  Every CTA starts its
+    // walk somewhere else so that the CTAs do not all ask the same L2 lines at once.
+    {
+        const int chunks = (N & 1) ? 0 : N >> 1;                   // 16-byte chunks per row
+        const int total = NBT * 8 * chunks;
+        const int rot = total ? (int)((blockIdx.x * 977u) % (unsigned)total) : 0;
+        for (int k0 = tid; k0 < total; k0 += NTHR) {
+            int k = k0 + rot;
+            if (k >= total) k -= total;
+            const int bb = k / chunks, cc = k - bb * chunks;
+            if (bcol0 + bb < B) cp_async16(s_f + (size_t)bb * LDN + 2 * cc, f + (size_t)(bcol0 + bb) * N + 2 * cc);
+            else *reinterpret_cast<double2*>(s_f + (size_t)bb * LDN + 2 * cc) = make_double2(0.0, 0.0);
+        }
+        if (!chunks)
+            for (int k = tid; k < NBT * 8 * N; k += NTHR) {
+                const int bb = k / N, nn = k - bb * N;
+                s_f[(size_t)bb * LDN + nn] = bcol0 + bb < B ? __ldcg(f + (size_t)(bcol0 + bb) * N + nn) : 0.0;
+            }
+        for (int k = tid; k < NBT * 8 * (LDN - N); k += NTHR) {
+            const int bb = k / (LDN - N), cc = k - bb * (LDN - N);
+            s_f[(size_t)bb * LDN + N + cc] = cc == 0 ? 1.0 : 0.0;
+        }
+    }
+    cp_async_commit();
+    cp_async_wait<0>();
+    __syncthreads();
+    if (tid == 0) stamp(trace, 1);
 
+    // acc: the tile's partial.  T: sum over the m of the current run (fixed n) of f_m A[(n,m), i]; when the run ends,
+    // acc += f_n T.  Lane holds out[b = 8 bt + lane/4][i = 8 rb + 2 (lane%4) + {0,1}], the same member b as its
+    // fragment of X, so f_n[b] scales its own accumulators.
+    double acc[NBT][2][2];
+#pragma unroll
+    for (int bt = 0; bt < NBT; ++bt)
+#pragma unroll
+        for (int rb = 0; rb < 2; ++rb) acc[bt][rb][0] = acc[bt][rb][1] = 0.0;
+
+    if (n > 0) {
         const double* xb = s_f + (size_t)lr * LDN + krow;    // + 8 bt LDN + column: the lane's member row of tile bt
         const int LD8 = 8 * LDN;
-        int vt = 0;
-        while (s_vt[vt + 1] <= g0) ++vt;
-        unsigned bnd = s_vt[vt + 1] - g0;                    // first group (relative) of the next tile
-
-        // acc: the tile's partial.  T: sum over the m of the current run (fixed n) of f_m A[(n,m), i]; when the run ends,
-        // acc += f_n T.  Lane holds out[b = 8 bt + lane/4][i = 8 rb + 2 (lane%4) + {0,1}], the same member b as its
-        // fragment of X, so f_n[b] scales its own accumulators.
-        double acc[NBT][2][2], T[NBT][2][2], sn[NBT];
+        double T[NBT][2][2], sn[NBT];
 #pragma unroll
         for (int bt = 0; bt < NBT; ++bt)
 #pragma unroll
-            for (int rb = 0; rb < 2; ++rb) { acc[bt][rb][0] = acc[bt][rb][1] = 0.0; T[bt][rb][0] = T[bt][rb][1] = 0.0; }
+            for (int rb = 0; rb < 2; ++rb) T[bt][rb][0] = T[bt][rb][1] = 0.0;
         auto fold = [&]() {
 #pragma unroll
             for (int bt = 0; bt < NBT; ++bt)
@@ -150,18 +154,6 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
                     T[bt][rb][0] = T[bt][rb][1] = 0.0;
                 }
         };
-        // one partial per (worker, tile), slot = worker + tile
-        auto flush = [&](int tile) {
-            double* dst = gpart + ((size_t)(wk + tile) * xstride + bcol0 + lr) * 16 + 2 * krow;
-#pragma unroll
-            for (int bt = 0; bt < NBT; ++bt)
-#pragma unroll
-                for (int rb = 0; rb < 2; ++rb) {
-                    *reinterpret_cast<double2*>(dst + (size_t)bt * 128 + rb * 8) = make_double2(acc[bt][rb][0], acc[bt][rb][1]);
-                    acc[bt][rb][0] = acc[bt][rb][1] = 0.0;
-                }
-        };
-
         // descriptors of the current group (dc) and the next one (dn) stay in registers: the f_m rows of a quad are
         // requested a whole quad before they are used
         uint4 dc = *reinterpret_cast<const uint4*>(ring + KX_GROUP_DBL * 8);
@@ -175,19 +167,13 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
         }
 
         for (unsigned gi = 0; gi < n; ++gi) {
-            if (gi == bnd) {                                 // the range crosses into the next tile
-                fold();
-                flush(vt);
-                do { ++vt; } while (s_vt[vt + 1] - g0 <= gi);
-                bnd = s_vt[vt + 1] - g0;
-            }
             // refill the slot freed by group gi-1, then make sure groups gi and gi+1 are in shared memory
             if (gi + STAGES - 1 < n) issue(gi + STAGES - 1);
             cp_async_commit();
             cp_async_wait<STAGES - 2>();
             __syncwarp();
-            const unsigned char* st = ring + (size_t)(gi % STAGES) * kStageBytes;
-            const double* wd = reinterpret_cast<const double*>(st) + lane;
+            const unsigned char* stg = ring + (size_t)(gi % STAGES) * kStageBytes;
+            const double* wd = reinterpret_cast<const double*>(stg) + lane;
             const bool last_group = gi + 1 >= n;
             uint4 dn = dc;
             if (!last_group) dn = *reinterpret_cast<const uint4*>(ring + (size_t)((gi + 1) % STAGES) * kStageBytes + KX_GROUP_DBL * 8);
@@ -222,281 +208,386 @@ k_dmma(KxDev dk, KxTiled t, int N, int B, unsigned Gtot, const double* __restric
             __syncwarp();     // every lane is done with this stage before it is refilled
         }
         fold();
-        flush(vt);
-        kx_pdl_wait();        // the grid must not complete before the kernels it follows have
-        return;
+        cp_async_wait<0>();
+        __syncwarp();
+        // the warp's accumulators -> its own (drained) ring: [8 NBT members][16 rows]
+        double* mine = reinterpret_cast<double*>(ring);
+#pragma unroll
+        for (int bt = 0; bt < NBT; ++bt)
+#pragma unroll
+            for (int rb = 0; rb < 2; ++rb)
+                *reinterpret_cast<double2*>(mine + (8 * bt + lr) * 16 + 8 * rb + 2 * krow) = make_double2(acc[bt][rb][0], acc[bt][rb][1]);
     }
-
-    // ---------------------------------------------------------------- loss role
-    {
-        constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
-        static_assert(WARPS == 8, "loss role: 8 warps (the coefficient pass maps warp <-> member tile)");
-        constexpr int MB = NBT * 8;               // members of this CTA
-        // brackets per coefficient pass: 256 threads = JB brackets x MB members, as many as the scratch holds at Q = 32
-        constexpr int JB = NBT == 1 ? 16 : 256 / MB;
-        constexpr int GS = MB + 4;                // row stride of the node values: 4 mod 8, conflict-free fragment reads
-        const int N_ = N, Q = t.Q;
-        const bool logm = dk.interp == KX_INTERP_LOG, tab = dk.exp_impl == KX_EXP_TABLE;
-        // shared memory: [A stages | scratch of the coefficient passes] [X window] [dct fragments, nodes, exp2 table]
-        unsigned char* sStage = smem;
-        double* sXw = reinterpret_cast<double*>(smem + (size_t)kLossStages * kLossABytes);          // [WC*16][LD]
-        double* s_afr = sXw + (size_t)WC * 16 * LD;                                                 // [(Q/8)(Q/4)][32]
-        double* s_node = s_afr + (KX_QMAX / 8) * (KX_QMAX / 4) * 32;                                // [QMAX]
-        double* s_tab = s_node + KX_QMAX;                                                           // [256]
-        double* s_G = reinterpret_cast<double*>(smem);                                              // [JB][Q][GS] (aliases the stages)
-        static_assert((size_t)JB * KX_QMAX * GS * 8 <= (size_t)kLossStages * kLossABytes, "coefficient scratch must fit the stages");
-        if (logm) {
-            for (int k = tid; k < (Q / 8) * (Q / 4) * 32; k += NTHR) {
-                const int ln = k & 31, fr = k >> 5, ct = fr / (Q / 4), ks = fr - ct * (Q / 4);
-                s_afr[k] = t.dct[(8 * ct + (ln >> 2)) * Q + 4 * ks + (ln & 3)];
-            }
-            if (tid < Q) s_node[tid] = t.nodes[tid];
-            if (tab) for (int k = tid; k < (1 << KX_EXP_BITS); k += NTHR) s_tab[k] = dk.exptab[k];
+    if (lane == 0) {
+        s_wtile[warp] = n > 0 ? tile : -1;
+        if (trace) {
+            const unsigned cta = blockIdx.x;
+            if (cta < KX_TRACE_CTAS) trace[cta * KX_TRACE_SLOTS + 8 + warp] = gtime();
         }
-        __syncthreads();
-
-        // Chebyshev coefficients a_c(b, j) of the window's k = (j, c) rows, k in [K0, K0 + 16 wn), straight into shared
-        // memory.  LOG: g(omega_q) = 2^(y_j + omega_q (y_(j+1) - y_j)) at the Q
-        // Chebyshev nodes, then the discrete Chebyshev transform as a (Q x Q) x (Q x 8 NBT) product on the tensor pipe;
-        // LINEAR: a_0 = (f_j + f_(j+1))/2, a_1 = (f_(j+1) - f_j)/2.  Also the member statistics (flags) of kx_internal.cuh.
-        auto build_window = [&](unsigned K0, unsigned wn) {
-            const unsigned K1 = K0 + 16u * wn;
-            const int jlo = (int)(K0 / (unsigned)Q);
-            const int jhi = min((int)((K1 - 1u) / (unsigned)Q), N_ - 2);
-            // rows beyond the last bracket are padding: zero
-            {
-                const unsigned kpad = (unsigned)(N_ - 1) * (unsigned)Q;
-                for (unsigned k = max(K0, kpad) + (unsigned)warp; k < K1; k += WARPS)
-                    for (int c2 = lane; c2 < LD; c2 += 32) sXw[(size_t)(k - K0) * LD + c2] = 0.0;
+    }
+    __syncthreads();
+    // one partial per (CTA, tile): the accumulators of the warps that worked on the same tile, added in warp order
+    const unsigned char* ring0 = smem + (size_t)(NBT * 8) * LDN * 8;
+    for (int wa = 0; wa < WARPS;) {
+        const int tl = s_wtile[wa];
+        int wb = wa + 1;
+        while (wb < WARPS && s_wtile[wb] == tl) ++wb;
+        if (tl >= 0) {
+            double* dst = gpart + ((size_t)(blockIdx.x + tl) * xstride + bcol0) * 16;
+            for (int o = tid; o < NBT * 128; o += NTHR) {
+                double s = 0.0;
+                for (int w = wa; w < wb; ++w) s += reinterpret_cast<const double*>(ring0 + (size_t)w * STAGES * kStageBytes)[o];
+                dst[o] = s;
             }
-            const int jj = tid / MB, bl = tid % MB;
-            if (!logm) {          // LINEAR: two exact coefficients per bracket, no transform: one flat loop
-                const int total = (jhi - jlo + 1) * MB;
-                for (int i0 = tid; i0 < total; i0 += 8 * NTHR) {          // 16 independent loads in flight per thread
-                    double v0[8], v1[8];
-#pragma unroll
-                    for (int u2 = 0; u2 < 8; ++u2) {
-                        const int idx = i0 + u2 * NTHR, j = jlo + idx / MB, bm = idx % MB, b = bcol0 + bm;
-                        const bool ok = idx < total && b < B;
-                        v0[u2] = ok ? __ldcg(f + (size_t)b * N_ + j) : 0.0;
-                        v1[u2] = ok ? __ldcg(f + (size_t)b * N_ + j + 1) : 0.0;
-                    }
-#pragma unroll
-                    for (int u2 = 0; u2 < 8; ++u2) {
-                        const int idx = i0 + u2 * NTHR, j = jlo + idx / MB, bm = idx % MB;
-                        if (idx < total) {
-                            const unsigned k = (unsigned)j * 2u;
-                            if (k >= K0 && k < K1) sXw[(size_t)(k - K0) * LD + bm] = 0.5 * (v0[u2] + v1[u2]);
-                            if (k + 1 >= K0 && k + 1 < K1) sXw[(size_t)(k + 1 - K0) * LD + bm] = 0.5 * (v1[u2] - v0[u2]);
-                        }
-                    }
-                }
-                __syncthreads();
-                return;
-            }
-            // the f values of a pass are requested one pass ahead
-            auto fetch = [&](int j0, double& a0, double& a1) {
-                const int j = j0 + jj, b = bcol0 + bl;
-                a0 = 0.0; a1 = 0.0;
-                if (jj < JB && j <= jhi && b < B) { a0 = __ldcg(f + (size_t)b * N_ + j); a1 = __ldcg(f + (size_t)b * N_ + j + 1); }
-            };
-            double fnx0, fnx1;
-            fetch(jlo, fnx0, fnx1);
-            for (int j0 = jlo; j0 <= jhi; j0 += JB) {
-                const int j = j0 + jj;
-                const bool valid = jj < JB && j <= jhi;
-                const int b = bcol0 + bl;
-                const double fj = fnx0, fj1 = fnx1;
-                if (j0 + JB <= jhi) fetch(j0 + JB, fnx0, fnx1);
-                if (valid && b < B) atomicMax(mstat + 2 * b + 1, __double_as_longlong(fmax(fabs(fj), fabs(fj1))));
-                if (valid) {
-                    const double y0 = log2(fmax(fj, dk.f_floor)), y1 = log2(fmax(fj1, dk.f_floor)), dy = y1 - y0;
-                    const double cabs = 0.6931471805599453 * fabs(dy);
-                    // log2 of the bracket's error bound (log2 max_i f_i is subtracted by the consumers); the atomics return
-                    // nothing, so nobody waits for them
-                    if (b < B && cabs > 0.0)
-                        atomicMax(mstat + 2 * b, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
-                    double* g = s_G + (size_t)jj * Q * GS + bl;
-                    if (tab) for (int q = 0; q < Q; ++q) g[q * GS] = kx_exp2_tab<1>(fma(s_node[q], dy, y0), s_tab);
-                    else for (int q = 0; q < Q; ++q) g[q * GS] = exp2(fma(s_node[q], dy, y0));
-                }
-                __syncthreads();
-                // transform: a task is (bracket of the pass, member tile); the 8 warps take 32 tasks at a time, 4 each, with
-                // 4 x (Q/8) independent accumulator chains so that the DMMA latency of one hides behind the others
-                for (int base = 0; base < JB * NBT; base += 32) {
-                    double D[4][KX_QMAX / 8][2];
-                    int tj[4], tm[4];
-#pragma unroll
-                    for (int u2 = 0; u2 < 4; ++u2) {
-                        const int idx = base + warp + 8 * u2;
-                        tj[u2] = idx < JB * NBT ? idx / NBT : -1;
-                        tm[u2] = idx % NBT;
-#pragma unroll
-                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[u2][ct][0] = D[u2][ct][1] = 0.0;
-                    }
-#pragma unroll
-                    for (int ks = 0; ks < KX_QMAX / 4; ++ks) {
-                        if (4 * ks < Q) {
-                            double afr[KX_QMAX / 8];
-#pragma unroll
-                            for (int ct = 0; ct < KX_QMAX / 8; ++ct) afr[ct] = 8 * ct < Q ? s_afr[(ct * (Q / 4) + ks) * 32 + lane] : 0.0;
-#pragma unroll
-                            for (int u2 = 0; u2 < 4; ++u2) {
-                                if (tj[u2] >= 0) {          // uniform over the warp
-                                    const double gv = s_G[((size_t)tj[u2] * Q + 4 * ks + krow) * GS + 8 * tm[u2] + lr];
-#pragma unroll
-                                    for (int ct = 0; ct < KX_QMAX / 8; ++ct)
-                                        if (8 * ct < Q) dmma884(D[u2][ct][0], D[u2][ct][1], afr[ct], gv);
-                                }
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int u2 = 0; u2 < 4; ++u2) {
-                        if (tj[u2] >= 0 && j0 + tj[u2] <= jhi) {
-#pragma unroll
-                            for (int ct = 0; ct < KX_QMAX / 8; ++ct) {
-                                if (8 * ct < Q) {
-                                    const unsigned k = (unsigned)(j0 + tj[u2]) * (unsigned)Q + 8u * ct + (unsigned)lr;
-                                    if (k >= K0 && k < K1)
-                                        *reinterpret_cast<double2*>(sXw + (size_t)(k - K0) * LD + 8 * tm[u2] + 2 * krow) = make_double2(D[u2][ct][0], D[u2][ct][1]);
-                                }
-                            }
-                        }
-                    }
-                }
-                __syncthreads();
-            }
-            __syncthreads();
-        };
-
-        const unsigned cl = blockIdx.x - GG;
-        const unsigned LC = (unsigned)t.LC;
-        const unsigned U = (unsigned)t.RS * LC;
-        const unsigned u0 = (unsigned)((unsigned long long)cl * U / (unsigned)GL);
-        const unsigned u1 = (unsigned)((unsigned long long)(cl + 1) * U / (unsigned)GL);
-        unsigned u = u0;
-        while (u < u1) {
-            const unsigned sp = u / LC;                                  // supertile
-            const unsigned ue = min(u1, (sp + 1) * LC);
-            const unsigned ka = u - sp * LC, n = ue - u;
-            const int nb = min(32, t.NR8 - 32 * (int)sp);                // 8-row blocks of this supertile
-            const int nbw = min(R8, max(0, nb - R8 * warp));             // ... of this warp
-
-            // every warp streams its own rows of the tensor (4 KiB per chunk: 4 eight-row blocks) through a private
-            // cp.async ring: no CTA-wide barrier inside a window
-            unsigned char* wring = sStage + (size_t)warp * (kLossStages * kLossABytes / WARPS);
-            constexpr int kWStage = kLossABytes / WARPS;                  // 4 KiB
-            auto issue = [&](unsigned kc, int slot) {
-                if (nbw > 0) {
-                    const double* srcA = t.AL + ((size_t)kc * t.NR8 + 32 * sp + R8 * warp) * 128;
-                    unsigned char* dstA = wring + (size_t)slot * kWStage;
-                    for (int k = lane; k < nbw * 64; k += 32) cp_async16(dstA + (size_t)k * 16, srcA + (size_t)k * 2);
-                }
-            };
-
-            double acc[R8][NBT][2];
-#pragma unroll
-            for (int r = 0; r < R8; ++r)
-#pragma unroll
-                for (int bt = 0; bt < NBT; ++bt) acc[r][bt][0] = acc[r][bt][1] = 0.0;
-
-            for (unsigned w0 = 0; w0 < n; w0 += (unsigned)WC) {
-                const unsigned wn = min((unsigned)WC, n - w0), kw = ka + w0;
-                build_window(16u * kw, wn);          // ends with a barrier: the scratch (= the rings) is free again
-#pragma unroll
-                for (int s2 = 0; s2 < kLossStages - 1; ++s2) {
-                    if ((unsigned)s2 < wn) issue(kw + s2, s2);
-                    cp_async_commit();
-                }
-                for (unsigned it = 0; it < wn; ++it) {
-                    if (it + kLossStages - 1 < wn) issue(kw + it + kLossStages - 1, (int)((it + kLossStages - 1) % kLossStages));
-                    cp_async_commit();
-                    cp_async_wait<kLossStages - 1>();        // chunk `it` of this warp has landed
-                    __syncwarp();
-                    if (nbw > 0) {
-                        const double* sA = reinterpret_cast<const double*>(wring + (size_t)(it % kLossStages) * kWStage) + lane;
-                        const double* sX = sXw + (size_t)(16 * it + krow) * LD + lr;
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            double xv[NBT];
-#pragma unroll
-                            for (int bt = 0; bt < NBT; ++bt) xv[bt] = sX[(size_t)(4 * q) * LD + 8 * bt];
-#pragma unroll
-                            for (int r = 0; r < R8; ++r) {
-                                const double w = sA[(r * 4 + q) * 32];
-#pragma unroll
-                                for (int bt = 0; bt < NBT; ++bt) dmma884(acc[r][bt][0], acc[r][bt][1], xv[bt], w);
-                            }
-                        }
-                    }
-                    __syncwarp();                            // the stage is refilled two iterations from now
-                }
-                cp_async_wait<0>();
-                __syncthreads();              // the rings are free again (next window's scratch, next piece)
-            }
-
-            double* dst = lpart + ((size_t)(cl + sp) * xstride + bcol0) * 256 + 8 * R8 * warp + 2 * krow;
-#pragma unroll
-            for (int r = 0; r < R8; ++r)
-                if (r < nbw)
-#pragma unroll
-                    for (int bt = 0; bt < NBT; ++bt)
-                        *reinterpret_cast<double2*>(dst + (size_t)(8 * bt + lr) * 256 + 8 * r) = make_double2(acc[r][bt][0], acc[r][bt][1]);
-            u = ue;
         }
+        wa = wb;
     }
 }
 
+// ---------------------------------------------------------------- loss role
+// A dense GEMM.  The CTA first computes the Chebyshev coefficients a_c(b,j) of its own share of k = (j,c) rows straight
+// into shared memory (window by window if the share does not fit): exp2 at the Chebyshev nodes, then the discrete
+// Chebyshev transform on the tensor pipe; it also accumulates the per-member statistics that route a member to the exact
+// fallback.  Then warp w streams its rows [32 w, 32 w + 32) of AL through a private 3-stage cp.async ring (4 KiB per chunk
+// of 16 k) and multiplies them with the resident coefficients (4 NBT DMMA per quad).  A range that crosses a supertile
+// (256 rows) boundary produces one partial per piece, slot = loss CTA + supertile.
+template <int NBT>
+__device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, const KxPlan& plan, int N, int B, int bcol0,
+                                          const double* __restrict__ f, long long* __restrict__ mstat, int xstride,
+                                          double* __restrict__ lpart, unsigned char* smem, unsigned long long* trace)
+{
+    constexpr int LD = NBT * 8 + 4;
+    constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
+    static_assert(WARPS == 8, "loss role: 8 warps (the coefficient pass maps warp <-> member tile)");
+    constexpr int MB = NBT * 8;               // members of this CTA
+    // brackets per coefficient pass: 256 threads = JB brackets x MB members, as many as the scratch holds at Q = 32
+    constexpr int JB = NBT == 1 ? 16 : 256 / MB;
+    constexpr int GS = MB + 4;                // row stride of the node values: 4 mod 8, conflict-free fragment reads
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int krow = lane & 3, lr = lane >> 2;
+    const int N_ = N, Q = t.Q, WC = plan.WC, GG = plan.GG, GL = plan.GL;
+    const bool logm = dk.interp == KX_INTERP_LOG, tab = dk.exp_impl == KX_EXP_TABLE;
+    // shared memory: [A stages | scratch of the coefficient passes] [X window] [dct fragments, nodes, exp2 table]
+    unsigned char* sStage = smem;
+    double* sXw = reinterpret_cast<double*>(smem + (size_t)kLossStages * kLossABytes);          // [WC*16][LD]
+    double* s_afr = sXw + (size_t)WC * 16 * LD;                                                 // [(Q/8)(Q/4)][32]
+    double* s_node = s_afr + (KX_QMAX / 8) * (KX_QMAX / 4) * 32;                                // [QMAX]
+    double* s_tab = s_node + KX_QMAX;                                                           // [256]
+    double* s_G = reinterpret_cast<double*>(smem);                                              // [JB][Q][GS] (aliases the stages)
+    static_assert((size_t)JB * KX_QMAX * GS * 8 <= (size_t)kLossStages * kLossABytes, "coefficient scratch must fit the stages");
+    if (logm) {
+        for (int k = tid; k < (Q / 8) * (Q / 4) * 32; k += NTHR) {
+            const int ln = k & 31, fr = k >> 5, ct = fr / (Q / 4), ks = fr - ct * (Q / 4);
+            s_afr[k] = t.dct[(8 * ct + (ln >> 2)) * Q + 4 * ks + (ln & 3)];
+        }
+        if (tid < Q) s_node[tid] = t.nodes[tid];
+        if (tab) for (int k = tid; k < (1 << KX_EXP_BITS); k += NTHR) s_tab[k] = dk.exptab[k];
+    }
+    __syncthreads();
+
+    // Chebyshev coefficients a_c(b, j) of the window's k = (j, c) rows, k in [K0, K0 + 16 wn), straight into shared
+    // memory.  LOG: g(omega_q) = 2^(y_j + omega_q (y_(j+1) - y_j)) at the Q
+    // Chebyshev nodes, then the discrete Chebyshev transform as a (Q x Q) x (Q x 8 NBT) product on the tensor pipe;
+    // LINEAR: a_0 = (f_j + f_(j+1))/2, a_1 = (f_(j+1) - f_j)/2.  Also the member statistics (flags) of kx_internal.cuh.
+    auto build_window = [&](unsigned K0, unsigned wn) {
+        const unsigned K1 = K0 + 16u * wn;
+        const int jlo = (int)(K0 / (unsigned)Q);
+        const int jhi = min((int)((K1 - 1u) / (unsigned)Q), N_ - 2);
+        // rows beyond the last bracket are padding: zero
+        {
+            const unsigned kpad = (unsigned)(N_ - 1) * (unsigned)Q;
+            for (unsigned k = max(K0, kpad) + (unsigned)warp; k < K1; k += WARPS)
+                for (int c2 = lane; c2 < LD; c2 += 32) sXw[(size_t)(k - K0) * LD + c2] = 0.0;
+        }
+        const int jj = tid / MB, bl = tid % MB;
+        if (!logm) {          // LINEAR: two exact coefficients per bracket, no transform: one flat loop
+            const int total = (jhi - jlo + 1) * MB;
+            for (int i0 = tid; i0 < total; i0 += 8 * NTHR) {          // 16 independent loads in flight per thread
+                double v0[8], v1[8];
+#pragma unroll
+                for (int u2 = 0; u2 < 8; ++u2) {
+                    const int idx = i0 + u2 * NTHR, j = jlo + idx / MB, bm = idx % MB, b = bcol0 + bm;
+                    const bool ok = idx < total && b < B;
+                    v0[u2] = ok ? __ldcg(f + (size_t)b * N_ + j) : 0.0;
+                    v1[u2] = ok ? __ldcg(f + (size_t)b * N_ + j + 1) : 0.0;
+                }
+#pragma unroll
+                for (int u2 = 0; u2 < 8; ++u2) {
+                    const int idx = i0 + u2 * NTHR, j = jlo + idx / MB, bm = idx % MB;
+                    if (idx < total) {
+                        const unsigned k = (unsigned)j * 2u;
+                        if (k >= K0 && k < K1) sXw[(size_t)(k - K0) * LD + bm] = 0.5 * (v0[u2] + v1[u2]);
+                        if (k + 1 >= K0 && k + 1 < K1) sXw[(size_t)(k + 1 - K0) * LD + bm] = 0.5 * (v1[u2] - v0[u2]);
+                    }
+                }
+            }
+            __syncthreads();
+            return;
+        }
+        // the f values of a pass are requested one pass ahead
+        auto fetch = [&](int j0, double& a0, double& a1) {
+            const int j = j0 + jj, b = bcol0 + bl;
+            a0 = 0.0; a1 = 0.0;
+            if (jj < JB && j <= jhi && b < B) { a0 = __ldcg(f + (size_t)b * N_ + j); a1 = __ldcg(f + (size_t)b * N_ + j + 1); }
+        };
+        double fnx0, fnx1;
+        fetch(jlo, fnx0, fnx1);
+        for (int j0 = jlo; j0 <= jhi; j0 += JB) {
+            const int j = j0 + jj;
+            const bool valid = jj < JB && j <= jhi;
+            const int b = bcol0 + bl;
+            const double fj = fnx0, fj1 = fnx1;
+            if (j0 + JB <= jhi) fetch(j0 + JB, fnx0, fnx1);
+            if (valid && b < B) atomicMax(mstat + 2 * b + 1, __double_as_longlong(fmax(fabs(fj), fabs(fj1))));
+            if (valid) {
+                const double y0 = log2(fmax(fj, dk.f_floor)), y1 = log2(fmax(fj1, dk.f_floor)), dy = y1 - y0;
+                const double cabs = 0.6931471805599453 * fabs(dy);
+                // log2 of the bracket's error bound (log2 max_i f_i is subtracted by the consumers); the atomics return
+                // nothing, so nobody waits for them
+                if (b < B && cabs > 0.0)
+                    atomicMax(mstat + 2 * b, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
+                double* g = s_G + (size_t)jj * Q * GS + bl;
+                // Q is a multiple of 8: eight independent exp2 chains at a time
+                if (tab) {
+                    for (int q0 = 0; q0 < Q; q0 += 8) {
+                        double e[8];
+#pragma unroll
+                        for (int u2 = 0; u2 < 8; ++u2) e[u2] = kx_exp2_tab<1>(fma(s_node[q0 + u2], dy, y0), s_tab);
+#pragma unroll
+                        for (int u2 = 0; u2 < 8; ++u2) g[(q0 + u2) * GS] = e[u2];
+                    }
+                } else {
+                    for (int q = 0; q < Q; ++q) g[q * GS] = exp2(fma(s_node[q], dy, y0));
+                }
+            }
+            __syncthreads();
+            // transform: a task is (bracket of the pass, member tile); the 8 warps take 32 tasks at a time, 4 each, with
+            // 4 x (Q/8) independent accumulator chains so that the DMMA latency of one hides behind the others
+            for (int base = 0; base < JB * NBT; base += 32) {
+                double D[4][KX_QMAX / 8][2];
+                int tj[4], tm[4];
+#pragma unroll
+                for (int u2 = 0; u2 < 4; ++u2) {
+                    const int idx = base + warp + 8 * u2;
+                    tj[u2] = (idx < JB * NBT && j0 + idx / NBT <= jhi) ? idx / NBT : -1;
+                    tm[u2] = idx % NBT;
+#pragma unroll
+                    for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[u2][ct][0] = D[u2][ct][1] = 0.0;
+                }
+#pragma unroll
+                for (int ks = 0; ks < KX_QMAX / 4; ++ks) {
+                    if (4 * ks < Q) {
+                        double afr[KX_QMAX / 8];
+#pragma unroll
+                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) afr[ct] = 8 * ct < Q ? s_afr[(ct * (Q / 4) + ks) * 32 + lane] : 0.0;
+#pragma unroll
+                        for (int u2 = 0; u2 < 4; ++u2) {
+                            if (tj[u2] >= 0) {          // uniform over the warp
+                                const double gv = s_G[((size_t)tj[u2] * Q + 4 * ks + krow) * GS + 8 * tm[u2] + lr];
+#pragma unroll
+                                for (int ct = 0; ct < KX_QMAX / 8; ++ct)
+                                    if (8 * ct < Q) dmma884(D[u2][ct][0], D[u2][ct][1], afr[ct], gv);
+                            }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int u2 = 0; u2 < 4; ++u2) {
+                    if (tj[u2] >= 0) {
+#pragma unroll
+                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) {
+                            if (8 * ct < Q) {
+                                const unsigned k = (unsigned)(j0 + tj[u2]) * (unsigned)Q + 8u * ct + (unsigned)lr;
+                                if (k >= K0 && k < K1)
+                                    *reinterpret_cast<double2*>(sXw + (size_t)(k - K0) * LD + 8 * tm[u2] + 2 * krow) = make_double2(D[u2][ct][0], D[u2][ct][1]);
+                            }
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        __syncthreads();
+    };
+
+    const unsigned cl = blockIdx.x - GG;
+    const unsigned LC = (unsigned)t.LC;
+    const unsigned U = (unsigned)t.RS * LC;
+    const unsigned u0 = (unsigned)((unsigned long long)cl * U / (unsigned)GL);
+    const unsigned u1 = (unsigned)((unsigned long long)(cl + 1) * U / (unsigned)GL);
+    unsigned u = u0;
+    bool first = true;
+    while (u < u1) {
+        const unsigned sp = u / LC;                                  // supertile
+        const unsigned ue = min(u1, (sp + 1) * LC);
+        const unsigned ka = u - sp * LC, n = ue - u;
+        const int nb = min(32, t.NR8 - 32 * (int)sp);                // 8-row blocks of this supertile
+        const int nbw = min(R8, max(0, nb - R8 * warp));             // ... of this warp
+
+        // every warp streams its own rows of the tensor (4 KiB per chunk: 4 eight-row blocks) through a private
+        // cp.async ring: no CTA-wide barrier inside a window
+        unsigned char* wring = sStage + (size_t)warp * (kLossStages * kLossABytes / WARPS);
+        constexpr int kWStage = kLossABytes / WARPS;                  // 4 KiB
+        auto issue = [&](unsigned kc, int slot) {
+            if (nbw > 0) {
+                const double* srcA = t.AL + ((size_t)kc * t.NR8 + 32 * sp + R8 * warp) * 128;
+                unsigned char* dstA = wring + (size_t)slot * kWStage;
+                for (int k = lane; k < nbw * 64; k += 32) cp_async16(dstA + (size_t)k * 16, srcA + (size_t)k * 2);
+            }
+        };
+
+        double acc[R8][NBT][2];
+#pragma unroll
+        for (int r = 0; r < R8; ++r)
+#pragma unroll
+            for (int bt = 0; bt < NBT; ++bt) acc[r][bt][0] = acc[r][bt][1] = 0.0;
+
+        for (unsigned w0 = 0; w0 < n; w0 += (unsigned)WC) {
+            const unsigned wn = min((unsigned)WC, n - w0), kw = ka + w0;
+            build_window(16u * kw, wn);          // ends with a barrier: the scratch (= the rings) is free again
+            if (first && tid == 0) stamp(trace, 1);
+            first = false;
+#pragma unroll
+            for (int s2 = 0; s2 < kLossStages - 1; ++s2) {
+                if ((unsigned)s2 < wn) issue(kw + s2, s2);
+                cp_async_commit();
+            }
+            for (unsigned it = 0; it < wn; ++it) {
+                if (it + kLossStages - 1 < wn) issue(kw + it + kLossStages - 1, (int)((it + kLossStages - 1) % kLossStages));
+                cp_async_commit();
+                cp_async_wait<kLossStages - 1>();        // chunk `it` of this warp has landed
+                __syncwarp();
+                if (nbw > 0) {
+                    const double* sA = reinterpret_cast<const double*>(wring + (size_t)(it % kLossStages) * kWStage) + lane;
+                    const double* sX = sXw + (size_t)(16 * it + krow) * LD + lr;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        double xv[NBT];
+#pragma unroll
+                        for (int bt = 0; bt < NBT; ++bt) xv[bt] = sX[(size_t)(4 * q) * LD + 8 * bt];
+#pragma unroll
+                        for (int r = 0; r < R8; ++r) {
+                            const double w = sA[(r * 4 + q) * 32];
+#pragma unroll
+                            for (int bt = 0; bt < NBT; ++bt) dmma884(acc[r][bt][0], acc[r][bt][1], xv[bt], w);
+                        }
+                    }
+                }
+                __syncwarp();                            // the stage is refilled two iterations from now
+            }
+            cp_async_wait<0>();
+            __syncthreads();              // the rings are free again (next window's scratch, next piece)
+        }
+
+        double* dst = lpart + ((size_t)(cl + sp) * xstride + bcol0) * 256 + 8 * R8 * warp + 2 * krow;
+#pragma unroll
+        for (int r = 0; r < R8; ++r)
+            if (r < nbw)
+#pragma unroll
+                for (int bt = 0; bt < NBT; ++bt)
+                    *reinterpret_cast<double2*>(dst + (size_t)(8 * bt + lr) * 256 + 8 * r) = make_double2(acc[r][bt][0], acc[r][bt][1]);
+        u = ue;
+    }
+}
+
+// ---------------------------------------------------------------- the fused kernel: one CTA per SM, cooperative
+// Clock stamps (st.trace, per CTA): 0 entry, 1 prologue done (f staged / first coefficient window built), 2 partials
+// written, 3 first barrier passed, 4 fallback done, 5 finishing phase done; 8..15 end of each gain warp's stream.
+template <int NBT, int STAGES>
+__global__ void __launch_bounds__(NTHR, 1)
+k_dmma(KxDev dk, KxTiled t, KxPlan plan, int B, const double* __restrict__ f, KxStage st)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ double s_red[8 * 8];
+    __shared__ int s_wtile[WARPS];
+    const int tid = threadIdx.x, N = dk.N;
+    if (tid == 0) stamp(st.trace, 0);
+
+    const int ny = (B + NBT * 8 - 1) / (NBT * 8);
+    for (int by = 0; by < ny; ++by) {          // member groups of 8 NBT: one pass each (more than one for B > 64 only)
+        const int bcol0 = by * NBT * 8;
+        if ((int)blockIdx.x < plan.GG) gain_role<NBT, STAGES>(t, plan, N, B, bcol0, f, st.xstride, st.gpart, smem, s_wtile, st.trace);
+        else loss_role<NBT>(dk, t, plan, N, B, bcol0, f, st.mstat, st.xstride, st.lpart, smem, st.trace);
+        __syncthreads();
+    }
+    if (tid == 0) stamp(st.trace, 2);
+    grid_barrier(st.bar, st.epoch);
+    if (tid == 0) stamp(st.trace, 3);
+
+    // members whose interpolation error bound is not negligible (rare): exact streaming contraction of their groups of
+    // KX_FB_BT members, the tasks dealt to all CTAs; every CTA takes the same decisions from the same statistics
+    bool any = false;
+    if (st.mstat) {
+        for (int b0 = 0; b0 < B; b0 += NTHR) any |= __syncthreads_or(b0 + tid < B && member_flagged(st.mstat, b0 + tid)) != 0;
+    }
+    if (any) {
+        for (int g0 = 0; g0 < B; g0 += KX_FB_BT) {
+            const int hit = __syncthreads_or(tid < KX_FB_BT && g0 + tid < B && member_flagged(st.mstat, g0 + tid));
+            if (!hit) continue;
+            if (dk.exp_impl == KX_EXP_LIBM) contract_group<KX_FB_BT, MODE_LOG_LIBM, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
+            else contract_group<KX_FB_BT, MODE_LOG_TAB, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
+        }
+        grid_barrier(st.bar, st.epoch + 1u);
+    }
+    if (tid == 0) stamp(st.trace, 4);
+
+    if (st.mstat_next && blockIdx.x == gridDim.x - 1)          // clean statistics for the next launch (the other buffer)
+        for (int k = tid; k < st.mstat_cap; k += NTHR) { st.mstat_next[2 * k] = KX_MSTAT_NONE; st.mstat_next[2 * k + 1] = 0; }
+    for (int b = blockIdx.x; b < B; b += gridDim.x) {
+        const bool flagged = st.mstat && member_flagged(st.mstat, b);
+        if (flagged && tid == 0 && st.fb_count) atomicAdd(st.fb_count, 1u);
+        finish_member(dk, f, B, st, &plan, !flagged, b, reinterpret_cast<double*>(smem), s_red);
+    }
+    if (tid == 0) stamp(st.trace, 5);
+}
+
 constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + ((KX_QMAX / 8) * (KX_QMAX / 4) * 32 + KX_QMAX + (1 << KX_EXP_BITS)) * 8;
+constexpr size_t kSmemMax = 226u * 1024u;       // dynamic shared memory: 227 KiB per CTA minus the kernel's static 544 bytes
 
 // chunks of 16 k whose Chebyshev coefficients a loss CTA keeps in shared memory at a time: its whole share if it fits
 int loss_window(const KxTiled& t, int GL, int nbt)
 {
     const long long U = (long long)t.RS * t.LC;
     const long long share = (U + GL - 1) / GL + 1;
-    const long long fit = (long long)((227u * 1024u - kLossFixedBytes) / ((size_t)16 * (nbt * 8 + 4) * 8));
+    const long long fit = (long long)((kSmemMax - kLossFixedBytes) / ((size_t)16 * (nbt * 8 + 4) * 8));
     long long wc = share < fit ? share : fit;
     return (int)(wc < 1 ? 1 : wc);
 }
 
-template <int NBT, int WARPS, int STAGES>
-size_t dmma_smem(const KxTiled& t, int N, int WC)
+int dmma_stages(int nbt) { return nbt <= 2 ? 8 : 4; }
+
+size_t dmma_smem(int nbt, int N, int WC)
 {
-    const size_t gain = (size_t)(((t.NT + 1) * 4 + 15) & ~15) + (size_t)(NBT * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * STAGES * kStageBytes;
-    const size_t loss = kLossFixedBytes + (size_t)WC * 16 * (NBT * 8 + 4) * 8;
-    return gain > loss ? gain : loss;
+    const size_t gain = (size_t)(nbt * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * dmma_stages(nbt) * kStageBytes;
+    const size_t loss = kLossFixedBytes + (size_t)WC * 16 * (nbt * 8 + 4) * 8;
+    const size_t fb = contract_smem<KX_FB_BT, MODE_LOG_TAB, 0>(N);
+    const size_t fin = finish_scratch_doubles(N) * 8;
+    size_t m = gain > loss ? gain : loss;
+    if (fb > m) m = fb;
+    if (fin > m) m = fin;
+    return m;
 }
 
-template <int NBT, int WARPS, int STAGES>
-cudaError_t launch_dmma_t(const KxDev& d, const KxTiled& t, unsigned Gtot, int GG, int GL, const double* f, long long* mstat,
-                          int xstride, double* gpart, double* lpart, int B, cudaStream_t s)
-{
-    const int WC = loss_window(t, GL, NBT);
-    const size_t smem = dmma_smem<NBT, WARPS, STAGES>(t, d.N, WC);
-    cudaError_t e = cudaFuncSetAttribute(k_dmma<NBT, WARPS, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid(GG + GL, (B + NBT * 8 - 1) / (NBT * 8));
-    // first kernel of the call: ordinary launch
-    return kx_launch(k_dmma<NBT, WARPS, STAGES>, grid, dim3(WARPS * 32), smem, s, false, d, t, d.N, B, Gtot, f, mstat, xstride,
-                     gpart, lpart, GG, GL, WC);
-}
-
-// member tiles (of 8) per CTA: limited by the batch and by the shared memory f^T of the gain role needs
-int kx_dmma_warps(int nbt) { (void)nbt; return 8; }
+// member tiles (of 8) per pass: limited by the batch and by the shared memory the rows of f need in the gain role
 int dmma_nbt(int N, int B)
 {
     int nbt = B <= 8 ? 1 : (B <= 16 ? 2 : (B <= 32 ? 4 : 8));
-    auto need = [&](int k) { return (size_t)(k * 8) * ((N + 7) & ~3) * 8 + (size_t)kx_dmma_warps(k) * (k <= 2 ? 8 : 4) * kStageBytes + 512; };
-    while (nbt > 1 && need(nbt) > 227u * 1024u) nbt >>= 1;
+    auto need = [&](int k) { return (size_t)(k * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * dmma_stages(k) * kStageBytes + 512; };
+    while (nbt > 1 && need(nbt) > kSmemMax) nbt >>= 1;
     return nbt;
+}
+
+template <int NBT, int STAGES>
+cudaError_t launch_dmma_t(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B, const KxStage& st,
+                          cudaStream_t s)
+{
+    const size_t smem = dmma_smem(NBT, d.N, plan.WC);
+    return kx_launch_coop(k_dmma<NBT, STAGES>, dim3(plan.GG + plan.GL), dim3(NTHR), smem, s, d, t, plan, B, f, st);
 }
 
 }  // namespace
 
-int kx_dmma_workers(int N, int B) { return kx_dmma_warps(dmma_nbt(N, B)); }
-
-// columns of the partials for a batch of B members: whole 8-member MMA tiles, whole CTA column groups
+// columns of the partials for a batch of B members: whole 8-member MMA tiles, whole passes
 int kx_xstride(int B)
 {
     if (B <= 8) return 8;
@@ -505,31 +596,80 @@ int kx_xstride(int B)
     return ((B + 63) / 64) * 64;
 }
 
-// CTAs per role.  Work in units of one gain group (8 DMMA per member tile): gain = groups, loss = LC * NR8 / 2.
-void kx_dmma_split(const KxDev& d, const KxTiled& t, int sm_count, long long groups, int B, int* GG, int* GL)
+cudaError_t kx_dmma_configure()
+{
+    static bool done = false;
+    if (done) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(k_dmma<1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    done = e == cudaSuccess;
+    return e;
+}
+
+// The plan of one launch.  Work in units of one gain group (8 DMMA per member tile): gain = groups, loss = LC NR8 / 2
+// (weighted by kLossCost).  Every CTA must be resident (grid barrier): at most one per SM.  The gain warps are dealt to the
+// tiles in proportion to the tiles' groups (largest remainder), at least one and at most one per group.
+void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned* vt_host, int B, KxPlan* plan)
 {
     const int nbt = dmma_nbt(d.N, B);
-    const int ny = (B + nbt * 8 - 1) / (nbt * 8);
-    const double wg = (double)(groups > 0 ? groups : 1);
+    const unsigned Gtot = vt_host[t.NT];
+    const double wg = (double)(Gtot > 0 ? Gtot : 1);
     const double wl = 0.5 * (double)t.LC * (double)t.NR8 * kLossCost;
     long long G = (long long)((wg + wl) / 8.0);
-    const long long cap = sm_count / ny > 2 ? sm_count / ny : 2;
-    if (G > cap) G = cap;
+    if (G > sm_count) G = sm_count;
     if (G < 2) G = 2;
     int gl = (int)((double)G * wl / (wg + wl) + 0.5);
     if (gl < 1) gl = 1;
     if (gl > (int)G - 1) gl = (int)G - 1;
-    *GL = gl;
-    *GG = (int)G - gl;
+    const long long U = (long long)t.RS * t.LC;
+    if (gl > U) gl = (int)U;                       // every loss CTA has at least one chunk
+    plan->nbt = nbt;
+    plan->GL = gl;
+    plan->GG = (int)G - gl;
+    plan->WC = loss_window(t, gl, nbt);
+
+    const int NT = t.NT;
+    const unsigned NW = (unsigned)plan->GG * WARPS;
+    std::vector<unsigned> w(NT, 0u), g(NT, 0u);
+    unsigned used = 0;
+    for (int k = 0; k < NT; ++k) {
+        g[k] = vt_host[k + 1] - vt_host[k];
+        if (g[k]) {
+            unsigned v = (unsigned)((unsigned long long)NW * g[k] / Gtot);
+            if (v < 1) v = 1;
+            if (v > g[k]) v = g[k];
+            w[k] = v; used += v;
+        }
+    }
+    while (used > NW) {            // the minimum of one warp per tile overshot: take from the lightest-loaded warps
+        int best = -1;
+        for (int k = 0; k < NT; ++k)
+            if (w[k] > 1 && (best < 0 || (unsigned long long)g[k] * w[best] < (unsigned long long)g[best] * w[k])) best = k;
+        if (best < 0) break;
+        --w[best]; --used;
+    }
+    while (used < NW) {            // left-over warps go where a warp has the most groups
+        int best = -1;
+        for (int k = 0; k < NT; ++k)
+            if (w[k] < g[k] && (best < 0 || (unsigned long long)g[k] * w[best] > (unsigned long long)g[best] * w[k])) best = k;
+        if (best < 0) break;
+        ++w[best]; ++used;
+    }
+    unsigned run = 0;
+    for (int k = 0; k < NT; ++k) { plan->wstart[k] = run; plan->vt[k] = vt_host[k]; run += w[k]; }
+    plan->wstart[NT] = run; plan->vt[NT] = vt_host[NT];
+    for (int k = NT + 1; k <= KX_MAX_NT; ++k) { plan->wstart[k] = run; plan->vt[k] = vt_host[NT]; }
 }
 
-cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, long long groups, int GG, int GL, const double* f,
-                           long long* mstat, int xstride, double* gpart, double* lpart, int B, cudaStream_t s)
+cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B,
+                           const KxStage& st, cudaStream_t s)
 {
-    switch (dmma_nbt(d.N, B)) {
-        case 1: return launch_dmma_t<1, 8, 8>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
-        case 2: return launch_dmma_t<2, 8, 8>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
-        case 4: return launch_dmma_t<4, 8, 4>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
-        default: return launch_dmma_t<8, 8, 4>(d, t, (unsigned)groups, GG, GL, f, mstat, xstride, gpart, lpart, B, s);
+    switch (plan.nbt) {
+        case 1: return launch_dmma_t<1, 8>(d, t, plan, f, B, st, s);
+        case 2: return launch_dmma_t<2, 8>(d, t, plan, f, B, st, s);
+        case 4: return launch_dmma_t<4, 4>(d, t, plan, f, B, st, s);
+        default: return launch_dmma_t<8, 4>(d, t, plan, f, B, st, s);
     }
 }

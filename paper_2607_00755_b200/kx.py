@@ -75,7 +75,9 @@ class _AdaptiveResult(C.Structure):
 # every symbol include/kx.h declares
 SYMBOLS = ["kx_build", "kx_set_mass", "kx_collide", "kx_collide_parts", "kx_collide_ex",
            "kx_collide_host", "kx_moments", "kx_evolve", "kx_evolve_adaptive", "kx_delta_source", "kx_info", "kx_tensor_export",
-           "kx_kinematics_export", "kx_profile", "kx_profile_read", "kx_probe_flops", "kx_last_error", "kx_destroy", "kx_version"]
+           "kx_kinematics_export", "kx_reserve", "kx_fallback_members", "kx_profile", "kx_profile_read", "kx_trace", "kx_trace_read",
+           "kx_probe_flops", "kx_last_error", "kx_destroy", "kx_version"]
+TRACE_CTAS, TRACE_SLOTS = 160, 32
 
 _lib = None
 
@@ -118,6 +120,10 @@ def _load():
     lib.kx_info.argtypes = [vp, i64p, i64p, C.POINTER(i32)]
     lib.kx_tensor_export.argtypes = [vp, C.c_int64, i64p, _dp, _dp, C.POINTER(C.c_uint32)]
     lib.kx_kinematics_export.argtypes = [vp, _dp, _dp, _dp]
+    lib.kx_reserve.argtypes = [vp, i32, vp]
+    lib.kx_fallback_members.argtypes = [vp, i64p]
+    lib.kx_trace.argtypes = [vp, i32]
+    lib.kx_trace_read.argtypes = [vp, C.POINTER(C.c_uint64)]
     lib.kx_profile.argtypes = [vp, i32]
     lib.kx_profile_read.argtypes = [vp, _dp, i64p]
     lib.kx_probe_flops.argtypes = [C.c_int, i32, _dp]
@@ -321,6 +327,25 @@ class Handle:
         G = torch.empty(self.N, dtype=torch.float64, device=f"cuda:{self.device}")
         self._check(self._lib.kx_delta_source(self._h, float(p0), C.c_void_p(G.data_ptr()), _stream(stream)))
         return G
+
+    def reserve(self, B, stream=None):
+        """kx_reserve: allocate workspaces and launch plan for batches up to B now (later calls only enqueue work)."""
+        self._check(self._lib.kx_reserve(self._h, int(B), _stream(stream)))
+
+    def fallback_members(self):
+        """kx_fallback_members: (member, evaluation) pairs that took the exact fallback since the last call."""
+        n = C.c_int64()
+        self._check(self._lib.kx_fallback_members(self._h, C.byref(n)))
+        return int(n.value)
+
+    def trace(self, enable=True):
+        self._check(self._lib.kx_trace(self._h, int(bool(enable))))
+
+    def trace_read(self):
+        """kx_trace_read: %globaltimer stamps [160 CTAs, 32 slots] (ns, 0 = not written) of the last launches."""
+        out = np.zeros((TRACE_CTAS, TRACE_SLOTS), dtype=np.uint64)
+        self._check(self._lib.kx_trace_read(self._h, out.ctypes.data_as(C.POINTER(C.c_uint64))))
+        return out
 
     def profile(self, enable=True):
         self._check(self._lib.kx_profile(self._h, int(bool(enable))))
