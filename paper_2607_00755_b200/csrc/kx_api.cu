@@ -203,10 +203,10 @@ kx_status_t launch_step(kx_handle_s* h, const double* f, int B, bool have_yd, bo
             st->mstat_cap = h->wsB;
         }
         st->NT = h->t.NT; st->LC = h->t.LC; st->RS = h->t.RS;
-        KX_CUDA(kx_launch_dmma(h->d, h->t, h->plan, f, B, *st, s));
+        KX_CUDA(kx_launch_dmma(h->d, h->t, h->plan, f, B, *st, &h->bar_total, s));
     } else {
         st->gpart = nullptr; st->lpart = nullptr; st->mstat = nullptr; st->mstat_next = nullptr;
-        KX_CUDA(kx_launch_stream(h->d, h->sm_count, f, have_yd ? h->yd : nullptr, B, *st, s));
+        KX_CUDA(kx_launch_stream(h->d, h->sm_count, f, have_yd ? h->yd : nullptr, B, *st, &h->bar_total, s));
     }
     if (h->profiling) {
         KX_CUDA(cudaEventRecord(h->prof_events[h->prof_used].second, s));

@@ -15,6 +15,20 @@ namespace {
 
 using namespace kxd;
 
+// barrier and finishing phase, NQ = ceil(N / 256) rows per thread
+template <int NQ>
+__device__ __forceinline__ void stream_tail(const KxDev& d, const double* __restrict__ f, int B, const KxStage& st,
+                                            unsigned char* smem_raw, double* s_red)
+{
+    const unsigned cta = blockIdx.y * gridDim.x + blockIdx.x, nctas = gridDim.x * gridDim.y;
+    FinishPre<NQ> pre;
+    if ((int)cta < B) finish_preload<NQ>(d, f, (int)cta, pre);    // static inputs of the finishing phase: before the barrier
+    grid_barrier_count(st.bar + 3, st.bar_target);
+    if (threadIdx.x == 0) stamp(st.trace, 2);
+    for (int b = (int)cta; b < B; b += (int)nctas)
+        finish_member<NQ>(d, f, B, st, nullptr, false, b, reinterpret_cast<double*>(smem_raw), s_red, b == (int)cta ? &pre : nullptr);
+}
+
 // grid (gx, gy): CTA (x, y) takes the member groups y, y + gy, ... and of each the tasks x, x + gx, ...; after the grid
 // barrier CTA c = y gx + x finishes the members c, c + gx gy, ...
 template <int BT, int MODE, int QS>
@@ -28,11 +42,9 @@ k_stream(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd, 
     for (int g = blockIdx.y; g < groups; g += gridDim.y)
         contract_group<BT, MODE, QS>(d, f, yd, st.part, B, g * BT, blockIdx.x, gridDim.x, smem_raw);
     if (threadIdx.x == 0) stamp(st.trace, 1);
-    grid_barrier(st.bar, st.epoch);
-    if (threadIdx.x == 0) stamp(st.trace, 2);
-    const unsigned cta = blockIdx.y * gridDim.x + blockIdx.x, nctas = gridDim.x * gridDim.y;
-    for (int b = (int)cta; b < B; b += (int)nctas)
-        finish_member(d, f, B, st, nullptr, false, b, reinterpret_cast<double*>(smem_raw), s_red);
+    if (d.N <= KX_CTA) stream_tail<1>(d, f, B, st, smem_raw, s_red);
+    else if (d.N <= 2 * KX_CTA) stream_tail<2>(d, f, B, st, smem_raw, s_red);
+    else stream_tail<4>(d, f, B, st, smem_raw, s_red);
     if (threadIdx.x == 0) stamp(st.trace, 3);
 }
 
@@ -128,12 +140,12 @@ template <int BT, int MODE, int QS>
 StreamCfg& stream_cfg() { static StreamCfg c = {false, 0, 0}; return c; }
 
 template <int BT, int MODE, int QS>
-cudaError_t launch_stream_t(const KxDev& d, int sm_count, const double* f, const double* yd, int B, const KxStage& st,
-                            cudaStream_t s)
+cudaError_t launch_stream_t(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st,
+                            unsigned* bar_total, cudaStream_t s)
 {
     const int N = d.N;
     size_t smem = contract_smem<BT, MODE, QS>(N);
-    const size_t fin = (size_t)N * 8;
+    const size_t fin = finish_scratch_bytes(N, 0, 0, 0, 0);
     if (smem < fin) smem = fin;
     StreamCfg& c = stream_cfg<BT, MODE, QS>();
     cudaError_t e;
@@ -157,21 +169,24 @@ cudaError_t launch_stream_t(const KxDev& d, int sm_count, const double* f, const
     const long long tasks_bound = (long long)N + (long long)N * ((long long)N * (N + 1) / 2) / (d.chunk > 0 ? d.chunk : 1024);
     if ((long long)gx > tasks_bound) gx = (int)tasks_bound;
     if (gx < 1) gx = 1;
-    return kx_launch_coop(k_stream<BT, MODE, QS>, dim3(gx, gy), dim3(KX_CTA), smem, s, d, f,
-                          reinterpret_cast<const double2*>(yd), B, st);
+    st.bar_target = *bar_total + (unsigned)(gx * gy);
+    e = kx_launch_coop(k_stream<BT, MODE, QS>, dim3(gx, gy), dim3(KX_CTA), smem, s, d, f,
+                       reinterpret_cast<const double2*>(yd), B, st);
+    if (e == cudaSuccess) *bar_total = st.bar_target;
+    return e;
 }
 
 template <int BT>
-cudaError_t launch_stream_m(const KxDev& d, int sm_count, const double* f, const double* yd, int B, const KxStage& st,
-                            cudaStream_t s)
+cudaError_t launch_stream_m(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st,
+                            unsigned* bar_total, cudaStream_t s)
 {
     if (d.eta) {         // quantum statistics: LOG interpolation only (checked in kx_build)
-        if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 1>(d, sm_count, f, yd, B, st, s);
-        return launch_stream_t<BT, MODE_LOG_TAB, 1>(d, sm_count, f, yd, B, st, s);
+        if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 1>(d, sm_count, f, yd, B, st, bar_total, s);
+        return launch_stream_t<BT, MODE_LOG_TAB, 1>(d, sm_count, f, yd, B, st, bar_total, s);
     }
-    if (d.interp == KX_INTERP_LINEAR) return launch_stream_t<BT, MODE_LINEAR, 0>(d, sm_count, f, yd, B, st, s);
-    if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 0>(d, sm_count, f, yd, B, st, s);
-    return launch_stream_t<BT, MODE_LOG_TAB, 0>(d, sm_count, f, yd, B, st, s);
+    if (d.interp == KX_INTERP_LINEAR) return launch_stream_t<BT, MODE_LINEAR, 0>(d, sm_count, f, yd, B, st, bar_total, s);
+    if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 0>(d, sm_count, f, yd, B, st, bar_total, s);
+    return launch_stream_t<BT, MODE_LOG_TAB, 0>(d, sm_count, f, yd, B, st, bar_total, s);
 }
 
 }  // namespace
@@ -196,13 +211,13 @@ int kx_pick_chunk(long long nnz_est, int N, int B, int sm_count)
 }
 
 cudaError_t kx_launch_stream(const KxDev& d, int sm_count, const double* f, const double* yd, int B,
-                             const KxStage& st, cudaStream_t s)
+                             KxStage st, unsigned* bar_total, cudaStream_t s)
 {
     switch (kx_pick_bt(d.N, B)) {
-        case 1: return launch_stream_m<1>(d, sm_count, f, yd, B, st, s);
-        case 2: return launch_stream_m<2>(d, sm_count, f, yd, B, st, s);
-        case 4: return launch_stream_m<4>(d, sm_count, f, yd, B, st, s);
-        default: return launch_stream_m<8>(d, sm_count, f, yd, B, st, s);
+        case 1: return launch_stream_m<1>(d, sm_count, f, yd, B, st, bar_total, s);
+        case 2: return launch_stream_m<2>(d, sm_count, f, yd, B, st, bar_total, s);
+        case 4: return launch_stream_m<4>(d, sm_count, f, yd, B, st, bar_total, s);
+        default: return launch_stream_m<8>(d, sm_count, f, yd, B, st, bar_total, s);
     }
 }
 

@@ -63,14 +63,32 @@ __device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned epoch)
     __syncthreads();
 }
 
-// statistics written by other CTAs of the same launch: read through L2
+// The first barrier of a launch, cheaper: a counter that only grows (bar[3]); the host knows how many CTAs every launch
+// adds and hands each launch its target.  Everybody polls the counter itself: one L2 round trip less than the epoch form.
+__device__ __forceinline__ void grid_barrier_count(unsigned* ctr, unsigned target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(ctr, 1u);
+        while ((int)(ld_acquire(ctr) - target) < 0) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// statistics written by other CTAs of the same launch: read through L2, one 16-byte load
 __device__ __forceinline__ bool member_flagged(const long long* mstat, int b)
 {
-    const double fm = __longlong_as_double(__ldcg(mstat + 2 * b + 1));
+    const longlong2 v = __ldcg(reinterpret_cast<const longlong2*>(mstat) + b);
+    const double fm = __longlong_as_double(v.y);
     if (!isfinite(fm)) return true;                        // Inf / NaN in f: the exact path treats them entry by entry
-    const long long k = __ldcg(mstat + 2 * b);
+    const long long k = v.x;
     if (k == KX_MSTAT_NONE) return false;
     const double lb = __longlong_as_double(k >= 0 ? k : (k ^ 0x7fffffffffffffffLL));
+    // log2(fm) >= its unbiased exponent: far below the threshold (the usual case) without evaluating the logarithm
+    const int ex = (int)((v.y >> 52) & 0x7ff) - 1023;
+    if (v.y != 0 && lb - (double)ex <= -49.82892142331043) return false;
     return lb - log2(fm) > -49.82892142331043;             // log2(1e-15)
 }
 
@@ -272,60 +290,72 @@ __device__ __forceinline__ double block_max(double v, double* s_red)
     return a;
 }
 
-__device__ __forceinline__ double4 ldcg4(const double* p)
+// ---------------------------------------------------------------- bulk copies (TMA, 1-D) and their mbarrier
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
 {
-    const double2 a = __ldcg(reinterpret_cast<const double2*>(p)), b = __ldcg(reinterpret_cast<const double2*>(p) + 1);
-    return make_double4(a.x, a.y, b.x, b.y);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_addr(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" :: "r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+// global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completion is signalled on `bar`
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+// orders earlier generic-proxy accesses (other CTAs' stores made visible by the grid barrier, this CTA's own shared-memory
+// traffic) before the async-proxy copies that follow
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 // ---------------------------------------------------------------- partials of the DMMA phase -> (gain, nu)[b, i]
 // gain: tile = i/16; the warps [wstart[tile], wstart[tile+1]) of the plan worked on it, i.e. the CTAs c0 = wstart[tile]/8
 // ... c1 = (wstart[tile+1]-1)/8, each of which wrote one partial into slot c + tile.  loss: supertile = i/256, chunk units
-// [sp LC, (sp+1) LC) of the RS LC units were taken by the loss CTAs d0..d1, slot = c + sp.  A thread adds the partials of
-// 4 consecutive rows (32-byte loads) for one of 4 interleaved slot subsets; the 4 subset sums are added in subset order:
-// a fixed order, bit-reproducible.  s_gn: [2][4][Npad], Npad = 4 ceil(N/4).
-constexpr size_t finish_scratch_doubles(int N) { return (size_t)N + 8 * (size_t)((N + 3) & ~3); }
-
-__device__ __forceinline__ void sum_dmma_partials(int N, const KxStage& st, const KxPlan& plan, int b, double* s_gn)
+// [sp LC, (sp+1) LC) of the RS LC units were taken by the loss CTAs ld0[sp]..ld1[sp], slot = c + sp.
+// The member's slice of every slot (128 bytes per gain slot, 2 KiB per loss slot) is fetched into shared memory by bulk
+// copies: about GG + NT + GL instructions for the whole CTA and every byte in flight at once; a thread then adds the
+// partials of its row in slot order: a fixed order, bit-reproducible.
+//   scratch: s_y [Npad] | s_gp [GG + NT][16] | s_lp [sum_sp (ld1 - ld0 + 1)][256]
+__host__ __device__ inline size_t finish_scratch_bytes(int N, int GG, int GL, int NT, int RS)
 {
-    const int tid = threadIdx.x, sub = tid >> 6;
+    return (size_t)((N + 3) & ~3) * 8 + (size_t)(GG + NT) * 128 + (size_t)(GL + RS) * 2048;
+}
+
+__device__ __forceinline__ void gather_partials(int N, const KxStage& st, const KxPlan& plan, int b, double* scratch,
+                                                unsigned long long* mbar)
+{
+    const int tid = threadIdx.x;
     const int Npad = (N + 3) & ~3;
-    const unsigned U = (unsigned)st.RS * (unsigned)st.LC;
-    for (int rq = tid & 63; 4 * rq < N; rq += 64) {
-        const int i0 = 4 * rq, tile = i0 >> 4;
-        double4 g = make_double4(0.0, 0.0, 0.0, 0.0), nu = g;
-        const unsigned w0 = plan.wstart[tile], w1 = plan.wstart[tile + 1];
-        // all loads of an output are in flight together
-        double4 vl[12];
-        const unsigned sp = (unsigned)i0 >> 8;
-        const unsigned l0 = sp * (unsigned)st.LC, l1 = l0 + (unsigned)st.LC;
-        const unsigned d0 = (unsigned)((((unsigned long long)l0 + 1ull) * (unsigned)plan.GL - 1ull) / U);
-        const unsigned d1 = (unsigned)(((unsigned long long)l1 * (unsigned)plan.GL - 1ull) / U);
-        const double* srl = st.lpart + ((size_t)sp * st.xstride + b) * 256 + (i0 & 255);
-#pragma unroll
-        for (int u = 0; u < 12; ++u) {
-            const unsigned c = d0 + (unsigned)sub + 4u * (unsigned)u;
-            vl[u] = c <= d1 ? ldcg4(srl + (size_t)c * st.xstride * 256) : make_double4(0.0, 0.0, 0.0, 0.0);
+    double* s_gp = scratch + Npad;
+    const int ng = plan.GG + st.NT;
+    double* s_lp = s_gp + (size_t)ng * 16;
+    int nl = 0;
+    for (int sp = 0; sp < st.RS; ++sp) nl += (int)(plan.ld1[sp] - plan.ld0[sp] + 1u);
+    fence_proxy_async();
+    if (tid == 0) mbar_expect_tx(mbar, (unsigned)ng * 128u + (unsigned)nl * 2048u);
+    for (int k = tid; k < ng + nl; k += KX_CTA) {
+        if (k < ng) {
+            bulk_g2s(s_gp + (size_t)k * 16, st.gpart + ((size_t)k * st.xstride + b) * 16, 128u, mbar);
+        } else {
+            int kk = k - ng, sp = 0;
+            while (kk >= (int)(plan.ld1[sp] - plan.ld0[sp] + 1u)) { kk -= (int)(plan.ld1[sp] - plan.ld0[sp] + 1u); ++sp; }
+            const unsigned c = plan.ld0[sp] + (unsigned)kk;
+            bulk_g2s(s_lp + (size_t)(k - ng) * 256, st.lpart + ((size_t)(c + sp) * st.xstride + b) * 256, 2048u, mbar);
         }
-        if (w1 > w0) {
-            const unsigned c0 = w0 / kDmmaWarps, c1 = (w1 - 1u) / kDmmaWarps;
-            const double* src = st.gpart + ((size_t)tile * st.xstride + b) * 16 + (i0 & 15);
-#pragma unroll 4
-            for (unsigned c = c0 + (unsigned)sub; c <= c1; c += 4) {
-                const double4 v = ldcg4(src + (size_t)c * st.xstride * 16);
-                g.x += v.x; g.y += v.y; g.z += v.z; g.w += v.w;
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < 12; ++u) { nu.x += vl[u].x; nu.y += vl[u].y; nu.z += vl[u].z; nu.w += vl[u].w; }
-        for (unsigned c = d0 + (unsigned)sub + 48u; c <= d1; c += 4) {
-            const double4 v = ldcg4(srl + (size_t)c * st.xstride * 256);
-            nu.x += v.x; nu.y += v.y; nu.z += v.z; nu.w += v.w;
-        }
-        *reinterpret_cast<double4*>(s_gn + (size_t)sub * Npad + i0) = g;
-        *reinterpret_cast<double4*>(s_gn + (size_t)(4 + sub) * Npad + i0) = nu;
     }
-    __syncthreads();
 }
 
 // ---------------------------------------------------------------- finishing phase: one CTA (256 threads) per member b
@@ -333,32 +363,110 @@ __device__ __forceinline__ void sum_dmma_partials(int N, const KxStage& st, cons
 //   a7  projection C.2-C.8 in the basis {1, K_i} (D3: same span as {1, E_i}, well conditioned), diag C.1, C.9
 //   a8  Runge-Kutta stage update                                                  eq. 4.9
 // from_dmma: the member's (gain, nu) come from the partials of the DMMA phase (plan != null), else from the partials
-// `st.part` of the exact streaming contraction.  scratch: finish_scratch_doubles(N) doubles of shared memory.
-__device__ __forceinline__ void finish_member(const KxDev& d, const double* __restrict__ fin, int B, const KxStage& st,
-                                              const KxPlan* plan, bool from_dmma, int b, double* scratch, double* s_red /* [64] */)
+// `st.part` of the exact streaming contraction.  scratch: finish_scratch_bytes() of shared memory (streaming path: the s_y part only).
+template <int NQ> struct FinishPre { double fi[NQ], h[NQ], E[NQ], K[NQ]; };      // NQ = ceil(N / 256) rows per thread
+
+// the member's stage input and the kinematics: nothing a kernel of this launch writes, so a finishing CTA may fetch them
+// before the grid barrier
+template <int NQ>
+__device__ __forceinline__ void finish_preload(const KxDev& d, const double* __restrict__ fin, int b, FinishPre<NQ>& pre)
 {
     const int N = d.N, tid = threadIdx.x;
     const double* fb = fin + (size_t)b * N;
-    double* s_y = scratch;                         // [N]
-    double* s_gn = scratch + N;                    // [2][4][Npad]
-    const int Npad = (N + 3) & ~3;
-    double C[kMaxPerThread], fi[kMaxPerThread], hi_[kMaxPerThread], Ei[kMaxPerThread], Ki[kMaxPerThread];
 #pragma unroll
-    for (int q = 0; q < kMaxPerThread; ++q) {
+    for (int q = 0; q < NQ; ++q) {
+        const int i = tid + q * KX_CTA;
+        pre.fi[q] = 0.0; pre.h[q] = 0.0; pre.E[q] = 0.0; pre.K[q] = 0.0;
+        if (i < N) { pre.fi[q] = fb[i]; pre.h[q] = d.h[i]; pre.E[q] = d.E[i]; pre.K[q] = d.K[i]; }
+    }
+}
+
+// (gain, nu) of row i from the gathered slots: four interleaved sums each (slot = first + k mod 4), added as
+// (s0 + s1) + (s2 + s3): short dependency chains, a fixed order
+__device__ __forceinline__ void sum_partials_row(int N, const KxStage& st, const KxPlan& plan, const double* scratch, int i,
+                                                 double& g, double& nu)
+{
+    const double* s_gp = scratch + ((N + 3) & ~3);
+    const double* s_lp = s_gp + (size_t)(plan.GG + st.NT) * 16;
+    const int tile = i >> 4, sp = i >> 8;
+    double a[4] = {0.0, 0.0, 0.0, 0.0}, l[4] = {0.0, 0.0, 0.0, 0.0};
+    const unsigned w0 = plan.wstart[tile], w1 = plan.wstart[tile + 1];
+    if (w1 > w0) {
+        const unsigned c0 = w0 / kDmmaWarps, ng = (w1 - 1u) / kDmmaWarps - c0 + 1u;
+        const double* pg = s_gp + (size_t)(c0 + tile) * 16 + (i & 15);
+        unsigned c = 0;
+        for (; c + 4 <= ng; c += 4) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) a[k] += pg[(size_t)(c + k) * 16];
+        }
+        for (int k = 0; c < ng; ++c, ++k) a[k] += pg[(size_t)c * 16];
+    }
+    unsigned lo = 0;
+    for (int s2 = 0; s2 < sp; ++s2) lo += plan.ld1[s2] - plan.ld0[s2] + 1u;
+    const unsigned nls = plan.ld1[sp] - plan.ld0[sp] + 1u;
+    const double* pl = s_lp + (size_t)lo * 256 + (i & 255);
+    unsigned c = 0;
+    for (; c + 4 <= nls; c += 4) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) l[k] += pl[(size_t)(c + k) * 256];
+    }
+    for (int k = 0; c < nls; ++c, ++k) l[k] += pl[(size_t)c * 256];
+    g = (a[0] + a[1]) + (a[2] + a[3]);
+    nu = (l[0] + l[1]) + (l[2] + l[3]);
+}
+
+// ---------------------------------------------------------------- finishing phase, the plain case of the tensor-core path
+// C_raw = gain - f_i nu_i only (a6): no projection, no diagnostics, no Runge-Kutta stage, no separate gain / loss outputs.
+// Kept apart from finish_member and as short as possible: this code runs once per launch, so what it costs is mostly the
+// instruction fetch (after an L2 flush the fetch comes from HBM).
+template <int NQ>
+__device__ __forceinline__ void finish_raw(int N, const KxStage& st, const KxPlan& plan, int b, const double* scratch,
+                                           const FinishPre<NQ>& pre, unsigned long long* mbar, unsigned parity)
+{
+    const int tid = threadIdx.x;
+    mbar_wait(mbar, parity);
+    if (tid == 0) stamp(st.trace, 7);
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        const int i = tid + q * KX_CTA;
+        if (i < N) {
+            double g, nu;
+            sum_partials_row(N, st, plan, scratch, i, g, nu);
+            st.C[(size_t)b * N + i] = fma(-pre.fi[q], nu, g);
+        }
+    }
+    __syncthreads();       // the scratch may be reused by the next member of this CTA
+}
+
+// from_dmma: the member's partials of the DMMA phase are on their way into the scratch (gather_partials(b) was issued by
+// the caller; `mbar` flips to `parity` when they have landed)
+template <int NQ>
+__device__ __forceinline__ void finish_member(const KxDev& d, const double* __restrict__ fin, int B, const KxStage& st,
+                                              const KxPlan* plan, bool from_dmma, int b, double* scratch, double* s_red /* [64] */,
+                                              const FinishPre<NQ>* pre = nullptr, unsigned long long* mbar = nullptr,
+                                              unsigned parity = 0)
+{
+    const int N = d.N, tid = threadIdx.x;
+    const double* fb = fin + (size_t)b * N;
+    const int Npad = (N + 3) & ~3;
+    double* s_y = scratch;                         // [Npad]
+    double C[NQ], fi[NQ], hi_[NQ], Ei[NQ], Ki[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
         const int i = tid + q * KX_CTA;
         C[q] = 0.0; fi[q] = 0.0; hi_[q] = 0.0; Ei[q] = 0.0; Ki[q] = 0.0;
-        if (i < N) { fi[q] = fb[i]; hi_[q] = d.h[i]; Ei[q] = d.E[i]; Ki[q] = d.K[i]; }
+        if (pre) { fi[q] = pre->fi[q]; hi_[q] = pre->h[q]; Ei[q] = pre->E[q]; Ki[q] = pre->K[q]; }
+        else if (i < N) { fi[q] = fb[i]; hi_[q] = d.h[i]; Ei[q] = d.E[i]; Ki[q] = d.K[i]; }
     }
-    if (from_dmma) sum_dmma_partials(N, st, *plan, b, s_gn);
+    if (from_dmma) mbar_wait(mbar, parity);
 
 #pragma unroll
-    for (int q = 0; q < kMaxPerThread; ++q) {
+    for (int q = 0; q < NQ; ++q) {
         const int i = tid + q * KX_CTA;
         if (i < N) {
             double g = 0.0, nu = 0.0, gq2 = 0.0, lq2 = 0.0;
             if (from_dmma) {
-                g = ((s_gn[i] + s_gn[Npad + i]) + s_gn[2 * Npad + i]) + s_gn[3 * Npad + i];
-                nu = ((s_gn[4 * Npad + i] + s_gn[5 * Npad + i]) + s_gn[6 * Npad + i]) + s_gn[7 * Npad + i];
+                sum_partials_row(N, st, *plan, scratch, i, g, nu);
             } else {
                 const unsigned t0 = d.taskptr[i], t1 = d.taskptr[i + 1];
                 const int nv = d.eta ? 4 : 2;
@@ -390,7 +498,7 @@ __device__ __forceinline__ void finish_member(const KxDev& d, const double* __re
         double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
         double fm = 0.0;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) {
+        for (int q = 0; q < NQ; ++q) {
             const double hc = hi_[q] * C[q];
             v[0] += hc;                       // R0 = sum h C
             v[1] += hc * Ki[q];               // RK = sum h K C
@@ -404,10 +512,10 @@ __device__ __forceinline__ void finish_member(const KxDev& d, const double* __re
         const double R0 = v[0], RK = v[1], R1 = v[2], S0 = v[3], S1 = v[4];
         double alpha = 0.0, beta = 0.0, D0 = 0.0, D1 = 0.0;
         if (project) {
-            double xi[kMaxPerThread];
+            double xi[NQ];
             double a[3] = {0.0, 0.0, 0.0};
 #pragma unroll
-            for (int q = 0; q < kMaxPerThread; ++q) {
+            for (int q = 0; q < NQ; ++q) {
                 const double r = fmax_ > 0.0 ? fabs(fi[q]) / fmax_ : 0.0;     // C.4
                 xi[q] = r > d.eps_supp ? r : 0.0;
                 const double hx = hi_[q] * xi[q];
@@ -424,7 +532,7 @@ __device__ __forceinline__ void finish_member(const KxDev& d, const double* __re
             }
             double dsum[2] = {0.0, 0.0};
 #pragma unroll
-            for (int q = 0; q < kMaxPerThread; ++q) {
+            for (int q = 0; q < NQ; ++q) {
                 const double corr = xi[q] * (alpha + beta * Ki[q]);
                 C[q] = C[q] - corr;                                          // C.3
                 dsum[0] += hi_[q] * fabs(corr);
@@ -443,7 +551,7 @@ __device__ __forceinline__ void finish_member(const KxDev& d, const double* __re
 
     if (st.C) {
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) {
+        for (int q = 0; q < NQ; ++q) {
             const int i = tid + q * KX_CTA;
             if (i < N) st.C[(size_t)b * N + i] = C[q];
         }
@@ -461,7 +569,7 @@ __device__ __forceinline__ void finish_member(const KxDev& d, const double* __re
     bool bad = false;
     double errmax = 0.0;
 #pragma unroll
-    for (int q = 0; q < kMaxPerThread; ++q) {
+    for (int q = 0; q < NQ; ++q) {
         const int i = tid + q * KX_CTA;
         if (i >= N) continue;
         const size_t o = (size_t)b * N + i;

@@ -97,6 +97,7 @@ struct KxPlan {
     int WC;                   // chunks of 16 k whose Chebyshev coefficients a loss CTA holds at a time
     unsigned wstart[KX_MAX_NT + 1];
     unsigned vt[KX_MAX_NT + 1];      // copy of vtptr: first group of every tile
+    unsigned ld0[4], ld1[4];         // first / last loss CTA (relative to GG) that worked on supertile sp (RS <= 4)
 };
 
 struct KxAdapt;
@@ -121,6 +122,7 @@ struct kx_handle_s {
     int plan_B;               // 0 = no plan
     unsigned *bar;            // device [4]: grid barrier of the fused kernels (arrival count, released epoch), fallback count
     unsigned epoch;           // launch serial number of the fused kernels (two barrier epochs per launch)
+    unsigned bar_total;       // CTAs that have arrived at bar[3] once every launch enqueued so far has run
     unsigned long long *trace;       // device [KX_TRACE_CTAS][KX_TRACE_SLOTS] clock stamps of the last fused launch, or null
     bool tracing;
     void *tiled_blob;         // one allocation holding the small tables of KxTiled
@@ -252,8 +254,9 @@ struct KxStage {             // what the finishing kernel does after the reducti
     int evolve;
     double *part;            // [tasks, B, 2 or 4] partials of the exact streaming contraction
     // grid barrier of the fused kernels (kx_device.cuh) and the optional clock-stamp trace
-    unsigned *bar;
+    unsigned *bar;           // [0] arrivals, [1] released epoch (second barrier of a launch); [2] fallback count; [3] growing counter
     unsigned epoch;
+    unsigned bar_target;     // value of bar[3] when every CTA of this launch has arrived at the first barrier
     unsigned long long *trace;
     unsigned *fb_count;      // device counter: members evaluated by the exact fallback (kx_fallback_count)
     // adaptive Heun (rk_method == KX_HEUN_ADAPT): dt and the rate come from the device controller state
@@ -262,8 +265,9 @@ struct KxStage {             // what the finishing kernel does after the reducti
 };
 #define KX_HEUN_ADAPT 3      // internal: Euler predictor / Heun corrector with the error norm of kx_evolve_adaptive
 // one operator evaluation on the exact streaming path: y = log2 f, contraction, grid barrier, finishing phase: ONE kernel
+// (bar_total: the handle's running count of barrier arrivals; the launcher adds its grid size and sets st.bar_target)
 cudaError_t kx_launch_stream(const KxDev& d, int sm_count, const double* f, const double* yd, int B,
-                             const KxStage& st, cudaStream_t s);
+                             KxStage st, unsigned* bar_total, cudaStream_t s);
 cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, int B, KxAdapt* ad, double u1, double safety,
                                  int* flag, cudaStream_t s);      // accept/reject + controller update
 cudaError_t kx_launch_delta_source(const KxDev& d, double p0, double* G, cudaStream_t s);
@@ -274,7 +278,7 @@ cudaError_t kx_launch_tile_runs(const KxDev& d, const KxTiled& t, cudaStream_t s
 cudaError_t kx_launch_tile_fill(const KxDev& d, const KxTiled& t, cudaStream_t s);     // A, desc (gain + loss)
 // one operator evaluation on the tensor-core path: DMMA phase, grid barrier, (exact fallback, barrier,) finishing phase
 cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B,
-                           const KxStage& st, cudaStream_t s);
+                           KxStage st, unsigned* bar_total, cudaStream_t s);
 cudaError_t kx_dmma_configure(); // shared-memory attributes of every instantiation (once per process)
 int kx_xstride(int B);
 void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned* vt_host, int B, KxPlan* plan);

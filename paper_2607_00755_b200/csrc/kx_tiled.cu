@@ -61,7 +61,8 @@ constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256
 template <int NBT, int STAGES>
 __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, int N, int B, int bcol0,
                                           const double* __restrict__ f, int xstride, double* __restrict__ gpart,
-                                          unsigned char* smem, int* s_wtile, unsigned long long* trace)
+                                          unsigned char* smem, int* s_wtile, unsigned long long* trace,
+                                          unsigned long long* mbar, unsigned& mpar)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int krow = lane & 3, lr = lane >> 2;
@@ -101,29 +102,36 @@ __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, 
     // s_f[b][n] = f[bcol0 + b][n], n < N; s_f[b][N] = 1 (the scale of padding quads), s_f[b][N+1..] = 0.  The rows of
     // f are copied as they are (16-byte cp.async when N is even); members beyond B are zero.  Every CTA starts its
     // walk somewhere else so that the CTAs do not all ask the same L2 lines at once.
+    // N even: one bulk copy (TMA) per row, completion on the CTA's mbarrier; else element by element.
     {
-        const int chunks = (N & 1) ? 0 : N >> 1;                   // 16-byte chunks per row
-        const int total = NBT * 8 * chunks;
-        const int rot = total ? (int)((blockIdx.x * 977u) % (unsigned)total) : 0;
-        for (int k0 = tid; k0 < total; k0 += NTHR) {
-            int k = k0 + rot;
-            if (k >= total) k -= total;
-            const int bb = k / chunks, cc = k - bb * chunks;
-            if (bcol0 + bb < B) cp_async16(s_f + (size_t)bb * LDN + 2 * cc, f + (size_t)(bcol0 + bb) * N + 2 * cc);
-            else *reinterpret_cast<double2*>(s_f + (size_t)bb * LDN + 2 * cc) = make_double2(0.0, 0.0);
-        }
-        if (!chunks)
-            for (int k = tid; k < NBT * 8 * N; k += NTHR) {
-                const int bb = k / N, nn = k - bb * N;
-                s_f[(size_t)bb * LDN + nn] = bcol0 + bb < B ? __ldcg(f + (size_t)(bcol0 + bb) * N + nn) : 0.0;
+        const bool bulk = (N & 1) == 0;
+        const int nrows = min(NBT * 8, B - bcol0);
+        if (bulk) {
+            if (tid == 0) mbar_expect_tx(mbar, (unsigned)nrows * (unsigned)N * 8u);
+            const int rot = (int)(blockIdx.x % (unsigned)nrows);     // every CTA starts its walk somewhere else
+            for (int k = tid; k < nrows; k += NTHR) {
+                int bb = k + rot;
+                if (bb >= nrows) bb -= nrows;
+                bulk_g2s(s_f + (size_t)bb * LDN, f + (size_t)(bcol0 + bb) * N, (unsigned)N * 8u, mbar);
             }
+        } else {
+            for (int k = tid; k < nrows * N; k += NTHR) {
+                const int bb = k / N, nn = k - bb * N;
+                s_f[(size_t)bb * LDN + nn] = __ldcg(f + (size_t)(bcol0 + bb) * N + nn);
+            }
+        }
+        for (int k = tid; k < (NBT * 8 - nrows) * N; k += NTHR) {          // members beyond B: zero
+            const int bb = nrows + k / N, nn = k % N;
+            s_f[(size_t)bb * LDN + nn] = 0.0;
+        }
         for (int k = tid; k < NBT * 8 * (LDN - N); k += NTHR) {
             const int bb = k / (LDN - N), cc = k - bb * (LDN - N);
             s_f[(size_t)bb * LDN + N + cc] = cc == 0 ? 1.0 : 0.0;
         }
+        cp_async_wait<0>();
+        if (bulk) mbar_wait(mbar, mpar);
+        mpar ^= bulk ? 1u : 0u;
     }
-    cp_async_commit();
-    cp_async_wait<0>();
     __syncthreads();
     if (tid == 0) stamp(trace, 1);
 
@@ -490,6 +498,74 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
     }
 }
 
+// ---------------------------------------------------------------- what follows the DMMA phase (NQ = rows per thread)
+template <int NQ>
+__device__ __forceinline__ void dmma_tail(const KxDev& dk, const KxPlan& plan, int B, const double* __restrict__ f,
+                                          const KxStage& st, unsigned char* smem, double* s_red, int& s_myflag,
+                                          unsigned long long* mbar, unsigned parity)
+{
+    const int tid = threadIdx.x, N = dk.N;
+    const bool mine = (int)blockIdx.x < B;          // this CTA finishes member blockIdx.x (and blockIdx.x + gridDim.x, ...)
+    FinishPre<NQ> pre;
+    if (mine) finish_preload(dk, f, blockIdx.x, pre);              // static inputs of the finishing phase: before the barrier
+    if (tid == 0) s_myflag = 0;
+    grid_barrier_count(st.bar + 3, st.bar_target);
+    if (tid == 0) stamp(st.trace, 3);
+
+    // The statistics of all members (one 16-byte load per thread) and the partials of this CTA's own member are requested
+    // together: one L2 round trip.  Members whose interpolation error bound is not negligible (rare) take the exact
+    // streaming contraction: their groups of KX_FB_BT members, the tasks dealt to all CTAs; every CTA takes the same
+    // decisions from the same statistics.
+    bool any = false;
+    {
+        // (the gather first: its proxy fence would otherwise wait for the statistics load)
+        if (mine) gather_partials(N, st, plan, blockIdx.x, reinterpret_cast<double*>(smem), mbar);
+        const bool fl0 = st.mstat && tid < B && member_flagged(st.mstat, tid);
+        if (fl0 && tid == (int)blockIdx.x) s_myflag = 1;
+        any = __syncthreads_or(fl0) != 0;
+        if (st.mstat) {
+#pragma unroll 1
+            for (int b0 = NTHR; b0 < B; b0 += NTHR) {
+                const bool fl = b0 + tid < B && member_flagged(st.mstat, b0 + tid);
+                if (fl && b0 + tid == (int)blockIdx.x) s_myflag = 1;
+                any |= __syncthreads_or(fl) != 0;
+            }
+        }
+    }
+    bool gathered = mine;
+    if (any) {
+        if (gathered) { mbar_wait(mbar, parity); parity ^= 1u; gathered = false; }      // the contraction reuses the scratch
+        __syncthreads();
+        for (int g0 = 0; g0 < B; g0 += KX_FB_BT) {
+            const int hit = __syncthreads_or(tid < KX_FB_BT && g0 + tid < B && member_flagged(st.mstat, g0 + tid));
+            if (!hit) continue;
+            if (dk.exp_impl == KX_EXP_LIBM) contract_group<KX_FB_BT, MODE_LOG_LIBM, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
+            else contract_group<KX_FB_BT, MODE_LOG_TAB, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
+        }
+        grid_barrier(st.bar, st.epoch);
+    }
+    if (tid == 0) stamp(st.trace, 4);
+
+    if (st.mstat_next && blockIdx.x == gridDim.x - 1)          // clean statistics for the next launch (the other buffer)
+        for (int k = tid; k < st.mstat_cap; k += NTHR) { st.mstat_next[2 * k] = KX_MSTAT_NONE; st.mstat_next[2 * k + 1] = 0; }
+    const bool plain = st.C && !st.gain && !st.loss && !st.diag && !st.evolve && !(st.flags & KX_PROJECT);
+    for (int b = blockIdx.x; b < B; b += gridDim.x) {
+        const bool first = b == (int)blockIdx.x;
+        const bool flagged = st.mstat && (first ? s_myflag != 0 : member_flagged(st.mstat, b));
+        if (flagged && tid == 0 && st.fb_count) atomicAdd(st.fb_count, 1u);
+        // (a flagged member implies `any`, so a gather still in flight belongs to an unflagged first member)
+        if (!flagged && !(first && gathered)) gather_partials(N, st, plan, b, reinterpret_cast<double*>(smem), mbar);
+        if (plain && !flagged) {
+            if (!first) finish_preload(dk, f, b, pre);
+            finish_raw<NQ>(N, st, plan, b, reinterpret_cast<const double*>(smem), pre, mbar, parity);
+        } else {
+            finish_member<NQ>(dk, f, B, st, &plan, !flagged, b, reinterpret_cast<double*>(smem), s_red, first ? &pre : nullptr,
+                          mbar, parity);
+        }
+        if (!flagged) parity ^= 1u;
+    }
+}
+
 // ---------------------------------------------------------------- the fused kernel: one CTA per SM, cooperative
 // Clock stamps (st.trace, per CTA): 0 entry, 1 prologue done (f staged / first coefficient window built), 2 partials
 // written, 3 first barrier passed, 4 fallback done, 5 finishing phase done; 8..15 end of each gain warp's stream.
@@ -500,45 +576,25 @@ k_dmma(KxDev dk, KxTiled t, KxPlan plan, int B, const double* __restrict__ f, Kx
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ double s_red[8 * 8];
     __shared__ int s_wtile[WARPS];
+    __shared__ int s_myflag;
+    __shared__ __align__(8) unsigned long long s_mbar;      // completion of the bulk copies of the finishing phase
     const int tid = threadIdx.x, N = dk.N;
-    if (tid == 0) stamp(st.trace, 0);
+    if (tid == 0) { stamp(st.trace, 0); mbar_init(&s_mbar, 1u); if (st.trace && blockIdx.x < KX_TRACE_CTAS) st.trace[blockIdx.x * KX_TRACE_SLOTS + 22] = clock64(); }
 
     const int ny = (B + NBT * 8 - 1) / (NBT * 8);
+    unsigned mpar = 0;                              // phase of s_mbar
+    __syncthreads();                                // the barrier is initialised
     for (int by = 0; by < ny; ++by) {          // member groups of 8 NBT: one pass each (more than one for B > 64 only)
         const int bcol0 = by * NBT * 8;
-        if ((int)blockIdx.x < plan.GG) gain_role<NBT, STAGES>(t, plan, N, B, bcol0, f, st.xstride, st.gpart, smem, s_wtile, st.trace);
+        if ((int)blockIdx.x < plan.GG) gain_role<NBT, STAGES>(t, plan, N, B, bcol0, f, st.xstride, st.gpart, smem, s_wtile, st.trace, &s_mbar, mpar);
         else loss_role<NBT>(dk, t, plan, N, B, bcol0, f, st.mstat, st.xstride, st.lpart, smem, st.trace);
         __syncthreads();
     }
     if (tid == 0) stamp(st.trace, 2);
-    grid_barrier(st.bar, st.epoch);
-    if (tid == 0) stamp(st.trace, 3);
-
-    // members whose interpolation error bound is not negligible (rare): exact streaming contraction of their groups of
-    // KX_FB_BT members, the tasks dealt to all CTAs; every CTA takes the same decisions from the same statistics
-    bool any = false;
-    if (st.mstat) {
-        for (int b0 = 0; b0 < B; b0 += NTHR) any |= __syncthreads_or(b0 + tid < B && member_flagged(st.mstat, b0 + tid)) != 0;
-    }
-    if (any) {
-        for (int g0 = 0; g0 < B; g0 += KX_FB_BT) {
-            const int hit = __syncthreads_or(tid < KX_FB_BT && g0 + tid < B && member_flagged(st.mstat, g0 + tid));
-            if (!hit) continue;
-            if (dk.exp_impl == KX_EXP_LIBM) contract_group<KX_FB_BT, MODE_LOG_LIBM, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
-            else contract_group<KX_FB_BT, MODE_LOG_TAB, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
-        }
-        grid_barrier(st.bar, st.epoch + 1u);
-    }
-    if (tid == 0) stamp(st.trace, 4);
-
-    if (st.mstat_next && blockIdx.x == gridDim.x - 1)          // clean statistics for the next launch (the other buffer)
-        for (int k = tid; k < st.mstat_cap; k += NTHR) { st.mstat_next[2 * k] = KX_MSTAT_NONE; st.mstat_next[2 * k + 1] = 0; }
-    for (int b = blockIdx.x; b < B; b += gridDim.x) {
-        const bool flagged = st.mstat && member_flagged(st.mstat, b);
-        if (flagged && tid == 0 && st.fb_count) atomicAdd(st.fb_count, 1u);
-        finish_member(dk, f, B, st, &plan, !flagged, b, reinterpret_cast<double*>(smem), s_red);
-    }
-    if (tid == 0) stamp(st.trace, 5);
+    if (N <= KX_CTA) dmma_tail<1>(dk, plan, B, f, st, smem, s_red, s_myflag, &s_mbar, mpar);
+    else if (N <= 2 * KX_CTA) dmma_tail<2>(dk, plan, B, f, st, smem, s_red, s_myflag, &s_mbar, mpar);
+    else dmma_tail<4>(dk, plan, B, f, st, smem, s_red, s_myflag, &s_mbar, mpar);
+    if (tid == 0) { stamp(st.trace, 5); if (st.trace && blockIdx.x < KX_TRACE_CTAS) st.trace[blockIdx.x * KX_TRACE_SLOTS + 23] = clock64(); }
 }
 
 constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + ((KX_QMAX / 8) * (KX_QMAX / 4) * 32 + KX_QMAX + (1 << KX_EXP_BITS)) * 8;
@@ -556,12 +612,13 @@ int loss_window(const KxTiled& t, int GL, int nbt)
 
 int dmma_stages(int nbt) { return nbt <= 2 ? 8 : 4; }
 
-size_t dmma_smem(int nbt, int N, int WC)
+size_t dmma_smem(int nbt, int N, const KxTiled& t, const KxPlan& plan)
 {
+    const int WC = plan.WC;
     const size_t gain = (size_t)(nbt * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * dmma_stages(nbt) * kStageBytes;
     const size_t loss = kLossFixedBytes + (size_t)WC * 16 * (nbt * 8 + 4) * 8;
     const size_t fb = contract_smem<KX_FB_BT, MODE_LOG_TAB, 0>(N);
-    const size_t fin = finish_scratch_doubles(N) * 8;
+    const size_t fin = finish_scratch_bytes(N, plan.GG, plan.GL, t.NT, t.RS);
     size_t m = gain > loss ? gain : loss;
     if (fb > m) m = fb;
     if (fin > m) m = fin;
@@ -578,11 +635,14 @@ int dmma_nbt(int N, int B)
 }
 
 template <int NBT, int STAGES>
-cudaError_t launch_dmma_t(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B, const KxStage& st,
-                          cudaStream_t s)
+cudaError_t launch_dmma_t(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B, KxStage& st,
+                          unsigned* bar_total, cudaStream_t s)
 {
-    const size_t smem = dmma_smem(NBT, d.N, plan.WC);
-    return kx_launch_coop(k_dmma<NBT, STAGES>, dim3(plan.GG + plan.GL), dim3(NTHR), smem, s, d, t, plan, B, f, st);
+    const size_t smem = dmma_smem(NBT, d.N, t, plan);
+    st.bar_target = *bar_total + (unsigned)(plan.GG + plan.GL);
+    const cudaError_t e = kx_launch_coop(k_dmma<NBT, STAGES>, dim3(plan.GG + plan.GL), dim3(NTHR), smem, s, d, t, plan, B, f, st);
+    if (e == cudaSuccess) *bar_total = st.bar_target;
+    return e;
 }
 
 }  // namespace
@@ -660,16 +720,21 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
     unsigned run = 0;
     for (int k = 0; k < NT; ++k) { plan->wstart[k] = run; plan->vt[k] = vt_host[k]; run += w[k]; }
     plan->wstart[NT] = run; plan->vt[NT] = vt_host[NT];
+    for (int sp = 0; sp < 4; ++sp) {
+        const unsigned long long l0 = (unsigned long long)sp * t.LC, l1 = l0 + t.LC;
+        plan->ld0[sp] = sp < t.RS ? (unsigned)(((l0 + 1ull) * (unsigned)gl - 1ull) / (unsigned long long)U) : 1u;
+        plan->ld1[sp] = sp < t.RS ? (unsigned)((l1 * (unsigned)gl - 1ull) / (unsigned long long)U) : 0u;
+    }
     for (int k = NT + 1; k <= KX_MAX_NT; ++k) { plan->wstart[k] = run; plan->vt[k] = vt_host[NT]; }
 }
 
 cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B,
-                           const KxStage& st, cudaStream_t s)
+                           KxStage st, unsigned* bar_total, cudaStream_t s)
 {
     switch (plan.nbt) {
-        case 1: return launch_dmma_t<1, 8>(d, t, plan, f, B, st, s);
-        case 2: return launch_dmma_t<2, 8>(d, t, plan, f, B, st, s);
-        case 4: return launch_dmma_t<4, 4>(d, t, plan, f, B, st, s);
-        default: return launch_dmma_t<8, 4>(d, t, plan, f, B, st, s);
+        case 1: return launch_dmma_t<1, 8>(d, t, plan, f, B, st, bar_total, s);
+        case 2: return launch_dmma_t<2, 8>(d, t, plan, f, B, st, bar_total, s);
+        case 4: return launch_dmma_t<4, 4>(d, t, plan, f, B, st, bar_total, s);
+        default: return launch_dmma_t<8, 4>(d, t, plan, f, B, st, bar_total, s);
     }
 }
