@@ -25,7 +25,9 @@ using namespace kxd;
 
 // cost of one loss DMMA relative to one gain DMMA in the CTA split (the loss CTAs also compute their Chebyshev
 // coefficients first; calibrated with the clock-stamp trace on cfg3 so that both roles reach the barrier together)
-constexpr double kLossCost = 1.22;
+constexpr double kLossCost = 1.26;
+// cost of one run (tile, n) of the gain stream in units of one group (see kx_dmma_plan)
+constexpr double kRunCost = 0.09;
 
 // D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
@@ -143,6 +145,8 @@ __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, 
     for (int bt = 0; bt < NBT; ++bt)
 #pragma unroll
         for (int rb = 0; rb < 2; ++rb) acc[bt][rb][0] = acc[bt][rb][1] = 0.0;
+    const long long ck0_ = clock64();
+    unsigned nfold_ = 0;
 
     if (n > 0) {
         const double* xb = s_f + (size_t)lr * LDN + krow;    // + 8 bt LDN + column: the lane's member row of tile bt
@@ -202,8 +206,8 @@ __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, 
                     dmma884(T[bt][1][0], T[bt][1][1], xv[bt], w1);
                 }
                 const unsigned srow = dsc >> 20;
-                if (more && srow != srow_cur) {              // the run (n) ends with this quad
-                    fold();
+                if (__builtin_expect(more && srow != srow_cur, 0)) {              // the run (n) ends with this quad
+                    fold(); ++nfold_;
                     srow_cur = srow;
                     const double* sr = xb + srow - krow;
 #pragma unroll
@@ -230,7 +234,7 @@ __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, 
         s_wtile[warp] = n > 0 ? tile : -1;
         if (trace) {
             const unsigned cta = blockIdx.x;
-            if (cta < KX_TRACE_CTAS) trace[cta * KX_TRACE_SLOTS + 8 + warp] = gtime();
+            if (cta < KX_TRACE_CTAS) { trace[cta * KX_TRACE_SLOTS + 8 + warp] = gtime(); trace[cta * KX_TRACE_SLOTS + 24 + warp] = ((unsigned long long)(clock64() - ck0_) << 24) | ((unsigned long long)nfold_ << 12) | n; }
         }
     }
     __syncthreads();
@@ -266,37 +270,30 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
 {
     constexpr int LD = NBT * 8 + 4;
     constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
-    static_assert(WARPS == 8, "loss role: 8 warps (the coefficient pass maps warp <-> member tile)");
+    static_assert(WARPS == 8, "loss role: 8 warps");
     constexpr int MB = NBT * 8;               // members of this CTA
-    // brackets per coefficient pass: 256 threads = JB brackets x MB members, as many as the scratch holds at Q = 32
-    constexpr int JB = NBT == 1 ? 16 : 256 / MB;
-    constexpr int GS = MB + 4;                // row stride of the node values: 4 mod 8, conflict-free fragment reads
+    constexpr int PARTS = NTHR / MB;          // threads per member in the coefficient pass: each takes every PARTS-th node
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int krow = lane & 3, lr = lane >> 2;
     const int N_ = N, Q = t.Q, WC = plan.WC, GG = plan.GG, GL = plan.GL;
     const bool logm = dk.interp == KX_INTERP_LOG, tab = dk.exp_impl == KX_EXP_TABLE;
-    // shared memory: [A stages | scratch of the coefficient passes] [X window] [dct fragments, nodes, exp2 table]
+    // shared memory: [A stages | scratch of the coefficient pass] [X window] [nodes, exp2 table]
     unsigned char* sStage = smem;
     double* sXw = reinterpret_cast<double*>(smem + (size_t)kLossStages * kLossABytes);          // [WC*16][LD]
-    double* s_afr = sXw + (size_t)WC * 16 * LD;                                                 // [(Q/8)(Q/4)][32]
-    double* s_node = s_afr + (KX_QMAX / 8) * (KX_QMAX / 4) * 32;                                // [QMAX]
+    double* s_node = sXw + (size_t)WC * 16 * LD;                                                // [QMAX]
     double* s_tab = s_node + KX_QMAX;                                                           // [256]
-    double* s_G = reinterpret_cast<double*>(smem);                                              // [JB][Q][GS] (aliases the stages)
-    static_assert((size_t)JB * KX_QMAX * GS * 8 <= (size_t)kLossStages * kLossABytes, "coefficient scratch must fit the stages");
+    double* s_y = reinterpret_cast<double*>(smem);                                              // [brackets + 1][MB] (aliases the stages)
     if (logm) {
-        for (int k = tid; k < (Q / 8) * (Q / 4) * 32; k += NTHR) {
-            const int ln = k & 31, fr = k >> 5, ct = fr / (Q / 4), ks = fr - ct * (Q / 4);
-            s_afr[k] = t.dct[(8 * ct + (ln >> 2)) * Q + 4 * ks + (ln & 3)];
-        }
         if (tid < Q) s_node[tid] = t.nodes[tid];
-        if (tab) for (int k = tid; k < (1 << KX_EXP_BITS); k += NTHR) s_tab[k] = dk.exptab[k];
+        for (int k = tid; k < (1 << KX_EXP_BITS); k += NTHR) s_tab[k] = dk.exptab[k];
     }
-    __syncthreads();
+    int npass_ = 0;
 
-    // Chebyshev coefficients a_c(b, j) of the window's k = (j, c) rows, k in [K0, K0 + 16 wn), straight into shared
-    // memory.  LOG: g(omega_q) = 2^(y_j + omega_q (y_(j+1) - y_j)) at the Q
-    // Chebyshev nodes, then the discrete Chebyshev transform as a (Q x Q) x (Q x 8 NBT) product on the tensor pipe;
-    // LINEAR: a_0 = (f_j + f_(j+1))/2, a_1 = (f_(j+1) - f_j)/2.  Also the member statistics (flags) of kx_internal.cuh.
+    // The operand X of the window's rows k = (j, q), k in [K0, K0 + 16 wn), straight into shared memory.
+    // LOG: X = g(omega_q) = 2^(y_j + omega_q (y_(j+1) - y_j)), the interpolated occupation at the Q Chebyshev nodes (the
+    // tensor holds the bucket moments in the Lagrange basis of these nodes, kx_tiled_build.cu), y = log2 max(f, f_floor);
+    // LINEAR: the two exact coefficients a_0 = (f_j + f_(j+1))/2, a_1 = (f_(j+1) - f_j)/2.  Also the member statistics
+    // (flags) of kx_internal.cuh.
     auto build_window = [&](unsigned K0, unsigned wn) {
         const unsigned K1 = K0 + 16u * wn;
         const int jlo = (int)(K0 / (unsigned)Q);
@@ -307,7 +304,6 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
             for (unsigned k = max(K0, kpad) + (unsigned)warp; k < K1; k += WARPS)
                 for (int c2 = lane; c2 < LD; c2 += 32) sXw[(size_t)(k - K0) * LD + c2] = 0.0;
         }
-        const int jj = tid / MB, bl = tid % MB;
         if (!logm) {          // LINEAR: two exact coefficients per bracket, no transform: one flat loop
             const int total = (jhi - jlo + 1) * MB;
             for (int i0 = tid; i0 < total; i0 += 8 * NTHR) {          // 16 independent loads in flight per thread
@@ -332,90 +328,68 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
             __syncthreads();
             return;
         }
-        // the f values of a pass are requested one pass ahead
-        auto fetch = [&](int j0, double& a0, double& a1) {
-            const int j = j0 + jj, b = bcol0 + bl;
-            a0 = 0.0; a1 = 0.0;
-            if (jj < JB && j <= jhi && b < B) { a0 = __ldcg(f + (size_t)b * N_ + j); a1 = __ldcg(f + (size_t)b * N_ + j + 1); }
-        };
-        double fnx0, fnx1;
-        fetch(jlo, fnx0, fnx1);
-        for (int j0 = jlo; j0 <= jhi; j0 += JB) {
-            const int j = j0 + jj;
-            const bool valid = jj < JB && j <= jhi;
-            const int b = bcol0 + bl;
-            const double fj = fnx0, fj1 = fnx1;
-            if (j0 + JB <= jhi) fetch(j0 + JB, fnx0, fnx1);
-            if (valid && b < B) atomicMax(mstat + 2 * b + 1, __double_as_longlong(fmax(fabs(fj), fabs(fj1))));
-            if (valid) {
-                const double y0 = log2(fmax(fj, dk.f_floor)), y1 = log2(fmax(fj1, dk.f_floor)), dy = y1 - y0;
-                const double cabs = 0.6931471805599453 * fabs(dy);
-                // log2 of the bracket's error bound (log2 max_i f_i is subtracted by the consumers); the atomics return
-                // nothing, so nobody waits for them
-                if (b < B && cabs > 0.0)
-                    atomicMax(mstat + 2 * b, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
-                double* g = s_G + (size_t)jj * Q * GS + bl;
-                // Q is a multiple of 8: eight independent exp2 chains at a time
-                if (tab) {
-                    for (int q0 = 0; q0 < Q; q0 += 8) {
-                        double e[8];
-#pragma unroll
-                        for (int u2 = 0; u2 < 8; ++u2) e[u2] = kx_exp2_tab<1>(fma(s_node[q0 + u2], dy, y0), s_tab);
-#pragma unroll
-                        for (int u2 = 0; u2 < 8; ++u2) g[(q0 + u2) * GS] = e[u2];
-                    }
-                } else {
-                    for (int q = 0; q < Q; ++q) g[q * GS] = exp2(fma(s_node[q], dy, y0));
-                }
-            }
-            __syncthreads();
-            // transform: a task is (bracket of the pass, member tile); the 8 warps take 32 tasks at a time, 4 each, with
-            // 4 x (Q/8) independent accumulator chains so that the DMMA latency of one hides behind the others
-            for (int base = 0; base < JB * NBT; base += 32) {
-                double D[4][KX_QMAX / 8][2];
-                int tj[4], tm[4];
+        // step 1: y_j = log2 max(f_j, f_floor) of the brackets' end points j = jlo .. jhi + 1, and max |f|
+        const int nj = jhi - jlo + 1;
+        {
+            const int total = (nj + 1) * MB;
+            for (int i0 = tid; i0 < total; i0 += 4 * NTHR) {
+                double v[4];
 #pragma unroll
                 for (int u2 = 0; u2 < 4; ++u2) {
-                    const int idx = base + warp + 8 * u2;
-                    tj[u2] = (idx < JB * NBT && j0 + idx / NBT <= jhi) ? idx / NBT : -1;
-                    tm[u2] = idx % NBT;
-#pragma unroll
-                    for (int ct = 0; ct < KX_QMAX / 8; ++ct) D[u2][ct][0] = D[u2][ct][1] = 0.0;
-                }
-#pragma unroll
-                for (int ks = 0; ks < KX_QMAX / 4; ++ks) {
-                    if (4 * ks < Q) {
-                        double afr[KX_QMAX / 8];
-#pragma unroll
-                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) afr[ct] = 8 * ct < Q ? s_afr[(ct * (Q / 4) + ks) * 32 + lane] : 0.0;
-#pragma unroll
-                        for (int u2 = 0; u2 < 4; ++u2) {
-                            if (tj[u2] >= 0) {          // uniform over the warp
-                                const double gv = s_G[((size_t)tj[u2] * Q + 4 * ks + krow) * GS + 8 * tm[u2] + lr];
-#pragma unroll
-                                for (int ct = 0; ct < KX_QMAX / 8; ++ct)
-                                    if (8 * ct < Q) dmma884(D[u2][ct][0], D[u2][ct][1], afr[ct], gv);
-                            }
-                        }
-                    }
+                    const int idx = i0 + u2 * NTHR, b = bcol0 + idx % MB;
+                    v[u2] = (idx < total && b < B) ? __ldcg(f + (size_t)b * N_ + jlo + idx / MB) : 0.0;
                 }
 #pragma unroll
                 for (int u2 = 0; u2 < 4; ++u2) {
-                    if (tj[u2] >= 0) {
-#pragma unroll
-                        for (int ct = 0; ct < KX_QMAX / 8; ++ct) {
-                            if (8 * ct < Q) {
-                                const unsigned k = (unsigned)(j0 + tj[u2]) * (unsigned)Q + 8u * ct + (unsigned)lr;
-                                if (k >= K0 && k < K1)
-                                    *reinterpret_cast<double2*>(sXw + (size_t)(k - K0) * LD + 8 * tm[u2] + 2 * krow) = make_double2(D[u2][ct][0], D[u2][ct][1]);
-                            }
-                        }
+                    const int idx = i0 + u2 * NTHR, b = bcol0 + idx % MB;
+                    if (idx < total) {
+                        if (b < B) atomicMax(mstat + 2 * b + 1, __double_as_longlong(fabs(v[u2])));
+                        s_y[idx] = log2(fmax(v[u2], dk.f_floor));
                     }
                 }
             }
-            __syncthreads();
         }
         __syncthreads();
+        if (tid == 0 && npass_ < 2) stamp(trace, 17 + 2 * npass_);
+        // step 2: thread (member bl, part) takes the nodes q = part, part + PARTS, ... of every bracket
+        {
+            const int bl = tid % MB, part = tid / MB;
+            const int b = bcol0 + bl;
+            constexpr int QP = (KX_QMAX + PARTS - 1) / PARTS;       // nodes per thread and bracket, at most
+            for (int jj = 0; jj < nj; ++jj) {
+                const double y0 = s_y[jj * MB + bl], y1 = s_y[(jj + 1) * MB + bl], dy = y1 - y0;
+                if (part == (jj & (PARTS - 1)) && b < B) {
+                    // log2 of the bracket's error bound (log2 max_i f_i is subtracted by the consumers); the atomics return
+                    // nothing, so nobody waits for them
+                    const double cabs = 0.6931471805599453 * fabs(dy);
+                    if (cabs > 0.0)
+                        atomicMax(mstat + 2 * b, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
+                }
+                if (tid == 0 && npass_ == 0 && (jj == 1 || jj == 2 || jj == 5)) stamp(trace, jj == 1 ? 19 : (jj == 2 ? 20 : 21));
+                const unsigned kb = (unsigned)(jlo + jj) * (unsigned)Q;
+                double e[QP];
+#pragma unroll
+                for (int u2 = 0; u2 < QP; ++u2) {
+                    // branch-free (nodes beyond Q are clamped and their value dropped below): the QP chains interleave
+                    const int q = min(part + u2 * PARTS, Q - 1);
+                    const double arg = fma(s_node[q], dy, y0);
+                    e[u2] = kx_exp2_tab<1>(arg, s_tab);
+                }
+                if (!tab) {
+#pragma unroll 1
+                    for (int u2 = 0; u2 < QP; ++u2) e[u2] = exp2(fma(s_node[min(part + u2 * PARTS, Q - 1)], dy, y0));
+                }
+#pragma unroll
+                for (int u2 = 0; u2 < QP; ++u2) {
+                    const int q = part + u2 * PARTS;
+                    const unsigned k = kb + (unsigned)q;
+                    if (q < Q && k >= K0 && k < K1) sXw[(size_t)(k - K0) * LD + bl] = e[u2];
+                }
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && npass_ < 2) stamp(trace, 18 + 2 * npass_);
+        ++npass_;
     };
 
     const unsigned cl = blockIdx.x - GG;
@@ -499,6 +473,24 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
 }
 
 // ---------------------------------------------------------------- what follows the DMMA phase (NQ = rows per thread)
+// The code after the grid barrier runs once per launch, so what it costs is mostly instruction fetch (about 0.3 us per
+// jump into code that is not in the instruction cache, measured as stall_no_instruction with ncu).  The plain case
+// (finish_raw) is kept short and inline; everything else is called out of line so that the kernel body stays compact.
+template <int NQ>
+__device__ __noinline__ void finish_member_cold(const KxDev& d, const double* __restrict__ fin, int B, const KxStage& st,
+                                                const KxPlan* plan, bool from_dmma, int b, double* scratch, double* s_red,
+                                                const FinishPre<NQ>* pre, unsigned long long* mbar, unsigned parity)
+{
+    finish_member<NQ>(d, fin, B, st, plan, from_dmma, b, scratch, s_red, pre, mbar, parity);
+}
+
+__device__ __noinline__ void fallback_cold(const KxDev& dk, const double* __restrict__ f, double* __restrict__ part, int B, int g0,
+                                           unsigned char* smem)
+{
+    if (dk.exp_impl == KX_EXP_LIBM) contract_group<KX_FB_BT, MODE_LOG_LIBM, 0>(dk, f, nullptr, part, B, g0, blockIdx.x, gridDim.x, smem);
+    else contract_group<KX_FB_BT, MODE_LOG_TAB, 0>(dk, f, nullptr, part, B, g0, blockIdx.x, gridDim.x, smem);
+}
+
 template <int NQ>
 __device__ __forceinline__ void dmma_tail(const KxDev& dk, const KxPlan& plan, int B, const double* __restrict__ f,
                                           const KxStage& st, unsigned char* smem, double* s_red, int& s_myflag,
@@ -539,8 +531,7 @@ __device__ __forceinline__ void dmma_tail(const KxDev& dk, const KxPlan& plan, i
         for (int g0 = 0; g0 < B; g0 += KX_FB_BT) {
             const int hit = __syncthreads_or(tid < KX_FB_BT && g0 + tid < B && member_flagged(st.mstat, g0 + tid));
             if (!hit) continue;
-            if (dk.exp_impl == KX_EXP_LIBM) contract_group<KX_FB_BT, MODE_LOG_LIBM, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
-            else contract_group<KX_FB_BT, MODE_LOG_TAB, 0>(dk, f, nullptr, st.part, B, g0, blockIdx.x, gridDim.x, smem);
+            fallback_cold(dk, f, st.part, B, g0, smem);
         }
         grid_barrier(st.bar, st.epoch);
     }
@@ -559,8 +550,8 @@ __device__ __forceinline__ void dmma_tail(const KxDev& dk, const KxPlan& plan, i
             if (!first) finish_preload(dk, f, b, pre);
             finish_raw<NQ>(N, st, plan, b, reinterpret_cast<const double*>(smem), pre, mbar, parity);
         } else {
-            finish_member<NQ>(dk, f, B, st, &plan, !flagged, b, reinterpret_cast<double*>(smem), s_red, first ? &pre : nullptr,
-                          mbar, parity);
+            finish_member_cold<NQ>(dk, f, B, st, &plan, !flagged, b, reinterpret_cast<double*>(smem), s_red, first ? &pre : nullptr,
+                                   mbar, parity);
         }
         if (!flagged) parity ^= 1u;
     }
@@ -571,7 +562,8 @@ __device__ __forceinline__ void dmma_tail(const KxDev& dk, const KxPlan& plan, i
 // written, 3 first barrier passed, 4 fallback done, 5 finishing phase done; 8..15 end of each gain warp's stream.
 template <int NBT, int STAGES>
 __global__ void __launch_bounds__(NTHR, 1)
-k_dmma(KxDev dk, KxTiled t, KxPlan plan, int B, const double* __restrict__ f, KxStage st)
+k_dmma(const __grid_constant__ KxDev dk, const __grid_constant__ KxTiled t, const __grid_constant__ KxPlan plan, int B,
+       const double* __restrict__ f, const __grid_constant__ KxStage st)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ double s_red[8 * 8];
@@ -597,7 +589,7 @@ k_dmma(KxDev dk, KxTiled t, KxPlan plan, int B, const double* __restrict__ f, Kx
     if (tid == 0) { stamp(st.trace, 5); if (st.trace && blockIdx.x < KX_TRACE_CTAS) st.trace[blockIdx.x * KX_TRACE_SLOTS + 23] = clock64(); }
 }
 
-constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + ((KX_QMAX / 8) * (KX_QMAX / 4) * 32 + KX_QMAX + (1 << KX_EXP_BITS)) * 8;
+constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + (KX_QMAX + (1 << KX_EXP_BITS)) * 8;
 constexpr size_t kSmemMax = 226u * 1024u;       // dynamic shared memory: 227 KiB per CTA minus the kernel's static 544 bytes
 
 // chunks of 16 k whose Chebyshev coefficients a loss CTA keeps in shared memory at a time: its whole share if it fits
@@ -692,12 +684,21 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
 
     const int NT = t.NT;
     const unsigned NW = (unsigned)plan->GG * WARPS;
+    // cost of a tile in units of one group: its groups plus kRunCost per run (one run per n: the fold at the end of a run and
+    // the short runs of the high tiles cost DMMA issue slots; measured with the clock-stamp trace: 0.83 of the DMMA peak on
+    // tile 0, 0.76 on the last tile of cfg3)
     std::vector<unsigned> w(NT, 0u), g(NT, 0u);
-    unsigned used = 0;
+    std::vector<double> c(NT, 0.0);
+    double Ctot = 0.0;
     for (int k = 0; k < NT; ++k) {
         g[k] = vt_host[k + 1] - vt_host[k];
+        c[k] = g[k] ? (double)g[k] + kRunCost * (double)d.N : 0.0;
+        Ctot += c[k];
+    }
+    unsigned used = 0;
+    for (int k = 0; k < NT; ++k) {
         if (g[k]) {
-            unsigned v = (unsigned)((unsigned long long)NW * g[k] / Gtot);
+            unsigned v = (unsigned)((double)NW * c[k] / Ctot);
             if (v < 1) v = 1;
             if (v > g[k]) v = g[k];
             w[k] = v; used += v;
@@ -706,14 +707,14 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
     while (used > NW) {            // the minimum of one warp per tile overshot: take from the lightest-loaded warps
         int best = -1;
         for (int k = 0; k < NT; ++k)
-            if (w[k] > 1 && (best < 0 || (unsigned long long)g[k] * w[best] < (unsigned long long)g[best] * w[k])) best = k;
+            if (w[k] > 1 && (best < 0 || c[k] * w[best] < c[best] * w[k])) best = k;
         if (best < 0) break;
         --w[best]; --used;
     }
-    while (used < NW) {            // left-over warps go where a warp has the most groups
+    while (used < NW) {            // left-over warps go where a warp has the most work
         int best = -1;
         for (int k = 0; k < NT; ++k)
-            if (w[k] < g[k] && (best < 0 || (unsigned long long)g[k] * w[best] > (unsigned long long)g[best] * w[k])) best = k;
+            if (w[k] < g[k] && (best < 0 || c[k] * w[best] > c[best] * w[k])) best = k;
         if (best < 0) break;
         ++w[best]; ++used;
     }

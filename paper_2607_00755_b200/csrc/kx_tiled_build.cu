@@ -4,7 +4,8 @@
 // kx_entry.cuh and from the same run table), regrouped in two ways:
 //
 //   gain operand  A[k=(n,m), i] = W_inm + W_imn for 16-row tiles, runs (tile, n) -> interval of m     eq. 4.6/4.7
-//   loss operand  M_c(i,j) = sum over the bucket {(n<=m): j_L(i,n,m) = j} of Wsym T_c(2 omega_R - 1), c < Q
+//   loss operand  M_c(i,j) = sum over the bucket {(n<=m): j_L(i,n,m) = j} of Wsym T_c(2 omega_R - 1), c < Q, stored for
+//                 LOG interpolation in the Lagrange basis of the Chebyshev nodes (see k_cheb_moments)
 //
 // Why Chebyshev moments: inside bracket j the interpolated occupation of eq. B.20 (eta = 0) is the smooth function
 // g(omega) = f_j^(1-omega) f_(j+1)^omega, omega in [0,1] (eq. B.19).  Its degree-(Q-1) interpolant at the Q
@@ -134,6 +135,16 @@ __global__ void __launch_bounds__(256) k_pack_gain(KxDev d, KxTiled t)
 template <int Q>
 __global__ void __launch_bounds__(128) k_cheb_moments(KxDev d, KxTiled t)
 {
+    // LOG: the moments are stored in the Lagrange basis of the Chebyshev nodes, L_q(omega) = sum_c D[c][q] T_c(2 omega - 1)
+    // with D = t.dct (the discrete Chebyshev transform, a_c = sum_q D[c][q] g(omega_q)):
+    //     sum_c a_c M_c = sum_q g(omega_q) ML_q,   ML_q = sum_c D[c][q] M_c,
+    // so that the operand X of the contraction is the interpolated occupation at the nodes itself and k_dmma needs no
+    // transform.  LINEAR (Q = 2) keeps the two exact Chebyshev coefficients.
+    __shared__ double s_D[Q > 2 ? Q * Q : 1];
+    if (Q > 2) {
+        for (int k = threadIdx.x; k < Q * Q; k += blockDim.x) s_D[k] = t.dct[k];
+        __syncthreads();
+    }
     const int N = d.N;
     const int i = blockIdx.x;
     const int rb8 = i >> 3, ir = i & 7;
@@ -188,10 +199,18 @@ __global__ void __launch_bounds__(128) k_cheb_moments(KxDev d, KxTiled t)
                 }
             }
         }
+#pragma unroll 1
+        for (int q = 0; q < Q; ++q) {
+            double v;
+            if (Q > 2) {
+                v = 0.0;
 #pragma unroll
-        for (int c = 0; c < Q; ++c) {
-            const int k = j * Q + c;
-            t.AL[(((size_t)(k >> 4) * t.NR8 + rb8) * 4 + ((k >> 2) & 3)) * 32 + ir * 4 + (k & 3)] = M[c];
+                for (int c = 0; c < Q; ++c) v = fma(s_D[c * Q + q], M[c], v);
+            } else {
+                v = q == 0 ? M[0] : M[Q > 1 ? 1 : 0];
+            }
+            const int k = j * Q + q;
+            t.AL[(((size_t)(k >> 4) * t.NR8 + rb8) * 4 + ((k >> 2) & 3)) * 32 + ir * 4 + (k & 3)] = v;
         }
     }
 }
