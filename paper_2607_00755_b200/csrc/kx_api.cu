@@ -4,6 +4,7 @@
 #include "kx_internal.cuh"
 
 #include <math.h>
+#include <stdlib.h>
 #include <new>
 #include <vector>
 
@@ -124,6 +125,14 @@ kx_status_t ensure_ws(kx_handle_s* h, int B)
         h->plan_B = 0;
     }
     h->wsB = nB; h->ws_tasks = need_tasks;
+    // test aid (tests/test_gpu_parity.py): KX_POISON_WS=1 fills every partial-sum workspace with NaN bit patterns, so that a
+    // slot the kernels read without having written it shows up in the result instead of passing on freshly zeroed memory
+    if (const char* e = getenv("KX_POISON_WS"); e && e[0] == '1') {
+        KX_CUDA(cudaMemset(h->part, 0xFF, (size_t)need_tasks * nB * 4 * 8));
+        KX_CUDA(cudaMemset(h->yd, 0xFF, bn * 2 * 8));
+        if (h->gpart) KX_CUDA(cudaMemset(h->gpart, 0xFF, (size_t)(h->sm_count + h->t.NT + 1) * h->ws_xstride * 16 * 8));
+        if (h->lpart) KX_CUDA(cudaMemset(h->lpart, 0xFF, (size_t)(h->sm_count + h->t.RS + 1) * h->ws_xstride * 256 * 8));
+    }
     return KX_OK;
 }
 

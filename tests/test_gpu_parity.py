@@ -307,9 +307,47 @@ def test_tiled_fallback_sharp_features(torch_cuda, oracle):
     assert (np.abs(Cp - Cp0) / scale).max() <= TOL
     # the same members in another order and batch size give the same bits (fallback is per member)
     perm = [3, 0, 5, 1]
+    assert h.fallback_members() == 6                     # members 1, 2, 3 in each of the two calls above, nobody else
     Cq = h.collide(_dev(torch, f[perm]), flags=1).cpu().numpy()
     assert np.array_equal(Cq, Cp[perm])
+    assert h.fallback_members() == 2                     # members 3 and 1 of the permuted batch
+    # smooth members only: nobody takes the exact path
+    h.collide(_dev(torch, c["f"]), flags=1)
+    assert h.fallback_members() == 0
     h.close()
+
+
+@pytest.mark.parametrize("N,log", [(6, False), (8, False), (12, False), (22, False), (32, True), (33, True), (44, True), (52, True)])
+def test_tiled_small_grids_poisoned_workspace(torch_cuda, oracle, monkeypatch, N, log):
+    """Grids with fewer gain groups than gain workers, on workspaces filled with NaN patterns (KX_POISON_WS) and after a
+    larger handle was created and destroyed in the same process: every partial slot the finishing phase adds must have been
+    written by the same launch.  Also across batch sizes on one handle, and bit-equal gain with the streaming storage."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    monkeypatch.setenv("KX_POISON_WS", "1")
+    big = kin.config(3, N=96, B=16)
+    hb = _handle(big)
+    hb.collide(_dev(torch, big["f"]))
+    hb.close()
+    p = kin.log_grid(N, 1e-2, 20.0) if log else kin.uniform_grid(N, 0.05, 8.0)
+    dp = kin.trapezoid_widths(p)
+    T = oracle.Tables(p, dp, 1.0)
+    h = kx.Handle(p, dp, 1.0, interp=kx.INTERP_LINEAR)
+    hs = kx.Handle(p, dp, 1.0, interp=kx.INTERP_LINEAR, storage=kx.STORE_SYM_ROWS)
+    for B in (3, 9, 1, 20):
+        f = np.stack([kin._random_bimodal(p, 7000 + b) for b in range(B)])
+        g0, l0, C0 = oracle.collide(T, f, 1)
+        g, l = h.collide_parts(_dev(torch, f))
+        assert torch.isfinite(g).all() and torch.isfinite(l).all()
+        assert _relerr(g.cpu().numpy(), g0, g0) <= TOL
+        assert _relerr(l.cpu().numpy(), l0, g0) <= TOL
+        gs, ls = hs.collide_parts(_dev(torch, f))
+        assert _relerr(gs.cpu().numpy(), g0, g0) <= TOL
+    hl = kx.Handle(p, dp, 1.0)                           # LOG interpolation: the Chebyshev-moment loss on the same grids
+    f = np.stack([kin._random_bimodal(p, 7100 + b) for b in range(5)])
+    g0, l0, C0 = oracle.collide(T, f, 0)
+    assert _relerr(hl.collide(_dev(torch, f)).cpu().numpy(), C0, g0) <= TOL
+    h.close(); hs.close(); hl.close()
 
 
 @pytest.mark.parametrize("B", [1, 7, 8, 9, 17, 33, 64, 65, 130])
