@@ -28,6 +28,9 @@ using namespace kxd;
 constexpr double kLossCost = 1.26;
 // cost of one run (tile, n) of the gain stream in units of one group (see kx_dmma_plan)
 constexpr double kRunCost = 0.09;
+// loss role in the plan's time model (units of one gain group of a warp): DMMA cost of a chunk relative to the same DMMA count of
+// the gain stream, and what the loss prologue (operand X: log2, exp2 at the nodes) takes longer than staging f
+constexpr double kLossChunk = 1.05, kLossPrologue = 5.5;
 
 // D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
@@ -666,28 +669,19 @@ cudaError_t kx_dmma_configure()
 void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned* vt_host, int B, KxPlan* plan)
 {
     const int nbt = dmma_nbt(d.N, B);
-    const unsigned Gtot = vt_host[t.NT];
+    const int NT = t.NT;
+    const unsigned Gtot = vt_host[NT];
     const double wg = (double)(Gtot > 0 ? Gtot : 1);
     const double wl = 0.5 * (double)t.LC * (double)t.NR8 * kLossCost;
     long long G = (long long)((wg + wl) / 8.0);
     if (G > sm_count) G = sm_count;
     if (G < 2) G = 2;
-    int gl = (int)((double)G * wl / (wg + wl) + 0.5);
-    if (gl < 1) gl = 1;
-    if (gl > (int)G - 1) gl = (int)G - 1;
     const long long U = (long long)t.RS * t.LC;
-    if (gl > U) gl = (int)U;                       // every loss CTA has at least one chunk
-    plan->nbt = nbt;
-    plan->GL = gl;
-    plan->GG = (int)G - gl;
-    plan->WC = loss_window(t, gl, nbt);
 
-    const int NT = t.NT;
-    const unsigned NW = (unsigned)plan->GG * WARPS;
     // cost of a tile in units of one group: its groups plus kRunCost per run (one run per n: the fold at the end of a run and
     // the short runs of the high tiles cost DMMA issue slots; measured with the clock-stamp trace: 0.83 of the DMMA peak on
     // tile 0, 0.76 on the last tile of cfg3)
-    std::vector<unsigned> w(NT, 0u), g(NT, 0u);
+    std::vector<unsigned> g(NT, 0u);
     std::vector<double> c(NT, 0.0);
     double Ctot = 0.0;
     for (int k = 0; k < NT; ++k) {
@@ -695,29 +689,79 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
         c[k] = g[k] ? (double)g[k] + kRunCost * (double)d.N : 0.0;
         Ctot += c[k];
     }
-    unsigned used = 0;
-    for (int k = 0; k < NT; ++k) {
-        if (g[k]) {
-            unsigned v = (unsigned)((double)NW * c[k] / Ctot);
-            if (v < 1) v = 1;
-            if (v > g[k]) v = g[k];
-            w[k] = v; used += v;
+    // the gain warps of GG CTAs dealt to the tiles in proportion to the tiles' costs (largest remainder), at least one and at
+    // most one per group; returns the load of the busiest warp in group units
+    auto deal = [&](int GG, std::vector<unsigned>& w) -> double {
+        const unsigned NW = (unsigned)GG * WARPS;
+        w.assign(NT, 0u);
+        unsigned used = 0;
+        for (int k = 0; k < NT; ++k) {
+            if (g[k]) {
+                unsigned v = (unsigned)((double)NW * c[k] / Ctot);
+                if (v < 1) v = 1;
+                if (v > g[k]) v = g[k];
+                w[k] = v; used += v;
+            }
         }
-    }
-    while (used > NW) {            // the minimum of one warp per tile overshot: take from the lightest-loaded warps
-        int best = -1;
+        while (used > NW) {            // the minimum of one warp per tile overshot: take from the lightest-loaded warps
+            int best = -1;
+            for (int k = 0; k < NT; ++k)
+                if (w[k] > 1 && (best < 0 || c[k] * w[best] < c[best] * w[k])) best = k;
+            if (best < 0) break;
+            --w[best]; --used;
+        }
+        while (used < NW) {            // left-over warps go where a warp has the most work
+            int best = -1;
+            for (int k = 0; k < NT; ++k)
+                if (w[k] < g[k] && (best < 0 || c[k] * w[best] > c[best] * w[k])) best = k;
+            if (best < 0) break;
+            ++w[best]; ++used;
+        }
+        // whole groups per warp: move warps from the tile that can best spare one to the tile with the busiest warp while
+        // that lowers the maximum
+        auto load_of = [&](int k, unsigned wk) { return (double)((g[k] + wk - 1) / wk) * (c[k] / (double)g[k]); };
+        for (int it = 0; it < 4 * NT; ++it) {
+            int kmax = -1, kmin = -1;
+            double lmax = 0.0, lmin = 1e300;
+            for (int k = 0; k < NT; ++k)
+                if (w[k]) { const double l = load_of(k, w[k]); if (l > lmax) { lmax = l; kmax = k; } }
+            for (int k = 0; k < NT; ++k)
+                if (w[k] > 1 && k != kmax) { const double l = load_of(k, w[k] - 1); if (l < lmin) { lmin = l; kmin = k; } }
+            if (kmax < 0 || kmin < 0 || w[kmax] >= g[kmax] || !(lmin < lmax)) break;
+            ++w[kmax]; --w[kmin];
+        }
+        double load = 0.0;
         for (int k = 0; k < NT; ++k)
-            if (w[k] > 1 && (best < 0 || c[k] * w[best] < c[best] * w[k])) best = k;
-        if (best < 0) break;
-        --w[best]; --used;
+            if (w[k]) { const double l = load_of(k, w[k]); if (l > load) load = l; }
+        return load;
+    };
+
+    // Role split.  First guess: in proportion to the DMMA counts.  Both roles are quantised (whole groups per gain warp,
+    // whole chunks of 16 k per loss CTA: 10 or 11 chunks at cfg3 is a 10 % step), so the neighbours of the guess are tried
+    // and the split with the earliest barrier wins: gain = load of the busiest warp; loss = chunks of the busiest CTA, one
+    // chunk of a full supertile being two groups' worth of DMMA per warp, plus the longer prologue of the loss role
+    // (kLossPrologue groups, from the clock-stamp trace).
+    int gl0 = (int)((double)G * wl / (wg + wl) + 0.5);
+    if (gl0 < 1) gl0 = 1;
+    if (gl0 > (int)G - 1) gl0 = (int)G - 1;
+    const double chunk_groups = 2.0 * (double)(t.NR8 < 32 * t.RS ? t.NR8 : 32 * t.RS) / (32.0 * t.RS) * kLossChunk;
+    int gl = gl0;
+    double best_t = 1e300;
+    std::vector<unsigned> w, wtry;
+    for (int cand = gl0 - 4; cand <= gl0 + 4; ++cand) {
+        if (cand < 1 || cand > (int)G - 1 || cand > U) continue;
+        const double tg = deal((int)G - cand, wtry);
+        const double tl = (double)((U + cand - 1) / cand) * chunk_groups + kLossPrologue;
+        const double tt = tg > tl ? tg : tl;
+        if (tt < best_t - 1e-9) { best_t = tt; gl = cand; }
     }
-    while (used < NW) {            // left-over warps go where a warp has the most work
-        int best = -1;
-        for (int k = 0; k < NT; ++k)
-            if (w[k] < g[k] && (best < 0 || c[k] * w[best] > c[best] * w[k])) best = k;
-        if (best < 0) break;
-        ++w[best]; ++used;
-    }
+    if (gl > U) gl = (int)U;                       // every loss CTA has at least one chunk
+    plan->nbt = nbt;
+    plan->GL = gl;
+    plan->GG = (int)G - gl;
+    plan->WC = loss_window(t, gl, nbt);
+    deal(plan->GG, w);
+
     unsigned run = 0;
     for (int k = 0; k < NT; ++k) { plan->wstart[k] = run; plan->vt[k] = vt_host[k]; run += w[k]; }
     plan->wstart[NT] = run; plan->vt[NT] = vt_host[NT];
