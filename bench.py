@@ -48,7 +48,7 @@ LOSS_NODES = {"log": 24, "linear": 2}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM; DMMA.8x8x4 runs at the same 37.2 TFLOP/s
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_dmma launch, from the committed `ncu --set full` capture named in
 # TRAFFIC_SOURCE (cfg3, LOG, B=64, raw operator); null for every other configuration
-NCU_TRAFFIC = {("log", 64): 61.09e6}
+NCU_TRAFFIC = {("log", 64): 61.34e6}
 TRAFFIC_SOURCE = "profiles/r02_k_dmma_full.md"
 
 
@@ -285,7 +285,7 @@ def time_evolve(torch, kx, dev, local, cfg, steps=None, with_oracle=False):
         B = 8
         c = kin.config(5, B=B)
         S = steps or 300
-        full = kin.config5_schedule(c["p"], c["dp"], B=B, S=10_000)
+        full = kin.config5_schedule(c["p"], c["p"] ** 2 * c["dp"], B=B, S=10_000)
         k0 = 3900                             # around x = 1: source 1 on, then off
         sch = dict(tau=full["tau"][k0:k0 + S + 1], rate=full["rate"][2 * k0:2 * (k0 + S) + 1],
                    mass=full["mass"][2 * k0:2 * (k0 + S) + 1], amp=np.ascontiguousarray(full["amp"][:, k0:k0 + S]))

@@ -120,12 +120,14 @@ def config(k: int, *, B: int | None = None, N: int | None = None) -> dict:
                 M2_0=1.0, m_med=m_med, f=np.ascontiguousarray(f, dtype=np.float64))
 
 
-def config5_schedule(p: np.ndarray, dp: np.ndarray, *, B: int = 8, S: int = 10_000) -> dict:
+def config5_schedule(p: np.ndarray, w: np.ndarray, *, B: int = 8, S: int = 10_000) -> dict:
     """Schedule arrays of config 5 (reading D11; every constant is a stated proposal).
 
     u = ln x from x=1e-2 to 1e3 in S steps; kinematic mass m(u)=x; rate = R1*x with
     R1 = 128 pi^3 (radiation domination, H ~ x^-2, in the kernel's units); two Gaussian
-    sources in q normalised to sum_i q_i^2 dq_i G_i = 1, centres (3, 30), widths (1, 3);
+    sources in q, centres (3, 30), widths (1, 3), each scaled so that sum_i w_i G_i = 1 for the
+    weights w the caller hands in (the callers pass w_i = q_i^2 dq_i: unit injected number per unit
+    amplitude; the generator itself holds none of the method's arithmetic);
     source 1 active while x<1, source 2 while 10<x<100, each adding 1e-3*G per step;
     kappa_b log-spaced 1e-4..1e2.
     """
@@ -139,9 +141,7 @@ def config5_schedule(p: np.ndarray, dp: np.ndarray, *, B: int = 8, S: int = 10_0
     R1 = 128.0 * math.pi ** 3
     G = np.stack([np.exp(-((p - 3.0) ** 2) / (2 * 1.0 ** 2)),
                   np.exp(-((p - 30.0) ** 2) / (2 * 3.0 ** 2))])
-    # input recipe, not the method's arithmetic: each shape is scaled so that its plain Riemann sum
-    # sum_i q_i^2 dq_i G_i over the grid handed in equals 1 (neither side consumes this sum as a result)
-    G /= (G * (p * p * dp)).sum(axis=1, keepdims=True)
+    G /= (G * np.asarray(w, dtype=np.float64)).sum(axis=1, keepdims=True)
     xs = np.exp(u[:-1])                       # x at the start of each step
     amp = np.zeros((2, S))
     amp[0, xs < 1.0 - 1e-12] = 1e-3 / du

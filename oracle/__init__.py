@@ -53,8 +53,11 @@ def _load():
                                       C.c_int, C.c_int, _dp, _dp, _dp]
         _lib.okx_evolve_q.restype = C.c_int
         _lib.okx_evolve_adaptive.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp] + [C.c_double] * 6 + [_dp] + \
-            [C.c_double] * 8 + [_dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp]
+            [C.c_double] * 9 + [_dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp]
         _lib.okx_evolve_adaptive.restype = C.c_int
+        _lib.okx_evolve_regimes.argtypes = [C.c_int, C.c_int, _dp, _dp] + [C.c_double] * 6 + [_dp] + \
+            [C.c_double] * 11 + [_dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp]
+        _lib.okx_evolve_regimes.restype = C.c_int
         _lib.okx_delta_source.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_double, _dp]
         _lib.okx_delta_source.restype = C.c_int
         _lib.okx_requadrature.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int,
@@ -208,9 +211,10 @@ def evolve(p, dp, f, *, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, interp=LOG, f_flo
 
 
 def evolve_adaptive(p, dp, f, *, u0, u1, du0=1e-4, rtol=1e-2, atol=2e-8, safety=0.9, rate0=1.0, rate_slope=0.0,
-                    m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, f_floor=1e-300, eps_supp=1e-12, kappa=None, project=True,
-                    G=None, amp=None, max_steps=100000, eta=0):
-    """Adaptive Heun of Sec. 4.2 (reading D15): returns f_final [B,N] and dict(u, du, accepted, rejected, done)."""
+                    mass_slope=0.0, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, f_floor=1e-300, eps_supp=1e-12, kappa=None,
+                    project=True, G=None, amp=None, max_steps=100000, eta=0):
+    """Adaptive Heun of Sec. 4.2 (reading D15): returns f_final [B,N] and dict(u, du, accepted, rejected, done).
+    Kinematic mass m(u) = m exp(mass_slope (u - u0))."""
     p, dp = _c(p), _c(dp)
     f = _c(np.atleast_2d(f)).copy()
     B, n = f.shape
@@ -222,9 +226,33 @@ def evolve_adaptive(p, dp, f, *, u0, u1, du0=1e-4, rtol=1e-2, atol=2e-8, safety=
     rc = _load().okx_evolve_adaptive(int(eta), n, B, _d(p), _d(dp), float(m), float(g_chi), float(M2_0), float(m_med),
                                      float(f_floor), float(eps_supp), _d(f), float(u0), float(u1), float(du0),
                                      float(rtol), float(atol), float(safety), float(rate0), float(rate_slope),
-                                     _d(kappa), int(bool(project)), nsrc, _d(G), _d(amp), int(max_steps), _d(out))
+                                     float(mass_slope), _d(kappa), int(bool(project)), nsrc, _d(G), _d(amp), int(max_steps),
+                                     _d(out))
     assert rc == 0
     return f, dict(u=out[0], du=out[1], accepted=int(out[2]), rejected=int(out[3]), done=bool(out[4]))
+
+
+def evolve_regimes(p, dp, f, *, u0, u1, du_fixed, eps_switch=1e-2, du0=1e-4, rtol=1e-2, atol=2e-8, safety=0.9, rate0=1.0,
+                   rate_slope=0.0, mass_slope=0.0, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, f_floor=1e-300, eps_supp=1e-12,
+                   kappa=None, project=True, G=None, amp=None, max_steps=100000):
+    """The two regimes of Sec. 4.2 (reading D16): sources only on fixed intervals until Gamma_2->2/H > eps_switch, then
+    adaptive Heun.  Returns f_final [B,N] and dict(u, du, accepted, rejected, done, u_switch, fixed_steps, ratio)."""
+    p, dp = _c(p), _c(dp)
+    f = _c(np.atleast_2d(f)).copy()
+    B, n = f.shape
+    kappa = None if kappa is None else _c(kappa)
+    nsrc = 0 if (G is None or amp is None) else int(np.atleast_2d(G).shape[0])
+    G = None if nsrc == 0 else _c(np.atleast_2d(G))
+    amp = None if nsrc == 0 else _c(np.atleast_1d(amp))
+    out = np.zeros(8)
+    rc = _load().okx_evolve_regimes(n, B, _d(p), _d(dp), float(m), float(g_chi), float(M2_0), float(m_med),
+                                    float(f_floor), float(eps_supp), _d(f), float(u0), float(u1), float(du_fixed),
+                                    float(eps_switch), float(du0), float(rtol), float(atol), float(safety), float(rate0),
+                                    float(rate_slope), float(mass_slope), _d(kappa), int(bool(project)), nsrc, _d(G),
+                                    _d(amp), int(max_steps), _d(out))
+    assert rc == 0
+    return f, dict(u=out[0], du=out[1], accepted=int(out[2]), rejected=int(out[3]), done=bool(out[4]),
+                   u_switch=out[5], fixed_steps=int(out[6]), ratio=out[7])
 
 
 def delta_source(p, dp, m, p0):

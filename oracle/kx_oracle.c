@@ -479,39 +479,42 @@ int okx_delta_source(int N, const double *p, const double *dp, double m, double 
 /* ---- Adaptive Heun in u = ln a (Sec. 4.2: "first computes an Euler predictor and then corrects it
  * using the average of the slopes at the beginning and end of the step. The difference between the predictor and
  * corrected value provides a local error estimate used to adjust the step size"; settings rtol, atol, du0, safety of
- * PAPER.md:474).  df/du = kappa_b R(u) C[f] + sum_s amp_s G_s, R(u) = rate0 exp(slope (u - u0)), static mass.
+ * PAPER.md:474).  df/du = kappa_b R(u) C[f; m(u)] + sum_s amp_s G_s, R(u) = rate0 exp(slope (u - u0)),
+ * m(u) = mass0 exp(mass_slope (u - u0)) (comoving momenta q = a p: the kinematics of eq. 4.4/B.17 see the mass m a,
+ * PAPER.md:166; mass_slope = 0: static mass).
  * Controller (the paper does not print it; reading D15): err = max_{b,i} |f_H - f_P| / (atol + rtol
  * max(|f|, |f_H|)) over the whole batch; accept iff err <= 1; du <- du clamp(safety / sqrt(max(err, 1e-10)), 0.2, 5);
- * du <= u1 - u; stop when u1 - u <= 1e-14 max(|u1|, 1).  out = {u, du, accepted, rejected, done}. */
-int okx_evolve_adaptive(int eta, int N, int B, const double *p, const double *dp, double m, double g_chi,
-                        double M2_0, double m_med, double f_floor, double eps_supp, double *f,
-                        double u0, double u1, double du0, double rtol, double atol, double safety,
-                        double rate0, double slope, const double *kappa, int project,
-                        int nsrc, const double *G, const double *amp, int max_steps, double *out)
+ * du <= u1 - u; stop when u1 - u <= 1e-14 max(|u1|, 1).  The loop runs from ustart (>= u0) with first step du_first. */
+static void okx_adaptive_core(okx_ctx *c, int B, double *f, double u0, double ustart, double u1, double du_first,
+                              double rtol, double atol, double safety, double rate0, double slope,
+                              double mass0, double mass_slope, const double *kappa, int project,
+                              int nsrc, const double *G, const double *amp, int max_steps,
+                              double *u_out, double *du_out, long *acc_out, long *rej_out, int *done_out)
 {
-    size_t N3 = (size_t)N * N * N;
-    okx_ctx c = { N, p, dp, m, g_chi, M2_0, m_med, 0, f_floor, eps_supp,
-                  malloc(sizeof(double) * N3), malloc(sizeof(int32_t) * N3), malloc(sizeof(double) * N3),
-                  malloc(sizeof(double) * N), malloc(sizeof(double) * N), malloc(sizeof(double) * N), m };
-    c.eta = eta;
-    okx_build(N, p, dp, m, g_chi, M2_0, m_med, c.W, c.jL, c.wR);
-    okx_kinematics(N, p, dp, m, c.E, c.K, c.h);
-    double *k1 = malloc(sizeof(double) * N), *k2 = malloc(sizeof(double) * N);
-    double *fP = malloc(sizeof(double) * N), *fH = malloc(sizeof(double) * (size_t)B * N);
-    double u = u0, du = du0 < u1 - u0 ? du0 : u1 - u0;
+    int N = c->N;
+    int use_mass = mass_slope != 0.0;
+    double *K1 = malloc(sizeof(double) * (size_t)B * N), *k2 = malloc(sizeof(double) * N);
+    double *fP = malloc(sizeof(double) * (size_t)B * N), *fH = malloc(sizeof(double) * (size_t)B * N);
+    double u = ustart, du = du_first < u1 - ustart ? du_first : u1 - ustart;
     long acc = 0, rej = 0;
-    int done = 0;
+    int done = u1 - u <= 1e-14 * fmax(fabs(u1), 1.0);
     for (int step = 0; step < max_steps && !done; ++step) {
         double err = 0.0;
+        double ma = use_mass ? mass0 * exp(mass_slope * (u - u0)) : mass0;
+        double mb = use_mass ? mass0 * exp(mass_slope * (u + du - u0)) : mass0;
+        /* stage-major over the members, so that a time-dependent mass needs one rebuild per stage */
         for (int b = 0; b < B; ++b) {
             double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
-            okx_rhs(&c, fb, m, 0, kb * rate0 * exp(slope * (u - u0)), project, nsrc, G, amp, k1, NULL);
-            for (int i = 0; i < N; ++i) fP[i] = fb[i] + du * k1[i];                        /* Euler predictor */
-            okx_rhs(&c, fP, m, 0, kb * rate0 * exp(slope * (u + du - u0)), project, nsrc, G, amp, k2, NULL);
+            okx_rhs(c, fb, ma, use_mass, kb * rate0 * exp(slope * (u - u0)), project, nsrc, G, amp, K1 + (size_t)b * N, NULL);
+            for (int i = 0; i < N; ++i) fP[(size_t)b * N + i] = fb[i] + du * K1[(size_t)b * N + i];   /* Euler predictor */
+        }
+        for (int b = 0; b < B; ++b) {
+            double kb = kappa ? kappa[b] : 1.0, *fb = f + (size_t)b * N;
+            okx_rhs(c, fP + (size_t)b * N, mb, use_mass, kb * rate0 * exp(slope * (u + du - u0)), project, nsrc, G, amp, k2, NULL);
             for (int i = 0; i < N; ++i) {
-                double fh = fb[i] + 0.5 * du * (k1[i] + k2[i]);                             /* Heun corrector */
+                double fh = fb[i] + 0.5 * du * (K1[(size_t)b * N + i] + k2[i]);                       /* Heun corrector */
                 fH[(size_t)b * N + i] = fh;
-                double e = fabs(fh - fP[i]) / (atol + rtol * fmax(fabs(fb[i]), fabs(fh)));
+                double e = fabs(fh - fP[(size_t)b * N + i]) / (atol + rtol * fmax(fabs(fb[i]), fabs(fh)));
                 if (!(e <= err)) err = isfinite(e) ? e : INFINITY;
             }
         }
@@ -524,8 +527,109 @@ int okx_evolve_adaptive(int eta, int N, int B, const double *p, const double *dp
         if (u1 - u <= 1e-14 * fmax(fabs(u1), 1.0)) { done = 1; u = u1; }
         else if (du > u1 - u) du = u1 - u;
     }
+    *u_out = u; *du_out = du; *acc_out = acc; *rej_out = rej; *done_out = done;
+    free(K1); free(k2); free(fP); free(fH);
+}
+
+static okx_ctx okx_ctx_new(int eta, int N, const double *p, const double *dp, double m, double g_chi, double M2_0,
+                           double m_med, double f_floor, double eps_supp)
+{
+    size_t N3 = (size_t)N * N * N;
+    okx_ctx c = { N, p, dp, m, g_chi, M2_0, m_med, 0, f_floor, eps_supp,
+                  malloc(sizeof(double) * N3), malloc(sizeof(int32_t) * N3), malloc(sizeof(double) * N3),
+                  malloc(sizeof(double) * N), malloc(sizeof(double) * N), malloc(sizeof(double) * N), m };
+    c.eta = eta;
+    okx_build(N, p, dp, m, g_chi, M2_0, m_med, c.W, c.jL, c.wR);
+    okx_kinematics(N, p, dp, m, c.E, c.K, c.h);
+    return c;
+}
+static void okx_ctx_free(okx_ctx *c) { free(c->W); free(c->jL); free(c->wR); free(c->E); free(c->K); free(c->h); }
+
+/* out = {u, du, accepted, rejected, done} */
+int okx_evolve_adaptive(int eta, int N, int B, const double *p, const double *dp, double m, double g_chi,
+                        double M2_0, double m_med, double f_floor, double eps_supp, double *f,
+                        double u0, double u1, double du0, double rtol, double atol, double safety,
+                        double rate0, double slope, double mass_slope, const double *kappa, int project,
+                        int nsrc, const double *G, const double *amp, int max_steps, double *out)
+{
+    okx_ctx c = okx_ctx_new(eta, N, p, dp, m, g_chi, M2_0, m_med, f_floor, eps_supp);
+    double u, du; long acc, rej; int done;
+    okx_adaptive_core(&c, B, f, u0, u0, u1, du0, rtol, atol, safety, rate0, slope, m, mass_slope, kappa, project,
+                      nsrc, G, amp, max_steps, &u, &du, &acc, &rej, &done);
     out[0] = u; out[1] = du; out[2] = (double)acc; out[3] = (double)rej; out[4] = (double)done;
-    free(c.W); free(c.jL); free(c.wR); free(c.E); free(c.K); free(c.h); free(k1); free(k2); free(fP); free(fH);
+    okx_ctx_free(&c);
+    return 0;
+}
+
+/* ---- The two regimes of Sec. 4.2.
+ * Regime 1, "the self-scattering rate is negligible compared with the Hubble rate, and the evolution is driven only by
+ * the freeze-in source terms.  In this regime, we set the self-collisions to zero, C_el[f] = 0, and evolve the
+ * distribution with a fourth-order Runge-Kutta method on fixed intervals in u": steps of du_fixed (the last one cut at
+ * u1).  The source rates amp_s are constant in u here, so all four Runge-Kutta slopes are the same vector
+ * k = sum_s amp_s G_s and the RK4 update f + (du/6)(k + 2k + 2k + k) is f + du k: that is what is evaluated.
+ * "The code also monitors the effective self-scattering rate, Gamma_2->2 = n_chi <sigma v>, and compares it with the
+ * Hubble rate.  Once Gamma_2->2 / H > eps_switch = 1e-2, the elastic self-collision operator is included."  Reading D16
+ * (the paper gives only the definition): the discretized n_chi <sigma v> seen by a particle of bin i is the loss
+ * frequency nu_i = loss_i / f_i = sum_nm W_inm f_j~ of eq. 4.6, its average over the population is
+ * nu_bar = sum_i h_i loss_i / sum_i h_i f_i, and with the time variable u of eq. 4.9 the ratio is
+ *     Gamma_2->2 / H = kappa_b R(u) nu_bar[f(u); m(u)]          (0 when sum h f = 0).
+ * It is evaluated at u0 and after every fixed step; the whole batch switches at the first such point where the LARGEST
+ * member ratio exceeds eps_switch (eps_switch <= 0: regime 2 from the start).
+ * Regime 2: adaptive Heun (okx_adaptive_core) from the switch point to u1 with first step du0.
+ * out = {u, du, accepted, rejected, done, u_switch, fixed_steps, ratio_at_switch}; max_steps bounds the attempted Heun
+ * steps; u_switch = u1 and ratio = the last monitored value if the switch never happens. */
+int okx_evolve_regimes(int N, int B, const double *p, const double *dp, double m, double g_chi,
+                       double M2_0, double m_med, double f_floor, double eps_supp, double *f,
+                       double u0, double u1, double du_fixed, double eps_switch,
+                       double du0, double rtol, double atol, double safety,
+                       double rate0, double slope, double mass_slope, const double *kappa, int project,
+                       int nsrc, const double *G, const double *amp, int max_steps, double *out)
+{
+    okx_ctx c = okx_ctx_new(0, N, p, dp, m, g_chi, M2_0, m_med, f_floor, eps_supp);
+    int use_mass = mass_slope != 0.0;
+    double *loss = malloc(sizeof(double) * N);
+    double u = u0, ratio = 0.0;
+    long fixed = 0;
+    int switched = 0, done = 0;
+    for (;;) {
+        /* monitor at u */
+        double mu_ = use_mass ? m * exp(mass_slope * (u - u0)) : m;
+        if (use_mass && mu_ != c.cur_m) {
+            okx_build(N, p, dp, mu_, g_chi, M2_0, m_med, c.W, c.jL, c.wR);
+            okx_kinematics(N, p, dp, mu_, c.E, c.K, c.h);
+            c.cur_m = mu_;
+        }
+        ratio = 0.0;
+        for (int b = 0; b < B; ++b) {
+            const double *fb = f + (size_t)b * N;
+            okx_collide(N, 1, fb, c.W, c.jL, c.wR, 0, f_floor, NULL, loss, NULL);
+            long double sl = 0.0L, sf = 0.0L;
+            for (int i = 0; i < N; ++i) { sl += (long double)c.h[i] * loss[i]; sf += (long double)c.h[i] * fb[i]; }
+            double r = sf > 0.0L ? (kappa ? kappa[b] : 1.0) * rate0 * exp(slope * (u - u0)) * (double)(sl / sf) : 0.0;
+            if (r > ratio) ratio = r;
+        }
+        if (!(eps_switch > 0.0) || ratio > eps_switch) { switched = 1; break; }
+        if (u1 - u <= 1e-14 * fmax(fabs(u1), 1.0)) { done = 1; u = u1; break; }
+        /* one fixed step with C_el = 0 */
+        double du = du_fixed < u1 - u ? du_fixed : u1 - u;
+        for (int b = 0; b < B; ++b)
+            for (int i = 0; i < N; ++i) {
+                double k = 0.0;
+                for (int q = 0; q < nsrc; ++q) k += amp[q] * G[(size_t)q * N + i];
+                f[(size_t)b * N + i] += du * k;
+            }
+        u += du;
+        ++fixed;
+    }
+    double usw = switched ? u : u1, du_next = du0;
+    long acc = 0, rej = 0;
+    if (switched)
+        okx_adaptive_core(&c, B, f, u0, u, u1, du0, rtol, atol, safety, rate0, slope, m, mass_slope, kappa, project,
+                          nsrc, G, amp, max_steps, &u, &du_next, &acc, &rej, &done);
+    out[0] = u; out[1] = du_next; out[2] = (double)acc; out[3] = (double)rej; out[4] = (double)done;
+    out[5] = usw; out[6] = (double)fixed; out[7] = ratio;
+    free(loss);
+    okx_ctx_free(&c);
     return 0;
 }
 

@@ -110,7 +110,7 @@ def test_cfg5_reduced_freeze_in(torch_cuda, oracle):
     import paper_2607_00755_b200 as kx
     B, S = 8, 1000
     c = kin.config(5, N=64, B=B)
-    sch = kin.config5_schedule(c["p"], c["dp"], B=B, S=S)
+    sch = kin.config5_schedule(c["p"], c["p"] ** 2 * c["dp"], B=B, S=S)
     f_ref, d_ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], method=oracle.RK4, tau=sch["tau"],
                                  rate=sch["rate"], mass=sch["mass"], kappa=sch["kappa"], G=sch["G"],
                                  amp=sch["amp"], want_diag=True)
@@ -147,7 +147,7 @@ def test_cfg5_full_size_steps_against_oracle(torch_cuda, oracle):
     import paper_2607_00755_b200 as kx
     B, S = 8, 10_000
     c = kin.config(5, B=B)
-    sch = kin.config5_schedule(c["p"], c["dp"], B=B, S=S)
+    sch = kin.config5_schedule(c["p"], c["p"] ** 2 * c["dp"], B=B, S=S)
     h = kx.Handle(c["p"], c["dp"], c["m"])
     G = _dev(torch, sch["G"])
     f = _dev(torch, c["f"])
@@ -229,7 +229,7 @@ def test_cfg5_sources_only_and_heun_euler_mass(torch_cuda, oracle):
     import paper_2607_00755_b200 as kx
     B, S = 2, 40
     c = kin.config(5, N=32, B=B)
-    sch = kin.config5_schedule(c["p"], c["dp"], B=B, S=S)
+    sch = kin.config5_schedule(c["p"], c["p"] ** 2 * c["dp"], B=B, S=S)
     expect = (sch["amp"] * np.diff(sch["tau"])[None, :]).sum(axis=1) @ sch["G"]
     h = kx.Handle(c["p"], c["dp"], c["m"])
     G = _dev(torch, sch["G"])
@@ -270,7 +270,7 @@ def test_cfg5_full_size_invariants(torch_cuda):
     import paper_2607_00755_b200 as kx
     B, S = 8, 10_000
     c = kin.config(5, B=B)
-    sch = kin.config5_schedule(c["p"], c["dp"], B=B, S=S)
+    sch = kin.config5_schedule(c["p"], c["p"] ** 2 * c["dp"], B=B, S=S)
     h = kx.Handle(c["p"], c["dp"], c["m"])
     f = _dev(torch, c["f"])
     h.evolve(f, sch["tau"], method=kx.RK4, rate=sch["rate"], mass=sch["mass"], kappa=sch["kappa"],

@@ -316,7 +316,7 @@ def test_moments_closed_form(oracle):
 def test_evolve_sources_only_closed_form(oracle):
     """kappa = 0 switches the collision term off: f(S) = f(0) + sum_k amp[:,k] dtau_k G exactly, any method."""
     c = kin.config(5, N=24, B=3)
-    sch = kin.config5_schedule(c["p"], c["dp"], B=3, S=40)
+    sch = kin.config5_schedule(c["p"], c["p"] ** 2 * c["dp"], B=3, S=40)
     expect = (sch["amp"] * np.diff(sch["tau"])[None, :]).sum(axis=1) @ sch["G"]
     for method in (oracle.EULER, oracle.HEUN, oracle.RK4):
         f = oracle.evolve(c["p"], c["dp"], c["f"], method=method, tau=sch["tau"], rate=sch["rate"],
@@ -607,3 +607,116 @@ def test_A3_adaptive_rate_slope_by_reparametrisation(oracle):
         errs.append(np.abs(f - ref).max() / np.abs(ref).max())
     assert errs[0] < 2e-4 and errs[1] < 2e-5, errs
     assert errs[0] / errs[1] > 5.0, errs
+
+
+def test_A4_adaptive_mass_slope_against_fixed_step_reference(oracle):
+    """okx_evolve_adaptive's kinematic mass m(u) = m e^{mass_slope (u - u0)} (comoving momenta: the kinematics see m a,
+    PAPER.md:166).  Independent reference: the fixed-step RK4 integrator fed the sampled arrays mass[2S+1] (whose stage
+    positions are pinned by E2) on a fine grid.  The adaptive solution approaches it with an error proportional to rtol;
+    taking the mass at u for both Heun stages would be first order (error ~ sqrt(rtol)), and ignoring the slope is off at
+    O(1)."""
+    N = 24
+    p = kin.log_grid(N, 2e-2, 20.0)
+    dp = kin.trapezoid_widths(p)
+    f0 = kin._random_bimodal(p, 91)[None, :]
+    m0, slope = 0.4, 1.0
+    T = oracle.Tables(p, dp, m0)
+    g, l, C = oracle.collide(T, f0, oracle.LOG)
+    nu = float((l[0] / f0[0]).max())
+    u0, u1 = 0.0, 1.2                                     # the mass grows by e^1.2 = 3.3
+    rate0 = 6.0 / nu / (u1 - u0)
+    S = 600
+    tau = np.linspace(u0, u1, S + 1)
+    th = np.empty(2 * S + 1)
+    th[0::2] = tau
+    th[1::2] = 0.5 * (tau[:-1] + tau[1:])
+    ref = oracle.evolve(p, dp, f0, m=m0, method=oracle.RK4, tau=tau, rate=np.full(2 * S + 1, rate0),
+                        mass=m0 * np.exp(slope * (th - u0)))
+    scale = np.abs(ref).max()
+    errs = []
+    for rtol in (1e-4, 1e-5):
+        f, info = oracle.evolve_adaptive(p, dp, f0, m=m0, u0=u0, u1=u1, du0=1e-4, rtol=rtol, atol=rtol * 1e-9, rate0=rate0,
+                                         mass_slope=slope)
+        assert info["done"]
+        errs.append(np.abs(f - ref).max() / scale)
+    assert errs[0] < 3e-4 and errs[1] < 3e-5, errs
+    assert errs[0] / errs[1] > 5.0, errs
+    f_static, _ = oracle.evolve_adaptive(p, dp, f0, m=m0, u0=u0, u1=u1, du0=1e-4, rtol=1e-5, atol=1e-14, rate0=rate0)
+    assert np.abs(f_static - ref).max() / scale > 1e-3
+
+
+def test_R1_regime_switch_closed_form(oracle):
+    """The Gamma_2->2/H switch of Sec. 4.2 (reading D16) where it has a closed form: before the switch f(u) = (u - u0) S
+    with S = sum_s amp_s G_s (f0 = 0, sources only), the LOG-interpolated loss is homogeneous of degree two in f, so
+        Gamma/H (u) = kappa R(u) (u - u0) nu_bar[S],   nu_bar[S] = sum h loss[S] / sum h S
+    with one oracle.collide of S.  The whole batch switches at the first fixed step boundary where the LARGEST member ratio
+    exceeds eps_switch; the monitor sees R(u) at the boundary."""
+    c = kin.config(1)
+    p, dp = c["p"], c["dp"]
+    G = np.stack([np.exp(-0.5 * (p - 3.0) ** 2), np.exp(-0.5 * ((p - 6.0) / 2.0) ** 2)])
+    amp = np.array([0.3, 0.05])
+    Ssrc = (amp[:, None] * G).sum(axis=0)[None, :]
+    T = oracle.Tables(p, dp, c["m"])
+    g, l, C = oracle.collide(T, Ssrc, oracle.LOG)
+    nubar = float((T.h * l[0]).sum() / (T.h * Ssrc[0]).sum())
+    u0, u1, duf, eps = 0.5, 3.0, 0.05, 1e-2
+    kappa = np.array([0.2, 1.0, 0.05])
+    slope = 0.8
+    rate0 = eps / (kappa.max() * nubar * 1.02)            # the largest member crosses eps near u - u0 = 0.6
+    ks = np.arange(1, 60)
+    ratio = kappa.max() * rate0 * np.exp(slope * ks * duf) * (ks * duf) * nubar
+    k_star = int(ks[np.argmax(ratio > eps)])
+    assert 5 < k_star < 40
+    f0 = np.zeros((3, p.size))
+    f, info = oracle.evolve_regimes(p, dp, f0, m=c["m"], u0=u0, u1=u1, du_fixed=duf, eps_switch=eps, du0=1e-3, rtol=1e-3,
+                                    atol=1e-12, rate0=rate0, rate_slope=slope, kappa=kappa, G=G, amp=amp, max_steps=1)
+    assert info["fixed_steps"] == k_star
+    assert abs(info["u_switch"] - (u0 + k_star * duf)) <= 1e-12
+    assert info["ratio"] == pytest.approx(float(ratio[k_star - 1]), rel=1e-10)
+    # teeth: a rule based on the smallest member, or a monitor without R(u), switches at another step
+    k_min = int(ks[np.argmax(kappa.min() * rate0 * np.exp(slope * ks * duf) * (ks * duf) * nubar > eps)]) if \
+        (kappa.min() * rate0 * np.exp(slope * ks * duf) * (ks * duf) * nubar > eps).any() else 10 ** 9
+    k_noR = int(ks[np.argmax(kappa.max() * rate0 * (ks * duf) * nubar > eps)])
+    assert k_min != k_star and k_noR != k_star
+    # never switching: sources only to the end, f = (u1 - u0) S exactly, no Heun step taken
+    f2, info2 = oracle.evolve_regimes(p, dp, f0, m=c["m"], u0=u0, u1=u1, du_fixed=duf, eps_switch=1e30, rate0=rate0,
+                                      rate_slope=slope, kappa=kappa, G=G, amp=amp)
+    assert info2["done"] and info2["accepted"] == 0 and info2["u_switch"] == u1
+    assert np.abs(f2 - (u1 - u0) * Ssrc).max() <= 1e-13 * np.abs(Ssrc).max() * (u1 - u0)
+
+
+def test_R2_regimes_compose(oracle):
+    """After the switch the run IS the adaptive Heun integration started from the switch state: regimes(u0 -> u1) equals
+    sources-only to u_switch followed by okx_evolve_adaptive(u_switch -> u1) with the rate and the mass continued
+    (rate0' = R(u_switch), m' = m(u_switch)); eps_switch <= 0 is plain adaptive Heun from u0.  With a mass slope the monitor
+    uses the kinematics of m(u) (the monitored ratio moves when the slope is ignored)."""
+    N = 24
+    p = kin.log_grid(N, 2e-2, 20.0)
+    dp = kin.trapezoid_widths(p)
+    G = np.exp(-0.5 * ((p - 2.0) / 0.7) ** 2)[None, :]
+    amp = np.array([0.4])
+    m0, mslope, rslope = 0.3, 1.0, 0.5
+    u0, u1, duf = 0.0, 1.5, 0.1
+    f0 = np.zeros((2, N))
+    kappa = np.array([1.0, 0.3])
+    T = oracle.Tables(p, dp, m0)
+    g, l, C = oracle.collide(T, amp[0] * G, oracle.LOG)
+    nubar = float((T.h * l[0]).sum() / (T.h * amp[0] * G[0]).sum())
+    rate0 = 1e-2 / (nubar * 0.45)
+    kw = dict(du0=1e-3, rtol=1e-4, atol=1e-13, kappa=kappa, G=G, amp=amp)
+    f, info = oracle.evolve_regimes(p, dp, f0, m=m0, u0=u0, u1=u1, du_fixed=duf, eps_switch=1e-2, rate0=rate0,
+                                    rate_slope=rslope, mass_slope=mslope, **kw)
+    assert info["done"] and 1 <= info["fixed_steps"] < 14 and info["accepted"] > 3
+    us = info["u_switch"]
+    start = f0 + (us - u0) * amp[0] * G
+    f2, info2 = oracle.evolve_adaptive(p, dp, start, m=m0 * math.exp(mslope * (us - u0)), u0=us, u1=u1,
+                                       rate0=rate0 * math.exp(rslope * (us - u0)), rate_slope=rslope, mass_slope=mslope, **kw)
+    assert info2["accepted"] == info["accepted"] and info2["rejected"] == info["rejected"]
+    assert np.abs(f - f2).max() <= 1e-12 * np.abs(f2).max()
+    f3, info3 = oracle.evolve_regimes(p, dp, start, m=m0, u0=u0, u1=u1, du_fixed=duf, eps_switch=0.0, rate0=rate0,
+                                      rate_slope=rslope, mass_slope=mslope, **kw)
+    f4, info4 = oracle.evolve_adaptive(p, dp, start, m=m0, u0=u0, u1=u1, rate0=rate0, rate_slope=rslope, mass_slope=mslope, **kw)
+    assert info3["fixed_steps"] == 0 and info3["accepted"] == info4["accepted"] and np.array_equal(f3, f4)
+    _, info5 = oracle.evolve_regimes(p, dp, f0, m=m0, u0=u0, u1=u1, du_fixed=duf, eps_switch=1e-2, rate0=rate0,
+                                     rate_slope=rslope, mass_slope=0.0, **kw)
+    assert info5["fixed_steps"] != info["fixed_steps"] or abs(info5["ratio"] / info["ratio"] - 1.0) > 1e-2
