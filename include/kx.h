@@ -176,8 +176,18 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
  * G: DEVICE [N].  KX_ERR_INVALID_ARG unless p[0] <= p0 <= p[N-1].  Asynchronous. */
 kx_status_t kx_delta_source(kx_handle_t h, double p0, double* G, void* stream);
 
-/* Adaptive Heun integration in u = ln a (Sec. 4.2; settings of PAPER.md:474), static kinematic mass:
- *     df/du = kappa_b R(u) C[f] + sum_s amp_s G_s,   R(u) = rate0 exp(rate_slope (u - u0))        (eq. 4.9)
+/* The time integration of Sec. 4.2 in u = ln a (settings of PAPER.md:474):
+ *     df/du = kappa_b R(u) C[f; m(u)] + sum_s amp_s G_s,   R(u) = rate0 exp(rate_slope (u - u0))        (eq. 4.9)
+ *     m(u) = m exp(mass_slope (u - u0)), m = the handle's current mass: with comoving momenta q = a p the kinematics see the
+ *     mass m a; mass_slope != 0 re-evaluates a1-a3 on the device at every stage (m(u) is computed on the
+ *     device from the controller's u: a rejected step costs no host round trip).
+ * Regime 1 (eps_switch > 0 and du_fixed > 0): "the self-scattering rate is negligible ... we set the self-collisions to zero
+ * and evolve the distribution with a fourth-order Runge-Kutta method on fixed intervals in u" (steps of du_fixed; with source
+ * rates constant in u the RK4 update is f + du sum_s amp_s G_s).  At u0 and after every fixed step the monitor
+ *     Gamma_2->2 / H = kappa_b R(u) sum_i h_i loss_i[f; m(u)] / sum_i h_i f_i          (reading D16)
+ * is evaluated on the device (one operator evaluation); at the first such point where the LARGEST member ratio exceeds
+ * eps_switch (1e-2) the whole batch enters regime 2 there.  eps_switch <= 0: regime 2 from u0.
+ * Regime 2: adaptive Heun.
  * Every attempted step is an Euler predictor f_P = f + du k1 and the Heun corrector f_H = f + du (k1 + k2)/2 (two
  * operator evaluations); err = max_{b,i} |f_H - f_P| / (atol + rtol max(|f|, |f_H|)) over the whole batch; the step is
  * accepted iff err <= 1, and du <- du clamp(safety / sqrt(err), 0.2, 5), du <= u1 - u (reading D15).
@@ -191,19 +201,26 @@ typedef struct {
     double rate0, rate_slope;
     const double* kappa;   /* HOST [B] per-member coupling multiplier; NULL => 1 */
     const double* amp;     /* HOST [src->nsrc] constant source rates per unit u (src->amp is not used); NULL => no sources */
-    int32_t max_steps;     /* attempted steps at most (> 0) */
+    int32_t max_steps;     /* attempted Heun steps at most (> 0) */
     uint32_t flags;        /* KX_PROJECT */
+    double mass_slope;     /* m(u) = m exp(mass_slope (u - u0)); 0 = static mass */
+    double du_fixed;       /* regime 1: fixed interval in u (> 0 to enable regime 1) */
+    double eps_switch;     /* regime 1 ends when Gamma_2->2/H exceeds this (1e-2); <= 0: no regime 1 */
 } kx_adaptive_t;
 
 typedef struct {
     double u, du;          /* where the integration stopped, the step it would take next */
     int64_t accepted, rejected;
     int32_t done;          /* 1 iff u reached u1 */
+    int32_t switched;      /* 1 iff regime 2 was entered */
+    double u_switch;       /* where (u1 if never) */
+    int64_t fixed_steps;   /* regime-1 steps taken */
+    double ratio;          /* Gamma_2->2/H of the last monitor point (largest member) */
 } kx_adaptive_result_t;
 
 /* f: DEVICE [B,N] in/out; src: only nsrc and G are read (may be NULL); result: HOST (may be NULL).  Synchronises.
- * KX_ERR_NONFINITE if f left the finite range; KX_ERR_UNSUPPORTED on a handle whose mass was changed is not raised:
- * the current tensor is used throughout. */
+ * KX_ERR_NONFINITE if f left the finite range.  With mass_slope != 0 the handle is left with the kinematics and the tensor
+ * of m(u) at the u where the integration stopped (as after kx_set_mass). */
 kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_source_t* src,
                                const kx_adaptive_t* ctl, kx_adaptive_result_t* result, void* stream);
 

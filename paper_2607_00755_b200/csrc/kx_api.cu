@@ -631,38 +631,97 @@ kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_sou
     if (rc != KX_OK) return rc;
     if (!ctl || !(ctl->u1 > ctl->u0) || !(ctl->du0 > 0.0) || !(ctl->rtol >= 0.0) || !(ctl->atol >= 0.0) ||
         !(ctl->rtol + ctl->atol > 0.0) || !(ctl->safety > 0.0 && ctl->safety <= 1.0) || ctl->max_steps < 1 ||
-        !isfinite(ctl->rate0) || !isfinite(ctl->rate_slope)) {
-        h->err = "kx_evolve_adaptive: need u1 > u0, du0 > 0, rtol, atol >= 0 (not both 0), 0 < safety <= 1, max_steps >= 1";
+        !isfinite(ctl->rate0) || !isfinite(ctl->rate_slope) || !isfinite(ctl->mass_slope) || !isfinite(ctl->du_fixed) ||
+        !isfinite(ctl->eps_switch)) {
+        h->err = "kx_evolve_adaptive: need u1 > u0, du0 > 0, rtol, atol >= 0 (not both 0), 0 < safety <= 1, max_steps >= 1, finite rates and slopes";
         return KX_ERR_INVALID_ARG;
     }
+    const bool regime1 = ctl->eps_switch > 0.0;
+    if (regime1 && !(ctl->du_fixed > 0.0)) { h->err = "kx_evolve_adaptive: eps_switch > 0 needs du_fixed > 0"; return KX_ERR_INVALID_ARG; }
     const int nsrc = (src && ctl->amp) ? src->nsrc : 0;
     if (nsrc < 0 || nsrc > KX_MAX_SRC || (nsrc > 0 && !src->G)) { h->err = "bad source description"; return KX_ERR_INVALID_ARG; }
     DeviceGuard guard(h->device);
     cudaStream_t s = (cudaStream_t)stream;
     const int N = h->d.N;
+    const bool mass_var = ctl->mass_slope != 0.0;
+    const double mass0 = h->d.m;
+    if (mass_var && h->cap < tri_entries(N)) {       // another mass may keep more triples: size for every (i, n <= m)
+        KX_CUDA(cudaStreamSynchronize(s));
+        if ((rc = alloc_tensor(h, tri_entries(N))) != KX_OK) return rc;
+        if ((rc = rebuild(h, h->d.m, s)) != KX_OK) return rc;
+    }
     if ((rc = ensure_ws(h, B)) != KX_OK) return rc;
-    if (!h->adapt) KX_CUDA(cudaMalloc((void**)&h->adapt, sizeof(KxAdapt)));
+    if (!h->adapt) KX_CUDA(cudaMalloc((void**)&h->adapt, sizeof(KxAdapt) + 64 + KX_MAX_SRC * 8));
+    double* m_dev = reinterpret_cast<double*>(reinterpret_cast<char*>(h->adapt) + ((sizeof(KxAdapt) + 15) & ~(size_t)15));
+    double* amp_dev = m_dev + 2;
     double* kappa_d = nullptr;
     if (ctl->kappa) {
         kappa_d = h->Cbuf + (size_t)h->wsB * N;
         KX_CUDA(cudaMemcpyAsync(kappa_d, ctl->kappa, (size_t)B * 8, cudaMemcpyHostToDevice, s));
     }
+    if (nsrc > 0) KX_CUDA(cudaMemcpyAsync(amp_dev, ctl->amp, (size_t)nsrc * 8, cudaMemcpyHostToDevice, s));
     KxAdapt init = {};
     init.u = ctl->u0;
     init.du = ctl->du0 < ctl->u1 - ctl->u0 ? ctl->du0 : ctl->u1 - ctl->u0;
     init.errkey = 0;                 // key of +0.0
+    init.switched = regime1 ? 0 : 1;
+    init.u_switch = regime1 ? ctl->u1 : ctl->u0;
     KX_CUDA(cudaMemcpyAsync(h->adapt, &init, sizeof init, cudaMemcpyHostToDevice, s));
     KX_CUDA(cudaMemsetAsync(h->flag, 0, 4, s));
-    const bool use_tiled = h->storage == KX_STORE_TILED && nnz_estimate(h) * B > kSmallProblem;
+    // with m(u) every stage has new kinematics: the exact streaming path (as kx_evolve with a mass schedule)
+    const bool use_tiled = h->storage == KX_STORE_TILED && !mass_var && nnz_estimate(h) * B > kSmallProblem;
     if (use_tiled && (rc = ensure_tiled(h, s)) != KX_OK) return rc;
     if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
 
+    // a1-a3 for m(u_stage), u_stage read from the controller state on the device
+    auto rebuild_at = [&](int stage) -> kx_status_t {
+        KX_CUDA(kx_launch_adapt_mass(h->adapt, stage, ctl->u0, mass0, ctl->mass_slope, m_dev, s));
+        h->d.m_dev = m_dev;
+        KX_CUDA(kx_launch_kinematics(h->d, 0.0, s));
+        KX_CUDA(kx_launch_runs(h->d, s));
+        KX_CUDA(kx_launch_fill(h->d, s));
+        h->nnz_stale = true; h->chunk_for_B = 0; h->tiled_ok = false;
+        return ensure_tasks(h, B, s);
+    };
+    auto finish = [&](kx_status_t code) -> kx_status_t {      // leave the handle with a host-side mass again
+        if (mass_var) {
+            h->d.m_dev = nullptr;
+            KxAdapt st2 = {};
+            if (cudaMemcpyAsync(&st2, h->adapt, sizeof st2, cudaMemcpyDeviceToHost, s) == cudaSuccess &&
+                cudaStreamSynchronize(s) == cudaSuccess) {
+                const kx_status_t r2 = rebuild(h, mass0 * exp(ctl->mass_slope * (st2.u - ctl->u0)), s);
+                if (code == KX_OK && r2 != KX_OK) code = r2;
+            }
+        }
+        return code;
+    };
+
     KxAdapt state = init;
+    // ---- regime 1: sources only on fixed intervals, Gamma_2->2/H monitored at every interval boundary
+    while (regime1 && !state.switched && !state.done) {
+        for (int a = 0; a < 8; ++a) {
+            if (mass_var && (rc = rebuild_at(0)) != KX_OK) return finish(rc);
+            KxStage st = {};
+            st.loss = h->k3; st.diag_stride = 4; st.evolve = 0;
+            if ((rc = launch_step(h, f, B, false, use_tiled, &st, s)) != KX_OK) return finish(rc);
+            KX_CUDA(kx_launch_regime1_step(h->d, f, h->k3, B, kappa_d, nsrc, nsrc ? src->G : nullptr, amp_dev, h->adapt,
+                                           ctl->u0, ctl->u1, ctl->du_fixed, ctl->eps_switch, ctl->rate0, ctl->rate_slope, s));
+        }
+        KX_CUDA(cudaMemcpyAsync(&state, h->adapt, sizeof state, cudaMemcpyDeviceToHost, s));
+        KX_CUDA(cudaStreamSynchronize(s));
+    }
+    // ---- regime 2: adaptive Heun from the switch point
+    if (regime1 && state.switched && !state.done) {
+        state.du = ctl->du0 < ctl->u1 - state.u ? ctl->du0 : ctl->u1 - state.u;
+        state.errkey = 0;
+        KX_CUDA(cudaMemcpyAsync(h->adapt, &state, sizeof state, cudaMemcpyHostToDevice, s));
+    }
     int attempts = 0;
     while (attempts < ctl->max_steps && !state.done) {
         const int chunk = ctl->max_steps - attempts < 8 ? ctl->max_steps - attempts : 8;
         for (int a = 0; a < chunk; ++a) {
             for (int stg = 0; stg < 2; ++stg) {
+                if (mass_var && (rc = rebuild_at(stg)) != KX_OK) return finish(rc);
                 const double* fin = stg == 0 ? f : h->fstage;
                 KxStage st = {};
                 st.flags = ctl->flags & KX_PROJECT;
@@ -676,7 +735,7 @@ kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_sou
                 st.flag = h->flag;
                 st.ad = h->adapt; st.ad_u0 = ctl->u0; st.ad_rate0 = ctl->rate0; st.ad_slope = ctl->rate_slope;
                 st.ad_rtol = ctl->rtol; st.ad_atol = ctl->atol;
-                if ((rc = launch_step(h, fin, B, /*have_yd=*/stg == 1 && !use_tiled, use_tiled, &st, s)) != KX_OK) return rc;
+                if ((rc = launch_step(h, fin, B, /*have_yd=*/stg == 1 && !use_tiled, use_tiled, &st, s)) != KX_OK) return finish(rc);
             }
             KX_CUDA(kx_launch_adapt_step(h->d, f, h->k2, B, h->adapt, ctl->u1, ctl->safety, h->flag, s));
         }
@@ -690,7 +749,11 @@ kx_status_t kx_evolve_adaptive(kx_handle_t h, double* f, int32_t B, const kx_sou
     if (result) {
         result->u = state.u; result->du = state.du;
         result->accepted = state.accepted; result->rejected = state.rejected; result->done = state.done;
+        result->switched = state.switched; result->u_switch = state.u_switch; result->fixed_steps = state.fixed_steps;
+        result->ratio = state.ratio;
     }
+    rc = finish(KX_OK);
+    if (rc != KX_OK) return rc;
     if (flag) { h->err = "kx_evolve_adaptive: f became non-finite"; return KX_ERR_NONFINITE; }
     return KX_OK;
 }

@@ -25,6 +25,7 @@ __global__ void k_kinematics(KxDev d, double m)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.N) return;
+    if (d.m_dev) m = __ldg(d.m_dev);
     double p = d.p[i], dp = d.dp[i], E, K;
     kin_point(p, m, E, K);
     d.E[i] = E;

@@ -85,6 +85,70 @@ __global__ void k_adapt_ctrl(KxAdapt* ad, double u1, double safety)
     ad->errkey = kx_dkey(0.0);
 }
 
+// ---------------------------------------------------------------- m(u) of the adaptive integrator, on the device
+// comoving momenta q = a p: the kinematics of a stage at u see the mass m a, m(u) = mass0 e^{slope (u - u0)}
+__global__ void k_adapt_mass(const KxAdapt* ad, int stage, double u0, double mass0, double slope, double* m_dev)
+{
+    const double us = stage ? ad->u + ad->du : ad->u;
+    *m_dev = mass0 * exp(slope * (us - u0));
+}
+
+// ---------------------------------------------------------------- regime 1 of Sec. 4.2
+// k_regime1_monitor (one CTA): Gamma_2->2 / H = kappa_b R(u) sum_i h_i loss_i / sum_i h_i f_i per member (reading D16; `loss`
+// is the loss term of the operator evaluated on f with the kinematics of m(u)), the largest member decides: above eps_switch
+// the batch switches to regime 2 at this u; else, at u1, the run is done; else the step that follows is taken.
+__global__ void __launch_bounds__(KX_CTA)
+k_regime1_monitor(KxDev d, const double* __restrict__ f, const double* __restrict__ loss, int B, const double* __restrict__ kappa,
+                  KxAdapt* ad, double u0, double u1, double eps_switch, double rate0, double rate_slope)
+{
+    __shared__ double s_red[8 * 8];
+    if (ad->switched || ad->done) return;
+    const int N = d.N;
+    const double u = ad->u;
+    const double R = rate0 * exp(rate_slope * (u - u0));
+    double ratio = 0.0;
+    for (int b = 0; b < B; ++b) {
+        double v[2] = {0.0, 0.0};
+        for (int i = threadIdx.x; i < N; i += KX_CTA) {
+            v[0] += d.h[i] * loss[(size_t)b * N + i];
+            v[1] += d.h[i] * f[(size_t)b * N + i];
+        }
+        block_sum<2>(v, s_red);
+        const double r = v[1] > 0.0 ? (kappa ? kappa[b] : 1.0) * R * (v[0] / v[1]) : 0.0;
+        if (r > ratio) ratio = r;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        ad->ratio = ratio;
+        if (!(eps_switch > 0.0) || ratio > eps_switch) { ad->switched = 1; ad->u_switch = u; }
+        else if (u1 - u <= 1e-14 * fmax(fabs(u1), 1.0)) { ad->done = 1; ad->u = u1; }
+    }
+}
+
+// k_regime1_step (one CTA per member): "we set the self-collisions to zero ... and evolve the distribution with a fourth-order
+// Runge-Kutta method on fixed intervals in u": the source rates are constant in u, so the four slopes are the same vector
+// k = sum_s amp_s G_s and the RK4 update is f + du k, du = min(du_fixed, u1 - u).  k_regime1_advance then moves u.
+__global__ void __launch_bounds__(KX_CTA)
+k_regime1_step(int N, double* __restrict__ f, int nsrc, const double* __restrict__ G, const double* __restrict__ amp,
+               const KxAdapt* __restrict__ ad, double u1, double du_fixed)
+{
+    if (ad->switched || ad->done) return;
+    const double rem = u1 - ad->u, du = du_fixed < rem ? du_fixed : rem;
+    for (int i = threadIdx.x; i < N; i += KX_CTA) {
+        double k = 0.0;
+        for (int q = 0; q < nsrc; ++q) k += amp[q] * G[(size_t)q * N + i];
+        f[(size_t)blockIdx.x * N + i] += du * k;
+    }
+}
+
+__global__ void k_regime1_advance(KxAdapt* ad, double u1, double du_fixed)
+{
+    if (ad->switched || ad->done) return;
+    const double rem = u1 - ad->u, du = du_fixed < rem ? du_fixed : rem;
+    ad->u += du;
+    ad->fixed_steps += 1;
+}
+
 // ---------------------------------------------------------------- monoenergetic source deposition
 __global__ void __launch_bounds__(KX_CTA) k_delta_source(KxDev d, double p0, double* __restrict__ G)
 {
@@ -226,6 +290,22 @@ cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, 
 {
     k_adapt_accept<<<B, KX_CTA, 0, s>>>(d.N, f, fnew, ad, flag);
     k_adapt_ctrl<<<1, 1, 0, s>>>(ad, u1, safety);
+    return cudaGetLastError();
+}
+
+cudaError_t kx_launch_adapt_mass(KxAdapt* ad, int stage, double u0, double mass0, double slope, double* m_dev, cudaStream_t s)
+{
+    k_adapt_mass<<<1, 1, 0, s>>>(ad, stage, u0, mass0, slope, m_dev);
+    return cudaGetLastError();
+}
+
+cudaError_t kx_launch_regime1_step(const KxDev& d, double* f, const double* loss, int B, const double* kappa, int nsrc,
+                                   const double* G, const double* amp_dev, KxAdapt* ad, double u0, double u1, double du_fixed,
+                                   double eps_switch, double rate0, double rate_slope, cudaStream_t s)
+{
+    k_regime1_monitor<<<1, KX_CTA, 0, s>>>(d, f, loss, B, kappa, ad, u0, u1, eps_switch, rate0, rate_slope);
+    k_regime1_step<<<B, KX_CTA, 0, s>>>(d.N, f, nsrc, G, amp_dev, ad, u1, du_fixed);
+    k_regime1_advance<<<1, 1, 0, s>>>(ad, u1, du_fixed);
     return cudaGetLastError();
 }
 

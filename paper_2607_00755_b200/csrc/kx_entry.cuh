@@ -9,6 +9,9 @@ namespace kxe {
 
 constexpr double kPi = 3.14159265358979323846;
 
+// kinematic mass of this build: a host value, or read from the device (adaptive integration with m(u))
+__device__ __forceinline__ double kx_mass(const KxDev& d) { return d.m_dev ? __ldg(d.m_dev) : d.m; }
+
 // ---------------------------------------------------------------- a1
 __device__ __forceinline__ void kin_point(double p, double m, double& E, double& K)
 {
@@ -72,7 +75,7 @@ static __device__ double kx_J(double a, double b, double dK, double M2_0, double
 // clipped to [-1,1]; |M|^2 is evaluated at t(mu) = 2 m^2 - 2 E_i E_n + 2 p_i p_n mu (reading D5).
 static __device__ double kx_F_quad(const KxDev& d, double pi_, double pn, double pm)
 {
-    const double m = d.m;
+    const double m = kx_mass(d);
     const double Ei = sqrt(pi_ * pi_ + m * m), En = sqrt(pn * pn + m * m), Em = sqrt(pm * pm + m * m);
     double acc = 0.0;
     for (int q = 0; q < d.n_mu; ++q) {
@@ -118,12 +121,13 @@ __device__ __forceinline__ double kx_Wsym(const KxDev& d, const double* __restri
 {
     const double pm = P[m];
     if (d.n_mu > 0) {      // numerical angular kernel: W = dp_n dp_m F_inm / (2 E_i g_chi), both orderings       eq. 4.7
-        const double Ei = sqrt(pi_ * pi_ + d.m * d.m);
+        const double mq = kx_mass(d);
+        const double Ei = sqrt(pi_ * pi_ + mq * mq);
         double F = kx_F_quad(d, pi_, pn, pm);
         if (m != n) F += kx_F_quad(d, pi_, pm, pn);
         return d.dp[n] * d.dp[m] / (2.0 * Ei * d.g_chi) * F;
     }
-    const double pj = sqrt(Kt * (Kt + 2.0 * d.m));   // eq. 4.4
+    const double pj = sqrt(Kt * (Kt + 2.0 * kx_mass(d)));   // eq. 4.4
     // eq. B.15-B.16
     double J = kx_J(fmax(fabs(pi_ - pn), fabs(pm - pj)), fmin(pi_ + pn, pm + pj), Ki - Kn, d.M2_0, d.m_med);
     if (m != n)   // the (i,m,n) ordering: second half of the symmetrised entry

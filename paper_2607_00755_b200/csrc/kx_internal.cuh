@@ -33,6 +33,7 @@ struct KxDev {
     const double *gl_mu, *gl_w;
     int chunk;           // entries per contraction task
     double m, g_chi, M2_0, m_med, f_floor, eps_supp;
+    const double* m_dev;      // not null: the kinematic mass is read from the device (kx_evolve_adaptive with m(u)); else `m`
     // grid and kinematics [N]
     const double *p, *dp;
     double *E, *K, *h;        // eq. B.1; K_i = E_i - m evaluated as p^2/(E+m)
@@ -226,6 +227,10 @@ struct KxAdapt {
     long long errkey;        // ordered key (kx_dkey) of the largest scaled error of the attempt, atomicMax over the CTAs
     long long accepted, rejected;
     int done;
+    // regime 1 of Sec. 4.2 (sources only on fixed intervals, Gamma_2->2/H monitored)
+    int switched;            // the largest member ratio exceeded eps_switch at u_switch
+    long long fixed_steps;
+    double u_switch, ratio;  // ratio: Gamma_2->2/H of the last monitor point (largest member)
 };
 
 struct KxStage {             // what the finishing kernel does after the reduction
@@ -271,6 +276,12 @@ cudaError_t kx_launch_stream(const KxDev& d, int sm_count, const double* f, cons
 cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, int B, KxAdapt* ad, double u1, double safety,
                                  int* flag, cudaStream_t s);      // accept/reject + controller update
 cudaError_t kx_launch_delta_source(const KxDev& d, double p0, double* G, cudaStream_t s);
+// m(u) of the adaptive integrator on the device: *m_dev = mass0 exp(slope (u_stage - u0)), u_stage = ad->u (+ ad->du)
+cudaError_t kx_launch_adapt_mass(KxAdapt* ad, int stage, double u0, double mass0, double slope, double* m_dev, cudaStream_t s);
+// regime 1: monitor Gamma_2->2/H at ad->u (switch / stop), then one sources-only step of at most du_fixed
+cudaError_t kx_launch_regime1_step(const KxDev& d, double* f, const double* loss, int B, const double* kappa, int nsrc,
+                                   const double* G, const double* amp_dev, KxAdapt* ad, double u0, double u1, double du_fixed,
+                                   double eps_switch, double rate0, double rate_slope, cudaStream_t s);
 cudaError_t kx_launch_moments(const KxDev& d, const double* f, int B, double* n, double* rho,
                               double* p1, double* p2, int stride, cudaStream_t s);
 // ---- tiled path (kx_tiled_build.cu, kx_tiled.cu)

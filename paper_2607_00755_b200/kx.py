@@ -64,12 +64,14 @@ class _Evolve(C.Structure):
 class _Adaptive(C.Structure):
     _fields_ = [("u0", C.c_double), ("u1", C.c_double), ("du0", C.c_double), ("rtol", C.c_double), ("atol", C.c_double),
                 ("safety", C.c_double), ("rate0", C.c_double), ("rate_slope", C.c_double), ("kappa", _dp), ("amp", _dp),
-                ("max_steps", C.c_int32), ("flags", C.c_uint32)]
+                ("max_steps", C.c_int32), ("flags", C.c_uint32), ("mass_slope", C.c_double), ("du_fixed", C.c_double),
+                ("eps_switch", C.c_double)]
 
 
 class _AdaptiveResult(C.Structure):
     _fields_ = [("u", C.c_double), ("du", C.c_double), ("accepted", C.c_int64), ("rejected", C.c_int64),
-                ("done", C.c_int32)]
+                ("done", C.c_int32), ("switched", C.c_int32), ("u_switch", C.c_double), ("fixed_steps", C.c_int64),
+                ("ratio", C.c_double)]
 
 
 # every symbol include/kx.h declares
@@ -297,9 +299,11 @@ class Handle:
         return diag
 
     def evolve_adaptive(self, f, u0, u1, *, du0=1e-4, rtol=1e-2, atol=2e-8, safety=0.9, rate0=1.0, rate_slope=0.0,
-                        kappa=None, project=True, G=None, amp=None, max_steps=100000, stream=None):
-        """kx_evolve_adaptive: adaptive Heun in u (Sec. 4.2); f [B,N] in place; returns dict(u, du, accepted,
-        rejected, done)."""
+                        mass_slope=0.0, du_fixed=0.0, eps_switch=0.0, kappa=None, project=True, G=None, amp=None,
+                        max_steps=100000, stream=None):
+        """kx_evolve_adaptive: the time integration of Sec. 4.2 in u (sources only on fixed intervals until
+        Gamma_2->2/H > eps_switch when eps_switch > 0, then adaptive Heun; kinematic mass m exp(mass_slope (u - u0)));
+        f [B,N] in place; returns dict(u, du, accepted, rejected, done, switched, u_switch, fixed_steps, ratio)."""
         B = self._batch(f)
         kappa = None if kappa is None else _f64(kappa)
         if kappa is not None and kappa.size != B:
@@ -315,11 +319,13 @@ class Handle:
         else:
             amp = None
         ctl = _Adaptive(float(u0), float(u1), float(du0), float(rtol), float(atol), float(safety), float(rate0),
-                        float(rate_slope), _ptr(kappa), _ptr(amp), int(max_steps), PROJECT if project else 0)
+                        float(rate_slope), _ptr(kappa), _ptr(amp), int(max_steps), PROJECT if project else 0,
+                        float(mass_slope), float(du_fixed), float(eps_switch))
         res = _AdaptiveResult()
         self._check(self._lib.kx_evolve_adaptive(self._h, _dev(f), B, C.byref(src) if src is not None else None,
                                                  C.byref(ctl), C.byref(res), _stream(stream)))
-        return dict(u=res.u, du=res.du, accepted=int(res.accepted), rejected=int(res.rejected), done=bool(res.done))
+        return dict(u=res.u, du=res.du, accepted=int(res.accepted), rejected=int(res.rejected), done=bool(res.done),
+                    switched=bool(res.switched), u_switch=res.u_switch, fixed_steps=int(res.fixed_steps), ratio=res.ratio)
 
     def delta_source(self, p0, stream=None):
         """kx_delta_source: shape [N] of a monoenergetic source at p0 for the current mass."""
