@@ -270,6 +270,7 @@ void kx_destroy(kx_handle_t h)
         cudaFree(h->bar);
         cudaFree(h->trace);
         cudaFree(h->gl);
+        cudaFree(h->runbuf);
         for (auto& ev : h->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     }
     delete h;
@@ -563,6 +564,42 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
     // kinematics, and re-deriving the Chebyshev moments per stage costs more than the exact streaming path
     const bool use_tiled = h->storage == KX_STORE_TILED && !ctl->mass && nnz_estimate(h) * B > kSmallProblem;
     if (use_tiled && (rc = ensure_tiled(h, s)) != KX_OK) return rc;
+
+    // Small static-mass problems without per-step diagnostics: the whole integration is ONE cooperative launch
+    // (k_stream_run: two grid barriers per stage instead of a launch per stage)
+    if (!use_tiled && !ctl->mass && !diag && S > 0) {
+        const size_t need = (size_t)(S + 1) + (ctl->rate ? (size_t)(2 * S + 1) : 0) + (size_t)nsrc * S;
+        if (h->runbuf_cap < need) {
+            KX_CUDA(cudaStreamSynchronize(s));
+            cudaFree(h->runbuf); h->runbuf = nullptr; h->runbuf_cap = 0;
+            KX_CUDA(dalloc(&h->runbuf, need + 1024));
+            h->runbuf_cap = need + 1024;
+        }
+        double* tau_d = h->runbuf;
+        double* rate_d = ctl->rate ? tau_d + (S + 1) : nullptr;
+        double* amp_d = nsrc ? tau_d + (S + 1) + (ctl->rate ? (2 * S + 1) : 0) : nullptr;
+        KX_CUDA(cudaMemcpyAsync(tau_d, ctl->tau, (size_t)(S + 1) * 8, cudaMemcpyHostToDevice, s));
+        if (rate_d) KX_CUDA(cudaMemcpyAsync(rate_d, ctl->rate, (size_t)(2 * S + 1) * 8, cudaMemcpyHostToDevice, s));
+        if (amp_d) KX_CUDA(cudaMemcpyAsync(amp_d, src->amp, (size_t)nsrc * S * 8, cudaMemcpyHostToDevice, s));
+        if ((rc = ensure_tasks(h, B, s)) != KX_OK) return rc;
+        KxStage st = {};
+        st.flags = ctl->flags & KX_PROJECT;
+        st.diag_stride = 6;
+        st.evolve = 1; st.rk_method = ctl->method;
+        st.kappa = kappa_d;
+        st.nsrc = nsrc; st.G = nsrc ? src->G : nullptr;
+        st.f = f; st.fstage = h->fstage; st.k1 = h->k1; st.k2 = h->k2; st.k3 = h->k3;
+        st.ydnext = h->yd; st.flag = h->flag;
+        st.part = h->part; st.bar = h->bar; st.fb_count = h->bar + 2;
+        h->epoch += 2; st.epoch = h->epoch;
+        st.trace = nullptr;
+        KX_CUDA(kx_launch_stream_run(h->d, h->sm_count, f, B, st, ctl->method, S, tau_d, rate_d, amp_d, &h->bar_total, s));
+        int flag1 = 0;
+        KX_CUDA(cudaMemcpyAsync(&flag1, h->flag, 4, cudaMemcpyDeviceToHost, s));
+        KX_CUDA(cudaStreamSynchronize(s));
+        if (flag1) { h->err = "kx_evolve: f became non-finite"; return KX_ERR_NONFINITE; }
+        return KX_OK;
+    }
 
     for (int k = 0; k < S; ++k) {
         const double dt = ctl->tau[k + 1] - ctl->tau[k];

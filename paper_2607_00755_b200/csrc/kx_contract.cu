@@ -10,6 +10,7 @@
 //
 // Compiled with --fmad=false; every fused multiply-add is an explicit fma().
 #include "kx_device.cuh"
+#include <stdlib.h>
 
 namespace {
 
@@ -46,6 +47,68 @@ k_stream(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd, 
     else if (d.N <= 2 * KX_CTA) stream_tail<2>(d, f, B, st, smem_raw, s_red);
     else stream_tail<4>(d, f, B, st, smem_raw, s_red);
     if (threadIdx.x == 0) stamp(st.trace, 3);
+}
+
+// ---------------------------------------------------------------- a whole fixed-step integration in ONE launch
+// Small problems (configs 1 and 2: a stage is a few microseconds of work) are bound by the kernel launch and its grid
+// barrier when every Runge-Kutta stage is its own launch.  k_stream_run keeps the grid resident for all S steps of
+// kx_evolve (static mass, no per-step diagnostics): per stage, contraction -> grid barrier -> finishing phase (which writes
+// the next stage input and its y) -> grid barrier.  The step data (tau, rate, source amplitudes) is read from device
+// arrays; the barriers use the growing counter, one target per barrier.
+struct KxRun {
+    int method, S;            // KX_EULER | KX_HEUN | KX_RK4, number of steps
+    const double* tau;        // device [S+1]
+    const double* rate;       // device [2S+1] or null
+    const double* amp;        // device [nsrc, S] or null
+};
+
+template <int BT, int MODE, int QS, int NQ>
+__device__ __forceinline__ void stream_run(const KxDev& d, double* __restrict__ f, int B, const KxStage& st0, const KxRun& run,
+                                           unsigned char* smem_raw, double* s_red)
+{
+    const unsigned cta = blockIdx.y * gridDim.x + blockIdx.x, nctas = gridDim.x * gridDim.y;
+    const int groups = (B + BT - 1) / BT;
+    const int nstage = run.method == KX_EULER ? 1 : (run.method == KX_HEUN ? 2 : 4);
+    KxStage st = st0;
+    unsigned target = st0.bar_target;                 // value of the counter after the first barrier of this launch
+    bool have_yd = false;
+    for (int k = 0; k < run.S; ++k) {
+        const double t0 = run.tau[k], t1 = run.tau[k + 1];
+        st.dt = t1 - t0;
+        for (int q = 0; q < st.nsrc; ++q) st.amp[q] = run.amp[(size_t)q * run.S + k];
+        for (int stg = 0; stg < nstage; ++stg) {
+            int pos;                                  // node (0), midpoint (1) or end (2) of the step for this stage
+            if (run.method == KX_EULER) pos = 0;
+            else if (run.method == KX_HEUN) pos = stg == 0 ? 0 : 2;
+            else pos = stg == 0 ? 0 : (stg == 3 ? 2 : 1);
+            st.rate = run.rate ? run.rate[2 * k + pos] : 1.0;
+            st.rk_stage = stg;
+            const double* fin = stg == 0 ? f : st.fstage;
+            const double2* yd = have_yd ? reinterpret_cast<const double2*>(st.ydnext) : nullptr;
+            for (int g = blockIdx.y; g < groups; g += gridDim.y)
+                contract_group<BT, MODE, QS>(d, fin, yd, st.part, B, g * BT, blockIdx.x, gridDim.x, smem_raw, !have_yd);
+            grid_barrier_count(st.bar + 3, target);
+            target += nctas;
+            // (the finishing phase's scratch, N doubles at the head of the shared memory, lies inside the per-stage y rows: the
+            // tables behind them survive)
+            for (int b = (int)cta; b < B; b += (int)nctas)
+                finish_member<NQ>(d, fin, B, st, nullptr, false, b, reinterpret_cast<double*>(smem_raw), s_red, nullptr);
+            grid_barrier_count(st.bar + 3, target);
+            target += nctas;
+            have_yd = true;
+        }
+    }
+}
+
+template <int BT, int MODE, int QS>
+__global__ void __launch_bounds__(KX_CTA, 2)
+k_stream_run(KxDev d, double* __restrict__ f, int B, KxStage st, KxRun run)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double s_red[8 * 8];
+    if (d.N <= KX_CTA) stream_run<BT, MODE, QS, 1>(d, f, B, st, run, smem_raw, s_red);
+    else if (d.N <= 2 * KX_CTA) stream_run<BT, MODE, QS, 2>(d, f, B, st, run, smem_raw, s_red);
+    else stream_run<BT, MODE, QS, 4>(d, f, B, st, run, smem_raw, s_red);
 }
 
 // ---------------------------------------------------------------- adaptive Heun: accept / reject, controller update
@@ -205,7 +268,7 @@ StreamCfg& stream_cfg() { static StreamCfg c = {false, 0, 0}; return c; }
 
 template <int BT, int MODE, int QS>
 cudaError_t launch_stream_t(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st,
-                            unsigned* bar_total, cudaStream_t s)
+                            unsigned* bar_total, cudaStream_t s, const KxRun* run = nullptr)
 {
     const int N = d.N;
     size_t smem = contract_smem<BT, MODE, QS>(N);
@@ -215,6 +278,8 @@ cudaError_t launch_stream_t(const KxDev& d, int sm_count, const double* f, const
     cudaError_t e;
     if (!c.ready) {
         e = cudaFuncSetAttribute(k_stream<BT, MODE, QS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_stream_run<BT, MODE, QS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
         if (e != cudaSuccess) return e;
         c.ready = true;
     }
@@ -234,6 +299,13 @@ cudaError_t launch_stream_t(const KxDev& d, int sm_count, const double* f, const
     if ((long long)gx > tasks_bound) gx = (int)tasks_bound;
     if (gx < 1) gx = 1;
     st.bar_target = *bar_total + (unsigned)(gx * gy);
+    if (run) {          // the whole integration in one launch: two barriers per stage
+        const unsigned nstage = run->method == KX_EULER ? 1u : (run->method == KX_HEUN ? 2u : 4u);
+        const unsigned nbar = 2u * nstage * (unsigned)run->S;
+        e = kx_launch_coop(k_stream_run<BT, MODE, QS>, dim3(gx, gy), dim3(KX_CTA), smem, s, d, const_cast<double*>(f), B, st, *run);
+        if (e == cudaSuccess) *bar_total += nbar * (unsigned)(gx * gy);
+        return e;
+    }
     e = kx_launch_coop(k_stream<BT, MODE, QS>, dim3(gx, gy), dim3(KX_CTA), smem, s, d, f,
                        reinterpret_cast<const double2*>(yd), B, st);
     if (e == cudaSuccess) *bar_total = st.bar_target;
@@ -242,15 +314,15 @@ cudaError_t launch_stream_t(const KxDev& d, int sm_count, const double* f, const
 
 template <int BT>
 cudaError_t launch_stream_m(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st,
-                            unsigned* bar_total, cudaStream_t s)
+                            unsigned* bar_total, cudaStream_t s, const KxRun* run)
 {
     if (d.eta) {         // quantum statistics: LOG interpolation only (checked in kx_build)
-        if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 1>(d, sm_count, f, yd, B, st, bar_total, s);
-        return launch_stream_t<BT, MODE_LOG_TAB, 1>(d, sm_count, f, yd, B, st, bar_total, s);
+        if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 1>(d, sm_count, f, yd, B, st, bar_total, s, run);
+        return launch_stream_t<BT, MODE_LOG_TAB, 1>(d, sm_count, f, yd, B, st, bar_total, s, run);
     }
-    if (d.interp == KX_INTERP_LINEAR) return launch_stream_t<BT, MODE_LINEAR, 0>(d, sm_count, f, yd, B, st, bar_total, s);
-    if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 0>(d, sm_count, f, yd, B, st, bar_total, s);
-    return launch_stream_t<BT, MODE_LOG_TAB, 0>(d, sm_count, f, yd, B, st, bar_total, s);
+    if (d.interp == KX_INTERP_LINEAR) return launch_stream_t<BT, MODE_LINEAR, 0>(d, sm_count, f, yd, B, st, bar_total, s, run);
+    if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 0>(d, sm_count, f, yd, B, st, bar_total, s, run);
+    return launch_stream_t<BT, MODE_LOG_TAB, 0>(d, sm_count, f, yd, B, st, bar_total, s, run);
 }
 
 }  // namespace
@@ -278,10 +350,23 @@ cudaError_t kx_launch_stream(const KxDev& d, int sm_count, const double* f, cons
                              KxStage st, unsigned* bar_total, cudaStream_t s)
 {
     switch (kx_pick_bt(d.N, B)) {
-        case 1: return launch_stream_m<1>(d, sm_count, f, yd, B, st, bar_total, s);
-        case 2: return launch_stream_m<2>(d, sm_count, f, yd, B, st, bar_total, s);
-        case 4: return launch_stream_m<4>(d, sm_count, f, yd, B, st, bar_total, s);
-        default: return launch_stream_m<8>(d, sm_count, f, yd, B, st, bar_total, s);
+        case 1: return launch_stream_m<1>(d, sm_count, f, yd, B, st, bar_total, s, nullptr);
+        case 2: return launch_stream_m<2>(d, sm_count, f, yd, B, st, bar_total, s, nullptr);
+        case 4: return launch_stream_m<4>(d, sm_count, f, yd, B, st, bar_total, s, nullptr);
+        default: return launch_stream_m<8>(d, sm_count, f, yd, B, st, bar_total, s, nullptr);
+    }
+}
+
+cudaError_t kx_launch_stream_run(const KxDev& d, int sm_count, double* f, int B, KxStage st, int method, int S,
+                                 const double* tau_dev, const double* rate_dev, const double* amp_dev,
+                                 unsigned* bar_total, cudaStream_t s)
+{
+    KxRun run = {method, S, tau_dev, rate_dev, amp_dev};
+    switch (kx_pick_bt(d.N, B)) {
+        case 1: return launch_stream_m<1>(d, sm_count, f, nullptr, B, st, bar_total, s, &run);
+        case 2: return launch_stream_m<2>(d, sm_count, f, nullptr, B, st, bar_total, s, &run);
+        case 4: return launch_stream_m<4>(d, sm_count, f, nullptr, B, st, bar_total, s, &run);
+        default: return launch_stream_m<8>(d, sm_count, f, nullptr, B, st, bar_total, s, &run);
     }
 }
 

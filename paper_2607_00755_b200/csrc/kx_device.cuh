@@ -126,7 +126,7 @@ __host__ __device__ constexpr size_t contract_smem(int N)
 template <int BT, int MODE, int QS>
 __device__ __forceinline__ void contract_group(const KxDev& d, const double* __restrict__ f, const double2* __restrict__ yd,
                                                double* __restrict__ part, int B, int b0, unsigned task0, unsigned tstride,
-                                               unsigned char* smem_raw)
+                                               unsigned char* smem_raw, bool load_static = true)
 {
     const int N = d.N;
     double2* s_yd = reinterpret_cast<double2*>(smem_raw);                 // [BT][N]
@@ -141,11 +141,12 @@ __device__ __forceinline__ void contract_group(const KxDev& d, const double* __r
     for (int k = tid; k < BT * N; k += KX_CTA) {
         int b = k / N, j = k - b * N;
         if (b < nb) {
-            const double fv = f[(size_t)(b0 + b) * N + j];
-            if (yd) s_yd[k] = yd[(size_t)(b0 + b) * N + j];
+            // (read through L2: inside the one-launch integrator these were written by other CTAs a grid barrier ago)
+            const double fv = __ldcg(f + (size_t)(b0 + b) * N + j);
+            if (yd) s_yd[k] = __ldcg(yd + (size_t)(b0 + b) * N + j);
             else {        // no prepared y: computed here
                 const double y0 = yval(fv, d.interp, d.f_floor, d.eta);
-                const double y1 = j + 1 < N ? yval(f[(size_t)(b0 + b) * N + j + 1], d.interp, d.f_floor, d.eta) : y0;
+                const double y1 = j + 1 < N ? yval(__ldcg(f + (size_t)(b0 + b) * N + j + 1), d.interp, d.f_floor, d.eta) : y0;
                 s_yd[k] = make_double2(y0, y1 - y0);
             }
             s_f[k] = fv;
@@ -154,9 +155,11 @@ __device__ __forceinline__ void contract_group(const KxDev& d, const double* __r
             s_f[k] = 0.0;
         }
     }
-    if (MODE == MODE_LOG_TAB)
-        for (int k = tid; k < (KX_EXP_REP << KX_EXP_BITS); k += KX_CTA) s_tab[k] = d.exptab[k / KX_EXP_REP];
-    for (int k = tid; k <= N; k += KX_CTA) s_tp[k] = d.taskptr[k];
+    if (load_static) {        // the exp2 table and the task table do not change between the stages of a one-launch integration
+        if (MODE == MODE_LOG_TAB)
+            for (int k = tid; k < (KX_EXP_REP << KX_EXP_BITS); k += KX_CTA) s_tab[k] = d.exptab[k / KX_EXP_REP];
+        for (int k = tid; k <= N; k += KX_CTA) s_tp[k] = d.taskptr[k];
+    }
     __syncthreads();
 
     const unsigned ntasks = s_tp[N];

@@ -136,6 +136,8 @@ struct kx_handle_s {
     double *part;             // [ws_tasks, wsB, 2] per-task partial (gain, loss frequency)
     double *fstage, *k1, *k2, *k3, *Cbuf;   // [wsB, N] evolve buffers
     double *hostio;           // [wsB, N] x2 staging for kx_collide_host
+    double *runbuf;           // device copy of tau / rate / amp of a one-launch kx_evolve (grown on demand)
+    size_t runbuf_cap;        // in doubles
     int *flag;                // device non-finite flag
     KxAdapt *adapt;           // device controller state of kx_evolve_adaptive
     double p_lo, p_hi;        // host copies of p[0], p[N-1]
@@ -273,6 +275,10 @@ struct KxStage {             // what the finishing kernel does after the reducti
 // (bar_total: the handle's running count of barrier arrivals; the launcher adds its grid size and sets st.bar_target)
 cudaError_t kx_launch_stream(const KxDev& d, int sm_count, const double* f, const double* yd, int B,
                              KxStage st, unsigned* bar_total, cudaStream_t s);
+// a whole fixed-step integration (static mass, no diagnostics) on the exact streaming path in ONE cooperative launch
+cudaError_t kx_launch_stream_run(const KxDev& d, int sm_count, double* f, int B, KxStage st, int method, int S,
+                                 const double* tau_dev, const double* rate_dev, const double* amp_dev,
+                                 unsigned* bar_total, cudaStream_t s);
 cudaError_t kx_launch_adapt_step(const KxDev& d, double* f, const double* fnew, int B, KxAdapt* ad, double u1, double safety,
                                  int* flag, cudaStream_t s);      // accept/reject + controller update
 cudaError_t kx_launch_delta_source(const KxDev& d, double p0, double* G, cudaStream_t s);
