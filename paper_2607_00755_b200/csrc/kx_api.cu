@@ -205,6 +205,7 @@ kx_status_t launch_step(kx_handle_s* h, const double* f, int B, bool have_yd, bo
         }
         const int par = (int)((h->epoch >> 1) & 1u);
         st->gpart = h->gpart; st->lpart = h->lpart; st->xstride = h->ws_xstride;
+        st->gslots = h->sm_count + h->t.NT + 1; st->lslots = h->sm_count + h->t.RS + 1;
         st->mstat = nullptr; st->mstat_next = nullptr; st->mstat_cap = 0;
         if (h->d.interp == KX_INTERP_LOG) {      // LINEAR is exact: no statistics, no fallback
             st->mstat = h->mstat + (size_t)par * h->wsB * 2;

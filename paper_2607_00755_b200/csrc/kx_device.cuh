@@ -328,9 +328,10 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // gain: tile = i/16; the warps [wstart[tile], wstart[tile+1]) of the plan worked on it, i.e. the CTAs c0 = wstart[tile]/8
 // ... c1 = (wstart[tile+1]-1)/8, each of which wrote one partial into slot c + tile.  loss: supertile = i/256, chunk units
 // [sp LC, (sp+1) LC) of the RS LC units were taken by the loss CTAs ld0[sp]..ld1[sp], slot = c + sp.
-// The member's slice of every slot (128 bytes per gain slot, 2 KiB per loss slot) is fetched into shared memory by bulk
-// copies: about GG + NT + GL instructions for the whole CTA and every byte in flight at once; a thread then adds the
-// partials of its row in slot order: a fixed order, bit-reproducible.
+// The partials are stored member-major (gpart [member][slot][16], lpart [member][slot][256]), so the member's slice of all
+// gain slots is one contiguous piece and that of all loss slots another: two bulk copies (TMA) fetch them into shared
+// memory (164 small copies of 128 B / 2 KiB took 2 us: the copy engine handles them one after the other); a thread then
+// adds the partials of its row in slot order: a fixed order, bit-reproducible.
 //   scratch: s_y [Npad] | s_gp [GG + NT][16] | s_lp [sum_sp (ld1 - ld0 + 1)][256]
 __host__ __device__ inline size_t finish_scratch_bytes(int N, int GG, int GL, int NT, int RS)
 {
@@ -340,24 +341,18 @@ __host__ __device__ inline size_t finish_scratch_bytes(int N, int GG, int GL, in
 __device__ __forceinline__ void gather_partials(int N, const KxStage& st, const KxPlan& plan, int b, double* scratch,
                                                 unsigned long long* mbar)
 {
-    const int tid = threadIdx.x;
+    // member-major partials: all gain slots of member b are one contiguous piece, all loss slots another: two bulk copies
     const int Npad = (N + 3) & ~3;
     double* s_gp = scratch + Npad;
     const int ng = plan.GG + st.NT;
     double* s_lp = s_gp + (size_t)ng * 16;
-    int nl = 0;
-    for (int sp = 0; sp < st.RS; ++sp) nl += (int)(plan.ld1[sp] - plan.ld0[sp] + 1u);
+    const unsigned l0 = plan.ld0[0];
+    const unsigned nl = plan.ld1[st.RS - 1] + (unsigned)(st.RS - 1) - l0 + 1u;       // slots l0 .. ld1[RS-1] + RS - 1
     fence_proxy_async();
-    if (tid == 0) mbar_expect_tx(mbar, (unsigned)ng * 128u + (unsigned)nl * 2048u);
-    for (int k = tid; k < ng + nl; k += KX_CTA) {
-        if (k < ng) {
-            bulk_g2s(s_gp + (size_t)k * 16, st.gpart + ((size_t)k * st.xstride + b) * 16, 128u, mbar);
-        } else {
-            int kk = k - ng, sp = 0;
-            while (kk >= (int)(plan.ld1[sp] - plan.ld0[sp] + 1u)) { kk -= (int)(plan.ld1[sp] - plan.ld0[sp] + 1u); ++sp; }
-            const unsigned c = plan.ld0[sp] + (unsigned)kk;
-            bulk_g2s(s_lp + (size_t)(k - ng) * 256, st.lpart + ((size_t)(c + sp) * st.xstride + b) * 256, 2048u, mbar);
-        }
+    if (threadIdx.x == 0) {
+        mbar_expect_tx(mbar, (unsigned)ng * 128u + nl * 2048u);
+        bulk_g2s(s_gp, st.gpart + (size_t)b * st.gslots * 16, (unsigned)ng * 128u, mbar);
+        bulk_g2s(s_lp, st.lpart + ((size_t)b * st.lslots + l0) * 256, nl * 2048u, mbar);
     }
 }
 
@@ -404,8 +399,7 @@ __device__ __forceinline__ void sum_partials_row(int N, const KxStage& st, const
         }
         for (int k = 0; c < ng; ++c, ++k) a[k] += pg[(size_t)c * 16];
     }
-    unsigned lo = 0;
-    for (int s2 = 0; s2 < sp; ++s2) lo += plan.ld1[s2] - plan.ld0[s2] + 1u;
+    const unsigned lo = plan.ld0[sp] + (unsigned)sp - plan.ld0[0];     // the slots of supertile sp start at CTA ld0[sp] + sp
     const unsigned nls = plan.ld1[sp] - plan.ld0[sp] + 1u;
     const double* pl = s_lp + (size_t)lo * 256 + (i & 255);
     unsigned c = 0;

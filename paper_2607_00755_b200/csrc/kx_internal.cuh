@@ -116,8 +116,8 @@ struct kx_handle_s {
     int ws_xstride;           // members per partial slot (batch capacity padded)
     long long *mstat;         // [2][wsB][2] per member, double-buffered by launch parity: ordered key of the largest
                               // interpolation-error term over the brackets, bits of max_i |f_i| (see kx_member_flagged)
-    double *gpart;            // [sm_count + NT + 1, ws_xstride, 16]  gain partials of the DMMA kernel (one per CTA and tile)
-    double *lpart;            // [sm_count + RS + 1, ws_xstride, 256] loss partials (one per CTA and supertile)
+    double *gpart;            // [ws_xstride, sm_count + NT + 1, 16]  gain partials of the DMMA kernel (one per CTA and tile), member-major:
+    double *lpart;            // [ws_xstride, sm_count + RS + 1, 256] loss partials (one per CTA and supertile); a member's slots are contiguous
     std::vector<unsigned> vt_host;   // host copy of vtptr [NT + 1] (the plan of the DMMA kernel is made on the host)
     KxPlan plan;              // role split and warp -> tile map of the DMMA kernel for batch plan_B
     int plan_B;               // 0 = no plan
@@ -257,6 +257,7 @@ struct KxStage {             // what the finishing kernel does after the reducti
     long long *mstat_next;   // the other buffer: reset (all mstat_cap members) by the finishing phase for the next launch
     int mstat_cap;
     int NT, LC, RS, xstride;
+    int gslots, lslots;      // partial slots per member: gpart [member][gslots][16], lpart [member][lslots][256]
     int *flag;
     int evolve;
     double *part;            // [tasks, B, 2 or 4] partials of the exact streaming contraction

@@ -65,7 +65,7 @@ constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256
 // (CTA, tile), slot = CTA + tile.
 template <int NBT, int STAGES>
 __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, int N, int B, int bcol0,
-                                          const double* __restrict__ f, int xstride, double* __restrict__ gpart,
+                                          const double* __restrict__ f, int gslots, double* __restrict__ gpart,
                                           unsigned char* smem, int* s_wtile, unsigned long long* trace,
                                           unsigned long long* mbar, unsigned& mpar)
 {
@@ -248,11 +248,12 @@ __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, 
         int wb = wa + 1;
         while (wb < WARPS && s_wtile[wb] == tl) ++wb;
         if (tl >= 0) {
-            double* dst = gpart + ((size_t)(blockIdx.x + tl) * xstride + bcol0) * 16;
+            // member-major: member b's slots are contiguous, so the finishing phase fetches them with one bulk copy
+            double* dst = gpart + ((size_t)bcol0 * gslots + (blockIdx.x + tl)) * 16;
             for (int o = tid; o < NBT * 128; o += NTHR) {
                 double s = 0.0;
                 for (int w = wa; w < wb; ++w) s += reinterpret_cast<const double*>(ring0 + (size_t)w * STAGES * kStageBytes)[o];
-                dst[o] = s;
+                dst[(size_t)(o >> 4) * gslots * 16 + (o & 15)] = s;
             }
         }
         wa = wb;
@@ -268,7 +269,7 @@ __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, 
 // (256 rows) boundary produces one partial per piece, slot = loss CTA + supertile.
 template <int NBT>
 __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, const KxPlan& plan, int N, int B, int bcol0,
-                                          const double* __restrict__ f, long long* __restrict__ mstat, int xstride,
+                                          const double* __restrict__ f, long long* __restrict__ mstat, int lslots,
                                           double* __restrict__ lpart, unsigned char* smem, unsigned long long* trace)
 {
     constexpr int LD = NBT * 8 + 4;
@@ -464,13 +465,13 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
             __syncthreads();              // the rings are free again (next window's scratch, next piece)
         }
 
-        double* dst = lpart + ((size_t)(cl + sp) * xstride + bcol0) * 256 + 8 * R8 * warp + 2 * krow;
+        double* dst = lpart + ((size_t)bcol0 * lslots + (cl + sp)) * 256 + 8 * R8 * warp + 2 * krow;
 #pragma unroll
         for (int r = 0; r < R8; ++r)
             if (r < nbw)
 #pragma unroll
                 for (int bt = 0; bt < NBT; ++bt)
-                    *reinterpret_cast<double2*>(dst + (size_t)(8 * bt + lr) * 256 + 8 * r) = make_double2(acc[r][bt][0], acc[r][bt][1]);
+                    *reinterpret_cast<double2*>(dst + (size_t)(8 * bt + lr) * lslots * 256 + 8 * r) = make_double2(acc[r][bt][0], acc[r][bt][1]);
         u = ue;
     }
 }
@@ -581,8 +582,8 @@ k_dmma(const __grid_constant__ KxDev dk, const __grid_constant__ KxTiled t, cons
     __syncthreads();                                // the barrier is initialised
     for (int by = 0; by < ny; ++by) {          // member groups of 8 NBT: one pass each (more than one for B > 64 only)
         const int bcol0 = by * NBT * 8;
-        if ((int)blockIdx.x < plan.GG) gain_role<NBT, STAGES>(t, plan, N, B, bcol0, f, st.xstride, st.gpart, smem, s_wtile, st.trace, &s_mbar, mpar);
-        else loss_role<NBT>(dk, t, plan, N, B, bcol0, f, st.mstat, st.xstride, st.lpart, smem, st.trace);
+        if ((int)blockIdx.x < plan.GG) gain_role<NBT, STAGES>(t, plan, N, B, bcol0, f, st.gslots, st.gpart, smem, s_wtile, st.trace, &s_mbar, mpar);
+        else loss_role<NBT>(dk, t, plan, N, B, bcol0, f, st.mstat, st.lslots, st.lpart, smem, st.trace);
         __syncthreads();
     }
     if (tid == 0) stamp(st.trace, 2);
