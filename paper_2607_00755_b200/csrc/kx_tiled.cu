@@ -30,7 +30,7 @@ constexpr double kLossCost = 1.26;
 constexpr double kRunCost = 0.09;
 // loss role in the plan's time model (units of one gain group of a warp): DMMA cost of a chunk relative to the same DMMA count of
 // the gain stream, and what the loss prologue (operand X: log2, exp2 at the nodes) takes longer than staging f
-constexpr double kLossChunk = 1.05, kLossPrologue = 5.5;
+constexpr double kLossChunk = 1.05, kLossPrologue = 3.9;
 
 // D[8 members x 8 rows] += X[8 members x 4 k] * A[4 k x 8 rows]
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
@@ -286,6 +286,7 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
     double* sXw = reinterpret_cast<double*>(smem + (size_t)kLossStages * kLossABytes);          // [WC*16][LD]
     double* s_node = sXw + (size_t)WC * 16 * LD;                                                // [QMAX]
     double* s_tab = s_node + KX_QMAX;                                                           // [256]
+    long long* s_stat = reinterpret_cast<long long*>(s_tab + (1 << KX_EXP_BITS));               // [2][64] member statistics of this CTA
     double* s_y = reinterpret_cast<double*>(smem);                                              // [brackets + 1][MB] (aliases the stages)
     if (logm) {
         if (tid < Q) s_node[tid] = t.nodes[tid];
@@ -332,23 +333,28 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
             __syncthreads();
             return;
         }
-        // step 1: y_j = log2 max(f_j, f_floor) of the brackets' end points j = jlo .. jhi + 1, and max |f|
+        // step 1: y_j = log2 max(f_j, f_floor) of the brackets' end points j = jlo .. jhi + 1, and max |f|.  The member
+        // statistics are reduced inside the CTA first (shared-memory atomics) and sent with ONE global atomic per member:
+        // 39 CTAs x 600 same-address atomics each were queueing in L2 and throttling the loads behind them
         const int nj = jhi - jlo + 1;
+        if (tid < 2 * 64) s_stat[tid] = tid < 64 ? KX_MSTAT_NONE : 0;
+        __syncthreads();
         {
-            const int total = (nj + 1) * MB;
+            // consecutive threads read consecutive j of one member: nj + 1 doubles of a row are 2-3 sectors, not nj + 1
+            const int nj1 = nj + 1, total = nj1 * MB;
             for (int i0 = tid; i0 < total; i0 += 4 * NTHR) {
                 double v[4];
 #pragma unroll
                 for (int u2 = 0; u2 < 4; ++u2) {
-                    const int idx = i0 + u2 * NTHR, b = bcol0 + idx % MB;
-                    v[u2] = (idx < total && b < B) ? __ldcg(f + (size_t)b * N_ + jlo + idx / MB) : 0.0;
+                    const int idx = i0 + u2 * NTHR, b = bcol0 + idx / nj1;
+                    v[u2] = (idx < total && b < B) ? __ldcg(f + (size_t)b * N_ + jlo + idx % nj1) : 0.0;
                 }
 #pragma unroll
                 for (int u2 = 0; u2 < 4; ++u2) {
-                    const int idx = i0 + u2 * NTHR, b = bcol0 + idx % MB;
+                    const int idx = i0 + u2 * NTHR, bm = idx / nj1, b = bcol0 + bm;
                     if (idx < total) {
-                        if (b < B) atomicMax(mstat + 2 * b + 1, __double_as_longlong(fabs(v[u2])));
-                        s_y[idx] = log2(fmax(v[u2], dk.f_floor));
+                        if (b < B) atomicMax(s_stat + 64 + bm, __double_as_longlong(fabs(v[u2])));
+                        s_y[(idx % nj1) * MB + bm] = log2(fmax(v[u2], dk.f_floor));
                     }
                 }
             }
@@ -367,7 +373,7 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
                     // nothing, so nobody waits for them
                     const double cabs = 0.6931471805599453 * fabs(dy);
                     if (cabs > 0.0)
-                        atomicMax(mstat + 2 * b, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
+                        atomicMax(s_stat + bl, kx_dkey(fmax(y0, y1) + (double)Q * (log2(cabs) - 2.0) + t.flag_log2));
                 }
                 if (tid == 0 && npass_ == 0 && (jj == 1 || jj == 2 || jj == 5)) stamp(trace, jj == 1 ? 19 : (jj == 2 ? 20 : 21));
                 const unsigned kb = (unsigned)(jlo + jj) * (unsigned)Q;
@@ -392,6 +398,10 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
             }
         }
         __syncthreads();
+        if (tid < MB && bcol0 + tid < B) {
+            if (s_stat[tid] != KX_MSTAT_NONE) atomicMax(mstat + 2 * (bcol0 + tid), s_stat[tid]);
+            atomicMax(mstat + 2 * (bcol0 + tid) + 1, s_stat[64 + tid]);
+        }
         if (tid == 0 && npass_ < 2) stamp(trace, 18 + 2 * npass_);
         ++npass_;
     };
@@ -593,7 +603,7 @@ k_dmma(const __grid_constant__ KxDev dk, const __grid_constant__ KxTiled t, cons
     if (tid == 0) { stamp(st.trace, 5); if (st.trace && blockIdx.x < KX_TRACE_CTAS) st.trace[blockIdx.x * KX_TRACE_SLOTS + 23] = clock64(); }
 }
 
-constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + (KX_QMAX + (1 << KX_EXP_BITS)) * 8;
+constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + (KX_QMAX + (1 << KX_EXP_BITS) + 2 * 64) * 8;
 constexpr size_t kSmemMax = 226u * 1024u;       // dynamic shared memory: 227 KiB per CTA minus the kernel's static 544 bytes
 
 // chunks of 16 k whose Chebyshev coefficients a loss CTA keeps in shared memory at a time: its whole share if it fits
