@@ -219,6 +219,33 @@ def time_collide(torch, h, f, C, flags, K, Wm, flusher, barrier, reps=5, calls=2
                 kern_warm=kern_warm_ms * 1e-3 / max(kern_warm_n, 1), t_med=float(np.median(meds)), fallback=fb)
 
 
+def trace_phases(torch, h, f, C, flags, flusher, reps=5):
+    """Phases of the fused tensor-core kernel from its own clock stamps (kx_trace: %globaltimer per CTA), L2 flushed before
+    every traced launch; microseconds since the first CTA entered, median over `reps` launches."""
+    h.trace(True)
+    out = []
+    for _ in range(reps):
+        flusher()
+        h.collide(f, flags=flags, out=C)
+        torch.cuda.synchronize()
+        tr = h.trace_read().astype(np.int64).reshape(160, 32)
+        ent = tr[:, 0][tr[:, 0] > 0]
+        if ent.size == 0:
+            continue
+        t0 = ent.min()
+
+        def last(slot):
+            v = tr[:, slot][tr[:, slot] > 0]
+            return float(v.max() - t0) * 1e-3 if v.size else float("nan")
+        out.append((last(1), last(2), last(3), last(5)))
+    h.trace(False)
+    if not out:
+        return None
+    m = np.median(np.array(out), axis=0)
+    return {"prologue_done_us": m[0], "dmma_phase_done_us": m[1], "barrier_passed_us": m[2], "kernel_done_us": m[3],
+            "how": "last CTA to reach each point, microseconds since the first CTA entered (kx_trace), L2 flushed, median of %d" % len(out)}
+
+
 def roofline(info, B, mode, streaming, stat, kern_s, peaks, peak_src, probe):
     """Roofline of the fused kernel for this configuration."""
     sm_max_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
@@ -433,6 +460,7 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
     t = time_collide(torch, h, f, C, flags, K, Wm, flusher, barrier)
+    phases = trace_phases(torch, h, f, C, flags, flusher) if not streaming else None
 
     # ---- end to end through host buffers
     fh = torch.tensor(c["f"], dtype=torch.float64).pin_memory()
@@ -474,6 +502,10 @@ def main():
         "kernel_ms": t_kern * 1e3, "kernel_ms_l2_warm": t["kern_warm"] * 1e3,
         "step_frac": roof["work_per_launch"] / (t_cold / K) / (roof["peak"] * (1e9 if roof["unit"] == "GB/s" else 1e12)),
         "event_pair_around_empty_kernel_us": ev_over_us, "tensor_bytes_per_launch": info["tensor_bytes"]})
+    if phases is not None:
+        # the contraction alone (what round 1's k_dmma was): work over the time the last CTA needs to write its partials
+        phases["dmma_phase_frac"] = roof["work_per_launch"] / (phases["dmma_phase_done_us"] * 1e-6) / (roof["peak"] * (1e9 if roof["unit"] == "GB/s" else 1e12))
+        roof["phases"] = phases
     Ngrid = info["N"]
     line = {
         "metric": METRIC if args.config == 3 and B == 64 and stat == 0 else f"C[f] evals/s (fp64, N={Ngrid}, B={B})",
