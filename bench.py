@@ -281,23 +281,30 @@ def roofline(info, B, mode, streaming, stat, kern_s, peaks, peak_src, probe):
 
 
 def side_collide(torch, kx, dev, local, peaks, peak_src, flusher, barrier, *, cfg, B, mode="log", project=False,
-                 storage="tiled", statistics="classical", K=10):
+                 storage="tiled", statistics="classical", precision="fp64", K=10):
     """One short side measurement of the operator (same protocol as the headline, fewer steps)."""
     c = kin.config(cfg, B=B)
     stat = {"classical": kx.STAT_CLASSICAL, "bose": kx.STAT_BOSE, "fermi": kx.STAT_FERMI}[statistics]
-    streaming = storage == "rows" or stat != 0
+    fp32 = precision == "fp32"
+    streaming = storage == "rows" or stat != 0 or fp32
     if stat != 0:
         c["f"] = c["f"] / np.abs(c["f"]).max(axis=1, keepdims=True) * (0.8 if stat < 0 else 2.5)
     h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"], device=local,
                   interp=kx.INTERP_LOG if mode == "log" else kx.INTERP_LINEAR,
-                  storage=kx.STORE_SYM_ROWS if streaming else kx.STORE_TILED, statistics=stat)
+                  storage=kx.STORE_SYM_ROWS if streaming else kx.STORE_TILED, statistics=stat,
+                  precision=kx.FP32 if fp32 else kx.FP64)
     f = torch.tensor(c["f"], dtype=torch.float64, device=dev)
     C = torch.empty_like(f)
     t = time_collide(torch, h, f, C, kx.PROJECT if project else 0, K, 3, flusher, barrier, reps=3, calls=50)
     info = h.info()
     roof = roofline(info, B, mode, streaming, stat, t["kern_cold"], peaks, peak_src, None)
+    if fp32:    # fp32 contraction: 4 FP32-pipe FMA/MUL per (entry, member) + one MUFU.EX2; peak 148 SMs x 128 lanes x max clock
+        peak32 = SM_COUNT * 128 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+        ach32 = info["nnz"] * B * 4 / t["kern_cold"] / 1e12
+        roof.update({"bound": "alu", "achieved": ach32, "peak": peak32, "unit": "T FP32 inst/s", "frac": ach32 / peak32})
     h.close()
-    return {"N": info["N"], "B": B, "mode": mode, "projected": project, "storage": storage, "statistics": statistics,
+    return {"N": info["N"], "B": B, "mode": mode, "projected": project, "storage": "rows" if streaming else storage,
+            "statistics": statistics, "precision": precision,
             "evals_per_s": B * K / t["t_cold"], "ms_per_step": t["t_cold"] / K * 1e3,
             "ms_per_step_l2_warm": t["t_warm"] / K * 1e3, "ms_per_call_median": t["t_med"] * 1e3,
             "kernel_ms": t["kern_cold"] * 1e3, "bound": roof["bound"], "frac": roof["frac"], "achieved": roof["achieved"],
@@ -541,6 +548,7 @@ def main():
             extra["cfg3_projected"] = side_collide(**sc, cfg=3, B=64, project=True)
             extra["cfg3_rows"] = side_collide(**sc, cfg=3, B=64, storage="rows", K=5)
             extra["cfg3_bose"] = side_collide(**sc, cfg=3, B=64, statistics="bose", K=5)
+            extra["cfg3_fp32"] = side_collide(**sc, cfg=3, B=64, precision="fp32", K=5)
             extra["cfg4_b8"] = side_collide(**sc, cfg=4, B=8)
             extra["cfg4_b1"] = side_collide(**sc, cfg=4, B=1)
             for cfg in (1, 2, 5):

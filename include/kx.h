@@ -52,7 +52,8 @@ typedef enum {
     KX_ERR_INVALID_ARG = 1,   /* null pointer, N<4, non-monotone grid, dp<=0, B<1, misaligned pointer */
     KX_ERR_ALLOC = 2,         /* host or device allocation failed */
     KX_ERR_CUDA = 3,          /* CUDA runtime error (message in kx_last_error) */
-    KX_ERR_UNSUPPORTED = 4,   /* option not implemented (fp32 mode); N > 1024 (n, m, j_L are packed 10 bits each) */
+    KX_ERR_UNSUPPORTED = 4,   /* option not implemented (fp32 with quantum statistics, LINEAR with statistics); N > 1024 (n, m, j_L
+                                 are packed 10 bits each) */
     KX_ERR_NONFINITE = 5      /* kx_evolve produced a NaN/Inf in f */
 } kx_status_t;
 
@@ -68,7 +69,9 @@ typedef enum {
                                  interpolation error bound exceeds 1e-15 max f fall back to the streaming kernel */
 /* precision */
 #define KX_FP64 0
-#define KX_FP32 1             /* not implemented: KX_ERR_UNSUPPORTED */
+#define KX_FP32 1             /* optional: the contraction (a4-a5) in single precision on the streaming kernel (the paper's GPU timings
+                                 are fp32); interface arrays stay fp64; error <= 1e-4 of max |gain| (BASELINE.json);
+                                 classical statistics only (else KX_ERR_UNSUPPORTED); forces KX_STORE_SYM_ROWS */
 /* exp used by the LOG loss term */
 #define KX_EXP_TABLE 0        /* 256-entry table x degree-4 polynomial of the remainder, <= 2 ulp (default) */
 #define KX_EXP_LIBM  1        /* CUDA math library exp2() */
@@ -97,7 +100,7 @@ typedef struct { double M2_0; double m_med; } kx_msq_t;
 typedef struct {
     int32_t interp;      /* KX_INTERP_*  */
     int32_t storage;     /* KX_STORE_*   */
-    int32_t precision;   /* KX_FP64      */
+    int32_t precision;   /* KX_FP64 | KX_FP32 */
     int32_t exp_impl;    /* KX_EXP_*     */
     int32_t loss_nodes;  /* KX_STORE_TILED + LOG: Chebyshev nodes per bracket, 8|16|24|32; 0 = default (24) */
     int32_t statistics;  /* KX_STAT_*: eta = 0 | +1 | -1 */

@@ -5,8 +5,8 @@ There is no CPU fallback: importing works anywhere, every call needs an sm_100 G
 """
 from .kx import (Handle, KxError, build_library, library_path, exported_symbols,
                  INTERP_LOG, INTERP_LINEAR, EXP_TABLE, EXP_LIBM, STORE_SYM_ROWS, STORE_TILED, STAT_CLASSICAL, STAT_BOSE, STAT_FERMI, PROJECT, DIAG,
-                 EULER, HEUN, RK4)
+                 EULER, HEUN, RK4, FP64, FP32)
 
 __all__ = ["Handle", "KxError", "build_library", "library_path", "exported_symbols",
            "INTERP_LOG", "INTERP_LINEAR", "EXP_TABLE", "EXP_LIBM", "STORE_SYM_ROWS", "STORE_TILED", "STAT_CLASSICAL", "STAT_BOSE", "STAT_FERMI", "PROJECT", "DIAG",
-           "EULER", "HEUN", "RK4"]
+           "EULER", "HEUN", "RK4", "FP64", "FP32"]

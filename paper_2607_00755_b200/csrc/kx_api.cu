@@ -297,7 +297,11 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     kx_opts_t o = {KX_INTERP_LOG, KX_STORE_TILED, KX_FP64, KX_EXP_TABLE, 0, 0, 0, 0, 1e-300, 1e-12};
     if (opts) o = *opts;
     if (o.loss_nodes == 0) o.loss_nodes = 24;
-    if (o.precision != KX_FP64) { g_build_err = "fp32 mode is not implemented"; return KX_ERR_UNSUPPORTED; }
+    if (o.precision != KX_FP64 && o.precision != KX_FP32) { g_build_err = "unknown precision"; return KX_ERR_INVALID_ARG; }
+    if (o.precision == KX_FP32 && o.statistics != KX_STAT_CLASSICAL) {
+        g_build_err = "fp32 mode is implemented for classical statistics only";
+        return KX_ERR_UNSUPPORTED;
+    }
     if (o.storage != KX_STORE_SYM_ROWS && o.storage != KX_STORE_TILED) { g_build_err = "unknown storage mode"; return KX_ERR_UNSUPPORTED; }
     if (o.loss_nodes != 8 && o.loss_nodes != 16 && o.loss_nodes != 24 && o.loss_nodes != 32) {
         g_build_err = "loss_nodes must be 0 (default 24), 8, 16, 24 or 32";
@@ -313,6 +317,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         return KX_ERR_UNSUPPORTED;
     }
     if (o.statistics != KX_STAT_CLASSICAL) o.storage = KX_STORE_SYM_ROWS;     // evaluated by the exact streaming kernel
+    if (o.precision == KX_FP32) o.storage = KX_STORE_SYM_ROWS;                // the fp32 contraction is a streaming kernel
     if (o.n_mu < 0 || o.n_mu > 4096 || o.reserved != 0) { g_build_err = "n_mu must be in [0, 4096] and reserved 0"; return KX_ERR_INVALID_ARG; }
     if (o.exp_impl != KX_EXP_TABLE && o.exp_impl != KX_EXP_LIBM) { g_build_err = "unknown exp_impl"; return KX_ERR_INVALID_ARG; }
     if (!(o.f_floor >= 1e-300) || !(o.eps_supp >= 0.0)) { g_build_err = "need f_floor >= 1e-300 and eps_supp >= 0"; return KX_ERR_INVALID_ARG; }
@@ -340,7 +345,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
     KxDev& d = h->d;
     d = KxDev{};
     h->t = KxTiled{};
-    d.N = N; d.interp = o.interp; d.exp_impl = o.exp_impl; d.eta = o.statistics; d.chunk = 0;
+    d.N = N; d.interp = o.interp; d.exp_impl = o.exp_impl; d.eta = o.statistics; d.chunk = 0; d.prec = o.precision;
     d.m = sp->m; d.g_chi = sp->g_chi; d.M2_0 = msq->M2_0; d.m_med = msq->m_med;
     d.f_floor = o.f_floor; d.eps_supp = o.eps_supp;
     cudaStream_t s = (cudaStream_t)stream;

@@ -41,7 +41,7 @@ k_stream(KxDev d, const double* __restrict__ f, const double2* __restrict__ yd, 
     if (threadIdx.x == 0) stamp(st.trace, 0);
     const int groups = (B + BT - 1) / BT;
     for (int g = blockIdx.y; g < groups; g += gridDim.y)
-        contract_group<BT, MODE, QS>(d, f, yd, st.part, B, g * BT, blockIdx.x, gridDim.x, smem_raw);
+        contract_any<BT, MODE, QS>(d, f, yd, st.part, B, g * BT, blockIdx.x, gridDim.x, smem_raw);
     if (threadIdx.x == 0) stamp(st.trace, 1);
     if (d.N <= KX_CTA) stream_tail<1>(d, f, B, st, smem_raw, s_red);
     else if (d.N <= 2 * KX_CTA) stream_tail<2>(d, f, B, st, smem_raw, s_red);
@@ -86,7 +86,7 @@ __device__ __forceinline__ void stream_run(const KxDev& d, double* __restrict__ 
             const double* fin = stg == 0 ? f : st.fstage;
             const double2* yd = have_yd ? reinterpret_cast<const double2*>(st.ydnext) : nullptr;
             for (int g = blockIdx.y; g < groups; g += gridDim.y)
-                contract_group<BT, MODE, QS>(d, fin, yd, st.part, B, g * BT, blockIdx.x, gridDim.x, smem_raw, !have_yd);
+                contract_any<BT, MODE, QS>(d, fin, yd, st.part, B, g * BT, blockIdx.x, gridDim.x, smem_raw, !have_yd);
             grid_barrier_count(st.bar + 3, target);
             target += nctas;
             // (the finishing phase's scratch, N doubles at the head of the shared memory, lies inside the per-stage y rows: the
@@ -316,6 +316,10 @@ template <int BT>
 cudaError_t launch_stream_m(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st,
                             unsigned* bar_total, cudaStream_t s, const KxRun* run)
 {
+    if (d.prec == KX_FP32) {      // optional single-precision contraction (classical statistics only, checked in kx_build)
+        if (d.interp == KX_INTERP_LINEAR) return launch_stream_t<BT, MODE_LINEAR_F32, 0>(d, sm_count, f, yd, B, st, bar_total, s, run);
+        return launch_stream_t<BT, MODE_LOG_F32, 0>(d, sm_count, f, yd, B, st, bar_total, s, run);
+    }
     if (d.eta) {         // quantum statistics: LOG interpolation only (checked in kx_build)
         if (d.exp_impl == KX_EXP_LIBM) return launch_stream_t<BT, MODE_LOG_LIBM, 1>(d, sm_count, f, yd, B, st, bar_total, s, run);
         return launch_stream_t<BT, MODE_LOG_TAB, 1>(d, sm_count, f, yd, B, st, bar_total, s, run);

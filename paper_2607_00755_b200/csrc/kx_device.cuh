@@ -114,11 +114,13 @@ __device__ __forceinline__ double yval(double f, int interp, double f_floor, int
 // task0 + tstride, ...; each thread owns entries e0+tid, e0+tid+256, ... and keeps BT accumulators per sum (one per member
 // of the group b0 .. b0+BT-1) in registers; a fixed-order shuffle / shared-memory reduction writes one partial per
 // (task, member).
-enum { MODE_LOG_TAB = 0, MODE_LOG_LIBM = 1, MODE_LINEAR = 2 };
+enum { MODE_LOG_TAB = 0, MODE_LOG_LIBM = 1, MODE_LINEAR = 2, MODE_LOG_F32 = 3, MODE_LINEAR_F32 = 4 };
 
 template <int BT, int MODE, int QS>
 __host__ __device__ constexpr size_t contract_smem(int N)
 {
+    if (MODE >= MODE_LOG_F32)       // fp32 mode: float2 y rows, float f rows, double partials of the warps, task table
+        return (size_t)BT * N * 12 + (size_t)(KX_CTA / 32) * 2 * BT * 8 + 16 + (((size_t)(N + 1) * 4 + 15) & ~(size_t)15);
     return (size_t)BT * N * 24 + (size_t)(KX_CTA / 32) * (QS ? 4 : 2) * BT * 8
          + (MODE == MODE_LOG_TAB ? (size_t)(KX_EXP_REP << KX_EXP_BITS) * 8 : 0) + (((size_t)(N + 1) * 4 + 15) & ~(size_t)15);
 }
@@ -254,6 +256,107 @@ __device__ __forceinline__ void contract_group(const KxDev& d, const double* __r
         }
         __syncthreads();
     }
+}
+
+// ---------------------------------------------------------------- the same contraction in fp32 (KX_FP32, optional mode)
+// The paper times its GPU path in single precision (Fig. 3); BASELINE.json asks for <= 1e-4 of max |gain|.
+// W, omega are read as stored (fp64) and rounded; f, y = log2 max(f, 1e-37), the products and the per-thread sums are
+// float (exp2f: ex2.approx), the reduction over threads and everything after it (finishing phase) is fp64.
+template <int BT, int LIN>
+__device__ __forceinline__ void contract_group_f32(const KxDev& d, const double* __restrict__ f, double* __restrict__ part, int B,
+                                                   int b0, unsigned task0, unsigned tstride, unsigned char* smem_raw,
+                                                   bool load_static = true)
+{
+    const int N = d.N;
+    float2* s_yd = reinterpret_cast<float2*>(smem_raw);                    // [BT][N]
+    float* s_f = reinterpret_cast<float*>(s_yd + (size_t)BT * N);          // [BT][N]
+    double* s_red = reinterpret_cast<double*>(smem_raw + (((size_t)BT * N * 12 + 15) & ~(size_t)15));    // [8][2*BT]
+    unsigned* s_tp = reinterpret_cast<unsigned*>(s_red + (KX_CTA / 32) * 2 * BT);                         // [N+1]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nb = min(BT, B - b0);
+    const float floor32 = fmaxf((float)d.f_floor, 1e-37f);
+    for (int k = tid; k < BT * N; k += KX_CTA) {
+        const int b = k / N, j = k - b * N;
+        float fv = 0.f, y0 = 0.f, y1 = 0.f;
+        if (b < nb) {
+            fv = (float)__ldcg(f + (size_t)(b0 + b) * N + j);
+            const float fn = j + 1 < N ? (float)__ldcg(f + (size_t)(b0 + b) * N + j + 1) : fv;
+            y0 = LIN ? fv : log2f(fmaxf(fv, floor32));
+            y1 = LIN ? fn : log2f(fmaxf(fn, floor32));
+        }
+        s_yd[k] = make_float2(y0, y1 - y0);
+        s_f[k] = fv;
+    }
+    if (load_static) for (int k = tid; k <= N; k += KX_CTA) s_tp[k] = d.taskptr[k];
+    __syncthreads();
+    const unsigned ntasks = s_tp[N];
+    const unsigned chunk = (unsigned)d.chunk;
+    for (unsigned task = task0; task < ntasks; task += tstride) {
+        int lo = 0, hi = N - 1;
+        while (lo < hi) {
+            int mid = (lo + hi + 1) >> 1;
+            if (s_tp[mid] <= task) lo = mid; else hi = mid - 1;
+        }
+        const int i = lo;
+        const unsigned r0 = d.rowptr[i], r1 = d.rowptr[i + 1];
+        const unsigned e0 = r0 + (task - s_tp[i]) * chunk;
+        const unsigned e1 = min(e0 + chunk, r1);
+        float g[BT], l[BT];
+#pragma unroll
+        for (int b = 0; b < BT; ++b) { g[b] = 0.f; l[b] = 0.f; }
+        unsigned e = e0 + tid;
+        double W = 0.0, om = 0.0;
+        unsigned pk = 0;
+        if (e < e1) { W = d.W[e]; om = d.omega[e]; pk = d.nmj[e]; }
+        while (e < e1) {
+            const float Wc = (float)W, omc = (float)om;
+            const unsigned pkc = pk;
+            e += KX_CTA;
+            if (e < e1) { W = d.W[e]; om = d.omega[e]; pk = d.nmj[e]; }
+            const int n = pkc & 1023, m = (pkc >> 10) & 1023, j = pkc >> 20;
+#pragma unroll
+            for (int b = 0; b < BT; ++b) {
+                const float pn = s_f[b * N + n] * s_f[b * N + m];
+                g[b] = fmaf(Wc, pn, g[b]);
+                const float2 y = s_yd[b * N + j];
+                const float t = fmaf(omc, y.y, y.x);
+                l[b] = fmaf(Wc, LIN ? t : exp2f(t), l[b]);
+            }
+        }
+        double gd[BT], ld[BT];
+#pragma unroll
+        for (int b = 0; b < BT; ++b) {
+            gd[b] = (double)g[b]; ld[b] = (double)l[b];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                gd[b] += __shfl_xor_sync(0xffffffffu, gd[b], o);
+                ld[b] += __shfl_xor_sync(0xffffffffu, ld[b], o);
+            }
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int b = 0; b < BT; ++b) { s_red[warp * 2 * BT + 2 * b] = gd[b]; s_red[warp * 2 * BT + 2 * b + 1] = ld[b]; }
+        }
+        __syncthreads();
+        if (tid < 2 * BT) {
+            double acc = 0.0;
+#pragma unroll
+            for (int w = 0; w < KX_CTA / 32; ++w) acc += s_red[w * 2 * BT + tid];
+            const int b = tid / 2;
+            if (b < nb) part[((size_t)task * B + (b0 + b)) * 2 + (tid % 2)] = acc;
+        }
+        __syncthreads();
+    }
+}
+
+// one dispatch point for the kernels: fp64 (MODE 0-2) or fp32 (MODE 3-4) contraction of a member group
+template <int BT, int MODE, int QS>
+__device__ __forceinline__ void contract_any(const KxDev& d, const double* __restrict__ f, const double2* __restrict__ yd,
+                                             double* __restrict__ part, int B, int b0, unsigned task0, unsigned tstride,
+                                             unsigned char* smem_raw, bool load_static = true)
+{
+    if (MODE >= MODE_LOG_F32) contract_group_f32<BT, MODE == MODE_LINEAR_F32>(d, f, part, B, b0, task0, tstride, smem_raw, load_static);
+    else contract_group<BT, (MODE >= MODE_LOG_F32 ? MODE_LOG_TAB : MODE), QS>(d, f, yd, part, B, b0, task0, tstride, smem_raw, load_static);
 }
 
 // ---------------------------------------------------------------- block reductions (256 threads, fixed order)

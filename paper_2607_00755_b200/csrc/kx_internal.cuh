@@ -29,6 +29,7 @@ struct KxDev {
     int interp;          // KX_INTERP_*
     int exp_impl;        // KX_EXP_*
     int eta;             // KX_STAT_*: 0, +1 (Bose), -1 (Fermi)
+    int prec;            // KX_FP64 | KX_FP32 (arithmetic of the streaming contraction)
     int n_mu;            // > 0: numerical angular kernel with n_mu Gauss-Legendre nodes (gl_mu, gl_w)
     const double *gl_mu, *gl_w;
     int chunk;           // entries per contraction task

@@ -18,6 +18,7 @@ INTERP_LOG, INTERP_LINEAR = 0, 1
 STORE_SYM_ROWS, STORE_TILED = 0, 1
 STAT_CLASSICAL, STAT_BOSE, STAT_FERMI = 0, 1, -1
 FP64 = 0
+FP32 = 1
 EXP_TABLE, EXP_LIBM = 0, 1
 PROJECT, DIAG = 1, 2
 EULER, HEUN, RK4 = 0, 1, 2
@@ -177,7 +178,7 @@ class Handle:
 
     def __init__(self, p, dp, m=1.0, g_chi=1.0, M2_0=1.0, m_med=0.0, *, interp=INTERP_LOG,
                  exp_impl=EXP_TABLE, storage=STORE_TILED, loss_nodes=0, statistics=STAT_CLASSICAL, n_mu=0, f_floor=1e-300,
-                 eps_supp=1e-12, device=0, stream=None):
+                 eps_supp=1e-12, precision=FP64, device=0, stream=None):
         import torch
         if not torch.cuda.is_available():
             raise KxError(3, "no CUDA device: libkx has no CPU fallback")
@@ -192,7 +193,7 @@ class Handle:
         grid = _Grid(self.N, _ptr(p), _ptr(dp))
         sp = _Species(float(m), float(g_chi))
         msq = _Msq(float(M2_0), float(m_med))
-        opts = _Opts(int(interp), int(storage), FP64, int(exp_impl), int(loss_nodes), int(statistics), int(n_mu), 0, float(f_floor),
+        opts = _Opts(int(interp), int(storage), int(precision), int(exp_impl), int(loss_nodes), int(statistics), int(n_mu), 0, float(f_floor),
                      float(eps_supp))
         with torch.cuda.device(self.device):
             rc = lib.kx_build(C.byref(grid), C.byref(sp), C.byref(msq), C.byref(opts), self.device,

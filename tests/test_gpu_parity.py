@@ -459,3 +459,36 @@ def test_two_bump_eq51_workload(torch_cuda, oracle):
         assert v / 10 < corr[N] < v * 10, (N, corr[N], v)
     assert corr[256] < corr[128] < corr[96] and corr[256] < corr[96] / 3
     assert epsN[256] < epsN[96] / 3 and epsE[256] < epsE[96] / 3
+
+
+# --------------------------------------------------------------------------------------- optional fp32 mode
+@pytest.mark.parametrize("cfg,N,B,interp", [(1, None, None, 0), (3, 96, 9, 0), (3, 96, 9, 1), (4, 100, 3, 0)])
+def test_fp32_mode_within_1e4(torch_cuda, oracle, cfg, N, B, interp):
+    """KX_FP32 (BASELINE.json north_star: optional fp32 mode, max-abs error <= 1e-4 relative to max_i |gain_i|): the
+    contraction in single precision against the fp64 oracle; the projected operator still conserves at fp64 round-off
+    because the finishing phase stays in double."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(cfg, N=N, B=B)
+    T = oracle.Tables(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    g0, l0, C0 = oracle.collide(T, c["f"], interp)
+    h = _handle(c, interp=interp, precision=kx.FP32)
+    f = _dev(torch, c["f"])
+    o = h.collide_ex(f, flags=0, want=("C", "gain", "loss"))
+    for key, ref in (("gain", g0), ("loss", l0), ("C", C0)):
+        err = _relerr(o[key].cpu().numpy(), ref, g0)
+        assert err <= 1e-4, (key, err)
+        assert err >= 1e-12 or key == "C"                # it really is single precision
+    Cp = h.collide(f, flags=1).cpu().numpy()
+    Craw = o["C"].cpu().numpy()
+    assert (np.abs((T.h * Cp).sum(axis=1)) <= 1e-12 * (T.h * np.abs(Craw)).sum(axis=1)).all()
+    with pytest.raises(kx.KxError):
+        _handle(c, precision=kx.FP32, statistics=kx.STAT_BOSE)
+    # a few RK4 steps in fp32 stay within 1e-4 of the fp64 oracle's
+    pos = c["f"] > 0
+    nu = float((l0[pos] / c["f"][pos]).max())
+    tau = np.arange(4) * (0.5 / nu)
+    f_ref = oracle.evolve(c["p"], c["dp"], c["f"], m=c["m"], M2_0=c["M2_0"], m_med=c["m_med"], interp=interp, method=oracle.RK4, tau=tau)
+    h.evolve(f, tau, method=kx.RK4)
+    assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-4 * np.abs(f_ref).max()
+    h.close()
