@@ -52,7 +52,9 @@ constexpr int WARPS = kDmmaWarps;
 constexpr int NTHR = WARPS * 32;
 static_assert(NTHR == KX_CTA, "the finishing phase and the exact fallback run with 256 threads");
 constexpr int kStageBytes = KX_GROUP_DBL * 8 + 16;     // gain ring stage: 2 KiB of A + 4 descriptors
-constexpr int kLossStages = 3;
+// ring stages of a loss warp (4 KiB each).  (6 stages for small batches, where the kernel streams from HBM, were measured:
+// the X window no longer fits in one piece and every further window repeats the prologue: slower)
+__host__ __device__ constexpr int loss_stages(int nbt) { return 3; }
 constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256 rows of AL
 
 // ---------------------------------------------------------------- gain role
@@ -273,6 +275,7 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
                                           double* __restrict__ lpart, unsigned char* smem, unsigned long long* trace)
 {
     constexpr int LD = NBT * 8 + 4;
+    constexpr int kLossStages = loss_stages(NBT);
     constexpr int R8 = 32 / WARPS;            // 8-row blocks per warp: the CTA covers a 256-row supertile
     static_assert(WARPS == 8, "loss role: 8 warps");
     constexpr int MB = NBT * 8;               // members of this CTA
@@ -366,6 +369,7 @@ __device__ __forceinline__ void loss_role(const KxDev& dk, const KxTiled& t, con
             const int bl = tid % MB, part = tid / MB;
             const int b = bcol0 + bl;
             constexpr int QP = (KX_QMAX + PARTS - 1) / PARTS;       // nodes per thread and bracket, at most
+#pragma unroll(QP >= 4 ? 1 : 4)
             for (int jj = 0; jj < nj; ++jj) {
                 const double y0 = s_y[jj * MB + bl], y1 = s_y[(jj + 1) * MB + bl], dy = y1 - y0;
                 if (part == (jj & (PARTS - 1)) && b < B) {
@@ -603,7 +607,7 @@ k_dmma(const __grid_constant__ KxDev dk, const __grid_constant__ KxTiled t, cons
     if (tid == 0) { stamp(st.trace, 5); if (st.trace && blockIdx.x < KX_TRACE_CTAS) st.trace[blockIdx.x * KX_TRACE_SLOTS + 23] = clock64(); }
 }
 
-constexpr size_t kLossFixedBytes = (size_t)kLossStages * kLossABytes + (KX_QMAX + (1 << KX_EXP_BITS) + 2 * 64) * 8;
+constexpr size_t loss_fixed_bytes(int nbt) { return (size_t)loss_stages(nbt) * kLossABytes + (KX_QMAX + (1 << KX_EXP_BITS) + 2 * 64) * 8; }
 constexpr size_t kSmemMax = 226u * 1024u;       // dynamic shared memory: 227 KiB per CTA minus the kernel's static 544 bytes
 
 // chunks of 16 k whose Chebyshev coefficients a loss CTA keeps in shared memory at a time: its whole share if it fits
@@ -611,7 +615,7 @@ int loss_window(const KxTiled& t, int GL, int nbt)
 {
     const long long U = (long long)t.RS * t.LC;
     const long long share = (U + GL - 1) / GL + 1;
-    const long long fit = (long long)((kSmemMax - kLossFixedBytes) / ((size_t)16 * (nbt * 8 + 4) * 8));
+    const long long fit = (long long)((kSmemMax - loss_fixed_bytes(nbt)) / ((size_t)16 * (nbt * 8 + 4) * 8));
     long long wc = share < fit ? share : fit;
     return (int)(wc < 1 ? 1 : wc);
 }
@@ -622,7 +626,7 @@ size_t dmma_smem(int nbt, int N, const KxTiled& t, const KxPlan& plan)
 {
     const int WC = plan.WC;
     const size_t gain = (size_t)(nbt * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * dmma_stages(nbt) * kStageBytes;
-    const size_t loss = kLossFixedBytes + (size_t)WC * 16 * (nbt * 8 + 4) * 8;
+    const size_t loss = loss_fixed_bytes(nbt) + (size_t)WC * 16 * (nbt * 8 + 4) * 8;
     const size_t fb = contract_smem<KX_FB_BT, MODE_LOG_TAB, 0>(N);
     const size_t fin = finish_scratch_bytes(N, plan.GG, plan.GL, t.NT, t.RS);
     size_t m = gain > loss ? gain : loss;
@@ -697,7 +701,7 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
     double Ctot = 0.0;
     for (int k = 0; k < NT; ++k) {
         g[k] = vt_host[k + 1] - vt_host[k];
-        c[k] = g[k] ? (double)g[k] + kRunCost * (double)d.N : 0.0;
+        c[k] = g[k] ? (double)g[k] + (nbt <= 2 ? 0.0 : kRunCost) * (double)d.N : 0.0;     // small batches: bytes, not issue slots
         Ctot += c[k];
     }
     // the gain warps of GG CTAs dealt to the tiles in proportion to the tiles' costs (largest remainder), at least one and at
@@ -755,14 +759,17 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
     int gl0 = (int)((double)G * wl / (wg + wl) + 0.5);
     if (gl0 < 1) gl0 = 1;
     if (gl0 > (int)G - 1) gl0 = (int)G - 1;
-    const double chunk_groups = 2.0 * (double)(t.NR8 < 32 * t.RS ? t.NR8 : 32 * t.RS) / (32.0 * t.RS) * kLossChunk;
+    // small batches stream from HBM: a loss warp has 8 KiB in flight (2 of its 3 ring stages), a gain warp 14 KiB (7 of 8), and
+    // the loss chunk costs 2.7 instead of 2.1 groups (measured on cfg4: 0.78 us per chunk, 0.29 us per group)
+    const double chunk_w = nbt <= 2 ? 1.35 : kLossChunk, prologue_w = nbt <= 2 ? 13.0 : kLossPrologue;
+    const double chunk_groups = 2.0 * (double)(t.NR8 < 32 * t.RS ? t.NR8 : 32 * t.RS) / (32.0 * t.RS) * chunk_w;
     int gl = gl0;
     double best_t = 1e300;
     std::vector<unsigned> w, wtry;
-    for (int cand = gl0 - 4; cand <= gl0 + 4; ++cand) {
+    for (int cand = gl0 - 4; cand <= gl0 + 12; ++cand) {
         if (cand < 1 || cand > (int)G - 1 || cand > U) continue;
         const double tg = deal((int)G - cand, wtry);
-        const double tl = (double)((U + cand - 1) / cand) * chunk_groups + kLossPrologue;
+        const double tl = (double)((U + cand - 1) / cand) * chunk_groups + prologue_w;
         const double tt = tg > tl ? tg : tl;
         if (tt < best_t - 1e-9) { best_t = tt; gl = cand; }
     }
