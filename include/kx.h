@@ -267,6 +267,15 @@ kx_status_t kx_trace_read(kx_handle_t h, uint64_t* stamps);
  * contraction).  Synchronises the device; takes about 50 ms. */
 kx_status_t kx_probe_flops(int device, int32_t kind, double* tflops);
 
+/* Test aid, HOST only (no device is touched): the launch plan of the tensor-core kernel for a grid of N points, a batch of
+ * B members, Q loss nodes per bracket and `sm_count` SMs, given the number of gain groups of every 16-row tile
+ * (groups_per_tile[ceil(N/16)]).  head[8] = {gain CTAs, loss CTAs, member tiles per pass, loss window in chunks, tiles,
+ * supertiles, loss chunks, dynamic shared memory in bytes}; wstart[tiles + 1] = first gain warp of every tile (8 warps per
+ * CTA); ld[8] = first / last loss CTA of each of the (up to 4) supertiles.  tests/test_plan_cpu.py checks the invariants the
+ * kernel relies on (every gain warp owns at least one group, every partial slot that is summed was written, every CTA fits). */
+kx_status_t kx_plan_probe(int32_t N, int32_t B, int32_t Q, int32_t sm_count, const uint32_t* groups_per_tile,
+                          int32_t* head, uint32_t* wstart, uint32_t* ld);
+
 const char* kx_last_error(kx_handle_t h);   /* h may be NULL: returns the last build failure */
 void        kx_destroy(kx_handle_t h);
 int32_t     kx_version(void);

@@ -756,9 +756,16 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
     // and the split with the earliest barrier wins: gain = load of the busiest warp; loss = chunks of the busiest CTA, one
     // chunk of a full supertile being two groups' worth of DMMA per warp, plus the longer prologue of the loss role
     // (kLossPrologue groups, from the clock-stamp trace).
+    // the finishing phase gathers one 2 KiB slice per loss slot and one 128-byte slice per gain slot into shared memory: that
+    // bounds the number of loss CTAs (found by tests/test_plan_cpu.py on profiles with hardly any gain work)
+    const long long gl_cap = ((long long)kSmemMax - (long long)((d.N + 3) & ~3) * 8 - (G + NT) * 128) / 2048 - t.RS;
+    int gl_max = (int)G - 1;
+    if (gl_max > U) gl_max = (int)U;
+    if (gl_max > gl_cap) gl_max = (int)gl_cap;
+    if (gl_max < 1) gl_max = 1;
     int gl0 = (int)((double)G * wl / (wg + wl) + 0.5);
     if (gl0 < 1) gl0 = 1;
-    if (gl0 > (int)G - 1) gl0 = (int)G - 1;
+    if (gl0 > gl_max) gl0 = gl_max;
     // small batches stream from HBM: a loss warp has 8 KiB in flight (2 of its 3 ring stages), a gain warp 14 KiB (7 of 8), and
     // the loss chunk costs 2.7 instead of 2.1 groups (measured on cfg4: 0.78 us per chunk, 0.29 us per group)
     const double chunk_w = nbt <= 2 ? 1.35 : kLossChunk, prologue_w = nbt <= 2 ? 13.0 : kLossPrologue;
@@ -767,13 +774,13 @@ void kx_dmma_plan(const KxDev& d, const KxTiled& t, int sm_count, const unsigned
     double best_t = 1e300;
     std::vector<unsigned> w, wtry;
     for (int cand = gl0 - 4; cand <= gl0 + 12; ++cand) {
-        if (cand < 1 || cand > (int)G - 1 || cand > U) continue;
+        if (cand < 1 || cand > gl_max) continue;
         const double tg = deal((int)G - cand, wtry);
         const double tl = (double)((U + cand - 1) / cand) * chunk_groups + prologue_w;
         const double tt = tg > tl ? tg : tl;
         if (tt < best_t - 1e-9) { best_t = tt; gl = cand; }
     }
-    if (gl > U) gl = (int)U;                       // every loss CTA has at least one chunk
+    if (gl > gl_max) gl = gl_max;                  // every loss CTA has at least one chunk, the finishing scratch fits
     plan->nbt = nbt;
     plan->GL = gl;
     plan->GG = (int)G - gl;
@@ -800,4 +807,29 @@ cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, const KxPlan& plan,
         case 4: return launch_dmma_t<4, 4>(d, t, plan, f, B, st, bar_total, s);
         default: return launch_dmma_t<8, 4>(d, t, plan, f, B, st, bar_total, s);
     }
+}
+
+// Host-only view of the launch plan (no device needed): used by the CPU tests of the planner's invariants.
+extern "C" kx_status_t kx_plan_probe(int32_t N, int32_t B, int32_t Q, int32_t sm_count, const uint32_t* groups_per_tile,
+                                     int32_t* head, uint32_t* wstart, uint32_t* ld)
+{
+    if (N < 4 || N > KX_MAX_N || B < 1 || sm_count < 2 || !groups_per_tile || !head || !wstart || !ld) return KX_ERR_INVALID_ARG;
+    if (Q != 2 && Q != 8 && Q != 16 && Q != 24 && Q != 32) return KX_ERR_INVALID_ARG;
+    KxDev d = {};
+    d.N = N;
+    KxTiled t = {};
+    t.NT = (N + KX_TI - 1) / KX_TI;
+    t.Q = Q;
+    t.LC = ((N - 1) * Q + 15) / 16;
+    t.NR8 = (N + 7) / 8;
+    t.RS = (N + 255) / 256;
+    std::vector<unsigned> vt((size_t)t.NT + 1, 0u);
+    for (int k = 0; k < t.NT; ++k) vt[k + 1] = vt[k] + groups_per_tile[k];
+    KxPlan plan = {};
+    kx_dmma_plan(d, t, sm_count, vt.data(), B, &plan);
+    head[0] = plan.GG; head[1] = plan.GL; head[2] = plan.nbt; head[3] = plan.WC; head[4] = t.NT; head[5] = t.RS; head[6] = t.LC;
+    head[7] = (int32_t)dmma_smem(plan.nbt, N, t, plan);
+    for (int k = 0; k <= t.NT; ++k) wstart[k] = plan.wstart[k];
+    for (int k = 0; k < 4; ++k) { ld[k] = plan.ld0[k]; ld[4 + k] = plan.ld1[k]; }
+    return KX_OK;
 }

@@ -79,7 +79,7 @@ class _AdaptiveResult(C.Structure):
 SYMBOLS = ["kx_build", "kx_set_mass", "kx_collide", "kx_collide_parts", "kx_collide_ex",
            "kx_collide_host", "kx_moments", "kx_evolve", "kx_evolve_adaptive", "kx_delta_source", "kx_info", "kx_tensor_export",
            "kx_kinematics_export", "kx_reserve", "kx_fallback_members", "kx_profile", "kx_profile_read", "kx_trace", "kx_trace_read",
-           "kx_probe_flops", "kx_last_error", "kx_destroy", "kx_version"]
+           "kx_probe_flops", "kx_plan_probe", "kx_last_error", "kx_destroy", "kx_version"]
 TRACE_CTAS, TRACE_SLOTS = 160, 32
 
 _lib = None
@@ -130,6 +130,7 @@ def _load():
     lib.kx_profile.argtypes = [vp, i32]
     lib.kx_profile_read.argtypes = [vp, _dp, i64p]
     lib.kx_probe_flops.argtypes = [C.c_int, i32, _dp]
+    lib.kx_plan_probe.argtypes = [i32, i32, i32, i32, C.POINTER(C.c_uint32), C.POINTER(C.c_int32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
     lib.kx_last_error.argtypes = [vp]
     lib.kx_last_error.restype = C.c_char_p
     lib.kx_destroy.argtypes = [vp]
@@ -140,6 +141,23 @@ def _load():
             getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
+
+
+def plan_probe(N: int, B: int, groups_per_tile, Q: int = 24, sm_count: int = 148) -> dict:
+    """kx_plan_probe: the host-side launch plan of the tensor-core kernel (no device needed)."""
+    lib = _load()
+    g = np.ascontiguousarray(groups_per_tile, dtype=np.uint32)
+    NT = (N + 15) // 16
+    if g.size != NT:
+        raise ValueError("groups_per_tile must have ceil(N/16) entries")
+    head = (C.c_int32 * 8)()
+    wstart = (C.c_uint32 * (NT + 1))()
+    ld = (C.c_uint32 * 8)()
+    rc = lib.kx_plan_probe(N, B, Q, sm_count, g.ctypes.data_as(C.POINTER(C.c_uint32)), head, wstart, ld)
+    if rc != 0:
+        raise KxError(rc, "kx_plan_probe")
+    return dict(GG=head[0], GL=head[1], nbt=head[2], WC=head[3], NT=head[4], RS=head[5], LC=head[6], smem=head[7],
+                wstart=np.array(wstart[:], dtype=np.int64), ld0=np.array(ld[:4], dtype=np.int64), ld1=np.array(ld[4:], dtype=np.int64))
 
 
 def exported_symbols() -> list[str]:
