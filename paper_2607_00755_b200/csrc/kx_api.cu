@@ -573,7 +573,7 @@ kx_status_t kx_evolve(kx_handle_t h, double* f, int32_t B, const kx_source_t* sr
 
     // Small static-mass problems without per-step diagnostics: the whole integration is ONE cooperative launch
     // (k_stream_run: two grid barriers per stage instead of a launch per stage)
-    if (!use_tiled && !ctl->mass && !diag && S > 0) {
+    if (!use_tiled && !ctl->mass && !diag && S > 0 && kx_stream_run_supported(h->d)) {
         const size_t need = (size_t)(S + 1) + (ctl->rate ? (size_t)(2 * S + 1) : 0) + (size_t)nsrc * S;
         if (h->runbuf_cap < need) {
             KX_CUDA(cudaStreamSynchronize(s));

@@ -278,6 +278,19 @@ struct KxStage {             // what the finishing kernel does after the reducti
 cudaError_t kx_launch_stream(const KxDev& d, int sm_count, const double* f, const double* yd, int B,
                              KxStage st, unsigned* bar_total, cudaStream_t s);
 // a whole fixed-step integration (static mass, no diagnostics) on the exact streaming path in ONE cooperative launch
+// step data of a one-launch integration (k_stream_run), on the device
+struct KxRun {
+    int method, S;            // KX_EULER | KX_HEUN | KX_RK4, number of steps
+    const double* tau;        // device [S+1]
+    const double* rate;       // device [2S+1] or null
+    const double* amp;        // device [nsrc, S] or null
+};
+// the streaming kernels are instantiated per member-group size BT in kx_stream_bt{1,2,4,8}.cu (compiled in parallel)
+cudaError_t kx_launch_stream_bt1(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st, unsigned* bar_total, cudaStream_t s, const KxRun* run);
+cudaError_t kx_launch_stream_bt2(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st, unsigned* bar_total, cudaStream_t s, const KxRun* run);
+cudaError_t kx_launch_stream_bt4(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st, unsigned* bar_total, cudaStream_t s, const KxRun* run);
+cudaError_t kx_launch_stream_bt8(const KxDev& d, int sm_count, const double* f, const double* yd, int B, KxStage& st, unsigned* bar_total, cudaStream_t s, const KxRun* run);
+bool kx_stream_run_supported(const KxDev& d);      // built for the default fp64 paths only (LOG table exp2, LINEAR; classical)
 cudaError_t kx_launch_stream_run(const KxDev& d, int sm_count, double* f, int B, KxStage st, int method, int S,
                                  const double* tau_dev, const double* rate_dev, const double* amp_dev,
                                  unsigned* bar_total, cudaStream_t s);
