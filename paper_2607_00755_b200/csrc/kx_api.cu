@@ -355,7 +355,7 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         // one blob: 8 double arrays [N], exp table, int tables
         const size_t nd = (size_t)8 * N + (1u << KX_EXP_BITS);
         const size_t n2 = (size_t)N * N;
-        const size_t bytes = nd * 8 + (n2 * 2 + (n2 + 1) + 2 * (size_t)(N + 1) + 4) * 4;
+        const size_t bytes = nd * 8 + (n2 * 2 + (n2 + 1) + 2 * (size_t)(N + 1) + 4 + KX_BLUT_MAX + 4) * 4;
         KX_CUDA(cudaMalloc(&h->dev_blob, bytes));
         double* dp_ = (double*)h->dev_blob;
         double* P = dp_;            dp_ += N;
@@ -373,7 +373,8 @@ kx_status_t kx_build(const kx_grid_t* grid, const kx_species_t* sp, const kx_msq
         d.run_off = (unsigned*)ip;  ip += n2 + 1;
         d.rowptr = (unsigned*)ip;   ip += N + 1;
         d.taskptr = (unsigned*)ip;  ip += N + 1;
-        h->flag = ip;
+        h->flag = ip;               ip += 4;
+        d.blut = (unsigned*)ip;
         d.p = P; d.dp = DP; d.exptab = tab;
         std::vector<double> t(1u << KX_EXP_BITS);
         for (unsigned k = 0; k < (1u << KX_EXP_BITS); ++k)

@@ -42,6 +42,30 @@ __global__ void k_kinematics(KxDev d, double m)
     }
 }
 
+// bracket look-up table (kx_entry.cuh): one CTA; thread per key
+__global__ void __launch_bounds__(1024) k_bracket_lut(KxDev d)
+{
+    const int N = d.N;
+    const double* __restrict__ K = d.K;
+    const unsigned key0 = kx_key17(K[0]), key1 = kx_key17(K[N - 1]);
+    const unsigned size = key1 - key0 + 1u;
+    if (!(K[0] > 0.0) || size > KX_BLUT_MAX) {          // no table: k_fill falls back to the binary search
+        if (threadIdx.x == 0) { d.blut[0] = 0u; d.blut[1] = 0u; }
+        return;
+    }
+    if (threadIdx.x == 0) { d.blut[0] = key0; d.blut[1] = size; }
+    for (unsigned k = threadIdx.x; k < size; k += blockDim.x) {
+        // number of j with key(K_j) < key0 + k, minus one (clamped to 0): binary search on the monotone keys
+        int lo = 0, hi = N;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (kx_key17(K[mid]) < key0 + k) lo = mid + 1; else hi = mid;
+        }
+        const int j = lo - 1;
+        d.blut[2 + k] = (unsigned)(j < 0 ? 0 : (j > N - 2 ? N - 2 : j));
+    }
+}
+
 // one thread per (i,n): the interval of kept m in [n, N)
 __global__ void k_runs(KxDev d)
 {
@@ -124,7 +148,7 @@ __global__ void __launch_bounds__(1024) k_scan_base(KxDev d)
 }
 
 // one warp per run (i,n); lanes over m.  Writes W (symmetrised), omega_R and n|m<<10|jL<<20.
-__global__ void __launch_bounds__(256) k_fill(KxDev d)
+__global__ void __launch_bounds__(256, 4) k_fill(KxDev d)
 {
     const int N = d.N;
     const int lane = threadIdx.x & 31;
@@ -146,7 +170,7 @@ __global__ void __launch_bounds__(256) k_fill(KxDev d)
             const double Km = K[m];
             const double Kt = kx_Kt(Kn, Km, Ki, K0, KN1);       // D4: the kept triple's K~ snapped into the domain
             const double W = kx_Wsym(d, P, n, m, pi_, pn, Ki, Kn, Km, Kt, pref_in);
-            const int lo = kx_bracket(K, N, Kt);
+            const int lo = kx_bracket_lut(K, N, Kt, d.blut);
             const double om = (Kt - K[lo]) / (K[lo + 1] - K[lo]);   // eq. B.19
             const size_t e = (size_t)off + k;
             d.W[e] = W;
@@ -198,6 +222,7 @@ cudaError_t kx_launch_kinematics(const KxDev& d, double m, cudaStream_t s)
 cudaError_t kx_launch_runs(const KxDev& d, cudaStream_t s)
 {
     dim3 grid((d.N + 127) / 128, d.N);
+    k_bracket_lut<<<1, 1024, 0, s>>>(d);
     k_runs<<<grid, 128, 0, s>>>(d);
     k_scan_rows<<<d.N, 1024, 0, s>>>(d);
     k_scan_base<<<d.N, 1024, 0, s>>>(d);

@@ -135,6 +135,22 @@ __device__ __forceinline__ double kx_Wsym(const KxDev& d, const double* __restri
     return pref_in * d.ccol[m] * J;
 }
 
+// The same bracket through a look-up table: key(x) = the 18 leading bits of a positive double (exponent and 6 mantissa bits,
+// monotone in x); lut[key - key0] = the largest j whose key is BELOW that key (so K_j <= any value with the key), a lower
+// bound from which a short linear scan reaches the bracket: one table load and one or two comparisons instead of a binary
+// search of log2 N dependent loads.  The result is the same j by construction.  size 0 = no table (K spans too many binades).
+__device__ __forceinline__ unsigned kx_key17(double x) { return (unsigned)(__double_as_longlong(x) >> 46); }
+__device__ __forceinline__ int kx_bracket(const double* __restrict__ K, int N, double Kt);
+__device__ __forceinline__ int kx_bracket_lut(const double* __restrict__ K, int N, double Kt, const unsigned* __restrict__ lut)
+{
+    const unsigned key0 = __ldg(lut), size = __ldg(lut + 1);
+    if (size == 0) return kx_bracket(K, N, Kt);
+    const unsigned k = kx_key17(Kt);
+    int j = k <= key0 ? 0 : (int)__ldg(lut + 2 + min(k - key0, size - 1u));
+    while (j < N - 2 && K[j + 1] <= Kt) ++j;
+    return j;
+}
+
 // bracket: largest j in [0, N-2] with K_j <= K~                                   eq. B.19
 __device__ __forceinline__ int kx_bracket(const double* __restrict__ K, int N, double Kt)
 {

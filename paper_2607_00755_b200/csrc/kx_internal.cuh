@@ -22,6 +22,7 @@
 #define KX_TRACE_CTAS  160      // clock-stamp trace (kx_trace): CTAs x slots of 8 bytes
 #define KX_TRACE_SLOTS 32
 #define KX_FB_BT      4        // members per group of the exact fallback inside the DMMA kernel
+#define KX_BLUT_MAX   4096     // entries of the bracket look-up table (64 keys per binade of K)
 
 // Device-side view of a handle: plain pointers, passed by value to every kernel.
 struct KxDev {
@@ -52,6 +53,7 @@ struct KxDev {
     // contraction tasks: row i is cut into ceil(len_i/chunk) tasks
     unsigned *taskptr;        // [N+1] exclusive scan; taskptr[N] = ntasks
     const double *exptab;     // [2^KX_EXP_BITS] 2^(k/2^KX_EXP_BITS)
+    unsigned *blut;           // bracket look-up table of k_fill (kx_build.cu): [0] first key, [1] size, [2..] lower bound of j_L per key
 };
 
 // Tiled storage (KX_STORE_TILED), the operands of the DMMA contraction kernel (kx_tiled.cu).
