@@ -140,6 +140,20 @@ kx_status_t kx_collide_ex(kx_handle_t h, const double* f, double* C, double* gai
 kx_status_t kx_collide_host(kx_handle_t h, const double* f_host, double* C_host, int32_t B,
                             uint32_t flags, void* stream);
 
+/* The same operator (a4-a7, C only) through an entry point that ALLOCATES NOTHING: no cudaMalloc / cudaFree / allocating
+ * library routine, on any call (every other evaluation call may grow the handle's workspace on its first call with a larger
+ * batch).  For callers that cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid it.
+ * A variant of the fused exact streaming kernel evaluates the handle's row storage (any storage mode; classical statistics,
+ * fp64, else KX_ERR_UNSUPPORTED) with its scratch -- per-task partial sums, task table, grid-barrier words -- in a file-scope
+ * static __device__ array of about 2 MiB that every GPU loading the library holds until exit.
+ * Limit: (tasks x B) <= 131072 pairs of partial sums, tasks <= nnz / chunk + N with chunk = 4096 entries doubled up to 65536
+ * until it fits (BASELINE config 3, N = 256: B <= 81 at chunk 4096, more at larger chunks; config 4, N = 512: B <= 110); beyond
+ * that KX_ERR_UNSUPPORTED with a message naming the limit -- nothing is launched.
+ * All calls share the array and it keeps the last call's contents (what must start at zero is cleared by every call): calls
+ * that OVERLAP on one GPU (two streams, two host threads, two handles) race on it -- serialise them.  One cooperative launch
+ * plus a one-CTA set-up kernel; asynchronous on `stream`.  Results equal kx_collide's up to the order of the partial sums. */
+kx_status_t kx_collide_static(kx_handle_t h, const double* f, double* C, int32_t B, uint32_t flags, void* stream);
+
 /* a9: moments of eq. B.2.  f: DEVICE [B,N]; n, rho, p1 = <p>, p2 = <p^2>: DEVICE [B], any may be NULL. */
 kx_status_t kx_moments(kx_handle_t h, const double* f, int32_t B,
                        double* n, double* rho, double* p1, double* p2, void* stream);

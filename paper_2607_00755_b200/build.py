@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkx.so")
 SOURCES = ["kx_api.cu", "kx_build.cu", "kx_contract.cu", "kx_stream_bt1.cu", "kx_stream_bt2.cu", "kx_stream_bt4.cu", "kx_stream_bt8.cu",
-           "kx_tiled_build.cu", "kx_tiled.cu", "kx_probe.cu"]
+           "kx_tiled_build.cu", "kx_tiled.cu", "kx_probe.cu", "kx_static.cu"]
 HEADERS = [os.path.join(CSRC, "kx_internal.cuh"), os.path.join(CSRC, "kx_entry.cuh"), os.path.join(CSRC, "kx_device.cuh"), os.path.join(CSRC, "kx_stream.cuh"), os.path.join(HERE, "..", "include", "kx.h")]
 # --fmad=false: validity decisions, omega and the Runge-Kutta updates must not depend on implicit FMA
 # contraction; the hot loops call fma() explicitly.

@@ -76,7 +76,7 @@ class _AdaptiveResult(C.Structure):
 
 
 # every symbol include/kx.h declares
-SYMBOLS = ["kx_build", "kx_set_mass", "kx_collide", "kx_collide_parts", "kx_collide_ex",
+SYMBOLS = ["kx_build", "kx_set_mass", "kx_collide", "kx_collide_static", "kx_collide_parts", "kx_collide_ex",
            "kx_collide_host", "kx_moments", "kx_evolve", "kx_evolve_adaptive", "kx_delta_source", "kx_info", "kx_tensor_export",
            "kx_kinematics_export", "kx_reserve", "kx_fallback_members", "kx_profile", "kx_profile_read", "kx_trace", "kx_trace_read",
            "kx_probe_flops", "kx_plan_probe", "kx_last_error", "kx_destroy", "kx_version"]
@@ -112,6 +112,7 @@ def _load():
                              C.c_int, vp, C.POINTER(vp)]
     lib.kx_set_mass.argtypes = [vp, C.c_double, vp]
     lib.kx_collide.argtypes = [vp, vp, vp, i32, u32, vp]
+    lib.kx_collide_static.argtypes = [vp, vp, vp, i32, u32, vp]
     lib.kx_collide_parts.argtypes = [vp, vp, vp, vp, i32, vp]
     lib.kx_collide_ex.argtypes = [vp, vp, vp, vp, vp, vp, i32, u32, vp]
     lib.kx_collide_host.argtypes = [vp, vp, vp, i32, u32, vp]
@@ -246,6 +247,16 @@ class Handle:
         B = self._batch(f)
         out = torch.empty_like(f) if out is None else out
         self._check(self._lib.kx_collide(self._h, _dev(f), _dev(out), B, int(flags), _stream(stream)))
+        return out
+
+    def collide_static(self, f, flags=0, out=None, stream=None):
+        """kx_collide_static: the operator through the entry point that allocates nothing (static device scratch).  `out`
+        must be given by callers that may not allocate; it is created here only as a convenience when omitted."""
+        import torch
+        B = self._batch(f)
+        if out is None:
+            out = torch.empty_like(f)
+        self._check(self._lib.kx_collide_static(self._h, _dev(f), _dev(out), B, int(flags), _stream(stream)))
         return out
 
     def collide_parts(self, f, stream=None):
