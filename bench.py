@@ -48,7 +48,7 @@ LOSS_NODES = {"log": 24, "linear": 2}
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM; DMMA.8x8x4 runs at the same 37.2 TFLOP/s
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_dmma launch, from the committed `ncu --set full` capture named in
 # TRAFFIC_SOURCE (cfg3, LOG, B=64, raw operator); null for every other configuration
-NCU_TRAFFIC = {("log", 64): 61.34e6}
+NCU_TRAFFIC = {("log", 64): 61.27e6}
 TRAFFIC_SOURCE = "profiles/r02_k_dmma_full.md"
 
 
