@@ -492,3 +492,27 @@ def test_fp32_mode_within_1e4(torch_cuda, oracle, cfg, N, B, interp):
     h.evolve(f, tau, method=kx.RK4)
     assert np.abs(f.cpu().numpy() - f_ref).max() <= 1e-4 * np.abs(f_ref).max()
     h.close()
+
+
+def test_nonfinite_member_takes_the_exact_path(torch_cuda):
+    """structural zeros of the tiled operand are stored as A = 0, and 0 x Inf = NaN would leak into rows whose
+    (i, n, m) triple is dropped.  A member holding an Inf or a NaN is routed to the exact fallback (its max |f| statistic is
+    not finite), so the tiled and the row storage agree bit for bit on it, and its batch neighbours are untouched."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(3, N=64, B=4)
+    f = c["f"].copy()
+    f[1, 50] = np.inf
+    f[2, 3] = np.nan
+    ht, hr = _handle(c), _handle(c, storage=kx.STORE_SYM_ROWS)
+    fd = _dev(torch, f)
+    Ct = ht.collide(fd).cpu().numpy()
+    assert ht.fallback_members() == 2
+    Cr = hr.collide(fd).cpu().numpy()
+    for b in (1, 2):
+        assert np.array_equal(np.isnan(Ct[b]), np.isnan(Cr[b])) and np.array_equal(np.isinf(Ct[b]), np.isinf(Cr[b]))
+        ok = np.isfinite(Cr[b])
+        assert np.array_equal(Ct[b][ok], Cr[b][ok])
+    clean = ht.collide(_dev(torch, c["f"])).cpu().numpy()
+    assert np.array_equal(Ct[0], clean[0]) and np.array_equal(Ct[3], clean[3])
+    ht.close(); hr.close()
