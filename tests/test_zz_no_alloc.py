@@ -90,3 +90,29 @@ def test_static_entry_other_modes_and_limits(torch_cuda, oracle):
     with pytest.raises(kx.KxError):
         hb.collide_static(_dev(torch, np.full((1, 32), 0.1)))
     hb.close()
+
+
+def test_static_entry_leaves_device_memory_alone(torch_cuda):
+    """What "allocates nothing" means, observed from outside: after a first call (CUDA loads a kernel's code lazily on its
+    first launch), the free device memory reported by the driver does not move over further calls with new batch sizes --
+    whereas the ordinary entry point grows the handle's workspace when it first sees a larger batch."""
+    torch = torch_cuda
+    import paper_2607_00755_b200 as kx
+    c = kin.config(3, N=128, B=48)
+    h = kx.Handle(c["p"], c["dp"], c["m"], c["g_chi"], c["M2_0"], c["m_med"])
+    f = _dev(torch, c["f"])
+    outs = {B: torch.empty((B, 128), dtype=torch.float64, device="cuda") for B in (2, 7, 48)}
+    h.collide_static(f[:2].contiguous(), out=outs[2])
+    h.collide_static(f[:2].contiguous(), flags=kx.PROJECT, out=outs[2])
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for B in (7, 48, 2, 48):
+        fb = f[:B]                                           # a view of the leading rows: contiguous, no torch allocation
+        h.collide_static(fb, out=outs[B])
+        h.collide_static(fb, flags=kx.PROJECT, out=outs[B])
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free0
+    h.collide(f)                                             # the ordinary path allocates its workspace for B = 48 now
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] < free0
+    h.close()
