@@ -620,7 +620,7 @@ int loss_window(const KxTiled& t, int GL, int nbt)
     return (int)(wc < 1 ? 1 : wc);
 }
 
-int dmma_stages(int nbt) { return nbt <= 2 ? 8 : 4; }
+int dmma_stages(int nbt) { return nbt <= 2 ? 8 : (nbt == 8 ? 5 : 4); }
 
 size_t dmma_smem(int nbt, int N, const KxTiled& t, const KxPlan& plan)
 {
@@ -673,7 +673,7 @@ cudaError_t kx_dmma_configure()
     cudaError_t e = cudaFuncSetAttribute(k_dmma<1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
     done = e == cudaSuccess;
     return e;
 }
@@ -805,7 +805,7 @@ cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, const KxPlan& plan,
         case 1: return launch_dmma_t<1, 8>(d, t, plan, f, B, st, bar_total, s);
         case 2: return launch_dmma_t<2, 8>(d, t, plan, f, B, st, bar_total, s);
         case 4: return launch_dmma_t<4, 4>(d, t, plan, f, B, st, bar_total, s);
-        default: return launch_dmma_t<8, 4>(d, t, plan, f, B, st, bar_total, s);
+        default: return launch_dmma_t<8, 5>(d, t, plan, f, B, st, bar_total, s);
     }
 }
 
