@@ -65,7 +65,7 @@ constexpr int kLossABytes = 32 * 1024;                 // loss stage: 16 k x 256
 // run (fixed n) take X = f_m and accumulate into T; f_n multiplies T once, when the run ends.  When all warps are done
 // they leave their accumulators in shared memory and the CTA adds those of the same tile in warp order: one partial per
 // (CTA, tile), slot = CTA + tile.
-template <int NBT, int STAGES>
+template <int NBT, int STAGES, int LDNC>
 __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, int N, int B, int bcol0,
                                           const double* __restrict__ f, int gslots, double* __restrict__ gpart,
                                           unsigned char* smem, int* s_wtile, unsigned long long* trace,
@@ -73,7 +73,9 @@ __device__ __forceinline__ void gain_role(const KxTiled& t, const KxPlan& plan, 
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int krow = lane & 3, lr = lane >> 2;
-    const int LDN = (N + 7) & ~3;             // row stride of s_f: >= N + 4, = 0 mod 4; N = 0 mod 16 gives 4 mod 16
+    // row stride of s_f: >= N + 4, = 0 mod 4; N = 0 mod 16 gives 4 mod 16.  LDNC != 0: a compile-time stride (260 for N <= 256),
+    // so that the eight member-tile rows of a fragment load sit at immediate offsets (28 address adds less per group)
+    const int LDN = LDNC ? LDNC : ((N + 7) & ~3);
     double* s_f = reinterpret_cast<double*>(smem);                                    // [8 NBT][LDN]
     unsigned char* ring = smem + (size_t)(NBT * 8) * LDN * 8 + (size_t)warp * STAGES * kStageBytes;
 
@@ -578,7 +580,7 @@ __device__ __forceinline__ void dmma_tail(const KxDev& dk, const KxPlan& plan, i
 // ---------------------------------------------------------------- the fused kernel: one CTA per SM, cooperative
 // Clock stamps (st.trace, per CTA): 0 entry, 1 prologue done (f staged / first coefficient window built), 2 partials
 // written, 3 first barrier passed, 4 fallback done, 5 finishing phase done; 8..15 end of each gain warp's stream.
-template <int NBT, int STAGES>
+template <int NBT, int STAGES, int LDNC>
 __global__ void __launch_bounds__(NTHR, 1)
 k_dmma(const __grid_constant__ KxDev dk, const __grid_constant__ KxTiled t, const __grid_constant__ KxPlan plan, int B,
        const double* __restrict__ f, const __grid_constant__ KxStage st)
@@ -596,7 +598,7 @@ k_dmma(const __grid_constant__ KxDev dk, const __grid_constant__ KxTiled t, cons
     __syncthreads();                                // the barrier is initialised
     for (int by = 0; by < ny; ++by) {          // member groups of 8 NBT: one pass each (more than one for B > 64 only)
         const int bcol0 = by * NBT * 8;
-        if ((int)blockIdx.x < plan.GG) gain_role<NBT, STAGES>(t, plan, N, B, bcol0, f, st.gslots, st.gpart, smem, s_wtile, st.trace, &s_mbar, mpar);
+        if ((int)blockIdx.x < plan.GG) gain_role<NBT, STAGES, LDNC>(t, plan, N, B, bcol0, f, st.gslots, st.gpart, smem, s_wtile, st.trace, &s_mbar, mpar);
         else loss_role<NBT>(dk, t, plan, N, B, bcol0, f, st.mstat, st.lslots, st.lpart, smem, st.trace);
         __syncthreads();
     }
@@ -620,12 +622,15 @@ int loss_window(const KxTiled& t, int GL, int nbt)
     return (int)(wc < 1 ? 1 : wc);
 }
 
+// row stride of the staged f in the gain role (see gain_role): a constant 260 for the 8-tile kernel on grids up to 256
+int gain_ldn(int nbt, int N) { return (nbt == 8 && N <= 256) ? 260 : ((N + 7) & ~3); }
+
 int dmma_stages(int nbt) { return nbt <= 2 ? 8 : (nbt == 8 ? 5 : 4); }
 
 size_t dmma_smem(int nbt, int N, const KxTiled& t, const KxPlan& plan)
 {
     const int WC = plan.WC;
-    const size_t gain = (size_t)(nbt * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * dmma_stages(nbt) * kStageBytes;
+    const size_t gain = (size_t)(nbt * 8) * gain_ldn(nbt, N) * 8 + (size_t)WARPS * dmma_stages(nbt) * kStageBytes;
     const size_t loss = loss_fixed_bytes(nbt) + (size_t)WC * 16 * (nbt * 8 + 4) * 8;
     const size_t fb = contract_smem<KX_FB_BT, MODE_LOG_TAB, 0>(N);
     const size_t fin = finish_scratch_bytes(N, plan.GG, plan.GL, t.NT, t.RS);
@@ -639,18 +644,18 @@ size_t dmma_smem(int nbt, int N, const KxTiled& t, const KxPlan& plan)
 int dmma_nbt(int N, int B)
 {
     int nbt = B <= 8 ? 1 : (B <= 16 ? 2 : (B <= 32 ? 4 : 8));
-    auto need = [&](int k) { return (size_t)(k * 8) * ((N + 7) & ~3) * 8 + (size_t)WARPS * dmma_stages(k) * kStageBytes + 512; };
+    auto need = [&](int k) { return (size_t)(k * 8) * gain_ldn(k, N) * 8 + (size_t)WARPS * dmma_stages(k) * kStageBytes + 512; };
     while (nbt > 1 && need(nbt) > kSmemMax) nbt >>= 1;
     return nbt;
 }
 
-template <int NBT, int STAGES>
+template <int NBT, int STAGES, int LDNC>
 cudaError_t launch_dmma_t(const KxDev& d, const KxTiled& t, const KxPlan& plan, const double* f, int B, KxStage& st,
                           unsigned* bar_total, cudaStream_t s)
 {
     const size_t smem = dmma_smem(NBT, d.N, t, plan);
     st.bar_target = *bar_total + (unsigned)(plan.GG + plan.GL);
-    const cudaError_t e = kx_launch_coop(k_dmma<NBT, STAGES>, dim3(plan.GG + plan.GL), dim3(NTHR), smem, s, d, t, plan, B, f, st);
+    const cudaError_t e = kx_launch_coop(k_dmma<NBT, STAGES, LDNC>, dim3(plan.GG + plan.GL), dim3(NTHR), smem, s, d, t, plan, B, f, st);
     if (e == cudaSuccess) *bar_total = st.bar_target;
     return e;
 }
@@ -670,10 +675,11 @@ cudaError_t kx_dmma_configure()
 {
     static bool done = false;
     if (done) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(k_dmma<1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    cudaError_t e = cudaFuncSetAttribute(k_dmma<1, 8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<2, 8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<4, 4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<8, 5, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dmma<8, 5, 260>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
     done = e == cudaSuccess;
     return e;
 }
@@ -802,10 +808,12 @@ cudaError_t kx_launch_dmma(const KxDev& d, const KxTiled& t, const KxPlan& plan,
                            KxStage st, unsigned* bar_total, cudaStream_t s)
 {
     switch (plan.nbt) {
-        case 1: return launch_dmma_t<1, 8>(d, t, plan, f, B, st, bar_total, s);
-        case 2: return launch_dmma_t<2, 8>(d, t, plan, f, B, st, bar_total, s);
-        case 4: return launch_dmma_t<4, 4>(d, t, plan, f, B, st, bar_total, s);
-        default: return launch_dmma_t<8, 5>(d, t, plan, f, B, st, bar_total, s);
+        case 1: return launch_dmma_t<1, 8, 0>(d, t, plan, f, B, st, bar_total, s);
+        case 2: return launch_dmma_t<2, 8, 0>(d, t, plan, f, B, st, bar_total, s);
+        case 4: return launch_dmma_t<4, 4, 0>(d, t, plan, f, B, st, bar_total, s);
+        default:
+            if (d.N <= 256) return launch_dmma_t<8, 5, 260>(d, t, plan, f, B, st, bar_total, s);
+            return launch_dmma_t<8, 5, 0>(d, t, plan, f, B, st, bar_total, s);
     }
 }
 
